@@ -1,0 +1,562 @@
+"""Pins for the oracle (run with -m "not gpu").
+
+Each test checks ``oracle/`` against something other than itself: values printed by the paper or the
+literature (tests/golden), closed forms, invariants, brute force on tiny inputs.  Citations are
+PAPER.md line numbers (``:NNN``).
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate, optimize, special
+
+import oracle
+
+L = oracle.lib()
+
+RHO_W, SIGMA_W, R_V, R_D, C_PD, P1000 = 1000.0, 0.072, 461.5, 287.0, 1005.0, 1e5
+
+
+# ----------------------------------------------------------------------------- Philox
+def test_philox_known_answers(golden_dir):
+    rows = [l.split() for l in open(os.path.join(golden_dir, "philox_kat.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r if t != "->"]
+        out = oracle.philox(v[0:4], v[4:6])
+        assert [int(t) for t in out] == v[6:10]
+
+
+def test_philox_counter_sensitivity():
+    # a dropped counter word or key word would leave the output unchanged under that word's change
+    base = oracle.philox([1, 2, 3, 4], [5, 6])
+    for w in range(4):
+        c = [1, 2, 3, 4]
+        c[w] += 1
+        assert (oracle.philox(c, [5, 6]) != base).all()
+    assert (oracle.philox([1, 2, 3, 4], [6, 6]) != base).all()
+    assert (oracle.philox([1, 2, 3, 4], [5, 7]) != base).all()
+
+
+# ----------------------------------------------------------------------------- sort / pairing
+def _grid_oracle(nx=4, nz=3, **kw):
+    return oracle.Oracle(nx=nx, ny=0, nz=nz, dx=10.0, dy=1.0, dz=20.0, dt=1.0, **kw)
+
+
+def test_sort_is_lexicographic_definition():
+    """:624 + BASELINE north_star: order = sort on (cell, Philox key, id); key = Philox(id, step, 0, 0).w0."""
+    rng = np.random.default_rng(3)
+    N = 500
+    o = _grid_oracle(seed=0x1234567855AA)
+    x, z = rng.uniform(0, 40, N), rng.uniform(0, 60, N)
+    ids = rng.permutation(10 * N)[:N].astype(np.uint32)
+    n = rng.integers(1, 100, N).astype(np.uint64)
+    n[::17] = 0  # dead SDs never reach the sort
+    o.set_state(n, np.full(N, 1e-12), np.full(N, 1e-24), np.full(N, 0.5), x=x, z=z, id=ids)
+    o.set_step(7)
+    o.stage("sort")
+    got_ids, seg = o.get_order()
+    live = n > 0
+    cell = (np.floor(x / 10.0).astype(int) * 1 + 0) * 3 + np.floor(z / 20.0).astype(int)
+    key = [int(oracle.philox([int(i), 7, 0, 0], [0x567855AA, 0x1234])[0]) for i in ids]
+    tup = sorted((int(cell[s]), key[s], int(ids[s])) for s in range(N) if live[s])
+    assert [t[2] for t in tup] == [int(i) for i in got_ids]
+    counts = np.bincount([t[0] for t in tup], minlength=12)
+    assert (np.diff(seg) == counts).all()
+    assert o.n_sd() == live.sum()  # compaction happened
+
+
+def test_pairings_of_four_are_uniform():
+    """:624 "randomly grouped into non-overlapping pairs": each of the 3 pairings of 4 SDs has frequency 1/3."""
+    o = oracle.Oracle(dx=1, dy=1, dz=1, seed=99)
+    ones = np.ones(4)
+    counts = {}
+    T = 30000
+    for t in range(T):
+        o.set_state(np.full(4, 5, np.uint64), ones, ones, ones)
+        o.set_step(t)
+        o.stage("sort")
+        ids, _ = o.get_order()
+        p = frozenset([frozenset(ids[:2].tolist()), frozenset(ids[2:].tolist())])
+        counts[p] = counts.get(p, 0) + 1
+    assert len(counts) == 3
+    for c in counts.values():
+        assert abs(c / T - 1 / 3) < 4.5 * np.sqrt(2 / 9 / T)
+
+
+@pytest.mark.parametrize("nsd", [3, 4, 5, 6])
+def test_pair_probability_bruteforce(nsd):
+    """:626-631 eq. 27: thanks to the factor n(n-1)/2 / floor(n/2), the expected number of collision
+    events of every unordered pair (i,j) per step equals the unscaled max(N_i,N_j) K dt/dV."""
+    rng = np.random.default_rng(nsd)
+    n = (np.array([7, 11, 13, 17, 19, 23][:nsd]) * 1000).astype(np.uint64)
+    r = rng.uniform(10e-6, 30e-6, nsd)
+    v = 4 / 3 * np.pi * r**3
+    b, dV, dt = 1500.0, 1e-3, 1.0
+    o = oracle.Oracle(dx=0.1, dy=0.1, dz=0.1, dt=dt, kernel="golovin", golovin_b=b, seed=4242)
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True)
+    pairs = list(itertools.combinations(range(nsd), 2))
+    expect = {pr: max(n[pr[0]], n[pr[1]]) * b * (v[pr[0]] + v[pr[1]]) * dt / dV for pr in pairs}
+    scale = (nsd * (nsd - 1) / 2) / (nsd // 2)
+    assert max(expect.values()) * scale < 1.0  # stay in the single-collision regime
+    T = 60000
+    hits = dict.fromkeys(pairs, 0)
+    rw2, rd3, kap = r**2, np.full(nsd, 1e-27), np.full(nsd, 0.5)
+    for t in range(T):
+        o.set_state(n, rw2, rd3, kap)
+        o.set_step(t)
+        o.stage("sort")
+        o.stage("coal", op)
+        st = o.get_state()
+        grown = np.nonzero(st["rw2"] != rw2)[0]
+        shrunk = np.nonzero(st["n"] != n)[0]
+        assert len(grown) == len(shrunk)
+        for k in grown:  # the partner is the SD whose multiplicity dropped by n_k
+            j = [j for j in shrunk if n[j] - st["n"][j] == n[k]]
+            assert len(j) == 1
+            hits[tuple(sorted((int(k), int(j[0]))))] += 1
+    for pr in pairs:
+        p = expect[pr]
+        sd = np.sqrt(T * p * scale)  # event count ~ Binomial with variance <= T p scale / scale... use generous bound
+        assert abs(hits[pr] - T * p) < 4.5 * max(sd / np.sqrt(scale), 3.0), (pr, hits[pr], T * p)
+
+
+def test_collision_update_worked_example():
+    """:639-643 with DESIGN.md reading R-collision (Shima 2009 rule): hand-computed two-SD cell."""
+    b, dV, dt = 1.0, 1.0, 1.0
+    rj, rk = 2.0e-1, 1.0e-1
+    vj, vk = 4 / 3 * np.pi * rj**3, 4 / 3 * np.pi * rk**3
+    nj, nk = 8, 2
+    p = nj * b * (vj + vk) * dt / dV  # n_c = 2 -> scale factor 1
+    assert 0.3 < p < 0.31
+    # choose b so that p = 10.3 > floor(n_j/n_k) = 4  -> g = 4, SD j dies
+    o = oracle.Oracle(dx=1, dy=1, dz=1, dt=dt, kernel="golovin", golovin_b=10.3 / p, seed=1)
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True)
+    o.set_state(np.array([nj, nk], np.uint64), np.array([rj**2, rk**2]), np.array([3e-24, 1e-24]), np.array([0.2, 0.8]))
+    o.stage("sort")
+    o.stage("coal", op)
+    st = o.get_state()
+    j, k = (0, 1)
+    assert st["n"].tolist() == [0, 2]
+    assert st["rw2"][j] == rj**2 and st["rd3"][j] == 3e-24 and st["kappa"][j] == 0.2  # j keeps its radii
+    np.testing.assert_allclose(st["rw2"][k] ** 1.5, rk**3 + 4 * rj**3, rtol=1e-14)
+    np.testing.assert_allclose(st["rd3"][k], 1e-24 + 4 * 3e-24, rtol=1e-15)
+    np.testing.assert_allclose(st["kappa"][k], (4 * 3e-24 * 0.2 + 1e-24 * 0.8) / (13e-24), rtol=1e-15)
+    # p = 2.5 -> gamma in {2, 3} (multi_coal) but exactly {0 or 1} in the paper's variant (:645)
+    for multi, allowed in ((True, {2, 3}), (False, {1})):
+        seen = set()
+        o = oracle.Oracle(dx=1, dy=1, dz=1, dt=dt, kernel="golovin", golovin_b=2.5 / p, seed=1, multi_coal=multi)
+        for t in range(40):
+            o.set_state(np.array([nj, nk], np.uint64), np.array([rj**2, rk**2]), np.array([3e-24, 1e-24]), np.array([0.2, 0.8]))
+            o.set_step(t)
+            o.stage("sort")
+            o.stage("coal", op)
+            seen.add((nj - int(o.get_state()["n"][0])) // nk)
+        assert seen == allowed
+
+
+def test_equal_multiplicity_tie_break_first_in_order_is_j():
+    """DESIGN.md reading R-tie: on N_i = N_j the first SD in sorted order loses its multiplicity (:641)."""
+    o = oracle.Oracle(dx=1, dy=1, dz=1, dt=1.0, kernel="golovin", golovin_b=1e18, seed=5)
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True)
+    for t in range(20):
+        o.set_state(np.array([5, 5], np.uint64), np.array([1e-10, 4e-10]), np.full(2, 1e-27), np.full(2, 0.5))
+        o.set_step(t)
+        o.stage("sort")
+        first = int(o.get_order()[0][0])
+        o.stage("coal", op)
+        n = o.get_state()["n"]
+        assert n[first] == 0 and n[1 - first] == 5
+
+
+def test_coalescence_conserves_mass_and_sum_n_is_monotone():
+    """:643 extensive attributes are summed: sum N r_w^3 and sum N r_d^3 are conserved (this is what decides
+    reading R-collision, the printed wording of :639 does not conserve mass); sum N never grows."""
+    rng = np.random.default_rng(11)
+    N = 4000
+    o = _grid_oracle(kernel="geometric", seed=77)
+    o.set_fields(th=np.full(12, 289.0), rv=np.full(12, 7.5e-3), rhod=np.full(12, 1.1))
+    n = rng.integers(1, 10**6, N).astype(np.uint64) * 1000
+    r = np.exp(rng.uniform(np.log(1e-6), np.log(300e-6), N))
+    rd3 = np.exp(rng.uniform(np.log(1e-24), np.log(1e-20), N))
+    kap = rng.choice([0.3, 0.61, 1.2], N)
+    o.set_state(n, r**2, rd3, kap, x=rng.uniform(0, 40, N), z=rng.uniform(0, 60, N))
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, sstp_coal=3)
+    f = np.float64
+    m_w0, m_d0, s0 = (n.astype(f) * r**3).sum(), (n.astype(f) * rd3).sum(), int(n.sum())
+    kd0 = (n.astype(f) * rd3 * kap).sum()
+    for _ in range(20):
+        o.step(op)
+        st = o.get_state()
+        nn = st["n"].astype(f)
+        assert abs((nn * st["rw2"] ** 1.5).sum() / m_w0 - 1) < 1e-13
+        assert abs((nn * st["rd3"]).sum() / m_d0 - 1) < 1e-13
+        assert abs((nn * st["rd3"] * st["kappa"]).sum() / kd0 - 1) < 1e-13  # dry-volume-weighted kappa
+        s1 = int(st["n"].sum())
+        assert s1 <= s0
+        s0 = s1
+    c = o.counters()
+    assert c["collisions"] > 1000 and s0 < int(n.sum())  # the test did exercise collisions (incl. gamma > 1)
+
+
+# ----------------------------------------------------------------------------- Golovin box
+def golovin_n(v, t, n0, v0, b):
+    """Golovin (1963) solution for K = b(u+v), n(v,0) = n0/v0 exp(-v/v0)."""
+    T = b * n0 * v0 * t
+    tau = 1 - np.exp(-T)
+    x = v / v0
+    return n0 / v0 * (1 - tau) / (x * np.sqrt(tau)) * special.ive(1, 2 * x * np.sqrt(tau)) * np.exp(-x * (1 - np.sqrt(tau)) ** 2)
+
+
+def test_golovin_closed_form_moments():
+    n0, v0, b, t = 2.0**23, 4 / 3 * np.pi * 30.531e-6**3, 1500.0, 1200.0
+    T = b * n0 * v0 * t
+    lx = np.linspace(-30, 9, 400001)  # trapezoid in ln(v/v0); integrand is smooth and decays at both ends
+    M = [np.trapezoid(golovin_n(np.exp(lx) * v0, t, n0, v0, b) * (np.exp(lx) * v0) ** (k + 1), lx) for k in range(3)]
+    np.testing.assert_allclose(M[0], n0 * np.exp(-T), rtol=1e-6)
+    np.testing.assert_allclose(M[1], n0 * v0, rtol=1e-6)
+    np.testing.assert_allclose(M[2], 2 * n0 * v0**2 * np.exp(2 * T), rtol=1e-6)
+
+
+def test_box_golovin_against_analytic_solution():
+    """BASELINE.json configs[0]: V=1e6 m^3, 2^13 SDs, n0=2^23 m^-3, v0=(4/3)pi(30.531um)^3, b=1500/s, dt=1 s.
+    Pooled over 16 seeds, the zeroth moment and the binned mass spectrum follow the Golovin solution."""
+    N, n0, V, b = 2**13, 2.0**23, 1e6, 1500.0
+    v0 = 4 / 3 * np.pi * 30.531e-6**3
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True)
+    edges = np.exp(np.linspace(np.log(5e-6), np.log(2e-3), 25))
+    times = (1200, 2400, 3600)
+    M0 = {t: [] for t in times}
+    hist = {t: np.zeros(len(edges) - 1) for t in times}
+    mass = []
+    for seed in range(42, 58):
+        rng = np.random.default_rng(seed)
+        v = rng.exponential(v0, N)
+        o = oracle.Oracle(dx=100, dy=100, dz=100, dt=1.0, kernel="golovin", golovin_b=b, seed=seed)
+        n = np.full(N, int(n0 * V / N), np.uint64)
+        o.set_state(n, (v / (4 / 3 * np.pi)) ** (2 / 3), np.full(N, 1e-27), np.full(N, 0.5))
+        m_ini = (n * v).sum()
+        for t in range(1, 3601):
+            o.step(op)
+            if t in times:
+                st = o.get_state()
+                live = st["n"] > 0
+                r = np.sqrt(st["rw2"][live])
+                nn = st["n"][live].astype(float)
+                M0[t].append(nn.sum() / V)
+                hist[t] += np.histogram(r, edges, weights=nn * 4 / 3 * np.pi * r**3)[0] / V
+                mass.append((nn * 4 / 3 * np.pi * r**3).sum() / m_ini)
+    np.testing.assert_allclose(mass, 1.0, rtol=1e-12)  # first moment constant
+    tol_M0 = {1200: 0.06, 2400: 0.12, 3600: 0.35}  # sampling error grows as the SD count decays
+    for t in times:
+        T = b * n0 * v0 * t
+        ratio = np.mean(M0[t]) / (n0 * np.exp(-T))
+        assert abs(ratio - 1) < tol_M0[t], (t, ratio)
+    # mass density per bin at 1200 s against the integral of the closed form
+    t = 1200
+    ana = np.array([integrate.quad(lambda lr: golovin_n(4 / 3 * np.pi * np.exp(3 * lr), t, n0, v0, b)
+                                   * (4 / 3 * np.pi * np.exp(3 * lr)) ** 2 * 3, np.log(a), np.log(c))[0]
+                    for a, c in zip(edges[:-1], edges[1:])])
+    sim = hist[t] / 16
+    assert abs(ana.sum() / (n0 * v0) - 1) < 1e-3
+    big = ana > 0.02 * ana.sum()
+    assert big.sum() >= 5
+    assert np.abs(sim[big] / ana[big] - 1).max() < 0.2, (sim[big] / ana[big])
+    assert np.abs(sim - ana).sum() / ana.sum() < 0.1
+    # the mode of the mass spectrum moves to larger radii as in the closed form
+    assert np.argmax(hist[3600]) > np.argmax(hist[1200])
+
+
+# ----------------------------------------------------------------------------- thermodynamics
+def test_T_p_inversion_of_eq41():
+    """:1016-1018 eq. 41 theta = T (p_1000/p_d)^(R_d/c_pd), p_d = rho_d R_d T  <=>  eq. 43 (:1044)."""
+    for th, rhod in ((289.0, 1.2), (300.0, 0.9), (275.0, 1.05)):
+        T = L.orc_T(th, rhod)
+        pd = rhod * R_D * T
+        np.testing.assert_allclose(T * (P1000 / pd) ** (R_D / C_PD), th, rtol=1e-14)
+        np.testing.assert_allclose(L.orc_p(rhod, 0.01, T), rhod * (R_D + 0.01 * R_V) * T, rtol=1e-15)  # eq. 44
+
+
+def test_pvs_textbook_and_clausius_clapeyron(golden_dir):
+    for l in open(os.path.join(golden_dir, "textbook_values.txt")):
+        w = l.split()
+        if w and w[0] == "pvs":
+            np.testing.assert_allclose(L.orc_pvs(float(w[1])), float(w[2]), rtol=float(w[3]))
+    # d ln p_vs/dT = l_v/(R_v T^2) with l_v of Table 2 (:1087)
+    for T in (265.0, 280.0, 300.0):
+        h = 1e-3
+        d = (np.log(L.orc_pvs(T + h)) - np.log(L.orc_pvs(T - h))) / (2 * h)
+        lv = 2.5e6 + (1850.0 - 4218.0) * (T - 273.16)
+        np.testing.assert_allclose(L.orc_lv(T), lv, rtol=1e-15)
+        np.testing.assert_allclose(d, lv / (R_V * T * T), rtol=1e-7)
+
+
+def test_terminal_velocity_stokes_limit_and_textbook(golden_dir):
+    T, rhod = 293.15, 1.2
+    eta = L.orc_eta(T)
+    assert abs(eta / 1.81e-5 - 1) < 0.01  # air at 20 C
+    for r in (1e-8, 1e-7, 1e-6):
+        stokes = 2 * r * r * 9.81 * (RHO_W - rhod) / (9 * eta)
+        assert abs(L.orc_vterm(r, T, rhod, 0.0) / stokes - 1) < 3e-3
+    for l in open(os.path.join(golden_dir, "textbook_values.txt")):
+        w = l.split()
+        if w and w[0] == "vt":
+            np.testing.assert_allclose(L.orc_vterm(float(w[1]), T, rhod, 0.0), float(w[2]), rtol=float(w[3]))
+    v = [L.orc_vterm(r, T, rhod, 0.0) for r in np.geomspace(1e-9, 3e-3, 200)]
+    assert (np.diff(v) > 0).all()
+
+
+# ----------------------------------------------------------------------------- growth law
+TH, RHOD = 289.0, 1.1
+
+
+def _rv_for_RH(RH):
+    ct = oracle.cell_thermo(TH, 0.0, RHOD)
+    return RH * ct["rho_vs"] / RHOD
+
+
+def _S_eq(r, rd3, kappa):
+    """kappa-Koehler equilibrium saturation (eq. 22 with Table 2 :1056, :1074), written independently."""
+    T = L.orc_T(TH, RHOD)
+    A = 2 * SIGMA_W / (R_V * T * RHO_W)
+    return (r**3 - rd3) / (r**3 - rd3 * (1 - kappa)) * np.exp(A / r)
+
+
+def test_growth_rate_sign_changes_at_koehler_equilibrium():
+    rd3, kappa = (50e-9) ** 3, 0.61
+    for r in (60e-9, 0.2e-6, 1e-6, 10e-6):
+        S = _S_eq(r, rd3, kappa)
+        fp = L.orc_growth_f(r * r, rd3, kappa, TH, _rv_for_RH(S * (1 + 1e-6)), RHOD, 44.0, r * r)
+        fm = L.orc_growth_f(r * r, rd3, kappa, TH, _rv_for_RH(S * (1 - 1e-6)), RHOD, 44.0, r * r)
+        assert fp > 0 > fm
+
+
+def test_koehler_critical_point_closed_forms():
+    """r_c = sqrt(3 kappa r_d^3 / A), ln S_c = sqrt(4 A^3 / (27 kappa r_d^3)) (dilute limit)."""
+    T = L.orc_T(TH, RHOD)
+    A = 2 * SIGMA_W / (R_V * T * RHO_W)
+    for rd, kappa in ((30e-9, 0.61), (80e-9, 0.61), (50e-9, 1.2)):
+        rd3 = rd**3
+
+        def S_of_r(r):  # saturation at which the oracle's growth rate vanishes (f is linear in RH)
+            y = r * r
+            f1 = L.orc_growth_f(y, rd3, kappa, TH, _rv_for_RH(1.0), RHOD, 44.0, y)
+            f2 = L.orc_growth_f(y, rd3, kappa, TH, _rv_for_RH(1.01), RHOD, 44.0, y)
+            return 1.0 - f1 * 0.01 / (f2 - f1)
+
+        res = optimize.minimize_scalar(lambda lr: -S_of_r(np.exp(lr)), bounds=(np.log(1.5 * rd), np.log(100 * rd)), method="bounded",
+                                       options=dict(xatol=1e-10))
+        rc, Sc = np.exp(res.x), -res.fun
+        np.testing.assert_allclose(rc, np.sqrt(3 * kappa * rd3 / A), rtol=0.02)
+        np.testing.assert_allclose(np.log(Sc), np.sqrt(4 * A**3 / (27 * kappa * rd3)), rtol=0.02)
+
+
+def test_subsaturated_relaxation_reaches_koehler_root():
+    """at fixed RH < 1 without feedback the implicit scheme converges to RH = a_w exp(A/r)."""
+    for rd, RH in ((20e-9, 0.7), (60e-9, 0.9), (0.15e-6, 0.98)):
+        rd3, kappa = rd**3, 0.61
+        rv = _rv_for_RH(RH)
+        y = (3 * rd) ** 2
+        for _ in range(400):
+            y, _ill = oracle.cond_substep(y, rd3, kappa, TH, rv, RHOD, 44.0, 0.1)
+        np.testing.assert_allclose(_S_eq(np.sqrt(y), rd3, kappa), RH, rtol=1e-12)
+
+
+def test_large_drop_limit_is_linear_in_r2():
+    """for a big dilute drop a_w -> 1, exp(A/r) -> 1, beta -> 1: d r^2/dt constant, so the
+    implicit step (eq. 17) equals the explicit one."""
+    rd3, kappa, rv = (10e-9) ** 3, 0.61, _rv_for_RH(1.01)
+    y0 = (20e-6) ** 2
+    f0 = L.orc_growth_f(y0, rd3, kappa, TH, rv, RHOD, 44.0, y0)
+    y1, ill = oracle.cond_substep(y0, rd3, kappa, TH, rv, RHOD, 44.0, 0.1)
+    assert not ill and f0 > 0
+    assert abs((y1 - y0) / (0.1 * f0) - 1) < 2e-3
+    # Maxwell-Mason magnitude: r dr/dt = D_eff/rho_w * rho_vs * (S - 1), D_eff ~ O(1e-5) m^2/s
+    ct = oracle.cell_thermo(TH, rv, RHOD)
+    Deff = f0 * RHO_W / (2 * ct["rho_vs"] * (1.01 - _S_eq(20e-6, rd3, kappa)))
+    assert 0.5e-5 < Deff < 2.5e-5
+
+
+def test_implicit_equation_residual_and_bracket_rules():
+    """:568-579 eq. 17-19: the returned value solves y - y0 - dt' f(y) = 0 inside [a, b]; an ill-posed bracket
+    returns (a+b)/2 which is the explicit Euler step (:579)."""
+    rng = np.random.default_rng(5)
+    n_ill = n_ok = 0
+    for _ in range(3000):
+        rd = np.exp(rng.uniform(np.log(8e-9), np.log(0.5e-6)))
+        rd3, kappa = rd**3, 0.61
+        r0 = rd * np.exp(rng.uniform(np.log(1.02), np.log(40.0)))
+        RH = rng.choice([0.6, 0.95, 1.002, 1.05])
+        rv, dtp, y0 = _rv_for_RH(RH), 0.1, r0 * r0
+        f0 = L.orc_growth_f(y0, rd3, kappa, TH, rv, RHOD, 44.0, y0)
+        y1, ill = oracle.cond_substep(y0, rd3, kappa, TH, rv, RHOD, 44.0, dtp)
+        a = max(rd3 ** (2 / 3), y0 + min(2 * dtp * f0, 0))
+        b = y0 + max(2 * dtp * f0, 0)
+        assert a * (1 - 1e-15) <= y1 <= b * (1 + 1e-15)
+        if ill:
+            n_ill += 1
+            np.testing.assert_allclose(y1, 0.5 * (a + b), rtol=1e-15)
+            if a > rd3 ** (2 / 3) * (1 + 1e-12):
+                np.testing.assert_allclose(y1, y0 + dtp * f0, rtol=1e-14)  # Euler
+        else:
+            n_ok += 1
+            # g(y) = y - y0 - dt' f(y) changes sign within 2e-12 (relative) of the returned value; closer than
+            # that the rounding noise of RH - a_w exp(A/r) in f exceeds |g| (measured ~1e-13 y)
+            g = [y - y0 - dtp * L.orc_growth_f(y, rd3, kappa, TH, rv, RHOD, 44.0, y0) for y in (y1 * (1 - 2e-12), y1 * (1 + 2e-12))]
+            assert g[0] * g[1] <= 0.0
+    assert n_ok > 2000 and n_ill > 0
+
+
+def test_condensation_conserves_total_water_and_heats():
+    """:608-618 eq. 25-26: r_v + (4 pi rho_w/3) sum N r_w^3/(rho_d dV) is constant per cell to rounding."""
+    rng = np.random.default_rng(8)
+    nx, nz, N = 3, 4, 1500
+    o = oracle.Oracle(nx=nx, ny=0, nz=nz, dx=20.0, dy=1.0, dz=20.0, dt=1.0, seed=3)
+    ncell = nx * nz
+    th0 = np.full(ncell, 289.0)
+    rhod = np.linspace(1.15, 1.05, ncell)
+    rv0 = np.array([_rv_for_RH(s) for s in np.linspace(0.9, 1.04, ncell)]) * 1.1 / rhod
+    o.set_fields(th=th0, rv=rv0, rhod=rhod)
+    rd = np.exp(rng.uniform(np.log(10e-9), np.log(0.3e-6), N))
+    n = rng.integers(10**6, 10**9, N).astype(np.uint64)
+    x, z = rng.uniform(0, 60, N), rng.uniform(0, 80, N)
+    o.set_state(n, (2 * rd) ** 2, rd**3, np.full(N, 0.61), x=x, z=z)
+    cell = np.floor(x / 20).astype(int) * nz + np.floor(z / 20).astype(int)
+    dV = 20.0 * 1.0 * 20.0
+
+    def water(rv, st):
+        liq = np.bincount(cell, weights=st["n"].astype(float) * st["rw2"] ** 1.5, minlength=ncell)
+        return rv + 4 * np.pi * RHO_W / 3 * liq / (rhod * dV)
+
+    w0 = water(rv0, o.get_state())
+    op = oracle.make_opts(adve=False, sedi=False, cond=True, coal=False, RH_max=1.05, sstp_cond=10)
+    for _ in range(5):
+        o.step(op)
+    th1, rv1 = o.get_fields()
+    w1 = water(rv1, o.get_state())
+    np.testing.assert_allclose(w1, w0, rtol=2e-14)
+    assert np.abs(rv1 - rv0).max() > 1e-6  # something did condense / evaporate
+    # eq. 26: d theta = -theta l_v/(c_pd T) d r_v
+    T = np.array([L.orc_T(t, r) for t, r in zip(th0, rhod)])
+    lv = np.array([L.orc_lv(t) for t in T])
+    np.testing.assert_allclose((th1 - th0) / (rv1 - rv0), -th0 * lv / (C_PD * T), rtol=2e-3)
+    assert o.counters()["sd_substeps"] == 5 * 10 * N
+
+
+# ----------------------------------------------------------------------------- advection / sedimentation
+def test_advection_closed_form_solves_backward_euler():
+    """:536-556: eq. 16 is the solution of eq. 13-15."""
+    rng = np.random.default_rng(2)
+    for _ in range(200):
+        dx = rng.uniform(5, 50)
+        i = rng.integers(0, 70)
+        x = (i + rng.uniform(0, 1)) * dx
+        Clo, Chi = rng.uniform(-0.3, 0.3, 2)
+        xn = L.orc_adve_1d(x, dx, Clo, Chi)
+        omega = xn / dx - np.floor(x / dx)  # eq. 15
+        C = (1 - omega) * Clo + omega * Chi  # eq. 14
+        assert abs(xn - (x + dx * C)) < 1e-12 * dx * 70  # eq. 13
+        np.testing.assert_allclose(L.orc_adve_1d(x, dx, Clo, Clo), x + dx * Clo, rtol=1e-15)  # dC = 0
+    # a wall with C = 0 is never crossed
+    for x in (0.01, 5.0, 9.99):
+        assert L.orc_adve_1d(x, 10.0, 0.0, -0.5) >= 0.0
+        assert L.orc_adve_1d(x, 10.0, 0.5, 0.0) <= 10.0
+
+
+def test_move_stage_matches_eq16_per_dimension_and_sediments():
+    rng = np.random.default_rng(4)
+    nx, nz, N = 5, 4, 300
+    dx, dz, dt = 10.0, 20.0, 1.0
+    o = oracle.Oracle(nx=nx, ny=0, nz=nz, dx=dx, dy=1.0, dz=dz, dt=dt, seed=1)
+    rhod = rng.uniform(1.0, 1.2, nx * nz)
+    cx = rng.uniform(-0.2, 0.2, (nx + 1, nz))
+    cx[-1] = cx[0]
+    cz = rng.uniform(-0.1, 0.1, (nx, nz + 1))
+    cz[:, 0] = cz[:, -1] = 0
+    o.set_fields(th=np.full(nx * nz, 289.0), rv=np.full(nx * nz, 7e-3), rhod=rhod, cx=cx.ravel(), cz=cz.ravel())
+    x, z = rng.uniform(0, nx * dx, N), rng.uniform(0, nz * dz, N)
+    r = np.exp(rng.uniform(np.log(1e-6), np.log(1e-3), N))
+    z[:40] = rng.uniform(0, 3.0, 40)
+    r[:40] = 1e-3  # big drops near the ground will fall out
+    n = rng.integers(1, 10**6, N).astype(np.uint64)
+    o.set_state(n, r * r, np.full(N, 1e-24), np.full(N, 0.61), x=x, z=z)
+    op = oracle.make_opts(adve=True, sedi=True, cond=False, coal=False)
+    flux = o.step(op)
+    st = o.get_state()
+    i, k = np.floor(x / dx).astype(int), np.floor(z / dz).astype(int)
+    rd_ = rhod.reshape(nx, nz)[i, k]
+    xe = np.array([L.orc_adve_1d(a, dx, lo / q, hi / q) for a, lo, hi, q in zip(x, cx[i, k], cx[i + 1, k], rd_)])
+    ze = np.array([L.orc_adve_1d(a, dz, lo / q, hi / q) for a, lo, hi, q in zip(z, cz[i, k], cz[i, k + 1], rd_)])
+    T = L.orc_T(289.0, 1.0)
+    vt = np.array([L.orc_vterm(rr, L.orc_T(289.0, q), q, 7e-3) for rr, q in zip(r, rd_)])
+    ze = ze - vt * dt
+    xe = np.where(xe < 0, xe + nx * dx, xe)
+    xe = np.where(xe >= nx * dx, xe - nx * dx, xe)
+    np.testing.assert_allclose(st["x"], xe, rtol=1e-14)
+    np.testing.assert_allclose(st["z"], ze, rtol=1e-13, atol=1e-13)
+    out = ze < 0
+    assert out.sum() >= 30 and (st["n"][out] == 0).all() and (st["n"][~out] == n[~out]).all()
+    np.testing.assert_allclose(flux, (n[out] * 4 / 3 * np.pi * RHO_W * r[out] ** 3).sum(), rtol=1e-13)
+    # next step compacts the dead ones away, stably
+    o.step(oracle.make_opts(adve=False, sedi=False, cond=False, coal=False))
+    assert o.get_state()["id"].tolist() == np.nonzero(~out)[0].tolist()
+
+
+# ----------------------------------------------------------------------------- diagnostics / table / threads
+def test_moments_bruteforce():
+    """:818-823 eq. 29."""
+    rng = np.random.default_rng(6)
+    nx, ny, nz, N = 3, 2, 4, 2000
+    o = oracle.Oracle(nx=nx, ny=ny, nz=nz, dx=10.0, dy=5.0, dz=20.0, dt=1.0)
+    rhod = rng.uniform(1.0, 1.2, nx * ny * nz)
+    o.set_fields(rhod=rhod)
+    x, y, z = rng.uniform(0, 30, N), rng.uniform(0, 10, N), rng.uniform(0, 80, N)
+    rw, rd = np.exp(rng.uniform(np.log(1e-7), np.log(1e-4), N)), np.exp(rng.uniform(np.log(1e-9), np.log(1e-6), N))
+    n = rng.integers(0, 1000, N).astype(np.uint64)
+    o.set_state(n, rw**2, rd**3, np.full(N, 0.61), x=x, y=y, z=z)
+    cell = (np.floor(x / 10).astype(int) * ny + np.floor(y / 5).astype(int)) * nz + np.floor(z / 20).astype(int)
+    dV = 10.0 * 5.0 * 20.0
+    for wet, r in ((1, rw), (0, rd)):
+        for k in (0, 1, 3):
+            lo, hi = np.quantile(r, [0.2, 0.7])
+            m = (r >= lo) & (r < hi)
+            ref = np.zeros(nx * ny * nz)
+            for s in np.nonzero(m)[0]:
+                ref[cell[s]] += float(n[s]) * r[s] ** k
+            np.testing.assert_allclose(o.diag_mom(wet, lo, hi, k), ref / (rhod * dV), rtol=1e-13)
+    np.testing.assert_array_equal(o.diag_sd_conc(), np.bincount(cell[n > 0], minlength=nx * ny * nz))
+
+
+def test_efficiency_table_bilinear_and_clamped():
+    R = np.array([10e-6, 20e-6, 40e-6])
+    q = np.array([0.0, 0.5, 1.0])
+    tab = np.array([[0.0, 0.1, 0.2], [0.3, 0.5, 0.7], [1.0, 1.0, 0.9]])
+    o = oracle.Oracle(dx=1, dy=1, dz=1, kernel="hydro_tab", eff_R=R, eff_q=q, eff_tab=tab)
+    for a in range(3):
+        for c in range(3):
+            assert abs(o.eff(R[a], q[c]) - tab[a, c]) < 1e-15
+    np.testing.assert_allclose(o.eff(15e-6, 0.25), tab[:2, :2].mean(), rtol=1e-14)
+    np.testing.assert_allclose(o.eff(30e-6, 0.5), 0.75, rtol=1e-14)
+    assert o.eff(1e-6, 0.5) == o.eff(10e-6, 0.5) and o.eff(1e-3, 2.0) == tab[2, 2]
+
+
+def test_openmp_over_cells_is_bitwise_identical_to_serial():
+    rng = np.random.default_rng(21)
+    nx, nz, N = 6, 6, 3000
+    res = []
+    for threads in (1, 4):
+        o = oracle.Oracle(nx=nx, ny=0, nz=nz, dx=20.0, dy=1.0, dz=20.0, dt=1.0, seed=9)
+        o.set_threads(threads)
+        rr = np.random.default_rng(21)
+        rd = np.exp(rr.uniform(np.log(10e-9), np.log(0.3e-6), N))
+        o.set_fields(th=np.full(36, 289.0), rv=np.full(36, 9e-3), rhod=np.full(36, 1.1))
+        o.set_state(rr.integers(10**6, 10**9, N).astype(np.uint64), (30 * rd) ** 2, rd**3, np.full(N, 0.61),
+                    x=rr.uniform(0, 120, N), z=rr.uniform(0, 120, N))
+        op = oracle.make_opts(RH_max=1.05)
+        for _ in range(3):
+            o.step(op)
+        res.append((o.get_state(), o.get_fields()))
+    for k in res[0][0]:
+        np.testing.assert_array_equal(res[0][0][k], res[1][0][k])
+    np.testing.assert_array_equal(res[0][1][0], res[1][1][0])

@@ -1,0 +1,168 @@
+/* sdm.h -- C ABI of libsdm: the super-droplet (particle-based) warm-rain step of
+ * arxiv 1310.1905 (libcloudph++ 0.2, section 5) on one NVIDIA B200.
+ *
+ * The interface follows the paper's programming interface (PAPER.md :667-835,
+ * Listings 5.1-5.7): options fixed at creation (opts_init_t), per-step options
+ * (opts_t), array descriptors (arrinfo_t), a factory, step_sync / step_async
+ * and the diag_* / outbuf methods.  C has no templates, so real_t is the
+ * `real_bytes` field and backend_t is gone (CUDA only).
+ *
+ * Conventions
+ *  - Every function returns SDM_OK (0) or a negative sdm_status; the message is
+ *    available from sdm_last_error().  No exception crosses the boundary.
+ *  - "DEVICE pointer" = memory of the CUDA device the context was created on,
+ *    owned by the caller unless stated otherwise.  "HOST pointer" = ordinary
+ *    host memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy
+ *    default stream).  Work is enqueued on that stream; functions documented
+ *    as "blocking" synchronise with it.
+ *  - All floating-point arrays are IEEE double (real_bytes == 8).
+ *  - There is no CPU fallback: sdm_create fails with SDM_ERR_NO_DEVICE when no
+ *    sm_100 device is usable (PAPER.md :827 "does report an error").
+ */
+#ifndef SDM_H_
+#define SDM_H_
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sdm_ctx sdm_ctx;
+
+typedef enum {
+  SDM_OK = 0,
+  SDM_ERR_INVALID = -1,     /* bad argument (NULL, size, stride, option) */
+  SDM_ERR_NO_DEVICE = -2,   /* no usable sm_100 CUDA device */
+  SDM_ERR_CUDA = -3,        /* a CUDA runtime call or kernel failed */
+  SDM_ERR_CAPACITY = -4,    /* more super-droplets than max_sd, or a cell holds more SDs than a CTA can sort */
+  SDM_ERR_ORDER = -5        /* calls out of order (e.g. step_async without step_sync) */
+} sdm_status;
+
+/* PAPER.md Listing 5.3 (:722-726) has only `geometric`; BASELINE.json north_star adds the other two. */
+typedef enum {
+  SDM_KERNEL_GEOMETRIC = 0, /* eq. 28 with E = 1 */
+  SDM_KERNEL_GOLOVIN = 1,   /* K = b (v_i + v_j) */
+  SDM_KERNEL_HYDRO_TAB = 2  /* eq. 28 with E(r_large, r_small/r_large) bilinear from a table */
+} sdm_kernel;
+
+/* PAPER.md Listing 5.2 (:699-720) lgrngn::opts_init_t.  Copied by sdm_create. */
+typedef struct {
+  int nx, ny, nz;           /* Eulerian grid; 0 = dimension absent (:751: 0..3 Courant components) */
+  double dx, dy, dz, dt;    /* grid steps [m] and time step [s]; an absent dimension still
+                               contributes its d? to the cell volume dV = dx dy dz (2D: dy = 1 m; box: V) */
+  double x0, y0, z0, x1, y1, z1; /* Lagrangian sub-domain (:713); used by initialisation only */
+  double sd_conc_mean;      /* mean number of SDs per cell (:715); a sizing hint here */
+  int kernel;               /* sdm_kernel */
+  double golovin_b;         /* [1/s] for SDM_KERNEL_GOLOVIN */
+  int n_eff_R, n_eff_q;     /* collision-efficiency table shape (HYDRO_TAB) */
+  const double* eff_R;      /* HOST, n_eff_R collector radii [m], ascending */
+  const double* eff_q;      /* HOST, n_eff_q radius ratios small/large, ascending */
+  const double* eff_tab;    /* HOST, row-major [n_eff_R][n_eff_q] */
+  uint64_t seed;            /* Philox-4x32-10 key (low word, high word) */
+  int real_bytes;           /* 8 */
+  int multi_coal;           /* 1: gamma = floor(p) + [u < frac(p)] (north_star); 0: gamma = [u < p] (PAPER.md :645) */
+  uint64_t max_sd;          /* capacity in super-droplets (HBM is allocated once, at creation) */
+} sdm_opts_init;
+
+/* PAPER.md Listing 5.1 (:677-689) lgrngn::opts_t */
+typedef struct {
+  int adve, sedi, cond, coal; /* process toggles */
+  double RH_max;              /* RH limit for drop growth (:685) */
+  int sstp_cond, sstp_coal;   /* numbers of substeps (:688) */
+} sdm_opts;
+
+/* PAPER.md Listing 5.4 (:730-745) lgrngn::arrinfo_t: element (i,j,k) of the field lives at
+ * data_zero[i*strides[0] + j*strides[1] + k*strides[2]] (strides in elements, one per PRESENT
+ * dimension in x,y,z order; unused entries ignored).  data_zero == NULL means "argument omitted". */
+typedef struct {
+  double* data_zero;        /* DEVICE pointer to element (0,0,0) */
+  int64_t strides[3];
+} sdm_arrinfo;
+
+typedef struct {
+  uint64_t n_sd;            /* super-droplets in storage (live ones after the last step_sync) */
+  uint64_t max_cell_count;  /* largest number of SDs in one cell at the last step_sync */
+  uint64_t step;            /* completed steps */
+  uint64_t kernel_launches; /* CUDA kernels launched by this context since creation */
+  uint64_t pairs, collisions, near_ties; /* coalescence: candidate pairs, pairs with gamma > 0,
+                                            pairs with |u - frac(p)| < 1e-12 (summed since creation) */
+  uint64_t ill_posed;       /* condensation: SD-substeps that took the bracket branch of PAPER.md :579 */
+  uint64_t newton_iters;    /* condensation: growth-rate evaluations (summed) */
+  uint64_t sd_substeps;     /* condensation: SD-substeps solved */
+} sdm_stats_t;
+
+/* factory() of Listing 5.7 (:800-808).  Allocates all device memory for max_sd super-droplets on
+ * the current CUDA device.  Blocking. */
+int sdm_create(const sdm_opts_init* opts, sdm_ctx** out);
+void sdm_destroy(sdm_ctx* ctx);
+/* message of the last failed call on ctx (ctx == NULL: of the last failed sdm_create); library-owned */
+const char* sdm_last_error(const sdm_ctx* ctx);
+
+/* Load a particle population (parity tests, the box set-up, checkpoint restart) instead of the
+ * paper's init() (:759-766).  rhod and the Courant components (rho_d times Courant number on the
+ * Arakawa-C grid, shapes (nx+1) x ny x nz, nx x (ny+1) x nz, nx x ny x (nz+1); in 2D the second
+ * component is the vertical one and the third is omitted, :751) are copied into library-owned dense
+ * arrays.  n (multiplicity, uint64), rw2 (wet radius squared), rd3 (dry radius cubed), kappa, x, y,
+ * z, id (unique uint32) are DEVICE arrays of N elements, copied; coordinates of absent dimensions
+ * may be NULL.  Positions must lie inside the domain.  Blocking. */
+int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo rhod_courant_1,
+                         sdm_arrinfo rhod_courant_2, sdm_arrinfo rhod_courant_3, uint64_t N,
+                         const uint64_t* n, const double* rw2, const double* rd3, const double* kappa,
+                         const double* x, const double* y, const double* z, const uint32_t* id, void* stream);
+
+/* step_sync() of Listing 5.5 (:768-775, :816): the part of a step that alters the Eulerian fields.
+ * Removes N = 0 SDs, sorts the SDs by (cell, Philox key, id), and if opts->cond integrates
+ * opts->sstp_cond condensation substeps (eq. 17-26).  th and rv are read and OVERWRITTEN (final when
+ * the work enqueued on `stream` completes).  Courant components and rhod may be omitted
+ * (data_zero == NULL) when unchanged since initialisation (:816).  Blocks the host only until the
+ * sort histogram is known (it sizes the cell-resident launches). */
+int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* opts, sdm_arrinfo th, sdm_arrinfo rv,
+                  sdm_arrinfo rhod_courant_1, sdm_arrinfo rhod_courant_2, sdm_arrinfo rhod_courant_3,
+                  sdm_arrinfo rhod, void* stream);
+
+/* step_async() of Listing 5.5 (:776-777, :816): coalescence (eq. 27-28), advection (eq. 16) and
+ * sedimentation; only enqueues.  Must follow a step_sync of the same step. */
+int sdm_step_async(sdm_ctx* ctx, const sdm_opts* opts, void* stream);
+/* Waits for the last step_async and returns its rain flux through the bottom of the domain
+ * (:816), as the mass of water that left during that step [kg]. */
+int sdm_step_async_result(sdm_ctx* ctx, double* rain_flux);
+
+/* The same step for a caller whose Eulerian fields live in HOST memory (the paper's CPU solver,
+ * :845-848): copies th, rv (dense C order, nx*ny*nz doubles, pinned or pageable) to the device,
+ * runs step_sync, copies them back, runs step_async.  Blocking; *rain_flux as above. */
+int sdm_step_host(sdm_ctx* ctx, const sdm_opts* opts, double* th_host, double* rv_host,
+                  double* rain_flux, void* stream);
+
+/* diag_* of Listing 5.5 (:779-788, :818-823).  *_rng selects r in [r_mi, r_mx) for the following
+ * *_mom calls; *_mom(k) computes eq. 29 per cell into the output buffer; sd_conc counts SDs per
+ * cell.  Cells are those of the SDs' current positions.  Enqueue on `stream`. */
+int sdm_diag_sd_conc(sdm_ctx* ctx, void* stream);
+int sdm_diag_dry_rng(sdm_ctx* ctx, double r_mi, double r_mx);
+int sdm_diag_wet_rng(sdm_ctx* ctx, double r_mi, double r_mx);
+int sdm_diag_dry_mom(sdm_ctx* ctx, int k, void* stream);
+int sdm_diag_wet_mom(sdm_ctx* ctx, int k, void* stream);
+/* outbuf() (:788, :823): DEVICE pointer to nx*ny*nz doubles in dense C order, library-owned, valid
+ * until the next diag_* call; contents are final when the stream work of that diag call completes. */
+const double* sdm_outbuf(sdm_ctx* ctx);
+
+/* Parity / checkpoint access.  sdm_n_sd: number of SDs in storage (blocking).  sdm_export_state:
+ * copies the SoA state in storage order into DEVICE arrays of at least sdm_n_sd elements (NULL =
+ * skip that attribute); SDs whose multiplicity reached 0 during the last step are still present
+ * until the next step_sync.  sdm_export_order: after step_sync, the ids in sorted (cell, key, id)
+ * order and the nx*ny*nz+1 segment offsets (DEVICE arrays).  All enqueue on `stream`. */
+int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd);
+int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double* kappa,
+                     double* x, double* y, double* z, uint32_t* id, void* stream);
+int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, void* stream);
+/* Counters (blocking: synchronises the context's last stream). */
+int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out);
+/* Overrides the step counter used in the Philox counters (restart from a checkpoint, parity). */
+int sdm_set_step(sdm_ctx* ctx, uint64_t step);
+/* Tuning override for tests: threads cooperating on one cell in the cell-resident kernels
+ * (0 = automatic; 4, 8, 16, 32 = sub-warp groups; 256 = one CTA per cell). */
+int sdm_set_group_size(sdm_ctx* ctx, int group);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDM_H_ */

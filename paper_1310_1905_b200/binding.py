@@ -1,0 +1,247 @@
+"""Thin Python binding of libsdm (include/sdm.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+and streams.  Method names follow the C ABI / the paper's ``particles_t`` (Listing 5.5,
+:755-790).  There is no CPU fallback: importing works anywhere, but creating ``Particles`` raises
+unless ``libsdm.so`` is built and an sm_100 GPU is present.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libsdm.so")
+
+KERNELS = {"geometric": 0, "golovin": 1, "hydro_tab": 2}
+
+
+class SdmError(RuntimeError):
+    pass
+
+
+class OptsInit(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double), ("dt", C.c_double),
+                ("x0", C.c_double), ("y0", C.c_double), ("z0", C.c_double),
+                ("x1", C.c_double), ("y1", C.c_double), ("z1", C.c_double),
+                ("sd_conc_mean", C.c_double), ("kernel", C.c_int), ("golovin_b", C.c_double),
+                ("n_eff_R", C.c_int), ("n_eff_q", C.c_int),
+                ("eff_R", C.c_void_p), ("eff_q", C.c_void_p), ("eff_tab", C.c_void_p),
+                ("seed", C.c_uint64), ("real_bytes", C.c_int), ("multi_coal", C.c_int), ("max_sd", C.c_uint64)]
+
+
+class Opts(C.Structure):
+    _fields_ = [("adve", C.c_int), ("sedi", C.c_int), ("cond", C.c_int), ("coal", C.c_int),
+                ("RH_max", C.c_double), ("sstp_cond", C.c_int), ("sstp_coal", C.c_int)]
+
+
+class ArrInfo(C.Structure):
+    _fields_ = [("data_zero", C.c_void_p), ("strides", C.c_int64 * 3)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(k, C.c_uint64) for k in ("n_sd", "max_cell_count", "step", "kernel_launches", "pairs", "collisions",
+                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps")]
+
+
+EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
+           "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
+           "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size"]
+
+_lib = None
+
+
+def load_library():
+    """dlopen libsdm.so (built in-tree by paper_1310_1905_b200/build.py) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise SdmError(f"{_SO} is missing: build it with `python -m paper_1310_1905_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(_SO)
+    vp, u64p = C.c_void_p, C.POINTER(C.c_uint64)
+    L.sdm_create.argtypes = [C.POINTER(OptsInit), C.POINTER(vp)]
+    L.sdm_destroy.argtypes = [vp]
+    L.sdm_destroy.restype = None
+    L.sdm_last_error.argtypes = [vp]
+    L.sdm_last_error.restype = C.c_char_p
+    L.sdm_init_from_arrays.argtypes = [vp, ArrInfo, ArrInfo, ArrInfo, ArrInfo, C.c_uint64] + [vp] * 8 + [vp]
+    L.sdm_step_sync.argtypes = [vp, C.POINTER(Opts)] + [ArrInfo] * 6 + [vp]
+    L.sdm_step_async.argtypes = [vp, C.POINTER(Opts), vp]
+    L.sdm_step_async_result.argtypes = [vp, C.POINTER(C.c_double)]
+    L.sdm_step_host.argtypes = [vp, C.POINTER(Opts), vp, vp, C.POINTER(C.c_double), vp]
+    L.sdm_diag_sd_conc.argtypes = [vp, vp]
+    L.sdm_diag_dry_rng.argtypes = [vp, C.c_double, C.c_double]
+    L.sdm_diag_wet_rng.argtypes = [vp, C.c_double, C.c_double]
+    L.sdm_diag_dry_mom.argtypes = [vp, C.c_int, vp]
+    L.sdm_diag_wet_mom.argtypes = [vp, C.c_int, vp]
+    L.sdm_outbuf.argtypes = [vp]
+    L.sdm_outbuf.restype = vp
+    L.sdm_n_sd.argtypes = [vp, u64p]
+    L.sdm_export_state.argtypes = [vp] + [vp] * 8 + [vp]
+    L.sdm_export_order.argtypes = [vp, vp, vp, vp]
+    L.sdm_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.sdm_set_step.argtypes = [vp, C.c_uint64]
+    L.sdm_set_group_size.argtypes = [vp, C.c_int]
+    _lib = L
+    return L
+
+
+def make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=44.0, sstp_cond=10, sstp_coal=1):
+    return Opts(int(adve), int(sedi), int(cond), int(coal), float(RH_max), int(sstp_cond), int(sstp_coal))
+
+
+def arrinfo(t):
+    """arrinfo_t of a torch CUDA tensor (None -> omitted argument); strides in elements."""
+    a = ArrInfo()
+    if t is None:
+        a.data_zero = None
+        return a
+    assert t.is_cuda and t.dtype == torch.float64
+    a.data_zero = t.data_ptr()
+    for k, s in enumerate(t.stride()):
+        a.strides[k] = s
+    return a
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Particles:
+    """One ``particles_t`` (PAPER.md :747-790) living on the current CUDA device."""
+
+    def __init__(self, nx=0, ny=0, nz=0, dx=1.0, dy=1.0, dz=1.0, dt=1.0, kernel="geometric", golovin_b=1500.0,
+                 multi_coal=True, seed=42, eff_R=None, eff_q=None, eff_tab=None, max_sd=None, sd_conc_mean=0.0):
+        import numpy as np
+        self.L = load_library()
+        keep = [None if a is None else np.ascontiguousarray(a, dtype=np.float64) for a in (eff_R, eff_q, eff_tab)]
+        o = OptsInit()
+        o.nx, o.ny, o.nz, o.dx, o.dy, o.dz, o.dt = nx, ny, nz, dx, dy, dz, dt
+        o.x1, o.y1, o.z1 = dx * max(nx, 1), dy * max(ny, 1), dz * max(nz, 1)
+        o.sd_conc_mean, o.kernel, o.golovin_b = sd_conc_mean, KERNELS[kernel], golovin_b
+        if keep[0] is not None:
+            o.n_eff_R, o.n_eff_q = len(keep[0]), len(keep[1])
+            o.eff_R, o.eff_q, o.eff_tab = (k.ctypes.data for k in keep)
+        o.seed, o.real_bytes, o.multi_coal, o.max_sd = seed, 8, int(multi_coal), int(max_sd)
+        self.h = C.c_void_p()
+        rc = self.L.sdm_create(C.byref(o), C.byref(self.h))
+        if rc != 0:
+            raise SdmError(f"sdm_create failed ({rc}): {self.L.sdm_last_error(None).decode()}")
+        self.shape = tuple(n for n in (nx, ny, nz) if n > 0) or (1,)
+        self.ncell = max(nx, 1) * max(ny, 1) * max(nz, 1)
+        self.dims = (nx > 0, ny > 0, nz > 0)
+
+    def __del__(self):
+        try:
+            if self.h:
+                self.L.sdm_destroy(self.h)
+                self.h = None
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        if rc != 0:
+            raise SdmError(f"libsdm error {rc}: {self.L.sdm_last_error(self.h).decode()}")
+
+    def init_from_arrays(self, rhod, n, rw2, rd3, kappa, x=None, y=None, z=None, id=None, courant_1=None, courant_2=None,
+                         courant_3=None):
+        N = n.numel()
+        if id is None:
+            id = torch.arange(N, dtype=torch.int32, device=n.device)
+        self._ck(self.L.sdm_init_from_arrays(self.h, arrinfo(rhod), arrinfo(courant_1), arrinfo(courant_2), arrinfo(courant_3),
+                                             N, _ptr(n), _ptr(rw2), _ptr(rd3), _ptr(kappa), _ptr(x), _ptr(y), _ptr(z), _ptr(id),
+                                             _stream()))
+
+    def step_sync(self, opts, th, rv, courant_1=None, courant_2=None, courant_3=None, rhod=None):
+        self._ck(self.L.sdm_step_sync(self.h, C.byref(opts), arrinfo(th), arrinfo(rv), arrinfo(courant_1), arrinfo(courant_2),
+                                      arrinfo(courant_3), arrinfo(rhod), _stream()))
+
+    def step_async(self, opts):
+        self._ck(self.L.sdm_step_async(self.h, C.byref(opts), _stream()))
+
+    def step_async_result(self):
+        f = C.c_double()
+        self._ck(self.L.sdm_step_async_result(self.h, C.byref(f)))
+        return f.value
+
+    def step_host(self, opts, th_host, rv_host):
+        """th_host, rv_host: CPU float64 tensors (dense C order), overwritten."""
+        f = C.c_double()
+        self._ck(self.L.sdm_step_host(self.h, C.byref(opts), th_host.data_ptr(), rv_host.data_ptr(), C.byref(f), _stream()))
+        return f.value
+
+    def _out(self):
+        """Copy of the library-owned output buffer (PAPER.md :788 outbuf), shaped like the grid."""
+        src = _as_tensor(self.L.sdm_outbuf(self.h), self.ncell)
+        return src.clone().reshape(self.shape)
+
+    def diag_sd_conc(self):
+        self._ck(self.L.sdm_diag_sd_conc(self.h, _stream()))
+        return self._out()
+
+    def diag_dry_rng(self, r_mi, r_mx):
+        self._ck(self.L.sdm_diag_dry_rng(self.h, r_mi, r_mx))
+
+    def diag_wet_rng(self, r_mi, r_mx):
+        self._ck(self.L.sdm_diag_wet_rng(self.h, r_mi, r_mx))
+
+    def diag_dry_mom(self, k):
+        self._ck(self.L.sdm_diag_dry_mom(self.h, k, _stream()))
+        return self._out()
+
+    def diag_wet_mom(self, k):
+        self._ck(self.L.sdm_diag_wet_mom(self.h, k, _stream()))
+        return self._out()
+
+    def n_sd(self):
+        v = C.c_uint64()
+        self._ck(self.L.sdm_n_sd(self.h, C.byref(v)))
+        return v.value
+
+    def export_state(self):
+        N = self.n_sd()
+        dev = "cuda"
+        out = dict(n=torch.empty(N, dtype=torch.int64, device=dev), id=torch.empty(N, dtype=torch.int32, device=dev))
+        for k in ("rw2", "rd3", "kappa", "x", "y", "z"):
+            out[k] = torch.zeros(N, dtype=torch.float64, device=dev)
+        self._ck(self.L.sdm_export_state(self.h, *[_ptr(out[k]) for k in ("n", "rw2", "rd3", "kappa", "x", "y", "z", "id")],
+                                         _stream()))
+        torch.cuda.current_stream().synchronize()
+        return out
+
+    def export_order(self):
+        N = self.n_sd()
+        ids = torch.empty(N, dtype=torch.int32, device="cuda")
+        seg = torch.empty(self.ncell + 1, dtype=torch.int32, device="cuda")
+        self._ck(self.L.sdm_export_order(self.h, _ptr(ids), _ptr(seg), _stream()))
+        torch.cuda.current_stream().synchronize()
+        return ids, seg
+
+    def stats(self):
+        s = Stats()
+        self._ck(self.L.sdm_stats(self.h, C.byref(s)))
+        return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def set_step(self, step):
+        self._ck(self.L.sdm_set_step(self.h, step))
+
+    def set_group_size(self, g):
+        self._ck(self.L.sdm_set_group_size(self.h, g))
+
+
+def _as_tensor(ptr, n):
+    """Wrap a raw device pointer of n doubles as a torch tensor (no copy) via __cuda_array_interface__."""
+
+    class _Wrap:
+        pass
+
+    w = _Wrap()
+    w.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+    return torch.as_tensor(w, device="cuda")

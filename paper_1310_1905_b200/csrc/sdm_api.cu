@@ -1,0 +1,474 @@
+// C ABI of libsdm (include/sdm.h): context, memory, launch sizing.  All arithmetic of the step runs in
+// the kernels of sdm_sort.cu, sdm_cond.cu, sdm_coal_move.cu and sdm_diag.cu; there is no CPU path.
+#include "../../include/sdm.h"
+#include "sdm_kernels.cuh"
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace sdm;
+
+namespace {
+thread_local std::string g_create_error;
+constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are willing to ask for per CTA
+}
+
+struct sdm_ctx {
+  sdm_opts_init o{};
+  Grid g{};
+  int device = 0;
+  u64 cap_sd = 0;
+  SdArrays buf[2]{};
+  int cur = 0;
+  u32 *cell = nullptr, *off = nullptr, *count = nullptr, *blocksum = nullptr, *seg = nullptr;
+  u16* rank = nullptr;
+  u32* d_info = nullptr;     // [0],[1] slot counts (ping-pong), [2] max cell count, [3] error flag
+  u32* h_info = nullptr;     // pinned mirror
+  int cn = 0;                // which of d_info[0..1] is current
+  CellFields cf{};
+  double *cx = nullptr, *cy = nullptr, *cz = nullptr;
+  double* outbuf = nullptr;
+  double* flux_slots = nullptr;
+  double* d_flux = nullptr;  // [0] last step, [1] total
+  unsigned long long* cnt_mem = nullptr;
+  Counters cnt{};
+  CoalParams kp{};
+  double *d_effR = nullptr, *d_effq = nullptr, *d_efftab = nullptr;
+  double *th_dense = nullptr, *rv_dense = nullptr;   // for sdm_step_host
+  u64 nslots = 0;            // host-known number of slots in use
+  u64 max_nc = 0;
+  u64 step = 0;
+  bool synced = false;       // step_sync of the current step done
+  bool have_order = false;
+  int G = 32;                // group size chosen by the last step_sync
+  int group_override = 0;
+  cudaEvent_t ev_info = nullptr, ev_async = nullptr;
+  cudaStream_t last_stream = nullptr;
+  u64 launches = 0;
+  double dry_lo = 0, dry_hi = 1e300, wet_lo = 0, wet_hi = 1e300;
+  std::string err;
+};
+
+namespace {
+
+int fail(sdm_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e__ = (call);                                                                      \
+    if (e__ != cudaSuccess)                                                                        \
+      return fail(ctx, SDM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__));         \
+  } while (0)
+
+template <typename T>
+cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, std::max<size_t>(n, 1) * sizeof(T)); }
+
+Field make_field(const sdm_ctx* c, const sdm_arrinfo& a) {
+  Field f{a.data_zero, 0, 0, 0};
+  int idx = 0;
+  if (c->g.hx) f.s0 = a.strides[idx++];
+  if (c->g.hy) f.s1 = a.strides[idx++];
+  if (c->g.hz) f.s2 = a.strides[idx++];
+  return f;
+}
+
+// Courant component q (0-based among the PRESENT dimensions, PAPER.md :751) -> dense library copy
+int copy_courants(sdm_ctx* ctx, const sdm_arrinfo* comps, cudaStream_t st) {
+  const Grid& g = ctx->g;
+  int q = 0;
+  for (int dim = 0; dim < 3; ++dim) {
+    const bool present = dim == 0 ? g.hx : dim == 1 ? g.hy : g.hz;
+    if (!present) continue;
+    const sdm_arrinfo& a = comps[q++];
+    if (!a.data_zero) continue;
+    double* dst = dim == 0 ? ctx->cx : dim == 1 ? ctx->cy : ctx->cz;
+    launch_dense_copy(make_field(ctx, a), dst, g.NX + (dim == 0), g.NY + (dim == 1), g.NZ + (dim == 2), st);
+    ctx->launches++;
+  }
+  CK(cudaGetLastError());
+  return SDM_OK;
+}
+
+int pick_group(const sdm_ctx* c, double mean) {
+  if (c->group_override) return c->group_override;
+  if (mean < 12.0) return 4;
+  if (mean < 28.0) return 8;
+  if (mean < 80.0) return 16;
+  if (mean < 400.0) return 32;
+  return 256;
+}
+int ng_of(int G) { return (G <= 32 ? 128 : G) / G; }
+
+}  // namespace
+
+extern "C" {
+
+const char* sdm_last_error(const sdm_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
+  sdm_ctx* ctx = nullptr;
+  if (!o || !out) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: NULL argument");
+  *out = nullptr;
+  if (o->real_bytes != 8) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: real_bytes must be 8 (fp64 state)");
+  if (o->nx < 0 || o->ny < 0 || o->nz < 0 || !(o->dx > 0) || !(o->dy > 0) || !(o->dz > 0) || !(o->dt > 0))
+    return fail(nullptr, SDM_ERR_INVALID, "sdm_create: grid sizes must be >= 0 and dx, dy, dz, dt > 0");
+  if (o->kernel < 0 || o->kernel > 2) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: unknown kernel");
+  if (o->kernel == SDM_KERNEL_HYDRO_TAB && (o->n_eff_R < 2 || o->n_eff_q < 2 || !o->eff_R || !o->eff_q || !o->eff_tab))
+    return fail(nullptr, SDM_ERR_INVALID, "sdm_create: hydro_tab kernel needs an efficiency table of at least 2 x 2");
+  if (o->max_sd == 0 || o->max_sd >= 0xFFFFFFF0ull)
+    return fail(nullptr, SDM_ERR_INVALID, "sdm_create: max_sd must be in [1, 2^32 - 16)");
+  const long long ncell = (long long)std::max(o->nx, 1) * std::max(o->ny, 1) * std::max(o->nz, 1);
+  if (ncell >= (1ll << 31) - 8) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: too many cells");
+  int ndev = 0, dev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, SDM_ERR_NO_DEVICE, "sdm_create: no CUDA device (libsdm has no CPU fallback)");
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+    return fail(nullptr, SDM_ERR_NO_DEVICE, "sdm_create: cannot query the current CUDA device");
+  if (prop.major != 10)
+    return fail(nullptr, SDM_ERR_NO_DEVICE, std::string("sdm_create: device '") + prop.name + "' is not sm_100 (B200)");
+
+  ctx = new sdm_ctx();
+  ctx->o = *o;
+  ctx->device = dev;
+  Grid& g = ctx->g;
+  g.NX = std::max(o->nx, 1); g.NY = std::max(o->ny, 1); g.NZ = std::max(o->nz, 1);
+  g.hx = o->nx > 0; g.hy = o->ny > 0; g.hz = o->nz > 0;
+  g.ncell = (int)ncell;
+  g.dx = o->dx; g.dy = o->dy; g.dz = o->dz; g.dt = o->dt;
+  g.dV = o->dx * o->dy * o->dz;
+  g.X = o->dx * g.NX; g.Y = o->dy * g.NY; g.Z = o->dz * g.NZ;
+  ctx->cap_sd = o->max_sd;
+  const size_t N = (size_t)o->max_sd;
+  auto bail = [&](cudaError_t e, const char* what) {
+    std::string m = std::string("sdm_create: ") + what + ": " + cudaGetErrorString(e);
+    sdm_destroy(ctx);
+    return fail(nullptr, SDM_ERR_CUDA, m);
+  };
+  cudaError_t e;
+  for (int b = 0; b < 2; ++b) {
+    SdArrays& a = ctx->buf[b];
+    if ((e = dalloc(&a.n, N)) || (e = dalloc(&a.rw2, N)) || (e = dalloc(&a.rd3, N)) || (e = dalloc(&a.kappa, N)) ||
+        (e = dalloc(&a.x, g.hx ? N : 1)) || (e = dalloc(&a.y, g.hy ? N : 1)) || (e = dalloc(&a.z, g.hz ? N : 1)) ||
+        (e = dalloc(&a.id, N)))
+      return bail(e, "particle state");
+  }
+  const int nb = scan_num_blocks(g.ncell);
+  if ((e = dalloc(&ctx->cell, N)) || (e = dalloc(&ctx->off, N)) || (e = dalloc(&ctx->rank, N)) ||
+      (e = dalloc(&ctx->count, (size_t)g.ncell)) || (e = dalloc(&ctx->blocksum, (size_t)nb)) ||
+      (e = dalloc(&ctx->seg, (size_t)g.ncell + 1)) || (e = dalloc(&ctx->d_info, 4)) ||
+      (e = dalloc(&ctx->cf.rhod, (size_t)g.ncell)) || (e = dalloc(&ctx->cf.eta, (size_t)g.ncell)) ||
+      (e = dalloc(&ctx->cf.rho_a, (size_t)g.ncell)) || (e = dalloc(&ctx->outbuf, (size_t)g.ncell)) ||
+      (e = dalloc(&ctx->th_dense, (size_t)g.ncell)) || (e = dalloc(&ctx->rv_dense, (size_t)g.ncell)) ||
+      (e = dalloc(&ctx->cx, (size_t)(g.NX + 1) * g.NY * g.NZ)) || (e = dalloc(&ctx->cy, (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
+      (e = dalloc(&ctx->cz, (size_t)g.NX * g.NY * (g.NZ + 1))) || (e = dalloc(&ctx->flux_slots, NSLOT)) ||
+      (e = dalloc(&ctx->d_flux, 2)) || (e = dalloc(&ctx->cnt_mem, 6 * NSLOT)))
+    return bail(e, "scratch");
+  ctx->cf.cx = ctx->cx; ctx->cf.cy = ctx->cy; ctx->cf.cz = ctx->cz;
+  if ((e = cudaMallocHost((void**)&ctx->h_info, 4 * sizeof(u32)))) return bail(e, "pinned info");
+  if ((e = cudaMemset(ctx->count, 0, sizeof(u32) * g.ncell)) || (e = cudaMemset(ctx->seg, 0, sizeof(u32) * ((size_t)g.ncell + 1))) ||
+      (e = cudaMemset(ctx->d_info, 0, 4 * sizeof(u32))) ||
+      (e = cudaMemset(ctx->cx, 0, sizeof(double) * (size_t)(g.NX + 1) * g.NY * g.NZ)) ||
+      (e = cudaMemset(ctx->cy, 0, sizeof(double) * (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
+      (e = cudaMemset(ctx->cz, 0, sizeof(double) * (size_t)g.NX * g.NY * (g.NZ + 1))) ||
+      (e = cudaMemset(ctx->flux_slots, 0, sizeof(double) * NSLOT)) || (e = cudaMemset(ctx->d_flux, 0, 2 * sizeof(double))) ||
+      (e = cudaMemset(ctx->cnt_mem, 0, sizeof(unsigned long long) * 6 * NSLOT)) ||
+      (e = cudaMemset(ctx->outbuf, 0, sizeof(double) * g.ncell)))
+    return bail(e, "memset");
+  ctx->cnt.pairs = ctx->cnt_mem; ctx->cnt.collisions = ctx->cnt_mem + NSLOT; ctx->cnt.near_ties = ctx->cnt_mem + 2 * NSLOT;
+  ctx->cnt.ill_posed = ctx->cnt_mem + 3 * NSLOT; ctx->cnt.f_evals = ctx->cnt_mem + 4 * NSLOT; ctx->cnt.sd_substeps = ctx->cnt_mem + 5 * NSLOT;
+  CoalParams& kp = ctx->kp;
+  kp.kernel = o->kernel; kp.multi_coal = o->multi_coal; kp.golovin_b = o->golovin_b;
+  kp.seed_lo = (u32)o->seed; kp.seed_hi = (u32)(o->seed >> 32);
+  kp.n_eff_R = 0; kp.n_eff_q = 0;
+  if (o->kernel == SDM_KERNEL_HYDRO_TAB) {
+    kp.n_eff_R = o->n_eff_R; kp.n_eff_q = o->n_eff_q;
+    for (int t = 1; t < o->n_eff_R; ++t) if (!(o->eff_R[t] > o->eff_R[t - 1])) { sdm_destroy(ctx); return fail(nullptr, SDM_ERR_INVALID, "sdm_create: eff_R must ascend"); }
+    for (int t = 1; t < o->n_eff_q; ++t) if (!(o->eff_q[t] > o->eff_q[t - 1])) { sdm_destroy(ctx); return fail(nullptr, SDM_ERR_INVALID, "sdm_create: eff_q must ascend"); }
+    if ((e = dalloc(&ctx->d_effR, o->n_eff_R)) || (e = dalloc(&ctx->d_effq, o->n_eff_q)) ||
+        (e = dalloc(&ctx->d_efftab, (size_t)o->n_eff_R * o->n_eff_q)) ||
+        (e = cudaMemcpy(ctx->d_effR, o->eff_R, sizeof(double) * o->n_eff_R, cudaMemcpyHostToDevice)) ||
+        (e = cudaMemcpy(ctx->d_effq, o->eff_q, sizeof(double) * o->n_eff_q, cudaMemcpyHostToDevice)) ||
+        (e = cudaMemcpy(ctx->d_efftab, o->eff_tab, sizeof(double) * (size_t)o->n_eff_R * o->n_eff_q, cudaMemcpyHostToDevice)))
+      return bail(e, "efficiency table");
+    kp.eff_R = ctx->d_effR; kp.eff_q = ctx->d_effq; kp.eff_tab = ctx->d_efftab;
+  }
+  ctx->o.eff_R = ctx->o.eff_q = ctx->o.eff_tab = nullptr;   // host pointers are not retained
+  if ((e = cudaEventCreateWithFlags(&ctx->ev_info, cudaEventDisableTiming)) ||
+      (e = cudaEventCreateWithFlags(&ctx->ev_async, cudaEventDisableTiming)))
+    return bail(e, "events");
+  if ((e = cudaDeviceSynchronize())) return bail(e, "sync");
+  *out = ctx;
+  return SDM_OK;
+}
+
+void sdm_destroy(sdm_ctx* ctx) {
+  if (!ctx) return;
+  for (int b = 0; b < 2; ++b) {
+    SdArrays& a = ctx->buf[b];
+    cudaFree(a.n); cudaFree(a.rw2); cudaFree(a.rd3); cudaFree(a.kappa); cudaFree(a.x); cudaFree(a.y); cudaFree(a.z); cudaFree(a.id);
+  }
+  cudaFree(ctx->cell); cudaFree(ctx->off); cudaFree(ctx->rank); cudaFree(ctx->count); cudaFree(ctx->blocksum); cudaFree(ctx->seg);
+  cudaFree(ctx->d_info); cudaFree(ctx->cf.rhod); cudaFree(ctx->cf.eta); cudaFree(ctx->cf.rho_a); cudaFree(ctx->outbuf);
+  cudaFree(ctx->th_dense); cudaFree(ctx->rv_dense); cudaFree(ctx->cx); cudaFree(ctx->cy); cudaFree(ctx->cz);
+  cudaFree(ctx->flux_slots); cudaFree(ctx->d_flux); cudaFree(ctx->cnt_mem);
+  cudaFree(ctx->d_effR); cudaFree(ctx->d_effq); cudaFree(ctx->d_efftab);
+  if (ctx->h_info) cudaFreeHost(ctx->h_info);
+  if (ctx->ev_info) cudaEventDestroy(ctx->ev_info);
+  if (ctx->ev_async) cudaEventDestroy(ctx->ev_async);
+  cudaGetLastError();
+  delete ctx;
+}
+
+int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arrinfo c2, sdm_arrinfo c3, uint64_t N,
+                         const uint64_t* n, const double* rw2, const double* rd3, const double* kappa, const double* x,
+                         const double* y, const double* z, const uint32_t* id, void* stream) {
+  if (!ctx) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Grid& g = ctx->g;
+  if (N > ctx->cap_sd) return fail(ctx, SDM_ERR_CAPACITY, "sdm_init_from_arrays: N exceeds max_sd");
+  if (N && (!n || !rw2 || !rd3 || !kappa || !id || (g.hx && !x) || (g.hy && !y) || (g.hz && !z)))
+    return fail(ctx, SDM_ERR_INVALID, "sdm_init_from_arrays: NULL attribute array");
+  if (!rhod.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_init_from_arrays: rhod is mandatory");
+  launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st);
+  ctx->launches++;
+  const sdm_arrinfo comps[3] = {c1, c2, c3};
+  if (int rc = copy_courants(ctx, comps, st)) return rc;
+  ctx->cur = 0; ctx->cn = 0;
+  SdArrays& a = ctx->buf[0];
+  if (N) {
+    CK(cudaMemcpyAsync(a.n, n, N * 8, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.rw2, rw2, N * 8, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.rd3, rd3, N * 8, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.kappa, kappa, N * 8, cudaMemcpyDeviceToDevice, st));
+    if (g.hx) CK(cudaMemcpyAsync(a.x, x, N * 8, cudaMemcpyDeviceToDevice, st));
+    if (g.hy) CK(cudaMemcpyAsync(a.y, y, N * 8, cudaMemcpyDeviceToDevice, st));
+    if (g.hz) CK(cudaMemcpyAsync(a.z, z, N * 8, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.id, id, N * 4, cudaMemcpyDeviceToDevice, st));
+  }
+  const u32 info[4] = {(u32)N, 0u, 0u, 0u};
+  CK(cudaMemcpyAsync(ctx->d_info, info, sizeof(info), cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
+  CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * 6 * NSLOT, st));
+  CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
+  CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
+  CK(cudaStreamSynchronize(st));
+  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false;
+  ctx->last_stream = st;
+  return SDM_OK;
+}
+
+int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo c1, sdm_arrinfo c2,
+                  sdm_arrinfo c3, sdm_arrinfo rhod, void* stream) {
+  if (!ctx || !op) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Grid& g = ctx->g;
+  if (!th.data_zero || !rv.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: th and rv are mandatory");
+  if (op->cond && (op->sstp_cond < 1 || !(op->RH_max > 0))) return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: sstp_cond >= 1 and RH_max > 0 required");
+  if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_step_sync: called twice without step_async");
+  ctx->last_stream = st;
+  if (rhod.data_zero) { launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st); ctx->launches++; }
+  const sdm_arrinfo comps[3] = {c1, c2, c3};
+  if (int rc = copy_courants(ctx, comps, st)) return rc;
+
+  // a0-a3: compaction + cell index + counting sort by cell
+  u32* d_cur = ctx->d_info + ctx->cn;
+  u32* d_next = ctx->d_info + (ctx->cn ^ 1);
+  CK(cudaMemsetAsync(ctx->d_info + 2, 0, sizeof(u32), st));
+  launch_cellhist(ctx->buf[ctx->cur], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+  launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
+  ctx->launches += (ctx->nslots ? 1 : 0) + 3;
+  CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 4 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+  CK(cudaEventRecord(ctx->ev_info, st));
+  launch_scatter(ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
+  ctx->launches += ctx->nslots ? 1 : 0;
+  CK(cudaGetLastError());
+  CK(cudaEventSynchronize(ctx->ev_info));   // the scatter runs while the host sizes the next launches
+  ctx->cn ^= 1;
+  ctx->cur ^= 1;
+  ctx->nslots = ctx->h_info[ctx->cn];
+  ctx->max_nc = ctx->h_info[2];
+  if (ctx->h_info[3]) return fail(ctx, SDM_ERR_CUDA, "sdm_step_sync: device-side error flag set (corrupted segment sizes)");
+
+  // launch sizing from the measured occupancy
+  const double mean = (double)ctx->nslots / g.ncell;
+  int G = pick_group(ctx, mean);
+  const int P = std::max(next_pow2((int)ctx->max_nc), 2);
+  if ((size_t)ng_of(G) * P * 10 > kSmemLimit) G = 256;
+  if ((size_t)ng_of(G) * P * 10 > kSmemLimit || ctx->max_nc > 32768)
+    return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_sync: a cell holds more super-droplets than one CTA can sort (limit 16384)");
+  ctx->G = G;
+  const Field thf = make_field(ctx, th), rvf = make_field(ctx, rv);
+  if (ctx->nslots) {
+    CK(launch_rank(G, ctx->buf[ctx->cur].id, ctx->seg, g.ncell, (u32)ctx->step, ctx->kp.seed_lo, ctx->kp.seed_hi, P,
+                   ctx->rank, (int*)(ctx->d_info + 3), st));
+    ctx->launches++;
+  }
+  ctx->have_order = true;
+  if (op->cond) {
+    int cap = (int)((ctx->max_nc + 3) / 4 * 4);
+    cap = std::max(cap, 4);
+    if (cond_smem_bytes(G, cap) > kSmemLimit) cap = 0;   // work in place in HBM/L2
+    CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max};
+    CK(launch_cond(G, cap, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
+  } else {
+    launch_thermo(g, thf, rvf, ctx->cf, st);
+    CK(cudaGetLastError());
+  }
+  ctx->launches++;
+  ctx->synced = true;
+  return SDM_OK;
+}
+
+int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
+  if (!ctx || !op) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Grid& g = ctx->g;
+  if (!ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_step_async: step_sync of this step has not been called");
+  if (op->coal && op->sstp_coal < 1) return fail(ctx, SDM_ERR_INVALID, "sdm_step_async: sstp_coal >= 1 required");
+  ctx->last_stream = st;
+  if (ctx->nslots && (op->coal || op->adve || op->sedi)) {
+    const int G = ctx->G;
+    int cap = (int)((ctx->max_nc + 3) / 4 * 4);
+    cap = std::max(cap, 4);
+    const int sstp = op->coal ? op->sstp_coal : 1;
+    bool in_smem = coal_smem_bytes(G, cap, sstp, true) <= kSmemLimit;
+    if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
+      return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
+    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step};
+    CK(launch_coal_move(G, cap, in_smem, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
+                        ctx->cnt, st));
+    ctx->launches++;
+  }
+  launch_flux_sum(ctx->flux_slots, ctx->d_flux, ctx->d_flux + 1, st);
+  ctx->launches++;
+  CK(cudaGetLastError());
+  CK(cudaEventRecord(ctx->ev_async, st));
+  ctx->step += 1;
+  ctx->synced = false;
+  ctx->have_order = false;
+  return SDM_OK;
+}
+
+int sdm_step_async_result(sdm_ctx* ctx, double* rain_flux) {
+  if (!ctx) return SDM_ERR_INVALID;
+  CK(cudaEventSynchronize(ctx->ev_async));
+  if (rain_flux) CK(cudaMemcpy(rain_flux, ctx->d_flux, sizeof(double), cudaMemcpyDeviceToHost));
+  return SDM_OK;
+}
+
+int sdm_step_host(sdm_ctx* ctx, const sdm_opts* op, double* th_host, double* rv_host, double* rain_flux, void* stream) {
+  if (!ctx || !op || !th_host || !rv_host) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Grid& g = ctx->g;
+  const size_t bytes = sizeof(double) * g.ncell;
+  CK(cudaMemcpyAsync(ctx->th_dense, th_host, bytes, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(ctx->rv_dense, rv_host, bytes, cudaMemcpyHostToDevice, st));
+  sdm_arrinfo th{ctx->th_dense, {0, 0, 0}}, rv{ctx->rv_dense, {0, 0, 0}}, none{nullptr, {0, 0, 0}};
+  int idx = 0;   // dense C-order strides over the present dimensions
+  const long long sx = (long long)g.NY * g.NZ, sy = g.NZ, sz = 1;
+  if (g.hx) { th.strides[idx] = rv.strides[idx] = sx; ++idx; }
+  if (g.hy) { th.strides[idx] = rv.strides[idx] = sy; ++idx; }
+  if (g.hz) { th.strides[idx] = rv.strides[idx] = sz; ++idx; }
+  if (int rc = sdm_step_sync(ctx, op, th, rv, none, none, none, none, stream)) return rc;
+  CK(cudaMemcpyAsync(th_host, ctx->th_dense, bytes, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(rv_host, ctx->rv_dense, bytes, cudaMemcpyDeviceToHost, st));
+  if (int rc = sdm_step_async(ctx, op, stream)) return rc;
+  CK(cudaStreamSynchronize(st));
+  if (rain_flux) CK(cudaMemcpy(rain_flux, ctx->d_flux, sizeof(double), cudaMemcpyDeviceToHost));
+  return SDM_OK;
+}
+
+static int diag_launch(sdm_ctx* ctx, int wet, double lo, double hi, int k, int count_only, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  ctx->last_stream = st;
+  launch_diag_mom(ctx->buf[ctx->cur], ctx->d_info + ctx->cn, (u32)ctx->nslots, ctx->g, wet, lo, hi, k, count_only, ctx->cf.rhod,
+                  ctx->outbuf, st);
+  ctx->launches += (ctx->nslots ? 1 : 0) + (count_only ? 0 : 1);
+  CK(cudaGetLastError());
+  return SDM_OK;
+}
+int sdm_diag_sd_conc(sdm_ctx* ctx, void* stream) { return ctx ? diag_launch(ctx, 1, 0, 0, 0, 1, stream) : SDM_ERR_INVALID; }
+int sdm_diag_dry_rng(sdm_ctx* ctx, double r_mi, double r_mx) {
+  if (!ctx) return SDM_ERR_INVALID;
+  ctx->dry_lo = r_mi; ctx->dry_hi = r_mx;
+  return SDM_OK;
+}
+int sdm_diag_wet_rng(sdm_ctx* ctx, double r_mi, double r_mx) {
+  if (!ctx) return SDM_ERR_INVALID;
+  ctx->wet_lo = r_mi; ctx->wet_hi = r_mx;
+  return SDM_OK;
+}
+int sdm_diag_dry_mom(sdm_ctx* ctx, int k, void* stream) { return ctx ? diag_launch(ctx, 0, ctx->dry_lo, ctx->dry_hi, k, 0, stream) : SDM_ERR_INVALID; }
+int sdm_diag_wet_mom(sdm_ctx* ctx, int k, void* stream) { return ctx ? diag_launch(ctx, 1, ctx->wet_lo, ctx->wet_hi, k, 0, stream) : SDM_ERR_INVALID; }
+const double* sdm_outbuf(sdm_ctx* ctx) { return ctx ? ctx->outbuf : nullptr; }
+
+int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd) {
+  if (!ctx || !n_sd) return SDM_ERR_INVALID;
+  *n_sd = ctx->nslots;
+  return SDM_OK;
+}
+
+int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double* kappa, double* x, double* y, double* z,
+                     uint32_t* id, void* stream) {
+  if (!ctx) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const SdArrays& a = ctx->buf[ctx->cur];
+  const size_t N = ctx->nslots;
+  if (!N) return SDM_OK;
+  if (n) CK(cudaMemcpyAsync(n, a.n, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (rw2) CK(cudaMemcpyAsync(rw2, a.rw2, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (rd3) CK(cudaMemcpyAsync(rd3, a.rd3, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (kappa) CK(cudaMemcpyAsync(kappa, a.kappa, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (x && ctx->g.hx) CK(cudaMemcpyAsync(x, a.x, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (y && ctx->g.hy) CK(cudaMemcpyAsync(y, a.y, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (z && ctx->g.hz) CK(cudaMemcpyAsync(z, a.z, N * 8, cudaMemcpyDeviceToDevice, st));
+  if (id) CK(cudaMemcpyAsync(id, a.id, N * 4, cudaMemcpyDeviceToDevice, st));
+  return SDM_OK;
+}
+
+int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, void* stream) {
+  if (!ctx || !ids_sorted || !seg_start) return SDM_ERR_INVALID;
+  if (!ctx->have_order) return fail(ctx, SDM_ERR_ORDER, "sdm_export_order: valid only between step_sync and step_async");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (ctx->nslots) { launch_export_order(ctx->buf[ctx->cur].id, ctx->rank, ctx->seg, ctx->g.ncell, ids_sorted, st); ctx->launches++; }
+  CK(cudaMemcpyAsync(seg_start, ctx->seg, sizeof(u32) * ((size_t)ctx->g.ncell + 1), cudaMemcpyDeviceToDevice, st));
+  CK(cudaGetLastError());
+  return SDM_OK;
+}
+
+int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out) {
+  if (!ctx || !out) return SDM_ERR_INVALID;
+  CK(cudaStreamSynchronize(ctx->last_stream));
+  std::vector<unsigned long long> h(6 * NSLOT);
+  CK(cudaMemcpy(h.data(), ctx->cnt_mem, sizeof(unsigned long long) * 6 * NSLOT, cudaMemcpyDeviceToHost));
+  unsigned long long s[6] = {0, 0, 0, 0, 0, 0};
+  for (int q = 0; q < 6; ++q) for (int t = 0; t < NSLOT; ++t) s[q] += h[(size_t)q * NSLOT + t];
+  out->n_sd = ctx->nslots; out->max_cell_count = ctx->max_nc; out->step = ctx->step; out->kernel_launches = ctx->launches;
+  out->pairs = s[0]; out->collisions = s[1]; out->near_ties = s[2]; out->ill_posed = s[3]; out->newton_iters = s[4];
+  out->sd_substeps = s[5];
+  return SDM_OK;
+}
+
+int sdm_set_step(sdm_ctx* ctx, uint64_t step) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_set_step: not between step_sync and step_async");
+  ctx->step = step;
+  return SDM_OK;
+}
+
+int sdm_set_group_size(sdm_ctx* ctx, int group) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (!(group == 0 || group == 4 || group == 8 || group == 16 || group == 32 || group == 256))
+    return fail(ctx, SDM_ERR_INVALID, "sdm_set_group_size: 0, 4, 8, 16, 32 or 256");
+  ctx->group_override = group;
+  return SDM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,275 @@
+// Stages a5 + a6 in one cell-resident kernel: SDM coalescence on the pairs
+// (0,1),(2,3).. of the cell's sorted segment (PAPER.md :622-645, eq. 27-28) followed by advection
+// (eq. 16) and sedimentation (:647-651) of every SD of the cell.
+// This translation unit is compiled with -fmad=false: the collision probability and the new
+// positions use only IEEE +,-,*,/,sqrt in the oracle's order, so that collision decisions
+// (u < frac p) and cell-border decisions are taken on bit-identical numbers whenever the inputs are.
+#include "sdm_kernels.cuh"
+
+namespace sdm {
+
+// collision efficiency: bilinear in (collector radius, ratio), clamped at the table edges
+__device__ __forceinline__ double eff_lookup(const CoalParams& kp, double R, double q) {
+  const int nR = kp.n_eff_R, nq = kp.n_eff_q;
+  R = fmin(fmax(R, kp.eff_R[0]), kp.eff_R[nR - 1]);
+  q = fmin(fmax(q, kp.eff_q[0]), kp.eff_q[nq - 1]);
+  int iR = 0, iq = 0;
+  while (iR < nR - 2 && kp.eff_R[iR + 1] <= R) ++iR;   // last node <= R (upper_bound - 1), at most n-2
+  while (iq < nq - 2 && kp.eff_q[iq + 1] <= q) ++iq;
+  const double t = (R - kp.eff_R[iR]) / (kp.eff_R[iR + 1] - kp.eff_R[iR]);
+  const double s = (q - kp.eff_q[iq]) / (kp.eff_q[iq + 1] - kp.eff_q[iq]);
+  const double e00 = kp.eff_tab[iR * nq + iq], e01 = kp.eff_tab[iR * nq + iq + 1];
+  const double e10 = kp.eff_tab[(iR + 1) * nq + iq], e11 = kp.eff_tab[(iR + 1) * nq + iq + 1];
+  return (1.0 - t) * ((1.0 - s) * e00 + s * e01) + t * ((1.0 - s) * e10 + s * e11);
+}
+
+__device__ __forceinline__ double wrap(double x, double X) {
+  if (x < 0.0) x += X;
+  if (x >= X) x -= X;
+  return x;
+}
+
+// Shared memory per group: cap x {n (u64), rw2, rd3, kappa (double), id (u32)} (SMEM) or cap x u16 slot
+// indices (attributes left in HBM/L2), and for sstp_coal > 1 another P x {u64 key, u16 order}.
+template <int G, bool SMEM>
+__global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArrays a, const u16* __restrict__ rank,
+                                                                 const u32* __restrict__ seg, Grid g, CellFields cf,
+                                                                 CoalParams kp, CoalMoveParams mp, double* flux_slots,
+                                                                 Counters cnt, int cap, int P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NG = CtaOf<G>::threads / G;
+  __shared__ double red_scratch[32];
+  const int gi = threadIdx.x / G;
+  const Group<G> grp = make_group<G>(red_scratch);
+  const int c = blockIdx.x * NG + gi;
+  unsigned n_pairs = 0, n_coll = 0, n_tie = 0;
+  double flux = 0.0;
+  if (c < g.ncell) {
+    const u32 s0 = seg[c];
+    const int m = (int)(seg[c + 1] - s0);
+    // per-group shared arrays, indexed by sorted position e.  SMEM: the attributes themselves;
+    // otherwise (cells too large for shared memory) only the slot of position e, attributes stay in HBM/L2.
+    const size_t attr_bytes = SMEM ? (size_t)cap * 36 : (size_t)cap * 2;
+    unsigned char* base = smem_raw + (size_t)gi * (attr_bytes + (size_t)P * 10);
+    u64* pn; double *prw2, *prd3, *pkap; u32* pid;
+    u16* s_inv = reinterpret_cast<u16*>(base);
+    if constexpr (SMEM) {
+      pn = reinterpret_cast<u64*>(base);
+      prw2 = reinterpret_cast<double*>(base) + cap;
+      prd3 = reinterpret_cast<double*>(base) + 2 * cap;
+      pkap = reinterpret_cast<double*>(base) + 3 * cap;
+      pid = reinterpret_cast<u32*>(base + (size_t)cap * 32);
+    } else {
+      pn = a.n + s0; prw2 = a.rw2 + s0; prd3 = a.rd3 + s0; pkap = a.kappa + s0; pid = a.id + s0;
+    }
+    auto SL = [&](int e) -> int { if constexpr (SMEM) return e; else return (int)s_inv[e]; };
+    u64* s_key = reinterpret_cast<u64*>(base + attr_bytes);
+    u16* s_ord = reinterpret_cast<u16*>(base + attr_bytes + (size_t)P * 8);
+    const double eta = cf.eta[c], rho_a = cf.rho_a[c];
+    if (m > 0 && mp.coal) {
+      for (int t = grp.lane; t < m; t += G) {
+        const int e = rank[s0 + t];
+        if constexpr (SMEM) {
+          pn[e] = a.n[s0 + t];
+          prw2[e] = a.rw2[s0 + t];
+          prd3[e] = a.rd3[s0 + t];
+          pkap[e] = a.kappa[s0 + t];
+          pid[e] = a.id[s0 + t];
+        } else {
+          s_inv[e] = (u16)t;
+        }
+      }
+      grp.sync();
+      const double dtpp = g.dt / mp.sstp_coal;
+      int nc = m;   // SDs taking part in this substep
+      for (int sub = 0; sub < mp.sstp_coal; ++sub) {
+        if (sub > 0) {
+          // new random grouping (:624): drop SDs that reached N = 0, draw new keys, sort again
+          const int Pm = next_pow2(m);
+          for (int t = grp.lane; t < Pm; t += G) {
+            u64 key = ~0ull;
+            if (t < m && pn[SL(t)] != 0) { const u32 sid = pid[SL(t)]; key = ((u64)shuffle_key(sid, mp.step, (u32)sub, kp.seed_lo, kp.seed_hi) << 32) | sid; }
+            s_key[t] = key;
+            s_ord[t] = (u16)t;
+          }
+          bitonic_sort<G, u16>(grp, s_key, s_ord, Pm);
+          int live = 0;
+          for (int t = grp.lane; t < m; t += G) live += (s_key[t] != ~0ull);
+          nc = (int)grp.sum((unsigned long long)live);
+        }
+        if (nc >= 2) {
+          // eq. 27 last factor n(n-1)/2 / floor(n/2)
+          const double scale = (double)((u64)nc * (u64)(nc - 1) / 2) / (double)(nc / 2);
+          for (int pr = grp.lane; pr < nc / 2; pr += G) {
+            const int ea = SL((sub == 0) ? 2 * pr : s_ord[2 * pr]);
+            const int eb = SL((sub == 0) ? 2 * pr + 1 : s_ord[2 * pr + 1]);
+            const u64 na = pn[ea], nb = pn[eb];
+            const int j = (na >= nb) ? ea : eb, k = (na >= nb) ? eb : ea;   // j: larger N; tie -> first in order
+            const u64 nj = (na >= nb) ? na : nb, nk = (na >= nb) ? nb : na;
+            const double yj = prw2[j], yk = prw2[k];
+            const double rj = sqrt(yj), rk = sqrt(yk);
+            double K;
+            if (kp.kernel == 1) {   // Golovin
+              const double vj = (4.0 / 3.0) * cst::pi * (yj * rj), vk = (4.0 / 3.0) * cst::pi * (yk * rk);
+              K = kp.golovin_b * (vj + vk);
+            } else {                // eq. 28
+              const double vj = v_term(rj, eta, rho_a), vk = v_term(rk, eta, rho_a);
+              K = cst::pi * ((rj + rk) * (rj + rk)) * fabs(vj - vk);
+              if (kp.kernel == 2) {
+                const double rl = fmax(rj, rk), rs = fmin(rj, rk);
+                K = K * eff_lookup(kp, rl, rs / rl);
+              }
+            }
+            const double p = (((double)nj * K) * (dtpp / g.dV)) * scale;   // eq. 27
+            const double u = coal_uniform(pid[ea], mp.step, (u32)sub, kp.seed_lo, kp.seed_hi);
+            const u64 qmax = nj / nk;
+            u64 gam;
+            if (kp.multi_coal) {
+              const double pf = floor(p);
+              if (pf >= (double)qmax) gam = qmax;
+              else {
+                const double frac = p - pf;
+                if (fabs(u - frac) < 1e-12) ++n_tie;
+                gam = (u64)pf + (u < frac ? 1u : 0u);
+                if (gam > qmax) gam = qmax;
+              }
+            } else {
+              if (fabs(u - p) < 1e-12) ++n_tie;
+              gam = (u < p) ? 1u : 0u;   // :639, :645
+            }
+            ++n_pairs;
+            if (gam == 0) continue;
+            ++n_coll;
+            const double gd = (double)gam;
+            const double rw3 = yk * rk + gd * (yj * rj);    // extensive attributes are summed (:643)
+            const double rd3j = gd * prd3[j];
+            const double rd3k = prd3[k];
+            const double kj = pkap[j], kk = pkap[k];
+            if (kj != kk)                                    // intensive ones averaged (:643)
+              pkap[k] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
+            prd3[k] = rd3k + rd3j;
+            const double r = cbrt(rw3);
+            prw2[k] = r * r;
+            pn[j] = nj - gam * nk;
+          }
+        }
+        grp.sync();
+      }
+    }
+    // ---- advection + sedimentation, SD by SD in storage order --------------------------------------
+    if (m > 0 && (mp.coal || mp.adve || mp.sedi)) {
+      const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+      const double rhod = cf.rhod[c];
+      double Cxl = 0, Cxh = 0, Cyl = 0, Cyh = 0, Czl = 0, Czh = 0;
+      if (mp.adve) {
+        if (g.hx) { Cxl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod; Cxh = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod; }
+        if (g.hy) { Cyl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod; Cyh = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod; }
+        if (g.hz) { Czl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod; Czh = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod; }
+      }
+      for (int t = grp.lane; t < m; t += G) {
+        const u32 s = s0 + t;
+        u64 n; double y;
+        if (SMEM && mp.coal) {
+          const int e = rank[s];
+          n = pn[e]; y = prw2[e];
+          a.n[s] = n; a.rw2[s] = y; a.rd3[s] = prd3[e]; a.kappa[s] = pkap[e];
+        } else {
+          n = a.n[s]; y = a.rw2[s];
+        }
+        if (n == 0 || !(mp.adve || mp.sedi)) continue;
+        double xn = 0, yn = 0, zn = 0;
+        if (g.hx) xn = a.x[s];
+        if (g.hy) yn = a.y[s];
+        if (g.hz) zn = a.z[s];
+        if (mp.adve) {   // eq. 16 with the Courant numbers at the edges of the SD's time-n cell
+          if (g.hx) { const double dC = Cxh - Cxl; xn = (xn + g.dx * (Cxl - (double)i * dC)) / (1.0 - dC); }
+          if (g.hy) { const double dC = Cyh - Cyl; yn = (yn + g.dy * (Cyl - (double)j * dC)) / (1.0 - dC); }
+          if (g.hz) { const double dC = Czh - Czl; zn = (zn + g.dz * (Czl - (double)k * dC)) / (1.0 - dC); }
+        }
+        if (mp.sedi && g.hz) zn = zn - v_term(sqrt(y), eta, rho_a) * g.dt;   // explicit Euler (:649)
+        if (g.hx) { xn = wrap(xn, g.X); a.x[s] = xn; }                        // periodic (:558)
+        if (g.hy) { yn = wrap(yn, g.Y); a.y[s] = yn; }
+        if (g.hz) {
+          if (zn < 0.0 || !(zn < g.Z)) {                                       // left the domain (:651)
+            if (zn < 0.0) flux += (double)n * ((4.0 / 3.0) * cst::pi * cst::rho_w * (y * sqrt(y)));
+            a.n[s] = 0;
+          }
+          a.z[s] = zn;
+        }
+      }
+    }
+  }
+  // rain flux and counters: warp-reduce, then one atomic per warp on spread addresses
+  unsigned v0 = n_pairs, v1 = n_coll, v2 = n_tie;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    v0 += __shfl_xor_sync(0xffffffffu, v0, d);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, d);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, d);
+    flux += __shfl_xor_sync(0xffffffffu, flux, d);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    const int slot = (blockIdx.x * (CtaOf<G>::threads / 32) + (threadIdx.x >> 5)) & (NSLOT - 1);
+    if (v0) atomicAdd(&cnt.pairs[slot], (unsigned long long)v0);
+    if (v1) atomicAdd(&cnt.collisions[slot], (unsigned long long)v1);
+    if (v2) atomicAdd(&cnt.near_ties[slot], (unsigned long long)v2);
+    if (flux != 0.0) atomicAdd(&flux_slots[slot], flux);
+  }
+}
+
+// sums the NSLOT flux slots in a fixed order, then clears them
+__global__ void k_flux_sum(double* flux_slots, double* flux_out, double* flux_total) {
+  __shared__ double sh[NSLOT];
+  for (int t = threadIdx.x; t < NSLOT; t += blockDim.x) { sh[t] = flux_slots[t]; flux_slots[t] = 0.0; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double s = 0.0;
+    for (int t = 0; t < NSLOT; ++t) s += sh[t];
+    *flux_out = s;
+    *flux_total += s;
+  }
+}
+
+size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem) {
+  const int NG = (G <= 32 ? 128 : G) / G;
+  const int P = sstp_coal > 1 ? next_pow2(cap) : 0;
+  return (size_t)NG * ((size_t)cap * (in_smem ? 36 : 2) + (size_t)P * 10);
+}
+
+template <int G>
+static cudaError_t launch_coal_move_t(int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+                                      const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp,
+                                      double* flux_slots, const Counters& cnt, cudaStream_t st) {
+  constexpr int NG = CtaOf<G>::threads / G;
+  const int grid = (g.ncell + NG - 1) / NG;
+  const int P = mp.sstp_coal > 1 ? next_pow2(cap) : 0;
+  const size_t smem = coal_smem_bytes(G, cap, mp.sstp_coal, in_smem);
+  if (in_smem) {
+    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_coal_move<G, true><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
+  } else {
+    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_coal_move<G, false><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+                             const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
+                             const Counters& cnt, cudaStream_t st) {
+  switch (G) {
+    case 4: return launch_coal_move_t<4>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
+    case 8: return launch_coal_move_t<8>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
+    case 16: return launch_coal_move_t<16>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
+    case 32: return launch_coal_move_t<32>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
+    default: return launch_coal_move_t<256>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
+  }
+}
+
+void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st) {
+  k_flux_sum<<<1, 256, 0, st>>>(const_cast<double*>(flux_slots), flux_out, flux_total);
+}
+
+}  // namespace sdm

@@ -1,0 +1,58 @@
+// Host-side launch interface between sdm_api.cu and the kernel translation units.
+#pragma once
+#include "sdm_common.cuh"
+
+namespace sdm {
+
+// CTA shape of the cell-resident kernels: sub-warp / warp groups share a 128-thread CTA, a CTA-wide
+// group is the CTA.
+template <int G>
+struct CtaOf { static constexpr int threads = (G <= 32) ? 128 : G; };
+
+struct CondParams {
+  double dtp;        // dt / sstp_cond
+  int sstp;
+  double RH_max;
+};
+struct CoalMoveParams {
+  int coal, adve, sedi, sstp_coal;
+  u32 step;
+};
+struct CellFields {  // library-owned dense per-cell arrays
+  double* rhod;      // copy of the caller's rhod
+  double* eta;       // viscosity after the condensation feedback (for v_term)
+  double* rho_a;     // air density rhod (1 + rv)
+  const double *cx, *cy, *cz;   // rho_d * Courant on the Arakawa-C grid, dense C order
+};
+
+// sdm_sort.cu
+void launch_cellhist(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
+                     u32* count, cudaStream_t st);
+int scan_num_blocks(int ncell);
+void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_next, u32* d_maxcount, cudaStream_t st);
+void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
+                    const u32* cell, const u32* off, const u32* seg, cudaStream_t st);
+cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                        u16* rank, int* d_error, cudaStream_t st);
+void launch_export_order(const u32* id, const u16* rank, const u32* seg, int ncell, u32* ids_sorted, cudaStream_t st);
+
+// sdm_cond.cu
+// cap: shared-memory slots per group (>= largest cell) or 0 to work in place in global memory
+cudaError_t launch_cond(int G, int cap, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
+                        Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st);
+size_t cond_smem_bytes(int G, int cap);
+void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);
+
+// sdm_coal_move.cu
+cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+                             const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
+                             const Counters& cnt, cudaStream_t st);
+size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem);
+void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
+
+// sdm_diag.cu
+void launch_diag_mom(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
+                     double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st);
+void launch_dense_copy(Field src, double* dst, int n0, int n1, int n2, cudaStream_t st);
+
+}  // namespace sdm

@@ -1,0 +1,216 @@
+// Stage a0-a3 of the step: zero-multiplicity compaction, cell index, and the
+// sort on (cell, Philox key, id) as an MSD radix sort: one counting pass over the cell index (global
+// histogram + scan + scatter; dead SDs get no slot, which is the compaction) and a per-cell bitonic
+// sort of (key << 32 | id) in shared memory that yields each SD's rank inside its cell.
+// PAPER.md :547 (cell index), :624 (random non-overlapping pairs), :641/:651 (N = 0 SDs).
+#include "sdm_kernels.cuh"
+
+namespace sdm {
+
+// ---- a0/a1: cell index + histogram (warp-aggregated atomics) ----------------------------------------
+__global__ void __launch_bounds__(256) k_cellhist(SdArrays a, const u32* __restrict__ d_nslots, Grid g,
+                                                  u32* __restrict__ cell, u32* __restrict__ off,
+                                                  u32* __restrict__ count) {
+  const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+  const u32 nslots = *d_nslots;
+  u32 c = CELL_DEAD;
+  if (i < nslots && a.n[i] != 0) c = cell_of(g, g.hx ? a.x[i] : 0.0, g.hy ? a.y[i] : 0.0, g.hz ? a.z[i] : 0.0);
+  // lanes that fall in the same cell take consecutive slots with one atomic
+  const u32 peers = __match_any_sync(0xffffffffu, c);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  u32 base = 0;
+  if (c != CELL_DEAD && lane == leader) base = atomicAdd(&count[c], (u32)__popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  if (i < nslots) {
+    cell[i] = c;
+    if (c != CELL_DEAD) off[i] = base + __popc(peers & ((1u << lane) - 1u));
+  }
+}
+
+// ---- a2: exclusive scan of the histogram -> segment offsets (3 small kernels) -----------------------
+constexpr int SCAN_THREADS = 1024, SCAN_ITEMS = 4, SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__device__ __forceinline__ u32 block_excl_scan(u32 v, u32* warp_sums, u32& total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  u32 inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const u32 t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += t;
+  }
+  if (lane == 31) warp_sums[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    u32 s = warp_sums[lane];
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const u32 t = __shfl_up_sync(0xffffffffu, s, d);
+      if (lane >= d) s += t;
+    }
+    warp_sums[lane] = s;   // inclusive over warps
+  }
+  __syncthreads();
+  total = warp_sums[31];
+  return inc - v + (w ? warp_sums[w - 1] : 0u);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_partial(const u32* __restrict__ count, int ncell,
+                                                               u32* __restrict__ blocksum, u32* __restrict__ d_maxcount) {
+  __shared__ u32 ws[32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  u32 s = 0, mx = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k)
+    if (base + k < ncell) { const u32 v = count[base + k]; s += v; mx = max(mx, v); }
+  u32 total;
+  block_excl_scan(s, ws, total);
+  mx = __reduce_max_sync(0xffffffffu, mx);
+  if ((threadIdx.x & 31) == 0 && mx) atomicMax(d_maxcount, mx);
+  if (threadIdx.x == 0) blocksum[blockIdx.x] = total;
+}
+
+// one CTA: exclusive scan of the block sums; publishes the live count
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(u32* __restrict__ blocksum, int nblocks,
+                                                              u32* __restrict__ d_nslots_next, u32* __restrict__ seg_total) {
+  __shared__ u32 ws[32];
+  u32 carry = 0;
+  for (int b0 = 0; b0 < nblocks; b0 += SCAN_THREADS) {
+    const int b = b0 + threadIdx.x;
+    const u32 v = b < nblocks ? blocksum[b] : 0u;
+    u32 total;
+    const u32 ex = block_excl_scan(v, ws, total);
+    if (b < nblocks) blocksum[b] = carry + ex;
+    carry += total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { *d_nslots_next = carry; *seg_total = carry; }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(u32* __restrict__ count, int ncell,
+                                                             const u32* __restrict__ blocksum, u32* __restrict__ seg) {
+  __shared__ u32 ws[32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  u32 v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = base + k < ncell ? count[base + k] : 0u; s += v[k]; }
+  u32 total;
+  u32 ex = block_excl_scan(s, ws, total) + blocksum[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k)
+    if (base + k < ncell) { seg[base + k] = ex; ex += v[k]; count[base + k] = 0u; }   // histogram is left zeroed
+}
+
+// ---- a3: scatter the SoA state into cell-sorted storage (drops dead SDs) ----------------------------
+__global__ void __launch_bounds__(256) k_scatter(SdArrays src, SdArrays dst, const u32* __restrict__ d_nslots, Grid g,
+                                                 const u32* __restrict__ cell, const u32* __restrict__ off,
+                                                 const u32* __restrict__ seg) {
+  const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= *d_nslots) return;
+  const u32 c = cell[i];
+  if (c == CELL_DEAD) return;
+  const u32 d = seg[c] + off[i];
+  dst.n[d] = src.n[i];
+  dst.rw2[d] = src.rw2[i];
+  dst.rd3[d] = src.rd3[i];
+  dst.kappa[d] = src.kappa[i];
+  if (g.hx) dst.x[d] = src.x[i];
+  if (g.hy) dst.y[d] = src.y[i];
+  if (g.hz) dst.z[d] = src.z[i];
+  dst.id[d] = src.id[i];
+}
+
+// ---- a2 (second level): rank of every SD inside its cell under (Philox key, id) ----------------------
+// One group of G threads per cell.  Shared memory per group: P u64 keys + P u16 indices.
+template <int G>
+__global__ void __launch_bounds__(CtaOf<G>::threads) k_rank(const u32* __restrict__ id, const u32* __restrict__ seg,
+                                                            int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                                                            u16* __restrict__ rank, int* __restrict__ d_error) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NG = CtaOf<G>::threads / G;
+  const int gi = threadIdx.x / G;
+  const Group<G> grp = make_group<G>(nullptr);
+  const int c = blockIdx.x * NG + gi;
+  if (c >= ncell) return;
+  u64* skey = reinterpret_cast<u64*>(smem_raw) + (size_t)gi * P;
+  u16* sidx = reinterpret_cast<u16*>(smem_raw + (size_t)NG * P * sizeof(u64)) + (size_t)gi * P;
+  const u32 s0 = seg[c];
+  const int m = (int)(seg[c + 1] - s0);
+  if (m > P) {   // host sized P from the measured maximum; cannot happen unless the state was corrupted
+    if (grp.lane == 0) atomicExch(d_error, 1);
+    return;
+  }
+  if (m == 0) return;
+  if (m == 1) { if (grp.lane == 0) rank[s0] = 0; return; }
+  const int Pm = next_pow2(m);   // sort only as many slots as this cell needs
+  for (int t = grp.lane; t < Pm; t += G) {
+    u64 key = ~0ull;
+    if (t < m) {
+      const u32 sid = id[s0 + t];
+      key = ((u64)shuffle_key(sid, step, 0u, seed_lo, seed_hi) << 32) | sid;
+    }
+    skey[t] = key;
+    sidx[t] = (u16)t;
+  }
+  bitonic_sort<G, u16>(grp, skey, sidx, Pm);
+  for (int t = grp.lane; t < m; t += G) rank[s0 + sidx[t]] = (u16)t;
+}
+
+// ids in sorted order (parity export)
+__global__ void k_export_order(const u32* __restrict__ id, const u16* __restrict__ rank, const u32* __restrict__ seg,
+                               int ncell, u32* __restrict__ ids_sorted) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const u32 s0 = seg[c], s1 = seg[c + 1];
+  for (u32 s = s0; s < s1; ++s) ids_sorted[s0 + rank[s]] = id[s];
+}
+
+// ---- host launchers ----------------------------------------------------------------------------------
+void launch_cellhist(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
+                     u32* count, cudaStream_t st) {
+  if (nslots_bound == 0) return;
+  k_cellhist<<<(nslots_bound + 255) / 256, 256, 0, st>>>(a, d_nslots, g, cell, off, count);
+}
+
+int scan_num_blocks(int ncell) { return (ncell + SCAN_TILE - 1) / SCAN_TILE; }
+
+void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_next, u32* d_maxcount, cudaStream_t st) {
+  const int nb = scan_num_blocks(ncell);
+  k_scan_partial<<<nb, SCAN_THREADS, 0, st>>>(count, ncell, blocksum, d_maxcount);
+  k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(blocksum, nb, d_nslots_next, seg + ncell);
+  k_scan_apply<<<nb, SCAN_THREADS, 0, st>>>(count, ncell, blocksum, seg);
+}
+
+void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
+                    const u32* cell, const u32* off, const u32* seg, cudaStream_t st) {
+  if (nslots_bound == 0) return;
+  k_scatter<<<(nslots_bound + 255) / 256, 256, 0, st>>>(src, dst, d_nslots, g, cell, off, seg);
+}
+
+template <int G>
+static cudaError_t launch_rank_t(const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                                 u16* rank, int* d_error, cudaStream_t st) {
+  constexpr int NG = CtaOf<G>::threads / G;
+  const size_t smem = (size_t)NG * P * (sizeof(u64) + sizeof(u16));
+  cudaError_t e = cudaFuncSetAttribute(k_rank<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_rank<G><<<(ncell + NG - 1) / NG, CtaOf<G>::threads, smem, st>>>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                        u16* rank, int* d_error, cudaStream_t st) {
+  switch (G) {
+    case 4: return launch_rank_t<4>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    case 8: return launch_rank_t<8>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    case 16: return launch_rank_t<16>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    case 32: return launch_rank_t<32>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    default: return launch_rank_t<256>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+  }
+}
+
+void launch_export_order(const u32* id, const u16* rank, const u32* seg, int ncell, u32* ids_sorted, cudaStream_t st) {
+  k_export_order<<<(ncell + 127) / 128, 128, 0, st>>>(id, rank, seg, ncell, ids_sorted);
+}
+
+}  // namespace sdm

@@ -1,0 +1,284 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star): multiplicities, ids, order and pairings bit-exact;
+radii, positions, th, rv within 1e-9 relative (fp64); near-tie collision decisions counted."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1310_1905_b200 import workloads as W
+from tests.util import make_oracle, make_particles, np_, sorted_by_id
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-9
+
+
+def binding():
+    from paper_1310_1905_b200 import binding as b
+
+    return b
+
+
+def rain_mix(w, seed=5, frac=0.25):
+    """Give a fraction of the SDs cloud/drizzle/rain sizes so that coalescence and sedimentation act within a
+    few steps (the t = 0 population is all haze), and put some large drops just above the ground."""
+    N = w.n_sd
+    idx = torch.arange(N, dtype=torch.int64)
+    u = W.hash_uniform(seed, 101, idx)
+    v = W.hash_uniform(seed, 102, idx)
+    big = u < frac
+    r = torch.exp(np.log(3e-6) + v * (np.log(400e-6) - np.log(3e-6)))
+    rw2 = torch.where(big, r * r, w.state["rw2"])
+    w.state["rw2"] = torch.maximum(rw2, (w.state["rd3"] ** (1.0 / 3.0)) ** 2 * 1.0001)
+    # rain-sized SDs carry far fewer real drops
+    w.state["n"] = torch.where(big, torch.clamp(w.state["n"] // 1000, min=1), w.state["n"])
+    if w.state["z"] is not None:
+        low = W.hash_uniform(seed, 103, idx) < 0.02
+        w.state["z"] = torch.where(low & big, w.state["z"] * 0.002, w.state["z"])
+    return w
+
+
+def compare_states(p, o, positions=True, rtol=RTOL):
+    g = sorted_by_id(p.export_state())
+    r = sorted_by_id(o.get_state())
+    assert len(g["id"]) == len(r["id"])
+    np.testing.assert_array_equal(g["id"].astype(np.uint32), r["id"])
+    np.testing.assert_array_equal(g["n"].astype(np.uint64), r["n"])      # multiplicities: bit-exact
+    live = r["n"] > 0
+    np.testing.assert_allclose(np.sqrt(g["rw2"]), np.sqrt(r["rw2"]), rtol=rtol)
+    np.testing.assert_allclose(np.cbrt(g["rd3"]), np.cbrt(r["rd3"]), rtol=rtol)
+    np.testing.assert_allclose(g["kappa"], r["kappa"], rtol=rtol)
+    if positions:
+        for k, present in zip("xyz", p.dims):
+            if present:
+                np.testing.assert_allclose(g[k][live], r[k][live], rtol=rtol, atol=1e-9)
+    return g, r
+
+
+def compare_fields(th, rv, o, rtol=RTOL):
+    oth, orv = o.get_fields()
+    np.testing.assert_allclose(np_(th).ravel(), oth, rtol=rtol)
+    np.testing.assert_allclose(np_(rv).ravel(), orv, rtol=rtol)
+
+
+def run_both(w, steps, group=0, opts=None, check_every=1, **override):
+    b = binding()
+    kw = dict(w.opts)
+    kw.update(opts or {})
+    o = make_oracle(w, threads=4, **override)
+    p, th, rv = make_particles(w, **override)
+    if group:
+        p.set_group_size(group)
+    oo, po = oracle.make_opts(**kw), b.make_opts(**kw)
+    for s in range(steps):
+        fo = o.step(oo)
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+        fp = p.step_async_result()
+        np.testing.assert_allclose(fp, fo, rtol=1e-12, atol=1e-300)
+        if (s + 1) % check_every == 0 or s == steps - 1:
+            compare_states(p, o, positions=True)
+            compare_fields(th, rv, o)
+    return p, o, th, rv
+
+
+# ----------------------------------------------------------------------------------------------- sort
+@pytest.mark.parametrize("group", [0, 4, 8, 16, 32, 256])
+def test_sort_permutation_and_segments_are_exact(group):
+    """a0-a2: compaction + (cell, Philox key, id) order identical to std::sort on the tuple."""
+    b = binding()
+    w = W.cfg2_2d(sd_per_cell=20, nx=23, nz=17, seed=3)
+    n = w.state["n"].clone()
+    n[::13] = 0   # dead SDs must be compacted away
+    w.state["n"] = n
+    w.state["id"] = torch.flip(w.state["id"], [0]).contiguous()   # ids unrelated to storage order
+    o = make_oracle(w)
+    p, th, rv = make_particles(w)
+    if group:
+        p.set_group_size(group)
+    for step in (0, 5):
+        o.set_step(step)
+        p.set_step(step)
+        o.stage("sort")
+        po = b.make_opts(adve=False, sedi=False, cond=False, coal=False)
+        p.step_sync(po, th, rv)
+        ids, seg = p.export_order()
+        oids, oseg = o.get_order()
+        np.testing.assert_array_equal(np_(seg).astype(np.int64), oseg)
+        np.testing.assert_array_equal(np_(ids).astype(np.uint32), oids)
+        assert p.n_sd() == o.n_sd() == int((n != 0).sum())
+        p.step_async(po)
+        o.step_async(oracle.make_opts(adve=False, sedi=False, cond=False, coal=False))
+    assert p.stats()["max_cell_count"] == np.diff(oseg).max()
+
+
+# ----------------------------------------------------------------------------------------------- box
+def test_box_golovin_trajectory_bit_exact_multiplicities():
+    """configs[0]: 2^13 SDs in one cell, Golovin kernel, coalescence only."""
+    w = W.box_golovin(seed=42)
+    p, o, _, _ = run_both(w, 400, check_every=100)
+    sp, so = p.stats(), o.counters()
+    assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"] and so["collisions"] > 1000
+    assert sp["near_ties"] == so["near_ties"] and so["near_ties"] <= 1e-6 * so["pairs"] + 1
+    assert p.n_sd() == o.n_sd() < w.n_sd
+
+
+# ----------------------------------------------------------------------------------------------- full step
+@pytest.mark.parametrize("group", [0, 8, 32, 256])
+def test_full_step_2d_single_and_few_steps(group):
+    w = rain_mix(W.cfg2_2d(sd_per_cell=32, nx=20, nz=24, seed=11))
+    p, o, th, rv = run_both(w, 4, group=group)
+    sp, so = p.stats(), o.counters()
+    assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"] and so["collisions"] > 50
+    assert sp["ill_posed"] == so["ill_posed"]
+    assert sp["sd_substeps"] == so["sd_substeps"]
+    assert o.rain_flux_total() > 0 and p.n_sd() < w.n_sd   # sedimentation removed SDs, compaction followed
+
+
+def test_trajectory_2d_30_steps():
+    w = rain_mix(W.cfg2_2d(sd_per_cell=16, nx=16, nz=16, seed=2))
+    p, o, th, rv = run_both(w, 30, check_every=10)
+    sp, so = p.stats(), o.counters()
+    assert sp["collisions"] == so["collisions"] and sp["ill_posed"] == so["ill_posed"]
+    assert so["near_ties"] <= 1e-6 * so["pairs"] + 1
+
+
+def test_full_step_3d():
+    w = rain_mix(W.cfg4_3d(sd_per_cell=64, nx=6, ny=5, nz=16, seed=4))
+    p, o, th, rv = run_both(w, 3)
+    assert p.stats()["collisions"] == o.counters()["collisions"] > 0
+
+
+def test_hydro_tab_kernel_and_paper_variant_without_multiple_coalescence():
+    w = rain_mix(W.cfg3_2d_drizzle(sd_per_cell=48, nx=10, nz=12, seed=6))
+    run_both(w, 3)
+    run_both(w, 2, multi_coal=False)
+
+
+def test_coalescence_substeps_reshuffle():
+    """sstp_coal > 1: new keys and a new sort inside the cell every substep, dead SDs dropped (:624)."""
+    w = rain_mix(W.cfg2_2d(sd_per_cell=40, nx=8, nz=8, seed=9), frac=0.6)
+    for group in (0, 256):
+        p, o, _, _ = run_both(w, 3, group=group, opts=dict(sstp_coal=4, cond=False))
+        assert p.stats()["collisions"] == o.counters()["collisions"] > 100
+
+
+def test_process_toggles():
+    w = rain_mix(W.cfg2_2d(sd_per_cell=16, nx=8, nz=8, seed=10))
+    for opts in (dict(adve=True, sedi=False, cond=False, coal=False), dict(adve=False, sedi=True, cond=False, coal=False),
+                 dict(adve=False, sedi=False, cond=True, coal=False), dict(adve=False, sedi=False, cond=False, coal=True),
+                 dict(adve=False, sedi=False, cond=False, coal=False)):
+        run_both(w, 2, opts=opts)
+
+
+def test_crowded_cells_fall_back_to_global_memory_paths():
+    """One cell with far more SDs than shared memory can stage: condensation and coalescence run in place."""
+    w = rain_mix(W.cfg2_2d(sd_per_cell=1500, nx=2, nz=3, seed=12), frac=0.3)
+    w.state["x"] = w.state["x"] * 0.4   # crowd everything into the first column: 3 cells with ~3000 SDs
+    p, o, _, _ = run_both(w, 2, group=32, opts=dict(sstp_cond=2))
+    assert p.stats()["max_cell_count"] > 2500
+
+
+# ----------------------------------------------------------------------------------------------- API
+def test_strided_fields_and_optional_arguments():
+    """arrinfo_t strides (:730-745): halo-padded, non-contiguous th/rv/rhod give the same result."""
+    b = binding()
+    w = rain_mix(W.cfg2_2d(sd_per_cell=16, nx=9, nz=7, seed=13))
+    p1, th1, rv1 = make_particles(w)
+    p2, _, _ = make_particles(w)
+    pad_th = torch.full((9 + 4, 7 + 6), -1.0, dtype=torch.float64, device="cuda")
+    pad_rv = torch.full((7 + 2, 9 + 2), -1.0, dtype=torch.float64, device="cuda")   # transposed storage
+    th2 = pad_th[2:-2, 3:-3]
+    rv2 = pad_rv[1:-1, 1:-1].t()
+    th2.copy_(w.th.cuda())
+    rv2.copy_(w.rv.cuda())
+    rhod_pad = torch.zeros((9, 2 * 7), dtype=torch.float64, device="cuda")
+    rhod2 = rhod_pad[:, ::2]
+    rhod2.copy_(w.rhod.cuda())
+    po = b.make_opts(**w.opts)
+    for _ in range(2):
+        p1.step_sync(po, th1, rv1)
+        p1.step_async(po)
+        p2.step_sync(po, th2, rv2, rhod=rhod2)
+        p2.step_async(po)
+    assert torch.equal(th1, th2) and torch.equal(rv1, rv2)
+    assert pad_th[0, 0] == -1 and pad_th[-1, -1] == -1 and pad_rv[0, 0] == -1   # halo untouched
+    a, c = sorted_by_id(p1.export_state()), sorted_by_id(p2.export_state())
+    for k in a:
+        np.testing.assert_array_equal(a[k], c[k])
+
+
+def test_step_host_matches_device_path():
+    b = binding()
+    w = rain_mix(W.cfg2_2d(sd_per_cell=16, nx=9, nz=7, seed=14))
+    p1, th1, rv1 = make_particles(w)
+    p2, _, _ = make_particles(w)
+    th_h, rv_h = w.th.clone().pin_memory(), w.rv.clone().pin_memory()
+    po = b.make_opts(**w.opts)
+    for _ in range(3):
+        p1.step_sync(po, th1, rv1)
+        p1.step_async(po)
+        f1 = p1.step_async_result()
+        f2 = p2.step_host(po, th_h, rv_h)
+        assert f1 == f2
+    assert torch.equal(th1.cpu(), th_h) and torch.equal(rv1.cpu(), rv_h)
+
+
+def test_diagnostics_match_oracle():
+    w = rain_mix(W.cfg2_2d(sd_per_cell=24, nx=11, nz=9, seed=15))
+    p, o, th, rv = run_both(w, 2)
+    np.testing.assert_array_equal(np_(p.diag_sd_conc()).ravel(), o.diag_sd_conc())
+    for lo, hi in ((0.5e-6, 25e-6), (25e-6, 1.0), (0.0, 1.0)):   # thresholds of PAPER.md :862
+        p.diag_wet_rng(lo, hi)
+        for k in (0, 3):
+            np.testing.assert_allclose(np_(p.diag_wet_mom(k)).ravel(), o.diag_mom(1, lo, hi, k), rtol=1e-12)
+    p.diag_dry_rng(10e-9, 1e-6)
+    np.testing.assert_allclose(np_(p.diag_dry_mom(1)).ravel(), o.diag_mom(0, 10e-9, 1e-6, 1), rtol=1e-12)
+
+
+def test_edge_cases_empty_single_and_errors():
+    b = binding()
+    w = W.cfg2_2d(sd_per_cell=4, nx=4, nz=4, seed=16)
+    po = b.make_opts(**w.opts)
+    # empty population
+    e = W.cfg2_2d(sd_per_cell=4, nx=4, nz=4, seed=16)
+    e.state = {k: (None if v is None else v[:0]) for k, v in e.state.items()}
+    p, th, rv = make_particles(e, max_sd=8)
+    for _ in range(2):
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+    assert p.step_async_result() == 0.0 and p.n_sd() == 0 and torch.equal(th.cpu(), w.th)
+    assert np_(p.diag_sd_conc()).sum() == 0
+    # a single SD
+    s = W.cfg2_2d(sd_per_cell=4, nx=4, nz=4, seed=16)
+    s.state = {k: (None if v is None else v[:1].clone()) for k, v in s.state.items()}
+    run_both(s, 2)
+    # errors, not UB
+    p, th, rv = make_particles(w)
+    with pytest.raises(b.SdmError, match="step_sync of this step"):
+        p.step_async(po)
+    p.step_sync(po, th, rv)
+    with pytest.raises(b.SdmError, match="called twice"):
+        p.step_sync(po, th, rv)
+    with pytest.raises(b.SdmError, match="exceeds max_sd"):
+        make_particles(w, max_sd=w.n_sd - 1)
+    with pytest.raises(b.SdmError, match="real_bytes|max_sd"):
+        b.Particles(nx=2, nz=2, max_sd=0)
+
+
+def test_runs_are_reproducible_bit_for_bit():
+    """Storage order inside a cell depends on atomics, results must not."""
+    b = binding()
+    w = rain_mix(W.cfg2_2d(sd_per_cell=32, nx=12, nz=12, seed=17))
+    outs = []
+    for _ in range(2):
+        p, th, rv = make_particles(w)
+        po = b.make_opts(**w.opts)
+        for _ in range(3):
+            p.step_sync(po, th, rv)
+            p.step_async(po)
+        outs.append((sorted_by_id(p.export_state()), th.clone(), rv.clone()))
+    for k in outs[0][0]:
+        np.testing.assert_array_equal(outs[0][0][k], outs[1][0][k])
+    assert torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])

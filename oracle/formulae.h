@@ -149,7 +149,9 @@ inline double cond_substep_sd(double y0, double rd3, double kappa, const CellThe
   if (ga == 0.0) return a;
   if (gb == 0.0) return b;
   if ((ga > 0.0) == (gb > 0.0)) {          // :579 bisection ill-posed -> (a+b)/2
-    if (ill_posed) *ill_posed = 1;
+    // counted only when the bracket is wider than 1e-9 b: below that the sign of g at the far end is
+    // rounding noise of f and either branch returns the same value to 1e-9
+    if (ill_posed) *ill_posed = (b - a > 1e-9 * b) ? 1 : 0;
     return 0.5 * (a + b);
   }
   while (b - a > 1e-15 * b) {               // bisection

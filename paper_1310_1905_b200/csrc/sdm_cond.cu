@@ -115,7 +115,7 @@ __device__ __forceinline__ double cond_solve(double y0, double rd2, double rd3, 
         ++n_eval;
         const double gb = b - y0 - dtp * fb;
         if (gb == 0.0) return b;
-        if (gb < 0.0) { ++n_ill; return 0.5 * (a + b); }   // :579
+        if (gb < 0.0) { n_ill += (b - a > 1e-9 * b); return 0.5 * (a + b); }   // :579; counted when wider than noise
         hi_unv = false;
       } else if (g > 0.0 && lo_unv) {
         double fa, dfa;
@@ -123,7 +123,7 @@ __device__ __forceinline__ double cond_solve(double y0, double rd2, double rd3, 
         ++n_eval;
         const double ga = a - y0 - dtp * fa;
         if (ga == 0.0) return a;
-        if (ga > 0.0) { ++n_ill; return 0.5 * (a + b); }
+        if (ga > 0.0) { n_ill += (b - a > 1e-9 * b); return 0.5 * (a + b); }
         lo_unv = false;
       }
       yn = 0.5 * (lo + hi);

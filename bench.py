@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py -- super-droplet-steps/s of the full particle step (sort + cond x10 + coal + adve/sedi +
+compaction) on the 3D prescribed-flow configuration of BASELINE.json (configs[3]: 128x128x64 cells,
+64 SD/cell, 67M SDs, fp64), one process per GPU.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 3d|2d|sweep]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the oracle (a deliberately plain CPU program)
+on a bounded sample of the same workload.  See DESIGN.md "Measurement" for every definition used here.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "super-droplet-steps/s (sort+coal+cond+sedi)"
+UNIT = "SD-steps/s"
+
+# Algorithmic work per unit:
+#  - whole step, fp64, 3D: 350 B of HBM traffic per SD-step;
+#  - condensation kernel: fp64 operations per growth-rate evaluation and per SD-substep set-up, counted
+#    from the formulae (an FMA counts 2; a division, sqrt, rsqrt, exp, cbrt count as the length of their
+#    fp64 instruction sequences).
+BYTES_PER_SD_STEP = {3: 350.0, 2: 350.0 - 16.0 - 8.0}
+FLOP_PER_EVAL = 190.0
+FLOP_PER_SETUP = 150.0
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="3d", choices=["3d", "2d", "sweep"])
+    ap.add_argument("--sd-per-cell", type=int, default=0)
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the horizontal grid (debugging only; reported in config)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--group", type=int, default=0)
+    return ap.parse_args()
+
+
+def workload_args(a):
+    if a.workload == "3d":
+        n = max(int(round(128 * a.scale)), 2)
+        return dict(kind="3d", nx=n, ny=n, nz=64, sd=a.sd_per_cell or 64)
+    if a.workload == "2d":
+        return dict(kind="2d", nx=75, ny=0, nz=75, sd=a.sd_per_cell or 128)
+    return dict(kind="sweep", nx=256, ny=0, nz=256, sd=a.sd_per_cell or 128)
+
+
+def make_workload(wa, seed, device):
+    from paper_1310_1905_b200 import workloads as W
+
+    if wa["kind"] == "3d":
+        return W.cfg4_3d(sd_per_cell=wa["sd"], nx=wa["nx"], ny=wa["ny"], nz=wa["nz"], seed=seed, device=device)
+    if wa["kind"] == "2d":
+        return W.cfg3_2d_drizzle(sd_per_cell=wa["sd"], seed=seed, device=device)
+    return W.cfg5_sweep(wa["sd"], seed=seed, device=device)
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def oracle_rate(wa, steps, warmup, seed=42):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload: a block of full
+    columns of the same recipe (same vertical profile, same SD/cell), OpenMP over cells."""
+    import oracle
+    from tests.util import make_oracle
+
+    nx = 8 if wa["kind"] == "3d" else 16
+    sub = dict(wa)
+    sub.update(nx=nx, ny=(4 if wa["kind"] == "3d" else 0))
+    if wa["kind"] != "3d":
+        sub["nz"] = min(wa["nz"], 75)
+    from paper_1310_1905_b200 import workloads as W
+
+    if wa["kind"] == "3d":
+        w = W.cfg4_3d(sd_per_cell=wa["sd"], nx=sub["nx"], ny=sub["ny"], nz=sub["nz"], seed=seed)
+    elif wa["kind"] == "2d":
+        w = W.cfg3_2d_drizzle(sd_per_cell=wa["sd"], nx=sub["nx"], nz=sub["nz"], seed=seed)
+    else:
+        w = W.kinematic(sub["nx"], 0, wa["nz"], 1500.0 / wa["nz"], wa["sd"], seed=seed)
+    cores = oracle.lib().orc_max_threads()
+    o = make_oracle(w, threads=cores)
+    oo = oracle.make_opts(**w.opts)
+    for _ in range(warmup):
+        o.step(oo)
+    n, t0 = 0, time.perf_counter()
+    for _ in range(steps):
+        n += o.n_live()
+        o.step(oo)
+    dt = time.perf_counter() - t0
+    desc = (f"{w.name}: {w.n_sd} SDs in {sub['nx']}x{max(sub['ny'], 1)}x{sub['nz']} full columns of the same recipe, "
+            f"{steps} steps after {warmup} warm-up, OpenMP over cells")
+    return n / dt, cores, desc, dt / steps * 1e3
+
+
+def run_reference(a, wa):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(a.steps, 3))
+    warm = max(1, min(a.warmup, 1))
+    v, cores, desc, ms = oracle_rate(wa, steps, warm)
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": steps, "warmup": warm,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": config_of(wa), "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def config_of(wa):
+    return {"workload": f"{wa['kind']} prescribed-flow {wa['nx']}x{max(wa['ny'], 1)}x{wa['nz']} cells, {wa['sd']} SD/cell, "
+                        "bimodal lognormal aerosol (kappa=0.61), sort+cond(10 substeps)+coal+adve+sedi+compaction, dt=1 s, RH_max=1.05",
+            "n_sd_per_gpu": wa["nx"] * max(wa["ny"], 1) * wa["nz"] * wa["sd"],
+            "l2": "state (60 B/SD) far exceeds the 126 MB L2; no flush needed",
+            "parallelism": "independent replicas (single-GPU path, no collective)"}
+
+
+def main():
+    a = parse()
+    wa = workload_args(a)
+    if a.impl == "reference":
+        return run_reference(a, wa)
+
+    import torch
+    import torch.distributed as dist
+
+    from paper_1310_1905_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = f"cuda:{local}"
+
+    w = make_workload(wa, seed=42 + rank, device=dev)
+    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], **w.init)
+    s = w.state
+    cs = list(w.courants) + [None] * (3 - len(w.courants))
+    p.init_from_arrays(w.rhod, s["n"], s["rw2"], s["rd3"], s["kappa"], s["x"], s["y"], s["z"], s["id"], courant_1=cs[0],
+                       courant_2=cs[1], courant_3=cs[2])
+    n_sd0 = w.n_sd
+    th, rv = w.th.clone(), w.rv.clone()
+    ndim = 3 if wa["ny"] > 0 else 2
+    del w, s
+    torch.cuda.empty_cache()
+    if a.group:
+        p.set_group_size(a.group)
+    po = binding.make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=1.05, sstp_cond=10, sstp_coal=1)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def one_step():
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+
+    for _ in range(max(a.warmup, 3)):
+        one_step()
+    # ---- device-resident timing ------------------------------------------------------------------
+    p.set_timing(True)
+    p.stage_times(reset=True)
+    st0 = p.stats()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sd_steps = 0
+    ev0.record()
+    for _ in range(a.steps):
+        p.step_sync(po, th, rv)
+        sd_steps += p.n_sd()      # live SDs of this step (host-known after the sort, no extra sync)
+        p.step_async(po)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    st1 = p.stats()
+    stages = p.stage_times(reset=True)
+    p.set_timing(False)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    tot = torch.tensor([float(sd_steps)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms_max, sd_total = float(t.item()), float(tot.item())
+    value = sd_total / (ms_max * 1e-3)
+
+    # ---- end to end: Eulerian fields in (pinned) host memory, copied in and out every step ---------
+    th_h, rv_h = th.cpu().pin_memory(), rv.cpu().pin_memory()
+    p.step_host(po, th_h, rv_h)
+    barrier()
+    e_sd, t0 = 0, time.perf_counter()
+    for _ in range(a.steps):
+        e_sd += p.n_sd()
+        p.step_host(po, th_h, rv_h)
+    torch.cuda.synchronize()
+    e_dt = time.perf_counter() - t0
+    et = torch.tensor([e_dt], dtype=torch.float64, device=dev)
+    etot = torch.tensor([float(e_sd)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(et, op=dist.ReduceOp.MAX)
+        dist.all_reduce(etot, op=dist.ReduceOp.SUM)
+    ncell = th.numel()
+    e2e = {"value": float(etot.item()) / float(et.item()), "unit": UNIT, "h2d_bytes_per_step": 2 * ncell * 8,
+           "d2h_bytes_per_step": 2 * ncell * 8 + 8, "api": "sdm_step_host (th, rv in pinned host memory)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (condensation), measured live ---------------------------
+    hbm_peak, peak_src = peaks()
+    cond_ms, cond_n = stages["cond"]
+    evals = st1["newton_iters"] - st0["newton_iters"]
+    subs = st1["sd_substeps"] - st0["sd_substeps"]
+    flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP
+    ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
+    stage_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in stages.items()}
+    step_ms = ms / a.steps
+    roofline = {"kernel": "k_cond (condensation, 10 fused substeps)", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                "evals_per_sd_substep": evals / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
+                "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms}
+    bytes_step = BYTES_PER_SD_STEP[ndim] * (sd_steps / a.steps)
+    hbm = {"bound": "hbm", "achieved": bytes_step / (step_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+           "frac": bytes_step / (step_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
+           "algorithmic_bytes_per_sd_step": BYTES_PER_SD_STEP[ndim]}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+           "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": config_of(wa), "clocks": clocks, "e2e": e2e,
+           "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm,
+           "stage_ms": stage_ms, "n_sd_live": p.n_sd(), "n_sd_initial": n_sd0}
+    if not a.no_cpu_baseline:
+        v, cores, desc, _ = oracle_rate(wa, 2, 1)
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

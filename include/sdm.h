@@ -156,6 +156,21 @@ int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double
 int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, void* stream);
 /* Counters (blocking: synchronises the context's last stream). */
 int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out);
+/* Per-stage device timing.  With timing enabled every stage of step_sync / step_async is bracketed by
+ * CUDA events on the launching stream.  sdm_stage_times synchronises that stream and returns, per
+ * sdm_stage, the summed elapsed milliseconds and the number of timed launches since the last reset
+ * (ms and launches: HOST arrays of SDM_N_STAGES elements; launches may be NULL). */
+typedef enum {
+  SDM_STAGE_HIST = 0,      /* a0-a1: cell index + histogram (compaction) */
+  SDM_STAGE_SCAN = 1,      /* a2: segment offsets */
+  SDM_STAGE_SCATTER = 2,   /* a3: reorder the state by cell */
+  SDM_STAGE_RANK = 3,      /* a2: (Philox key, id) order inside each cell */
+  SDM_STAGE_COND = 4,      /* a4: condensation substeps */
+  SDM_STAGE_COAL_MOVE = 5, /* a5-a6: coalescence + advection + sedimentation */
+  SDM_N_STAGES = 6
+} sdm_stage;
+int sdm_set_timing(sdm_ctx* ctx, int enable);
+int sdm_stage_times(sdm_ctx* ctx, double* ms, uint64_t* launches, int reset);
 /* Overrides the step counter used in the Philox counters (restart from a checkpoint, parity). */
 int sdm_set_step(sdm_ctx* ctx, uint64_t step);
 /* Tuning override for tests: threads cooperating on one cell in the cell-resident kernels

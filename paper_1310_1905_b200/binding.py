@@ -48,7 +48,9 @@ class Stats(C.Structure):
 EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
-           "sdm_stats", "sdm_set_step", "sdm_set_group_size"]
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_timing", "sdm_stage_times"]
+
+STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move")
 
 _lib = None
 
@@ -85,6 +87,8 @@ def load_library():
     L.sdm_stats.argtypes = [vp, C.POINTER(Stats)]
     L.sdm_set_step.argtypes = [vp, C.c_uint64]
     L.sdm_set_group_size.argtypes = [vp, C.c_int]
+    L.sdm_set_timing.argtypes = [vp, C.c_int]
+    L.sdm_stage_times.argtypes = [vp, C.POINTER(C.c_double), u64p, C.c_int]
     _lib = L
     return L
 
@@ -234,6 +238,16 @@ class Particles:
 
     def set_group_size(self, g):
         self._ck(self.L.sdm_set_group_size(self.h, g))
+
+    def set_timing(self, enable=True):
+        self._ck(self.L.sdm_set_timing(self.h, int(enable)))
+
+    def stage_times(self, reset=True):
+        """{stage: (milliseconds, timed launches)} since the last reset (synchronises the stream)."""
+        ms = (C.c_double * len(STAGES))()
+        cnt = (C.c_uint64 * len(STAGES))()
+        self._ck(self.L.sdm_stage_times(self.h, ms, cnt, int(reset)))
+        return {s: (ms[k], cnt[k]) for k, s in enumerate(STAGES)}
 
 
 def _as_tensor(ptr, n):

@@ -48,6 +48,12 @@ struct sdm_ctx {
   cudaStream_t last_stream = nullptr;
   u64 launches = 0;
   double dry_lo = 0, dry_hi = 1e300, wet_lo = 0, wet_hi = 1e300;
+  // optional per-stage timing with CUDA events on the launching stream (sdm_set_timing)
+  bool timing = false;
+  std::vector<cudaEvent_t> tev[SDM_N_STAGES];   // start/stop pairs not yet folded into t_ms
+  double t_ms[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0};
+  uint64_t t_cnt[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0};
+  std::vector<cudaEvent_t> ev_pool;
   std::string err;
 };
 
@@ -91,6 +97,36 @@ int copy_courants(sdm_ctx* ctx, const sdm_arrinfo* comps, cudaStream_t st) {
   }
   CK(cudaGetLastError());
   return SDM_OK;
+}
+
+// stage timers: t_begin/t_end bracket the launches of one stage with events on the stream
+void t_begin(sdm_ctx* c, int stage, cudaStream_t st) {
+  if (!c->timing) return;
+  cudaEvent_t e;
+  if (!c->ev_pool.empty()) { e = c->ev_pool.back(); c->ev_pool.pop_back(); }
+  else if (cudaEventCreate(&e) != cudaSuccess) return;
+  cudaEventRecord(e, st);
+  c->tev[stage].push_back(e);
+}
+void t_end(sdm_ctx* c, int stage, cudaStream_t st) {
+  if (!c->timing || (c->tev[stage].size() & 1) == 0) return;
+  cudaEvent_t e;
+  if (!c->ev_pool.empty()) { e = c->ev_pool.back(); c->ev_pool.pop_back(); }
+  else if (cudaEventCreate(&e) != cudaSuccess) { c->ev_pool.push_back(c->tev[stage].back()); c->tev[stage].pop_back(); return; }
+  cudaEventRecord(e, st);
+  c->tev[stage].push_back(e);
+}
+void t_fold(sdm_ctx* c) {   // caller has synchronised the stream
+  for (int s = 0; s < SDM_N_STAGES; ++s) {
+    auto& v = c->tev[s];
+    for (size_t k = 0; k + 1 < v.size(); k += 2) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, v[k], v[k + 1]) == cudaSuccess) { c->t_ms[s] += ms; c->t_cnt[s]++; }
+    }
+    for (cudaEvent_t e : v) c->ev_pool.push_back(e);
+    v.clear();
+  }
+  cudaGetLastError();
 }
 
 int pick_group(const sdm_ctx* c, double mean) {
@@ -222,6 +258,8 @@ void sdm_destroy(sdm_ctx* ctx) {
   if (ctx->h_info) cudaFreeHost(ctx->h_info);
   if (ctx->ev_info) cudaEventDestroy(ctx->ev_info);
   if (ctx->ev_async) cudaEventDestroy(ctx->ev_async);
+  for (int q = 0; q < SDM_N_STAGES; ++q) for (cudaEvent_t e : ctx->tev[q]) cudaEventDestroy(e);
+  for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
   cudaGetLastError();
   delete ctx;
 }
@@ -281,12 +319,18 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   u32* d_cur = ctx->d_info + ctx->cn;
   u32* d_next = ctx->d_info + (ctx->cn ^ 1);
   CK(cudaMemsetAsync(ctx->d_info + 2, 0, sizeof(u32), st));
+  t_begin(ctx, SDM_STAGE_HIST, st);
   launch_cellhist(ctx->buf[ctx->cur], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+  t_end(ctx, SDM_STAGE_HIST, st);
+  t_begin(ctx, SDM_STAGE_SCAN, st);
   launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
+  t_end(ctx, SDM_STAGE_SCAN, st);
   ctx->launches += (ctx->nslots ? 1 : 0) + 3;
   CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 4 * sizeof(u32), cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(ctx->ev_info, st));
+  t_begin(ctx, SDM_STAGE_SCATTER, st);
   launch_scatter(ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
+  t_end(ctx, SDM_STAGE_SCATTER, st);
   ctx->launches += ctx->nslots ? 1 : 0;
   CK(cudaGetLastError());
   CK(cudaEventSynchronize(ctx->ev_info));   // the scatter runs while the host sizes the next launches
@@ -306,8 +350,10 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   ctx->G = G;
   const Field thf = make_field(ctx, th), rvf = make_field(ctx, rv);
   if (ctx->nslots) {
+    t_begin(ctx, SDM_STAGE_RANK, st);
     CK(launch_rank(G, ctx->buf[ctx->cur].id, ctx->seg, g.ncell, (u32)ctx->step, ctx->kp.seed_lo, ctx->kp.seed_hi, P,
                    ctx->rank, (int*)(ctx->d_info + 3), st));
+    t_end(ctx, SDM_STAGE_RANK, st);
     ctx->launches++;
   }
   ctx->have_order = true;
@@ -316,7 +362,9 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     cap = std::max(cap, 4);
     if (cond_smem_bytes(G, cap) > kSmemLimit) cap = 0;   // work in place in HBM/L2
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max};
+    t_begin(ctx, SDM_STAGE_COND, st);
     CK(launch_cond(G, cap, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
+    t_end(ctx, SDM_STAGE_COND, st);
   } else {
     launch_thermo(g, thf, rvf, ctx->cf, st);
     CK(cudaGetLastError());
@@ -342,8 +390,10 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
       return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
     CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step};
+    t_begin(ctx, SDM_STAGE_COAL_MOVE, st);
     CK(launch_coal_move(G, cap, in_smem, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
                         ctx->cnt, st));
+    t_end(ctx, SDM_STAGE_COAL_MOVE, st);
     ctx->launches++;
   }
   launch_flux_sum(ctx->flux_slots, ctx->d_flux, ctx->d_flux + 1, st);
@@ -460,6 +510,24 @@ int sdm_set_step(sdm_ctx* ctx, uint64_t step) {
   if (!ctx) return SDM_ERR_INVALID;
   if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_set_step: not between step_sync and step_async");
   ctx->step = step;
+  return SDM_OK;
+}
+
+int sdm_set_timing(sdm_ctx* ctx, int enable) {
+  if (!ctx) return SDM_ERR_INVALID;
+  ctx->timing = enable != 0;
+  return SDM_OK;
+}
+
+int sdm_stage_times(sdm_ctx* ctx, double* ms, uint64_t* launches, int reset) {
+  if (!ctx || !ms) return SDM_ERR_INVALID;
+  CK(cudaStreamSynchronize(ctx->last_stream));
+  t_fold(ctx);
+  for (int q = 0; q < SDM_N_STAGES; ++q) {
+    ms[q] = ctx->t_ms[q];
+    if (launches) launches[q] = ctx->t_cnt[q];
+    if (reset) { ctx->t_ms[q] = 0; ctx->t_cnt[q] = 0; }
+  }
   return SDM_OK;
 }
 

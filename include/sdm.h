@@ -89,6 +89,7 @@ typedef struct {
   uint64_t ill_posed;       /* condensation: SD-substeps that took the bracket branch of PAPER.md :579 */
   uint64_t newton_iters;    /* condensation: growth-rate evaluations (summed) */
   uint64_t sd_substeps;     /* condensation: SD-substeps solved */
+  uint64_t cond_slow;       /* condensation: SD-substeps deferred to the second (compacted) solver pass */
 } sdm_stats_t;
 
 /* factory() of Listing 5.7 (:800-808).  Allocates all device memory for max_sd super-droplets on
@@ -176,6 +177,9 @@ int sdm_set_step(sdm_ctx* ctx, uint64_t step);
 /* Tuning override for tests: threads cooperating on one cell in the cell-resident kernels
  * (0 = automatic; 4, 8, 16, 32 = sub-warp groups; 256 = one CTA per cell). */
 int sdm_set_group_size(sdm_ctx* ctx, int group);
+/* Tuning override: growth-rate evaluations the dense condensation sweep spends on an SD before deferring it
+ * to the compacted second pass (1..200, default 4).  Does not change results beyond the solver tolerance. */
+int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast);
 
 #ifdef __cplusplus
 }

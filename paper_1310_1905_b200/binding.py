@@ -42,13 +42,13 @@ class ArrInfo(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("n_sd", "max_cell_count", "step", "kernel_launches", "pairs", "collisions",
-                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps")]
+                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow")]
 
 
 EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
-           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_timing", "sdm_stage_times"]
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move")
 
@@ -87,6 +87,7 @@ def load_library():
     L.sdm_stats.argtypes = [vp, C.POINTER(Stats)]
     L.sdm_set_step.argtypes = [vp, C.c_uint64]
     L.sdm_set_group_size.argtypes = [vp, C.c_int]
+    L.sdm_set_cond_kfast.argtypes = [vp, C.c_int]
     L.sdm_set_timing.argtypes = [vp, C.c_int]
     L.sdm_stage_times.argtypes = [vp, C.POINTER(C.c_double), u64p, C.c_int]
     _lib = L
@@ -238,6 +239,9 @@ class Particles:
 
     def set_group_size(self, g):
         self._ck(self.L.sdm_set_group_size(self.h, g))
+
+    def set_cond_kfast(self, kfast):
+        self._ck(self.L.sdm_set_cond_kfast(self.h, kfast))
 
     def set_timing(self, enable=True):
         self._ck(self.L.sdm_set_timing(self.h, int(enable)))

@@ -13,6 +13,9 @@ using namespace sdm;
 namespace {
 thread_local std::string g_create_error;
 constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are willing to ask for per CTA
+constexpr size_t kCondSmemTwoCtas = 110 * 1024;   // per CTA, so that two condensation CTAs share an SM
+constexpr double kCondTileTarget = 1792.0;  // SDs per condensation tile (mean); 6 sigma above fits 110 KB
+constexpr double kCondMaxCpb = 256.0;       // one thread per cell of the tile
 }
 
 struct sdm_ctx {
@@ -24,7 +27,7 @@ struct sdm_ctx {
   int cur = 0;
   u32 *cell = nullptr, *off = nullptr, *count = nullptr, *blocksum = nullptr, *seg = nullptr;
   u16* rank = nullptr;
-  u32* d_info = nullptr;     // [0],[1] slot counts (ping-pong), [2] max cell count, [3] error flag
+  u32* d_info = nullptr;     // [0],[1] slot counts (ping-pong), [2] max cell count, [3] error flag, [4..7] tile maxima
   u32* h_info = nullptr;     // pinned mirror
   int cn = 0;                // which of d_info[0..1] is current
   CellFields cf{};
@@ -44,6 +47,8 @@ struct sdm_ctx {
   bool have_order = false;
   int G = 32;                // group size chosen by the last step_sync
   int group_override = 0;
+  int cond_cpb0 = 1;         // candidate cells per condensation tile (halved up to 3 times if a tile overflows)
+  int kfast = 4;
   cudaEvent_t ev_info = nullptr, ev_async = nullptr;
   cudaStream_t last_stream = nullptr;
   u64 launches = 0;
@@ -198,27 +203,28 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   const int nb = scan_num_blocks(g.ncell);
   if ((e = dalloc(&ctx->cell, N)) || (e = dalloc(&ctx->off, N)) || (e = dalloc(&ctx->rank, N)) ||
       (e = dalloc(&ctx->count, (size_t)g.ncell)) || (e = dalloc(&ctx->blocksum, (size_t)nb)) ||
-      (e = dalloc(&ctx->seg, (size_t)g.ncell + 1)) || (e = dalloc(&ctx->d_info, 4)) ||
+      (e = dalloc(&ctx->seg, (size_t)g.ncell + 1)) || (e = dalloc(&ctx->d_info, 8)) ||
       (e = dalloc(&ctx->cf.rhod, (size_t)g.ncell)) || (e = dalloc(&ctx->cf.eta, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->cf.rho_a, (size_t)g.ncell)) || (e = dalloc(&ctx->outbuf, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->th_dense, (size_t)g.ncell)) || (e = dalloc(&ctx->rv_dense, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->cx, (size_t)(g.NX + 1) * g.NY * g.NZ)) || (e = dalloc(&ctx->cy, (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = dalloc(&ctx->cz, (size_t)g.NX * g.NY * (g.NZ + 1))) || (e = dalloc(&ctx->flux_slots, NSLOT)) ||
-      (e = dalloc(&ctx->d_flux, 2)) || (e = dalloc(&ctx->cnt_mem, 6 * NSLOT)))
+      (e = dalloc(&ctx->d_flux, 2)) || (e = dalloc(&ctx->cnt_mem, N_COUNTERS * NSLOT)))
     return bail(e, "scratch");
   ctx->cf.cx = ctx->cx; ctx->cf.cy = ctx->cy; ctx->cf.cz = ctx->cz;
-  if ((e = cudaMallocHost((void**)&ctx->h_info, 4 * sizeof(u32)))) return bail(e, "pinned info");
+  if ((e = cudaMallocHost((void**)&ctx->h_info, 8 * sizeof(u32)))) return bail(e, "pinned info");
   if ((e = cudaMemset(ctx->count, 0, sizeof(u32) * g.ncell)) || (e = cudaMemset(ctx->seg, 0, sizeof(u32) * ((size_t)g.ncell + 1))) ||
-      (e = cudaMemset(ctx->d_info, 0, 4 * sizeof(u32))) ||
+      (e = cudaMemset(ctx->d_info, 0, 8 * sizeof(u32))) ||
       (e = cudaMemset(ctx->cx, 0, sizeof(double) * (size_t)(g.NX + 1) * g.NY * g.NZ)) ||
       (e = cudaMemset(ctx->cy, 0, sizeof(double) * (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = cudaMemset(ctx->cz, 0, sizeof(double) * (size_t)g.NX * g.NY * (g.NZ + 1))) ||
       (e = cudaMemset(ctx->flux_slots, 0, sizeof(double) * NSLOT)) || (e = cudaMemset(ctx->d_flux, 0, 2 * sizeof(double))) ||
-      (e = cudaMemset(ctx->cnt_mem, 0, sizeof(unsigned long long) * 6 * NSLOT)) ||
+      (e = cudaMemset(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT)) ||
       (e = cudaMemset(ctx->outbuf, 0, sizeof(double) * g.ncell)))
     return bail(e, "memset");
   ctx->cnt.pairs = ctx->cnt_mem; ctx->cnt.collisions = ctx->cnt_mem + NSLOT; ctx->cnt.near_ties = ctx->cnt_mem + 2 * NSLOT;
   ctx->cnt.ill_posed = ctx->cnt_mem + 3 * NSLOT; ctx->cnt.f_evals = ctx->cnt_mem + 4 * NSLOT; ctx->cnt.sd_substeps = ctx->cnt_mem + 5 * NSLOT;
+  ctx->cnt.cond_slow = ctx->cnt_mem + 6 * NSLOT;
   CoalParams& kp = ctx->kp;
   kp.kernel = o->kernel; kp.multi_coal = o->multi_coal; kp.golovin_b = o->golovin_b;
   kp.seed_lo = (u32)o->seed; kp.seed_hi = (u32)(o->seed >> 32);
@@ -290,10 +296,10 @@ int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arr
     if (g.hz) CK(cudaMemcpyAsync(a.z, z, N * 8, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpyAsync(a.id, id, N * 4, cudaMemcpyDeviceToDevice, st));
   }
-  const u32 info[4] = {(u32)N, 0u, 0u, 0u};
+  const u32 info[8] = {(u32)N, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
   CK(cudaMemcpyAsync(ctx->d_info, info, sizeof(info), cudaMemcpyHostToDevice, st));
   CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
-  CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * 6 * NSLOT, st));
+  CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT, st));
   CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
   CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
   CK(cudaStreamSynchronize(st));
@@ -319,14 +325,18 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   u32* d_cur = ctx->d_info + ctx->cn;
   u32* d_next = ctx->d_info + (ctx->cn ^ 1);
   CK(cudaMemsetAsync(ctx->d_info + 2, 0, sizeof(u32), st));
+  CK(cudaMemsetAsync(ctx->d_info + 4, 0, 4 * sizeof(u32), st));
+  // condensation tiles: about kCondTileTarget SDs per CTA at the occupancy seen before this step
+  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, kCondTileTarget * g.ncell / std::max<double>(ctx->nslots, 1.0)));
   t_begin(ctx, SDM_STAGE_HIST, st);
   launch_cellhist(ctx->buf[ctx->cur], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
   t_end(ctx, SDM_STAGE_HIST, st);
   t_begin(ctx, SDM_STAGE_SCAN, st);
   launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
   t_end(ctx, SDM_STAGE_SCAN, st);
+  if (op->cond) { launch_tile_max(ctx->seg, g.ncell, ctx->cond_cpb0, ctx->d_info + 4, st); ctx->launches++; }
   ctx->launches += (ctx->nslots ? 1 : 0) + 3;
-  CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 4 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 8 * sizeof(u32), cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(ctx->ev_info, st));
   t_begin(ctx, SDM_STAGE_SCATTER, st);
   launch_scatter(ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
@@ -358,12 +368,19 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   }
   ctx->have_order = true;
   if (op->cond) {
-    int cap = (int)((ctx->max_nc + 3) / 4 * 4);
-    cap = std::max(cap, 4);
-    if (cond_smem_bytes(G, cap) > kSmemLimit) cap = 0;   // work in place in HBM/L2
-    CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max};
+    // largest candidate tile size whose most populated tile fits the shared memory of 2 CTAs per SM; a single
+    // crowded cell may take the whole SM; beyond that the kernel works in place in HBM/L2
+    int cpb = 1, cap = 0;
+    for (int k = 0; k < 4 && cap == 0; ++k) {
+      const int cand = std::max(1, ctx->cond_cpb0 >> k);
+      const int need = std::max(((int)ctx->h_info[4 + k] + 3) / 4 * 4, 4);
+      if (cond_smem_bytes(cand, need) <= (cand > 1 ? kCondSmemTwoCtas : kSmemLimit)) { cpb = cand; cap = need; }
+      if (cand == 1) break;
+    }
+    CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
     t_begin(ctx, SDM_STAGE_COND, st);
-    CK(launch_cond(G, cap, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
+    CK(launch_cond(cpb, cap, ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp,
+                   ctx->cnt, st));
     t_end(ctx, SDM_STAGE_COND, st);
   } else {
     launch_thermo(g, thf, rvf, ctx->cf, st);
@@ -496,13 +513,13 @@ int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, vo
 int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out) {
   if (!ctx || !out) return SDM_ERR_INVALID;
   CK(cudaStreamSynchronize(ctx->last_stream));
-  std::vector<unsigned long long> h(6 * NSLOT);
-  CK(cudaMemcpy(h.data(), ctx->cnt_mem, sizeof(unsigned long long) * 6 * NSLOT, cudaMemcpyDeviceToHost));
-  unsigned long long s[6] = {0, 0, 0, 0, 0, 0};
-  for (int q = 0; q < 6; ++q) for (int t = 0; t < NSLOT; ++t) s[q] += h[(size_t)q * NSLOT + t];
+  std::vector<unsigned long long> h(N_COUNTERS * NSLOT);
+  CK(cudaMemcpy(h.data(), ctx->cnt_mem, sizeof(unsigned long long) * N_COUNTERS * NSLOT, cudaMemcpyDeviceToHost));
+  unsigned long long s[N_COUNTERS] = {0, 0, 0, 0, 0, 0, 0};
+  for (int q = 0; q < N_COUNTERS; ++q) for (int t = 0; t < NSLOT; ++t) s[q] += h[(size_t)q * NSLOT + t];
   out->n_sd = ctx->nslots; out->max_cell_count = ctx->max_nc; out->step = ctx->step; out->kernel_launches = ctx->launches;
   out->pairs = s[0]; out->collisions = s[1]; out->near_ties = s[2]; out->ill_posed = s[3]; out->newton_iters = s[4];
-  out->sd_substeps = s[5];
+  out->sd_substeps = s[5]; out->cond_slow = s[6];
   return SDM_OK;
 }
 
@@ -528,6 +545,13 @@ int sdm_stage_times(sdm_ctx* ctx, double* ms, uint64_t* launches, int reset) {
     if (launches) launches[q] = ctx->t_cnt[q];
     if (reset) { ctx->t_ms[q] = 0; ctx->t_cnt[q] = 0; }
   }
+  return SDM_OK;
+}
+
+int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (kfast < 1 || kfast > 200) return fail(ctx, SDM_ERR_INVALID, "sdm_set_cond_kfast: 1..200");
+  ctx->kfast = kfast;
   return SDM_OK;
 }
 

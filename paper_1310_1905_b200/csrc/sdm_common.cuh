@@ -50,7 +50,9 @@ struct Counters {        // device accumulators, NSLOT spread slots each
   unsigned long long* ill_posed;
   unsigned long long* f_evals;
   unsigned long long* sd_substeps;
+  unsigned long long* cond_slow;
 };
+constexpr int N_COUNTERS = 7;
 struct CoalParams {
   int kernel, multi_coal;
   double golovin_b;

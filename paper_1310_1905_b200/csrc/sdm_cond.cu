@@ -1,42 +1,29 @@
 // Stage a4: condensational growth, all sstp_cond substeps fused in one
-// cell-resident kernel.  A group of G threads owns one grid cell: it stages the cell's SDs in shared
-// memory in sorted order, and per substep (i) diagnoses T, p, rho_vs, RH.. from theta, r_v, rho_d
-// (eq. 43-44, Table 2), (ii) solves eq. 17 for every SD by a bracketed Newton iteration on
-// r_w^2 inside the interval of eq. 18-19 (the paper bisects, :579, and names a faster root finder as
-// the first optimisation, :912), (iii) reduces sum N (r_w^3' - r_w^3) over the cell and applies the
-// feedback of eq. 25-26 to r_v and theta.  fp64 throughout; this kernel is fp64-ALU bound.
+// tile-resident kernel.  A CTA of 256 threads owns a TILE of consecutive grid cells (about 1800
+// super-droplets): the SDs are staged once in shared memory in sorted order and stay there for all
+// substeps.  Per substep
+//   A. one thread per cell applies the feedback of the previous substep (eq. 25-26) and
+//      diagnoses T, p, rho_vs, RH.. from theta, r_v, rho_d (eq. 43-44, Table 2),
+//   B. all threads sweep the tile's SDs DENSELY (lane utilisation does not depend on the cell
+//      populations) and solve eq. 17 by a bracketed Newton iteration on r_w^2 inside the interval of
+//      eq. 18-19 (the paper bisects, :579, and names a faster root finder as the first optimisation,
+//      :912); the sweep spends at most `kfast` growth-rate evaluations per SD,
+//   C. the few SDs that did not converge in B are collected in a list and solved to the end in a second,
+//      again densely packed, pass (so one slow SD does not hold 31 lanes for its whole iteration),
+//   D. one warp per cell sums N (r_w^3' - r_w^3) in sorted order (deterministic) for the next feedback.
+// The solver is a small state machine around ONE inlined growth-rate evaluation, so that lanes of a
+// warp differ only in their trip count.  fp64 throughout; this kernel is fp64-ALU bound.
 #include "sdm_kernels.cuh"
 
 namespace sdm {
 
-struct CellC {   // per-cell constants of one substep
-  double RH, A, c0, lD, lK, heat, eta, rho_a, Sc, Pr, T, lv;
-};
+constexpr int COND_THREADS = 256;
+constexpr int COND_WARPS = COND_THREADS / 32;
 
-__device__ __forceinline__ CellC cell_consts(double th, double rv, double rhod, double c_exn, double RH_max) {
-  CellC c;
-  // eq. 43: T = [theta (rhod R_d/p_1000)^(R_d/c_pd)]^(c_pd/(c_pd-R_d)); c_exn is the inner power (rhod is fixed)
-  const double T = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
-  const double p = rhod * (cst::R_d + rv * cst::R_v) * T;                 // eq. 44
-  const double lv = cst::l_v0 + (cst::c_pv - cst::c_l) * (T - cst::T_0);  // Table 2 :1087
-  // [L] Clausius-Clapeyron integral for the linear l_v(T)
-  const double ca = (cst::l_v0 + (cst::c_l - cst::c_pv) * cst::T_0) / cst::R_v;
-  const double cb = (cst::c_l - cst::c_pv) / cst::R_v;
-  const double pvs = cst::p_vs0 * exp(ca * (1.0 / cst::T_0 - 1.0 / T) - cb * log(T / cst::T_0));
-  const double rho_vs = pvs / (cst::R_v * T);
-  c.T = T; c.lv = lv;
-  c.RH = fmin(rv * rhod / rho_vs, RH_max);                                // eq. 30, :685
-  c.A = 2.0 * cst::sigma_w / (cst::R_v * T * cst::rho_w);                 // Table 2 :1056
-  c.c0 = 2.0 * rho_vs / cst::rho_w;
-  c.lD = 2.0 * cst::D_0 / sqrt(2.0 * cst::R_v * T);                       // [L] Fuchs-Sutugin lengths
-  c.lK = (4.0 / 5.0) * cst::K_0 * T / (p * sqrt(2.0 * cst::R_d * T));
-  c.heat = (rho_vs * lv / T) * (lv / (cst::R_v * T) - 1.0);               // eq. 21
-  c.eta = eta_air(T);
-  c.rho_a = rhod * (1.0 + rv);
-  c.Sc = c.eta / (c.rho_a * cst::D_0);
-  c.Pr = c.eta * cst::c_pd / cst::K_0;
-  return c;
-}
+struct CellK {   // per-cell constants of one substep (shared memory, SoA over the tile's cells)
+  double RH, A, c0, lD, lK, heat, kE, Sc, Pr;
+};
+constexpr int CELLK_N = 9;
 
 // [L] Sherwood / Nusselt number (Clift et al.): 1 + (1 + Re X)^(1/3) max(1, Re^0.077)
 __device__ __forceinline__ double vent(double Re, double X) {
@@ -51,189 +38,351 @@ __device__ __forceinline__ double vent(double Re, double X) {
   return 1.0 + cb * m;
 }
 
-// Growth rate f(y) = d r_w^2/dt (eq. 20-24) and df/dy at y = r_w^2, written with one division:
+struct SdK {   // per-SD constants of one substep
+  double rd3, krd3;   // r_d^3, kappa r_d^3
+  double Kc, hDc;     // K_0 Nu/2 (eq. 24 without beta_T), heat * D_0 Sh/2
+  double cDK;         // c0 * Dc * Kc
+};
+
+// Growth rate f(y) = d r_w^2/dt (eq. 20-24) and df/dy at y = r_w^2, written with one reciprocal:
 //   beta_M = N_M/D_M, beta_T = N_T/D_T (Fuchs-Sutugin multiplied through by r^2),
 //   D_eff = Dc Kc N_M N_T / Q,  Q = Kc N_T D_M + heat Dc N_M D_T,
 //   a_w = P/W, P = r^3 - r_d^3, W = P + kappa r_d^3,  f = c0 D_eff (RH - a_w exp(A/r)).
-__device__ __forceinline__ void growth_fd(double y, double rd3, double krd3, double Dc, double Kc, const CellC& c,
-                                          double& f, double& df) {
+__device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c, double& f, double& df) {
   const double invr = rsqrt(y);
   const double r = y * invr;
   const double lDr = c.lD * r, lKr = c.lK * r;
-  const double NM = y + lDr, DM = y + 1.71 * lDr + 1.33 * (c.lD * c.lD);
-  const double NT = y + lKr, DT = y + 1.71 * lKr + 1.33 * (c.lK * c.lK);
-  const double KN = Kc * NT, HN = c.heat * Dc * NM;
-  const double Q = KN * DM + HN * DT;
+  const double NM = y + lDr, DM = fma(1.71, lDr, y) + 1.33 * (c.lD * c.lD);
+  const double NT = y + lKr, DT = fma(1.71, lKr, y) + 1.33 * (c.lK * c.lK);
+  const double KN = s.Kc * NT, HN = s.hDc * NM;
+  const double Q = fma(KN, DM, HN * DT);
   const double r3 = y * r;
-  const double P = r3 - rd3, W = P + krd3;
+  const double P = r3 - s.rd3, W = P + s.krd3;
   const double ex = exp(c.A * invr);
   const double invQW = 1.0 / (Q * W);
   const double invQ = invQW * W, invW = invQW * Q;
-  const double Deff = Dc * KN * NM * invQ;
+  const double NN = NM * NT;
   const double aw = P * invW;
   const double S = c.RH - aw * ex;
-  f = c.c0 * Deff * S;
+  const double cD = s.cDK * invQ;
+  f = cD * NN * S;
   // derivative
   const double hr = 0.5 * invr;   // dr/dy
-  const double NMp = 1.0 + c.lD * hr, DMp = 1.0 + 1.71 * c.lD * hr;
-  const double NTp = 1.0 + c.lK * hr, DTp = 1.0 + 1.71 * c.lK * hr;
-  const double Qp = Kc * (NTp * DM + NT * DMp) + c.heat * Dc * (NMp * DT + NM * DTp);
-  const double dlnD = (NMp * NT + NTp * NM) / (NM * NT) - Qp * invQ;
-  const double invr3 = invr * invr * invr;
-  const double Sp = -ex * (1.5 * r * krd3 * invW * invW - aw * (0.5 * c.A * invr3));
-  df = c.c0 * Deff * (dlnD * S + Sp);
+  const double NMp = fma(c.lD, hr, 1.0), DMp = fma(1.71 * c.lD, hr, 1.0);
+  const double NTp = fma(c.lK, hr, 1.0), DTp = fma(1.71 * c.lK, hr, 1.0);
+  const double NNp = fma(NMp, NT, NM * NTp);
+  const double Qp = s.Kc * fma(NTp, DM, NT * DMp) + s.hDc * fma(NMp, DT, NM * DTp);
+  const double awp = 1.5 * r * s.krd3 * (invW * invW);
+  const double Sp = -ex * (awp - aw * (c.A * hr) * (invr * invr));
+  df = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
 }
 
 // One condensation substep of one SD: root of g(y) = y - y0 - dt' f(y) in [a, b] of eq. 18-19
-// (reading R-bracket), with the ill-posed-bracket rule of :579.
-__device__ __forceinline__ double cond_solve(double y0, double rd2, double rd3, double krd3, const CellC& c, double dtp,
-                                             unsigned& n_ill, unsigned& n_eval) {
-  const double r0 = sqrt(y0);
-  const double vt = v_term(r0, c.eta, c.rho_a);
-  const double Re = 2.0 * r0 * vt * c.rho_a / c.eta;
-  const double Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;   // eq. 23 without beta_M
-  const double Kc = cst::K_0 * vent(Re, c.Pr) * 0.5;   // eq. 24 without beta_T
-  double f, df;
-  growth_fd(y0, rd3, krd3, Dc, Kc, c, f, df);
-  ++n_eval;
-  const double two = 2.0 * dtp * f;
-  const double a = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
-  const double b = y0 + fmax(two, 0.0);              // eq. 19
-  if (!(a < b)) return a;
-  // g(lo) < 0 < g(hi); the end that is not y0 has not been evaluated yet
-  double lo = a, hi = b;
-  bool lo_unv = !(f > 0.0), hi_unv = (f > 0.0);
-  double y = y0, g = -dtp * f, gp = 1.0 - dtp * df;
-  for (int it = 0; it < 100; ++it) {
-    double yn = (gp > 0.0) ? y - g / gp : (g < 0.0 ? hi : lo);
-    bool newton = true;
-    if (!(yn > lo && yn < hi)) {
-      newton = false;
-      if (g < 0.0 && hi_unv) {   // heading out through b: is the bracket well-posed?
-        double fb, dfb;
-        growth_fd(b, rd3, krd3, Dc, Kc, c, fb, dfb);
-        ++n_eval;
-        const double gb = b - y0 - dtp * fb;
-        if (gb == 0.0) return b;
-        if (gb < 0.0) { n_ill += (b - a > 1e-9 * b); return 0.5 * (a + b); }   // :579; counted when wider than noise
-        hi_unv = false;
-      } else if (g > 0.0 && lo_unv) {
-        double fa, dfa;
-        growth_fd(a, rd3, krd3, Dc, Kc, c, fa, dfa);
-        ++n_eval;
-        const double ga = a - y0 - dtp * fa;
-        if (ga == 0.0) return a;
-        if (ga > 0.0) { n_ill += (b - a > 1e-9 * b); return 0.5 * (a + b); }
-        lo_unv = false;
-      }
-      yn = 0.5 * (lo + hi);
-    }
-    const double step = fabs(yn - y);
-    y = yn;
-    // a Newton step this small leaves an error of order step^2/y; a bisection step bounds it directly
-    if (step <= (newton ? 1e-9 : 2e-16) * y) break;
-    if (!(hi - lo > 1e-15 * hi)) break;
-    growth_fd(y, rd3, krd3, Dc, Kc, c, f, df);
-    ++n_eval;
-    g = y - y0 - dtp * f;
-    gp = 1.0 - dtp * df;
-    if (g == 0.0) break;
-    if (g < 0.0) { lo = y; lo_unv = false; } else { hi = y; hi_unv = false; }
+// (reading R-bracket), with the ill-posed-bracket rule of :579.  Newton steps are kept
+// inside the shrinking bracket [lo, hi]; a step that leaves it is replaced by a bisection, and before
+// the first departure through an end that has never been evaluated the sign of g there decides whether
+// the bracket is well-posed at all.  Returns false when `max_evals` evaluations did not suffice.
+//
+// Stopping rule for a Newton step of size d_k from an iterate whose previous step was d_(k-1):
+// the error left after the step is C d_k^2 with C = |g''/(2g')|, estimated by d_k/d_(k-1)^2 and
+// bounded below by 1/y (first step: 100/y); stop when that is below 1e-11 y.
+enum { M_FIRST = 0, M_MAIN = 1, M_CHK_A = 2, M_CHK_B = 3 };
+
+__device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, double krd3, const CellK& c, double dtp,
+                                           int max_evals, double& y_out, unsigned& n_ill, unsigned& n_eval) {
+  SdK s;
+  s.rd3 = rd3; s.krd3 = krd3;
+  {
+    // [L] ventilation at the substep's starting radius (reading R-vent); Re from the terminal
+    // velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2)
+    const double r0 = sqrt(y0);
+    const double e = c.kE * (r0 * sqrt(r0));
+    const double q = e / (sqrt(1.0 + e) + 1.0);
+    const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
+    const double Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;   // eq. 23 without beta_M
+    s.Kc = cst::K_0 * vent(Re, c.Pr) * 0.5;              // eq. 24 without beta_T
+    s.hDc = c.heat * Dc;
+    s.cDK = c.c0 * Dc * s.Kc;
   }
-  return y;
+  int mode = M_FIRST;
+  double yE = y0, y = y0, g = 0.0, gp = 1.0, a = 0.0, b = 0.0, lo = 0.0, hi = 0.0, dprev = 0.0;
+  bool lo_unv = false, hi_unv = false;
+  for (int it = 0; it < max_evals; ++it) {
+    double f, df;
+    growth_fd(yE, s, c, f, df);   // the only evaluation site
+    ++n_eval;
+    bool bisect = false;
+    if (mode == M_FIRST) {
+      const double two = 2.0 * dtp * f;
+      a = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
+      b = y0 + fmax(two, 0.0);              // eq. 19
+      if (!(a < b)) { y_out = a; return true; }
+      // g(lo) < 0 < g(hi) is what a well-posed bracket means; the end that is not y0 is unverified
+      lo = a; hi = b;
+      lo_unv = !(f > 0.0); hi_unv = (f > 0.0);
+      g = -dtp * f; gp = fma(-dtp, df, 1.0);
+    } else if (mode == M_CHK_B) {
+      const double gb = b - y0 - dtp * f;
+      if (gb == 0.0) { y_out = b; return true; }
+      if (gb < 0.0) { n_ill += (b - a > 1e-9 * b); y_out = 0.5 * (a + b); return true; }   // :579
+      hi_unv = false; bisect = true;
+    } else if (mode == M_CHK_A) {
+      const double ga = a - y0 - dtp * f;
+      if (ga == 0.0) { y_out = a; return true; }
+      if (ga > 0.0) { n_ill += (b - a > 1e-9 * b); y_out = 0.5 * (a + b); return true; }
+      lo_unv = false; bisect = true;
+    } else {
+      y = yE;
+      g = y - y0 - dtp * f; gp = fma(-dtp, df, 1.0);
+      if (g == 0.0) { y_out = y; return true; }
+      if (g < 0.0) { lo = y; lo_unv = false; } else { hi = y; hi_unv = false; }
+    }
+    // next point
+    double yn;
+    bool newton = !bisect;
+    if (newton) {
+      yn = (gp > 0.0) ? y - g / gp : (g < 0.0 ? hi : lo);
+      if (!(yn > lo && yn < hi)) {
+        newton = false;
+        if (g < 0.0 && hi_unv) { mode = M_CHK_B; yE = b; continue; }
+        if (g > 0.0 && lo_unv) { mode = M_CHK_A; yE = a; continue; }
+      }
+    }
+    if (!newton) yn = 0.5 * (lo + hi);
+    const double d = fabs(yn - y);
+    y = yn;
+    bool conv;
+    if (newton) {
+      const double tol = 1e-11 * y;
+      const double d2 = d * d;
+      conv = (dprev > 0.0) ? (d2 <= tol * y && d2 * d <= tol * (dprev * dprev)) : (100.0 * d2 <= tol * y);
+      dprev = d;
+    } else {
+      conv = d <= 2e-16 * y;   // a bisection step bounds the error directly
+      dprev = 0.0;
+    }
+    if (conv || !(hi - lo > 1e-15 * hi)) { y_out = y; return true; }
+    mode = M_MAIN; yE = y;
+  }
+  return false;
 }
 
-// Shared memory per group: cap x {dn, rw2, rd3, kappa*rd3, rd2} doubles.
-template <int G, bool SMEM>
-__global__ void __launch_bounds__(CtaOf<G>::threads) k_cond(SdArrays a, const u16* __restrict__ rank,
-                                                            const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
-                                                            CellFields cf, CondParams cp, Counters cnt, int cap) {
+// per-cell constants of one substep from theta, r_v, rho_d; returns T and l_v for the feedback of eq. 26
+__device__ __forceinline__ void cell_consts(double th, double rv, double rhod, double c_exn, double RH_max, CellK& c,
+                                            double& T_out, double& lv_out) {
+  // eq. 43: T = [theta (rhod R_d/p_1000)^(R_d/c_pd)]^(c_pd/(c_pd-R_d)); c_exn is the inner power (rhod is fixed)
+  const double T = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
+  const double p = rhod * (cst::R_d + rv * cst::R_v) * T;                 // eq. 44
+  const double lv = cst::l_v0 + (cst::c_pv - cst::c_l) * (T - cst::T_0);  // Table 2 :1087
+  // [L] Clausius-Clapeyron integral for the linear l_v(T)
+  const double ca = (cst::l_v0 + (cst::c_l - cst::c_pv) * cst::T_0) / cst::R_v;
+  const double cb = (cst::c_l - cst::c_pv) / cst::R_v;
+  const double pvs = cst::p_vs0 * exp(ca * (1.0 / cst::T_0 - 1.0 / T) - cb * log(T / cst::T_0));
+  const double rho_vs = pvs / (cst::R_v * T);
+  T_out = T; lv_out = lv;
+  c.RH = fmin(rv * rhod / rho_vs, RH_max);                                // eq. 30, :685
+  c.A = 2.0 * cst::sigma_w / (cst::R_v * T * cst::rho_w);                 // Table 2 :1056
+  c.c0 = 2.0 * rho_vs / cst::rho_w;
+  c.lD = 2.0 * cst::D_0 / sqrt(2.0 * cst::R_v * T);                       // [L] Fuchs-Sutugin lengths
+  c.lK = (4.0 / 5.0) * cst::K_0 * T / (p * sqrt(2.0 * cst::R_d * T));
+  c.heat = (rho_vs * lv / T) * (lv / (cst::R_v * T) - 1.0);               // eq. 21
+  const double eta = eta_air(T);
+  const double rho_a = rhod * (1.0 + rv);
+  // e = c1 sqrt(X), X = (32/3) r^3 (rho_w - rho_a) g rho_a / eta^2  ->  e = kE r^(3/2)
+  const double c1 = 4.0 / (cst::kc_delta0 * cst::kc_delta0 * sqrt(cst::kc_C0));
+  c.kE = c1 * sqrt((32.0 / 3.0) * (cst::rho_w - rho_a) * cst::g * rho_a) / eta;
+  c.Sc = eta / (rho_a * cst::D_0);
+  c.Pr = eta * cst::c_pd / cst::K_0;
+}
+
+// Shared memory of one CTA (SMEM variant), cap = SD slots, cpb = cells per tile:
+//   double cell[(CELLK_N + 1) * cpb]   constants of the substep + the cell's sum of N d(r_w^3)
+//   double sd[6 * cap]                 y = r_w^2, r_d^3, kappa r_d^3, N, r_d^2, N d(r_w^3)  (sorted order)
+//   u32 segl[cpb + 2]                  tile-local segment offsets, list counter
+//   u16 cidx[cap], list[cap]           local cell of each slot; slots left for the second pass
+// GMEM variant (a cell too crowded for shared memory; cpb = 1): the state stays in HBM/L2 in storage
+// order, contributions go to alt.rw2 in sorted order, the list to alt.id.
+size_t cond_smem_bytes(int cpb, int cap) {
+  return (size_t)(CELLK_N + 1) * cpb * 8 + (size_t)6 * cap * 8 + (size_t)(cpb + 2) * 4 + (size_t)cap * 4 + 16;
+}
+
+template <bool SMEM>
+__global__ void __launch_bounds__(COND_THREADS, 2)
+k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+       CellFields cf, CondParams cp, Counters cnt, int cpb, int cap) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NG = CtaOf<G>::threads / G;
-  __shared__ double red_scratch[32];
-  const int gi = threadIdx.x / G;
-  const Group<G> grp = make_group<G>(red_scratch);
-  const int c = blockIdx.x * NG + gi;
-  unsigned n_ill = 0, n_eval = 0, n_sub = 0;
-  if (c < g.ncell) {
-    double* sm = reinterpret_cast<double*>(smem_raw) + (size_t)gi * cap * 5;
-    double* s_dn = sm;
-    double* s_y = sm + cap;
-    double* s_rd3 = sm + 2 * cap;
-    double* s_krd3 = sm + 3 * cap;
-    double* s_rd2 = sm + 4 * cap;
-    const u32 s0 = seg[c];
-    const int m = (int)(seg[c + 1] - s0);
-    const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
-    double th = th_f.at(i, j, k), rv = rv_f.at(i, j, k);
-    const double rhod = cf.rhod[c];
-    const double c_exn = pow(rhod * cst::R_d / cst::p_1000, cst::R_d / cst::c_pd);
-    if (m > 0) {
-      if constexpr (SMEM) {
-        for (int t = grp.lane; t < m; t += G) {
-          const int e = rank[s0 + t];
-          const double rd3 = a.rd3[s0 + t];
-          const double q = cbrt(rd3);
-          s_dn[e] = (double)a.n[s0 + t];
-          s_y[e] = a.rw2[s0 + t];
-          s_rd3[e] = rd3;
-          s_krd3[e] = a.kappa[s0 + t] * rd3;
-          s_rd2[e] = q * q;
-        }
-        grp.sync();
-      }
-      const double fb = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
-      for (int sub = 0; sub < cp.sstp; ++sub) {
-        const CellC cc = cell_consts(th, rv, rhod, c_exn, cp.RH_max);
-        double acc = 0.0;
-        for (int e = grp.lane; e < m; e += G) {
-          double dn, y0, rd3, krd3, rd2;
-          if constexpr (SMEM) {
-            dn = s_dn[e]; y0 = s_y[e]; rd3 = s_rd3[e]; krd3 = s_krd3[e]; rd2 = s_rd2[e];
-          } else {
-            dn = (double)a.n[s0 + e]; y0 = a.rw2[s0 + e]; rd3 = a.rd3[s0 + e];
-            krd3 = a.kappa[s0 + e] * rd3;
-            const double q = cbrt(rd3);
-            rd2 = q * q;
-          }
-          const double y1 = cond_solve(y0, rd2, rd3, krd3, cc, cp.dtp, n_ill, n_eval);
-          ++n_sub;
-          acc += dn * (y1 * sqrt(y1) - y0 * sqrt(y0));
-          if constexpr (SMEM) s_y[e] = y1; else a.rw2[s0 + e] = y1;
-        }
-        const double sum = grp.sum(acc);
-        const double drv = fb * sum;                                          // eq. 25
-        const double dth = drv * (-th * cc.lv / (cst::c_pd * cc.T));          // eq. 26, old theta and T
-        rv += drv;
-        th += dth;
-      }
-      if constexpr (SMEM) {
-        grp.sync();
-        for (int t = grp.lane; t < m; t += G) a.rw2[s0 + t] = s_y[rank[s0 + t]];
-      }
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int c_first = blockIdx.x * cpb;
+  const int nc = min(cpb, g.ncell - c_first);
+  double* s_cell = reinterpret_cast<double*>(smem_raw);
+  double* s_sum = s_cell + CELLK_N * cpb;
+  double* s_sd = s_cell + (CELLK_N + 1) * cpb;
+  const int capd = SMEM ? cap : 0;
+  double *s_y = s_sd, *s_rd3 = s_sd + capd, *s_krd3 = s_sd + 2 * capd, *s_dn = s_sd + 3 * capd, *s_rd2 = s_sd + 4 * capd;
+  double* s_con = s_sd + 5 * capd;
+  u32* segl = reinterpret_cast<u32*>(s_sd + 6 * capd);
+  u32* list_n = segl + cpb + 1;
+  u16* cidx = reinterpret_cast<u16*>(segl + cpb + 2);
+  u16* list16 = cidx + capd;
+  const u32 s0 = seg[c_first];
+  const int M = (int)(seg[c_first + nc] - s0);
+  u32* list32 = alt.id + s0;
+  if constexpr (!SMEM) s_con = alt.rw2 + s0;
+
+  // thread `tid` owns cell c_first + tid for the whole kernel: theta, r_v and the feedback live in its registers
+  double th = 0, rv = 0, rhod = 1, c_exn = 0, fbk = 0, T = 0, lv = 0;
+  int ci = 0, cj = 0, ck = 0;
+  if (tid < nc) {
+    const int c = c_first + tid;
+    ck = c % g.NZ; cj = (c / g.NZ) % g.NY; ci = c / (g.NZ * g.NY);
+    th = th_f.at(ci, cj, ck); rv = rv_f.at(ci, cj, ck);
+    rhod = cf.rhod[c];
+    c_exn = pow(rhod * cst::R_d / cst::p_1000, cst::R_d / cst::c_pd);
+    fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
+    segl[tid] = seg[c] - s0;
+    s_sum[tid] = 0.0;
+  }
+  if (tid == 0) segl[nc] = (u32)M;
+  __syncthreads();
+
+  // stage the tile in sorted order (coalesced reads; the cell of a slot by binary search in segl)
+  if constexpr (SMEM) {
+    for (int t = tid; t < M; t += COND_THREADS) {
+      int lo = 0, hi = nc;   // segl[lo] <= t < segl[hi]
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+      const u32 s = s0 + t;
+      const int e = (int)segl[lo] + rank[s];
+      const double rd3 = a.rd3[s];
+      const double q = cbrt(rd3);
+      s_y[e] = a.rw2[s];
+      s_rd3[e] = rd3;
+      s_krd3[e] = a.kappa[s] * rd3;
+      s_dn[e] = (double)a.n[s];
+      s_rd2[e] = q * q;
+      cidx[e] = (u16)lo;
     }
-    if (grp.lane == 0) {
-      th_f.at(i, j, k) = th;
-      rv_f.at(i, j, k) = rv;
-      // air properties after the feedback, used by coalescence and sedimentation (v_term)
-      const double T = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
-      cf.eta[c] = eta_air(T);
-      cf.rho_a[c] = rhod * (1.0 + rv);
+  }
+
+  unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
+  for (int sub = 0; sub < cp.sstp && M > 0; ++sub) {
+    // A. feedback of the previous substep (eq. 25-26, old theta and T) and the new cell constants
+    if (tid < nc) {
+      if (sub > 0) {
+        const double drv = fbk * s_sum[tid];
+        th += drv * (-th * lv / (cst::c_pd * T));
+        rv += drv;
+      }
+      CellK c;
+      cell_consts(th, rv, rhod, c_exn, cp.RH_max, c, T, lv);
+      s_cell[0 * cpb + tid] = c.RH; s_cell[1 * cpb + tid] = c.A; s_cell[2 * cpb + tid] = c.c0;
+      s_cell[3 * cpb + tid] = c.lD; s_cell[4 * cpb + tid] = c.lK; s_cell[5 * cpb + tid] = c.heat;
+      s_cell[6 * cpb + tid] = c.kE; s_cell[7 * cpb + tid] = c.Sc; s_cell[8 * cpb + tid] = c.Pr;
+    }
+    if (tid == 0) *list_n = 0u;
+    __syncthreads();
+
+    // B/C. pass 0: dense sweep with at most kfast evaluations per SD; pass 1: the listed rest, to the end
+    for (int pass = 0; pass < 2; ++pass) {
+      const int count = pass == 0 ? M : (int)*list_n;
+      const int max_evals = pass == 0 ? cp.kfast : 200;
+      for (int q0 = warp * 32; q0 < count; q0 += COND_THREADS) {
+        const int q = q0 + lane;
+        const bool valid = q < count;
+        bool done = true;
+        int e = 0;
+        if (valid) {
+          if (pass == 0) e = q; else e = SMEM ? (int)list16[q] : (int)list32[q];
+          double y0, rd3, krd3, rd2, dn;
+          int cl = 0, econ = e;
+          if constexpr (SMEM) {
+            y0 = s_y[e]; rd3 = s_rd3[e]; krd3 = s_krd3[e]; rd2 = s_rd2[e]; dn = s_dn[e];
+            cl = cidx[e];
+          } else {
+            const u32 s = s0 + e;
+            y0 = a.rw2[s]; rd3 = a.rd3[s]; krd3 = a.kappa[s] * rd3; dn = (double)a.n[s];
+            const double qq = cbrt(rd3);
+            rd2 = qq * qq;
+            econ = rank[s];
+          }
+          CellK c;
+          c.RH = s_cell[0 * cpb + cl]; c.A = s_cell[1 * cpb + cl]; c.c0 = s_cell[2 * cpb + cl];
+          c.lD = s_cell[3 * cpb + cl]; c.lK = s_cell[4 * cpb + cl]; c.heat = s_cell[5 * cpb + cl];
+          c.kE = s_cell[6 * cpb + cl]; c.Sc = s_cell[7 * cpb + cl]; c.Pr = s_cell[8 * cpb + cl];
+          double y1 = y0;
+          unsigned ill = 0;
+          done = cond_solve(y0, rd2, rd3, krd3, c, cp.dtp, max_evals, y1, ill, n_eval);
+          if (done) {
+            n_ill += ill;
+            ++n_sub;
+            s_con[econ] = dn * (y1 * sqrt(y1) - y0 * sqrt(y0));
+            if constexpr (SMEM) s_y[e] = y1; else a.rw2[s0 + e] = y1;
+          }
+        }
+        if (pass == 0) {   // warp-aggregated append of the unfinished slots
+          const unsigned need = __ballot_sync(0xffffffffu, !done);
+          if (need) {
+            u32 base = 0;
+            if (lane == 0) base = atomicAdd(list_n, (u32)__popc(need));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (!done) {
+              const u32 pos = base + __popc(need & ((1u << lane) - 1u));
+              if constexpr (SMEM) list16[pos] = (u16)e; else list32[pos] = (u32)e;
+              ++n_slow;
+            }
+          }
+        }
+      }
+      __syncthreads();
+    }
+
+    // D. per-cell sum of N d(r_w^3) in sorted order: lane-strided partial sums, xor butterfly
+    for (int cl = warp; cl < nc; cl += COND_WARPS) {
+      const int b0 = (int)segl[cl], b1 = (int)segl[cl + 1];
+      double acc = 0.0;
+      for (int e = b0 + lane; e < b1; e += 32) acc += s_con[e];
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+      if (lane == 0) s_sum[cl] = acc;
+    }
+    __syncthreads();
+  }
+
+  if (tid < nc) {
+    if (M > 0) {   // feedback of the last substep
+      const double drv = fbk * s_sum[tid];
+      th += drv * (-th * lv / (cst::c_pd * T));
+      rv += drv;
+    }
+    th_f.at(ci, cj, ck) = th;
+    rv_f.at(ci, cj, ck) = rv;
+    // air properties after the feedback, used by coalescence and sedimentation (v_term)
+    const double Tn = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
+    cf.eta[c_first + tid] = eta_air(Tn);
+    cf.rho_a[c_first + tid] = rhod * (1.0 + rv);
+  }
+  if constexpr (SMEM) {
+    for (int t = tid; t < M; t += COND_THREADS) {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+      const u32 s = s0 + t;
+      a.rw2[s] = s_y[(int)segl[lo] + rank[s]];
     }
   }
   // counters: one atomic per warp and counter, spread over NSLOT addresses
-  unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub;
+  unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub, v3 = n_slow;
 #pragma unroll
   for (int d = 16; d >= 1; d >>= 1) {
     v0 += __shfl_xor_sync(0xffffffffu, v0, d);
     v1 += __shfl_xor_sync(0xffffffffu, v1, d);
     v2 += __shfl_xor_sync(0xffffffffu, v2, d);
+    v3 += __shfl_xor_sync(0xffffffffu, v3, d);
   }
-  if ((threadIdx.x & 31) == 0) {
-    const int slot = (blockIdx.x * (CtaOf<G>::threads / 32) + (threadIdx.x >> 5)) & (NSLOT - 1);
+  if (lane == 0) {
+    const int slot = (blockIdx.x * COND_WARPS + warp) & (NSLOT - 1);
     if (v0) atomicAdd(&cnt.ill_posed[slot], (unsigned long long)v0);
     if (v1) atomicAdd(&cnt.f_evals[slot], (unsigned long long)v1);
     if (v2) atomicAdd(&cnt.sd_substeps[slot], (unsigned long long)v2);
+    if (v3) atomicAdd(&cnt.cond_slow[slot], (unsigned long long)v3);
   }
 }
 
@@ -248,36 +397,22 @@ __global__ void k_thermo(Grid g, Field th_f, Field rv_f, CellFields cf) {
   cf.rho_a[c] = rhod * (1.0 + rv);
 }
 
-size_t cond_smem_bytes(int G, int cap) {
-  const int NG = (G <= 32 ? 128 : G) / G;
-  return (size_t)NG * cap * 5 * sizeof(double);
-}
-
-template <int G>
-static cudaError_t launch_cond_t(int cap, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
-                                 Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st) {
-  constexpr int NG = CtaOf<G>::threads / G;
-  const int grid = (g.ncell + NG - 1) / NG;
+// cpb cells per CTA; cap > 0: shared-memory slots per CTA (>= the most populated tile); cap == 0: GMEM
+// variant (cpb must be 1), `alt` = the idle ping-pong copy of the state used as scratch.
+cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+                        const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
+                        cudaStream_t st) {
+  const int grid = (g.ncell + cpb - 1) / cpb;
   if (cap > 0) {
-    const size_t smem = cond_smem_bytes(G, cap);
-    cudaError_t e = cudaFuncSetAttribute(k_cond<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = cond_smem_bytes(cpb, cap);
+    cudaError_t e = cudaFuncSetAttribute(k_cond<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_cond<G, true><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cap);
+    k_cond<true><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, cap);
   } else {
-    k_cond<G, false><<<grid, CtaOf<G>::threads, 0, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, 0);
+    const size_t smem = cond_smem_bytes(cpb, 0);
+    k_cond<false><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);
   }
   return cudaGetLastError();
-}
-
-cudaError_t launch_cond(int G, int cap, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
-                        Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st) {
-  switch (G) {
-    case 4: return launch_cond_t<4>(cap, a, rank, seg, g, th, rv, cf, cp, cnt, st);
-    case 8: return launch_cond_t<8>(cap, a, rank, seg, g, th, rv, cf, cp, cnt, st);
-    case 16: return launch_cond_t<16>(cap, a, rank, seg, g, th, rv, cf, cp, cnt, st);
-    case 32: return launch_cond_t<32>(cap, a, rank, seg, g, th, rv, cf, cp, cnt, st);
-    default: return launch_cond_t<256>(cap, a, rank, seg, g, th, rv, cf, cp, cnt, st);
-  }
 }
 
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st) {

@@ -13,6 +13,7 @@ struct CondParams {
   double dtp;        // dt / sstp_cond
   int sstp;
   double RH_max;
+  int kfast;         // growth-rate evaluations per SD in the dense sweep before an SD is deferred to the second pass
 };
 struct CoalMoveParams {
   int coal, adve, sedi, sstp_coal;
@@ -30,6 +31,7 @@ void launch_cellhist(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, c
                      u32* count, cudaStream_t st);
 int scan_num_blocks(int ncell);
 void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_next, u32* d_maxcount, cudaStream_t st);
+void launch_tile_max(const u32* seg, int ncell, int cpb0, u32* d_tilemax4, cudaStream_t st);
 void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
                     const u32* cell, const u32* off, const u32* seg, cudaStream_t st);
 cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
@@ -37,10 +39,12 @@ cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 ste
 void launch_export_order(const u32* id, const u16* rank, const u32* seg, int ncell, u32* ids_sorted, cudaStream_t st);
 
 // sdm_cond.cu
-// cap: shared-memory slots per group (>= largest cell) or 0 to work in place in global memory
-cudaError_t launch_cond(int G, int cap, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
-                        Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st);
-size_t cond_smem_bytes(int G, int cap);
+// cpb: cells per CTA; cap: shared-memory SD slots per CTA (>= most populated tile) or 0 to work in place in
+// global memory (cpb == 1, `alt` = idle ping-pong copy used as scratch)
+cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+                        const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
+                        cudaStream_t st);
+size_t cond_smem_bytes(int cpb, int cap);
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);
 
 // sdm_coal_move.cu

@@ -4,6 +4,7 @@
 // sort of (key << 32 | id) in shared memory that yields each SD's rank inside its cell.
 // PAPER.md :547 (cell index), :624 (random non-overlapping pairs), :641/:651 (N = 0 SDs).
 #include "sdm_kernels.cuh"
+#include <algorithm>
 
 namespace sdm {
 
@@ -101,6 +102,20 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(u32* __restrict__ c
     if (base + k < ncell) { seg[base + k] = ex; ex += v[k]; count[base + k] = 0u; }   // histogram is left zeroed
 }
 
+// Most populated tile of cpb consecutive cells, for the 4 candidate tile sizes cpb_k = max(1, cpb0 >> k):
+// sizes the shared memory of the tile-resident condensation kernel (sdm_cond.cu).
+__global__ void __launch_bounds__(256) k_tile_max(const u32* __restrict__ seg, int ncell, int cpb0, u32* __restrict__ out4) {
+  for (int k = 0; k < 4; ++k) {
+    const int cpb = max(1, cpb0 >> k);
+    const int ntile = (ncell + cpb - 1) / cpb;
+    u32 mx = 0;
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < ntile; t += gridDim.x * blockDim.x)
+      mx = max(mx, seg[min((t + 1) * cpb, ncell)] - seg[t * cpb]);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0 && mx) atomicMax(&out4[k], mx);
+  }
+}
+
 // ---- a3: scatter the SoA state into cell-sorted storage (drops dead SDs) ----------------------------
 __global__ void __launch_bounds__(256) k_scatter(SdArrays src, SdArrays dst, const u32* __restrict__ d_nslots, Grid g,
                                                  const u32* __restrict__ cell, const u32* __restrict__ off,
@@ -179,6 +194,11 @@ void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_n
   k_scan_partial<<<nb, SCAN_THREADS, 0, st>>>(count, ncell, blocksum, d_maxcount);
   k_scan_blocks<<<1, SCAN_THREADS, 0, st>>>(blocksum, nb, d_nslots_next, seg + ncell);
   k_scan_apply<<<nb, SCAN_THREADS, 0, st>>>(count, ncell, blocksum, seg);
+}
+
+void launch_tile_max(const u32* seg, int ncell, int cpb0, u32* d_tilemax4, cudaStream_t st) {
+  const int nb = std::min((ncell + 255) / 256, 1184);
+  k_tile_max<<<nb, 256, 0, st>>>(seg, ncell, cpb0, d_tilemax4);
 }
 
 void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,

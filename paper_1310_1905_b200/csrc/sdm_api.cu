@@ -13,9 +13,9 @@ using namespace sdm;
 namespace {
 thread_local std::string g_create_error;
 constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are willing to ask for per CTA
-constexpr size_t kCondSmemTwoCtas = 110 * 1024;   // per CTA, so that two condensation CTAs share an SM
-constexpr double kCondTileTarget = 1792.0;  // SDs per condensation tile (mean); 6 sigma above fits 110 KB
-constexpr double kCondMaxCpb = 256.0;       // one thread per cell of the tile
+constexpr size_t kCondSmemPerCta = 44 * 1024;    // per CTA, so that five condensation CTAs share an SM
+constexpr double kCondTileTarget = 700.0;   // SDs per condensation tile (mean); 5 sigma above fits 44 KB
+constexpr double kCondMaxCpb = 128.0;       // one thread per cell of the tile
 }
 
 struct sdm_ctx {
@@ -374,7 +374,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     for (int k = 0; k < 4 && cap == 0; ++k) {
       const int cand = std::max(1, ctx->cond_cpb0 >> k);
       const int need = std::max(((int)ctx->h_info[4 + k] + 3) / 4 * 4, 4);
-      if (cond_smem_bytes(cand, need) <= (cand > 1 ? kCondSmemTwoCtas : kSmemLimit)) { cpb = cand; cap = need; }
+      if (cond3_smem_bytes(cand, need) <= (cand > 1 ? kCondSmemPerCta : kSmemLimit)) { cpb = cand; cap = need; }
       if (cand == 1) break;
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};

@@ -77,6 +77,102 @@ __device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c
   df = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
 }
 
+// ---- fast path (k_cond3): the same equations written in r = sqrt(y), which stays resident in shared
+// memory over the substeps (no sqrt per substep), with one reciprocal per evaluation.
+// 1/a from the hardware seed (MUFU.RCP64H, ~2^-20) and NR Newton-Raphson refinements (2 -> < 1 ulp)
+template <int NR>
+__device__ __forceinline__ double rcp_nr(double a) {
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+#pragma unroll
+  for (int k = 0; k < NR; ++k) {
+    const double e = fma(-a, x, 1.0);
+    x = fma(x, e, x);
+  }
+  return x;
+}
+
+struct CellR {   // per-cell constants of one substep used by the fast path
+  double RH, A, lD, lK, qD, qK, lD171, lK171;
+  float kE, Sc, Pr;
+};
+
+// f(r) = d r_w^2/dt (eq. 20-24) and df/dr; also returns y = r^2.  Notation as growth_fd.
+__device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c, double& y, double& f, double& dfr) {
+  y = r * r;
+  const double lDr = c.lD * r, lKr = c.lK * r;
+  const double NM = y + lDr, DM = fma(1.71, lDr, y) + c.qD;
+  const double NT = y + lKr, DT = fma(1.71, lKr, y) + c.qK;
+  const double KN = s.Kc * NT, HN = s.hDc * NM;
+  const double Q = fma(KN, DM, HN * DT);
+  const double r3 = y * r;
+  const double P = r3 - s.rd3, W = P + s.krd3;
+  const double QW = Q * W;
+  const double inv = rcp_nr<2>(r * QW);
+  const double invr = inv * QW, invQ = inv * (r * W), invW = inv * (r * Q);
+  const double t = c.A * invr;
+  const double ex = exp(t);
+  const double NN = NM * NT;
+  const double aw = P * invW;
+  const double S = fma(-aw, ex, c.RH);
+  const double cD = s.cDK * invQ;
+  f = cD * NN * S;
+  const double r2 = r + r;
+  const double NMp = r2 + c.lD, DMp = r2 + c.lD171;
+  const double NTp = r2 + c.lK, DTp = r2 + c.lK171;
+  const double NNp = fma(NMp, NT, NM * NTp);
+  const double Qp = s.Kc * fma(NTp, DM, NT * DMp) + s.hDc * fma(NMp, DT, NM * DTp);
+  const double awp = 3.0 * y * s.krd3 * (invW * invW);
+  const double Sp = ex * fma(aw, t * invr, -awp);
+  dfr = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
+}
+
+// (1+x)^(1/3) - 1 by the binomial series, truncation < 1e-17 for 0 <= x < 0.02
+__device__ __forceinline__ double cbrt1pm1_small(double x) {
+  double p = -935.0 / 59049.0;
+  p = fma(p, x, 374.0 / 19683.0);
+  p = fma(p, x, -154.0 / 6561.0);
+  p = fma(p, x, 22.0 / 729.0);
+  p = fma(p, x, -10.0 / 243.0);
+  p = fma(p, x, 5.0 / 81.0);
+  p = fma(p, x, -1.0 / 9.0);
+  p = fma(p, x, 1.0 / 3.0);
+  return p * x;
+}
+
+// [L] ventilation at the substep's starting radius r0 (reading R-vent) -> per-SD constants.
+// Re·Sc below 2.5e-4 (r0 below ~3 um): Sh - 2 < 1e-4 enters D only through 2 + (Sh - 2), so Re and the
+// series are evaluated in fp32 (relative error 3e-7 of a 1e-4 term: < 3e-11 of D).  Above: fp64.
+__device__ __forceinline__ void sd_setup(double r0, double c0, double heat, double kE, double Sc, double Pr,
+                                         const CellR& c, SdK& s) {
+  const float rf = (float)r0;
+  const float ef = c.kE * rf * sqrtf(rf);
+  const float qf = ef / (sqrtf(1.0f + ef) + 1.0f);
+  const float Ref = (float)(cst::kc_delta0 * cst::kc_delta0 / 4.0) * (qf * qf);
+  const float xs = Ref * c.Sc, xp = Ref * c.Pr;
+  double shm, num;   // Sh - 2, Nu - 2
+  if (fmaxf(xs, xp) < 2.5e-4f) {
+    shm = (double)(xs * (1.0f / 3.0f + xs * (-1.0f / 9.0f + xs * (5.0f / 81.0f))));
+    num = (double)(xp * (1.0f / 3.0f + xp * (-1.0f / 9.0f + xp * (5.0f / 81.0f))));
+  } else {
+    const double e = kE * (r0 * sqrt(r0));
+    const double q = e / (sqrt(1.0 + e) + 1.0);
+    const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
+    const double x1 = Re * Sc, x2 = Re * Pr;
+    if (Re <= 1.0 && fmax(x1, x2) < 0.02) {
+      shm = cbrt1pm1_small(x1);
+      num = cbrt1pm1_small(x2);
+    } else {
+      shm = vent(Re, Sc) - 2.0;
+      num = vent(Re, Pr) - 2.0;
+    }
+  }
+  const double Dc = fma(0.5 * cst::D_0, shm, cst::D_0);   // eq. 23 without beta_M: D_0 Sh / 2
+  s.Kc = fma(0.5 * cst::K_0, num, cst::K_0);              // eq. 24 without beta_T: K_0 Nu / 2
+  s.hDc = heat * Dc;
+  s.cDK = c0 * Dc * s.Kc;
+}
+
 // One condensation substep of one SD: root of g(y) = y - y0 - dt' f(y) in [a, b] of eq. 18-19
 // (reading R-bracket), with the ill-posed-bracket rule of :579.  Newton steps are kept
 // inside the shrinking bracket [lo, hi]; a step that leaves it is replaced by a bisection, and before
@@ -386,6 +482,236 @@ k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __rest
   }
 }
 
+// ---- k_cond3: the shared-memory tile kernel, third version ---------------------------------------
+// Differences from k_cond<true> (kept above for cells too crowded for shared memory):
+//  * r_w (not r_w^2) is resident in shared memory: no sqrt per substep, N d(r_w^3) by two products;
+//  * the sweep is straight-line code around growth_r with a warp-uniform iteration loop; anything
+//    irregular (Newton leaving the bracket of eq. 18-19, an end to verify, slow convergence) is
+//    put on a WARP-private list and solved afterwards by cond_solve, the robust state machine;
+//  * small CTAs (T3 threads, several per SM) so that the serial phases of one tile (cell constants,
+//    slow list, barriers) overlap the sweeps of the others.
+// Shared memory: double cell[C3_N * cpb]; double sd[6 * cap] = r, r_d^3, kappa r_d^3, N, r_d^2,
+// N d(r_w^3); float cellf[3 * cpb]; u32 segl[cpb + 1]; u16 cidx[cap]; u16 list[lstride * warps].
+constexpr int C3_N = 12;   // RH, A, c0, lD, lK, heat, kE, Sc, Pr, qD, qK, sum
+constexpr int T3 = 128;
+static int c3_lstride(int cap) { return ((cap + T3 - 1) / T3) * 32; }
+size_t cond3_smem_bytes(int cpb, int cap) {
+  return (size_t)C3_N * cpb * 8 + (size_t)6 * cap * 8 + (size_t)3 * cpb * 4 + (size_t)(cpb + 1) * 4 + (size_t)cap * 2 +
+         (size_t)c3_lstride(cap) * (T3 / 32) * 2 + 32;
+}
+
+__global__ void __launch_bounds__(T3, 5)
+k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+        CellFields cf, CondParams cp, Counters cnt, int cpb, int cap, int lstride) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NW = T3 / 32;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int c_first = blockIdx.x * cpb;
+  const int nc = min(cpb, g.ncell - c_first);
+  double* s_cell = reinterpret_cast<double*>(smem_raw);
+  double* s_sum = s_cell + 11 * cpb;
+  double* s_r = s_cell + C3_N * cpb;
+  double *s_rd3 = s_r + cap, *s_krd3 = s_r + 2 * cap, *s_dn = s_r + 3 * cap, *s_rd2 = s_r + 4 * cap, *s_con = s_r + 5 * cap;
+  float* s_cf = reinterpret_cast<float*>(s_r + 6 * cap);
+  u32* segl = reinterpret_cast<u32*>(s_cf + 3 * cpb);
+  u16* cidx = reinterpret_cast<u16*>(segl + cpb + 1);
+  u16* mylist = cidx + ((cap + 1) & ~1) + warp * lstride;
+  const u32 s0 = seg[c_first];
+  const int M = (int)(seg[c_first + nc] - s0);
+
+  // thread `tid` owns cell c_first + tid: theta, r_v and the feedback live in its registers
+  double th = 0, rv = 0, rhod = 1, c_exn = 0, fbk = 0, T = 0, lv = 0;
+  int ci = 0, cj = 0, ck = 0;
+  if (tid < nc) {
+    const int c = c_first + tid;
+    ck = c % g.NZ; cj = (c / g.NZ) % g.NY; ci = c / (g.NZ * g.NY);
+    th = th_f.at(ci, cj, ck); rv = rv_f.at(ci, cj, ck);
+    rhod = cf.rhod[c];
+    c_exn = pow(rhod * cst::R_d / cst::p_1000, cst::R_d / cst::c_pd);
+    fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
+    segl[tid] = seg[c] - s0;
+    s_sum[tid] = 0.0;
+  }
+  if (tid == 0) segl[nc] = (u32)M;
+  __syncthreads();
+  for (int t = tid; t < M; t += T3) {   // stage the tile in sorted order
+    int lo = 0, hi = nc;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+    const u32 s = s0 + t;
+    const int e = (int)segl[lo] + rank[s];
+    const double rd3 = a.rd3[s];
+    const double q = cbrt(rd3);
+    s_r[e] = sqrt(a.rw2[s]);
+    s_rd3[e] = rd3;
+    s_krd3[e] = a.kappa[s] * rd3;
+    s_dn[e] = (double)a.n[s];
+    s_rd2[e] = q * q;
+    cidx[e] = (u16)lo;
+  }
+  unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
+  for (int sub = 0; sub < cp.sstp && M > 0; ++sub) {
+    // A. feedback of the previous substep (eq. 25-26, old theta and T) and the new cell constants
+    if (tid < nc) {
+      if (sub > 0) {
+        const double drv = fbk * s_sum[tid];
+        th += drv * (-th * lv / (cst::c_pd * T));
+        rv += drv;
+      }
+      CellK c;
+      cell_consts(th, rv, rhod, c_exn, cp.RH_max, c, T, lv);
+      s_cell[0 * cpb + tid] = c.RH; s_cell[1 * cpb + tid] = c.A; s_cell[2 * cpb + tid] = c.c0;
+      s_cell[3 * cpb + tid] = c.lD; s_cell[4 * cpb + tid] = c.lK; s_cell[5 * cpb + tid] = c.heat;
+      s_cell[6 * cpb + tid] = c.kE; s_cell[7 * cpb + tid] = c.Sc; s_cell[8 * cpb + tid] = c.Pr;
+      s_cell[9 * cpb + tid] = 1.33 * (c.lD * c.lD); s_cell[10 * cpb + tid] = 1.33 * (c.lK * c.lK);
+      s_cf[0 * cpb + tid] = (float)c.kE; s_cf[1 * cpb + tid] = (float)c.Sc; s_cf[2 * cpb + tid] = (float)c.Pr;
+    }
+    __syncthreads();
+    // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (warp-private list)
+    int nslow = 0;
+    const double dtp = cp.dtp;
+    for (int q0 = warp * 32; q0 < M; q0 += T3) {
+      const int e = q0 + lane;
+      const bool valid = e < M;
+      const int cl = valid ? (int)cidx[e] : 0;
+      const double r0 = valid ? s_r[e] : 1e-6;
+      const double rd2 = valid ? s_rd2[e] : 1e-14;
+      SdK s;
+      s.rd3 = valid ? s_rd3[e] : 1e-21;
+      s.krd3 = valid ? s_krd3[e] : 1e-21;
+      CellR c;
+      c.RH = s_cell[0 * cpb + cl]; c.A = s_cell[1 * cpb + cl]; c.lD = s_cell[3 * cpb + cl]; c.lK = s_cell[4 * cpb + cl];
+      c.qD = s_cell[9 * cpb + cl]; c.qK = s_cell[10 * cpb + cl];
+      c.lD171 = 1.71 * c.lD; c.lK171 = 1.71 * c.lK;
+      c.kE = s_cf[0 * cpb + cl]; c.Sc = s_cf[1 * cpb + cl]; c.Pr = s_cf[2 * cpb + cl];
+      sd_setup(r0, s_cell[2 * cpb + cl], s_cell[5 * cpb + cl], s_cell[6 * cpb + cl], s_cell[7 * cpb + cl],
+               s_cell[8 * cpb + cl], c, s);
+      double y0, f, dfr;
+      growth_r(r0, s, c, y0, f, dfr);
+      n_eval += valid;
+      const double two = 2.0 * dtp * f;
+      double lo = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
+      double hi = y0 + fmax(two, 0.0);              // eq. 19
+      double r = r0, dprev = 0.0;
+      int st;
+      if (!(lo < hi)) {
+        st = (lo == y0) ? 1 : 2;                    // a = b: the result is a
+      } else {
+        const double gp = fma(-dtp, dfr, r0 + r0);
+        const double rn = fma(dtp * f, rcp_nr<1>(gp), r0);
+        const double yn = rn * rn;
+        if (!(gp > 0.0 && yn > lo && yn < hi)) {
+          st = 2;
+        } else {
+          dprev = fabs(rn - r0);
+          r = rn;
+          st = (400.0 * (dprev * dprev) <= 1e-11 * (rn * rn)) ? 1 : 0;
+        }
+      }
+      if (!valid) st = 1;
+      for (int it = 1; it < cp.kfast; ++it) {
+        if (!__any_sync(0xffffffffu, st == 0)) break;
+        if (st == 0) {
+          double y;
+          growth_r(r, s, c, y, f, dfr);
+          ++n_eval;
+          const double gv = y - y0 - dtp * f;
+          const double gp = fma(-dtp, dfr, r + r);
+          if (gv < 0.0) lo = y; else hi = y;
+          const double rn = fma(-gv, rcp_nr<1>(gp), r);
+          const double yn = rn * rn;
+          if (!(gp > 0.0 && yn > lo && yn < hi)) {
+            st = 2;
+          } else {
+            const double d = fabs(rn - r);
+            const double tol = 1e-11 * rn, d2 = d * d;
+            const bool conv = (4.0 * d2 <= tol * rn) && (2.0 * d2 * d <= tol * (dprev * dprev));
+            r = rn; dprev = d;
+            if (conv || !(hi - lo > 1e-15 * hi)) st = 1;
+          }
+        }
+      }
+      if (st == 0) st = 2;
+      if (valid && st == 1) {
+        s_con[e] = s_dn[e] * (r * r * r - r0 * y0);
+        s_r[e] = r;
+        ++n_sub;
+      }
+      const unsigned need = __ballot_sync(0xffffffffu, st == 2);
+      if (st == 2) mylist[nslow + __popc(need & ((1u << lane) - 1u))] = (u16)e;
+      nslow += __popc(need);
+    }
+    __syncwarp();
+    // C. the listed rest: the bracketed state machine, from the start of the substep
+    for (int k0 = 0; k0 < nslow; k0 += 32) {
+      const int k = k0 + lane;
+      if (k < nslow) {
+        const int e = (int)mylist[k];
+        const int cl = (int)cidx[e];
+        CellK c;
+        c.RH = s_cell[0 * cpb + cl]; c.A = s_cell[1 * cpb + cl]; c.c0 = s_cell[2 * cpb + cl];
+        c.lD = s_cell[3 * cpb + cl]; c.lK = s_cell[4 * cpb + cl]; c.heat = s_cell[5 * cpb + cl];
+        c.kE = s_cell[6 * cpb + cl]; c.Sc = s_cell[7 * cpb + cl]; c.Pr = s_cell[8 * cpb + cl];
+        const double r0 = s_r[e], y0 = r0 * r0;
+        double y1 = y0;
+        unsigned ill = 0;
+        cond_solve(y0, s_rd2[e], s_rd3[e], s_krd3[e], c, dtp, 200, y1, ill, n_eval);
+        const double r1 = sqrt(y1);
+        n_ill += ill;
+        ++n_sub; ++n_slow;
+        s_con[e] = s_dn[e] * (r1 * r1 * r1 - r0 * y0);
+        s_r[e] = r1;
+      }
+    }
+    __syncthreads();
+    // D. per-cell sum of N d(r_w^3) in sorted order: lane-strided partial sums, xor butterfly
+    for (int cl = warp; cl < nc; cl += NW) {
+      const int b0 = (int)segl[cl], b1 = (int)segl[cl + 1];
+      double acc = 0.0;
+      for (int e = b0 + lane; e < b1; e += 32) acc += s_con[e];
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+      if (lane == 0) s_sum[cl] = acc;
+    }
+    __syncthreads();
+  }
+
+  if (tid < nc) {
+    if (M > 0) {   // feedback of the last substep
+      const double drv = fbk * s_sum[tid];
+      th += drv * (-th * lv / (cst::c_pd * T));
+      rv += drv;
+    }
+    th_f.at(ci, cj, ck) = th;
+    rv_f.at(ci, cj, ck) = rv;
+    // air properties after the feedback, used by coalescence and sedimentation (v_term)
+    const double Tn = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
+    cf.eta[c_first + tid] = eta_air(Tn);
+    cf.rho_a[c_first + tid] = rhod * (1.0 + rv);
+  }
+  for (int t = tid; t < M; t += T3) {
+    int lo = 0, hi = nc;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+    const u32 s = s0 + t;
+    const double r = s_r[(int)segl[lo] + rank[s]];
+    a.rw2[s] = r * r;
+  }
+  unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub, v3 = n_slow;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    v0 += __shfl_xor_sync(0xffffffffu, v0, d);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, d);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, d);
+    v3 += __shfl_xor_sync(0xffffffffu, v3, d);
+  }
+  if (lane == 0) {
+    const int slot = (blockIdx.x * NW + warp) & (NSLOT - 1);
+    if (v0) atomicAdd(&cnt.ill_posed[slot], (unsigned long long)v0);
+    if (v1) atomicAdd(&cnt.f_evals[slot], (unsigned long long)v1);
+    if (v2) atomicAdd(&cnt.sd_substeps[slot], (unsigned long long)v2);
+    if (v3) atomicAdd(&cnt.cond_slow[slot], (unsigned long long)v3);
+  }
+}
+
 // eta, rho_a per cell when condensation is switched off
 __global__ void k_thermo(Grid g, Field th_f, Field rv_f, CellFields cf) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -404,10 +730,10 @@ cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt
                         cudaStream_t st) {
   const int grid = (g.ncell + cpb - 1) / cpb;
   if (cap > 0) {
-    const size_t smem = cond_smem_bytes(cpb, cap);
-    cudaError_t e = cudaFuncSetAttribute(k_cond<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = cond3_smem_bytes(cpb, cap);
+    cudaError_t e = cudaFuncSetAttribute(k_cond3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_cond<true><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, cap);
+    k_cond3<<<grid, T3, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb, cap, c3_lstride(cap));
   } else {
     const size_t smem = cond_smem_bytes(cpb, 0);
     k_cond<false><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);

@@ -45,6 +45,7 @@ cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st);
 size_t cond_smem_bytes(int cpb, int cap);
+size_t cond3_smem_bytes(int cpb, int cap);   // the shared-memory tile kernel k_cond3 (cap > 0)
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);
 
 // sdm_coal_move.cu

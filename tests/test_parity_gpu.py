@@ -76,7 +76,8 @@ def run_both(w, steps, group=0, opts=None, check_every=1, **override):
         p.step_sync(po, th, rv)
         p.step_async(po)
         fp = p.step_async_result()
-        np.testing.assert_allclose(fp, fo, rtol=1e-12, atol=1e-300)
+        # rain flux = sum of N (4/3) pi rho_w r_w^3 over SDs whose radii match within RTOL -> 3 RTOL
+        np.testing.assert_allclose(fp, fo, rtol=3 * RTOL, atol=1e-300)
         if (s + 1) % check_every == 0 or s == steps - 1:
             compare_states(p, o, positions=True)
             compare_fields(th, rv, o)

@@ -285,7 +285,8 @@ def main():
     roofline = {"kernel": "k_cond (condensation, 10 fused substeps)", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": None,
                 "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
-                "evals_per_sd_substep": evals / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
+                "evals_per_sd_substep": evals / max(subs, 1),
+                "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
                 "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms}
     bytes_step = BYTES_PER_SD_STEP[ndim] * (sd_steps / a.steps)
     hbm = {"bound": "hbm", "achieved": bytes_step / (step_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",

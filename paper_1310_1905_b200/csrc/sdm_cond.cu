@@ -599,7 +599,7 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
         const double gp = fma(-dtp, dfr, r0 + r0);
         const double rn = fma(dtp * f, rcp_nr<1>(gp), r0);
         const double yn = rn * rn;
-        if (!(gp > 0.0 && yn > lo && yn < hi)) {
+        if (!(gp > 0.0 && yn >= lo && yn <= hi)) {   // a step that rounds to nothing stays on the end it started from
           st = 2;
         } else {
           dprev = fabs(rn - r0);
@@ -619,7 +619,7 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
           if (gv < 0.0) lo = y; else hi = y;
           const double rn = fma(-gv, rcp_nr<1>(gp), r);
           const double yn = rn * rn;
-          if (!(gp > 0.0 && yn > lo && yn < hi)) {
+          if (!(gp > 0.0 && yn >= lo && yn <= hi)) {   // a step that rounds to nothing stays on the end it started from
             st = 2;
           } else {
             const double d = fabs(rn - r);

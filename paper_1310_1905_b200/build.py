@@ -29,7 +29,11 @@ def _stale(target, sources):
 
 
 def build(force=False, verbose=False):
+    """Compiles csrc/*.cu and links libsdm.so.  SDM_NVCC_EXTRA (environment) appends flags, e.g. -D tuning macros,
+    to every unit and forces a rebuild."""
     os.makedirs(OBJ, exist_ok=True)
+    env_extra = os.environ.get("SDM_NVCC_EXTRA", "").split()
+    force = force or bool(env_extra)
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
     objs = []
     for src, extra in UNITS.items():
@@ -37,7 +41,7 @@ def build(force=False, verbose=False):
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + hdrs):
-            cmd = [NVCC] + ARCH + COMMON + extra + ["-c", s, "-o", o]
+            cmd = [NVCC] + ARCH + COMMON + extra + env_extra + ["-c", s, "-o", o]
             r = subprocess.run(cmd, capture_output=True, text=True)
             log = r.stdout + r.stderr
             with open(o + ".log", "w") as f:

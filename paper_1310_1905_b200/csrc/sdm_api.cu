@@ -13,8 +13,10 @@ using namespace sdm;
 namespace {
 thread_local std::string g_create_error;
 constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are willing to ask for per CTA
-constexpr size_t kCondSmemPerCta = 44 * 1024;    // per CTA, so that five condensation CTAs share an SM
-constexpr double kCondTileTarget = 700.0;   // SDs per condensation tile (mean); 5 sigma above fits 44 KB
+#ifndef SDM_COND_TILE_TARGET
+#define SDM_COND_TILE_TARGET 660.0
+#endif
+constexpr double kCondTileTarget = SDM_COND_TILE_TARGET;   // SDs per condensation tile (mean); 5 sigma above fits the 800 slots of k_cond4
 constexpr double kCondMaxCpb = 128.0;       // one thread per cell of the tile
 }
 
@@ -368,18 +370,19 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   }
   ctx->have_order = true;
   if (op->cond) {
-    // largest candidate tile size whose most populated tile fits the shared memory of 2 CTAs per SM; a single
-    // crowded cell may take the whole SM; beyond that the kernel works in place in HBM/L2
-    int cpb = 1, cap = 0;
-    for (int k = 0; k < 4 && cap == 0; ++k) {
-      const int cand = std::max(1, ctx->cond_cpb0 >> k);
-      const int need = std::max(((int)ctx->h_info[4 + k] + 3) / 4 * 4, 4);
-      if (cond3_smem_bytes(cand, need) <= (cand > 1 ? kCondSmemPerCta : kSmemLimit)) { cpb = cand; cap = need; }
-      if (cand == 1) break;
+    // largest candidate tile that fits the small tile kernel, else the large one, else one cell per CTA in place
+    int cpb = 1, variant = cond_variant(1, (int)ctx->max_nc);
+    for (int want = 1; want <= 2; ++want) {
+      bool found = false;
+      for (int k = 0; k < 4 && !found; ++k) {
+        const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
+        if (cond_variant(cand, (int)ctx->h_info[4 + k]) == want) { cpb = cand; variant = want; found = true; }
+      }
+      if (found || variant == want) break;
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
     t_begin(ctx, SDM_STAGE_COND, st);
-    CK(launch_cond(cpb, cap, ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp,
+    CK(launch_cond(cpb, variant, ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp,
                    ctx->cnt, st));
     t_end(ctx, SDM_STAGE_COND, st);
   } else {

@@ -77,8 +77,43 @@ __device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c
   df = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
 }
 
-// ---- fast path (k_cond3): the same equations written in r = sqrt(y), which stays resident in shared
+// ---- fast path (k_cond4): the same equations written in r = sqrt(y), which stays resident in shared
 // memory over the substeps (no sqrt per substep), with one reciprocal per evaluation.
+// fp64 literals cost two UMOV/MOV issue slots each on sm_100 (64-bit immediates do not exist), which in
+// a polynomial doubles the instruction count; constants that the hot loop needs therefore live in
+// constant memory, where one LDCU.128 fetches two of them into uniform registers.
+enum {
+  KC_LOG2E = 0, KC_MAGIC, KC_LN2_HI, KC_LN2_LO,   // exp: range reduction
+  KC_E13, KC_E12, KC_E11, KC_E10, KC_E9, KC_E8, KC_E7, KC_E6, KC_E5, KC_E4, KC_E3, KC_E2,   // 1/n!
+  KC_TOL, KC_TOL400, KC_EPSW, KC_D0, KC_HALF_D0, KC_K0, KC_HALF_K0, KC_171,
+  KC_D2Q, KC_B1, KC_B2, KC_B3, KC_B4, KC_B5,   // delta0^2/4; binomial series of (1+x)^(1/3) - 1
+  KC_N
+};
+__constant__ double KC[KC_N] = {
+    1.4426950408889634074, 6755399441055744.0 /* 1.5 * 2^52 */, 6.93147180369123816490e-01, 1.90821492927058770002e-10,
+    1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0, 1.0 / 5040.0,
+    1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5,
+    1e-11, 1e-11 / 400.0, 1e-15, cst::D_0, 0.5 * cst::D_0, cst::K_0, 0.5 * cst::K_0, 1.71,
+    cst::kc_delta0 * cst::kc_delta0 / 4.0, 1.0 / 3.0, -1.0 / 9.0, 5.0 / 81.0, -10.0 / 243.0, 22.0 / 729.0};
+
+// exp(t) for 0 <= t < 8 (t = A/r, the Kelvin exponent): n = rint(t log2 e) by the 1.5*2^52 trick,
+// s = t - n ln 2 in two parts (|s| <= 0.347), Taylor polynomial of degree 13 (remainder
+// 0.347^14/14! = 4e-18), result scaled by 2^n through the exponent field.  No overflow, underflow
+// or NaN handling: the caller keeps t in range and sends everything else to cond_solve.
+__device__ __forceinline__ double exp_kelvin(double t) {
+  const double z = fma(t, KC[KC_LOG2E], KC[KC_MAGIC]);
+  const int n = __double2loint(z);
+  const double fn = z - KC[KC_MAGIC];
+  double s = fma(-fn, KC[KC_LN2_HI], t);
+  s = fma(-fn, KC[KC_LN2_LO], s);
+  double p = KC[KC_E13];
+  p = fma(p, s, KC[KC_E12]); p = fma(p, s, KC[KC_E11]); p = fma(p, s, KC[KC_E10]); p = fma(p, s, KC[KC_E9]);
+  p = fma(p, s, KC[KC_E8]); p = fma(p, s, KC[KC_E7]); p = fma(p, s, KC[KC_E6]); p = fma(p, s, KC[KC_E5]);
+  p = fma(p, s, KC[KC_E4]); p = fma(p, s, KC[KC_E3]); p = fma(p, s, KC[KC_E2]);
+  p = fma(p, s, 1.0); p = fma(p, s, 1.0);
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+}
+
 // 1/a from the hardware seed (MUFU.RCP64H, ~2^-20) and NR Newton-Raphson refinements (2 -> < 1 ulp)
 template <int NR>
 __device__ __forceinline__ double rcp_nr(double a) {
@@ -94,15 +129,15 @@ __device__ __forceinline__ double rcp_nr(double a) {
 
 struct CellR {   // per-cell constants of one substep used by the fast path
   double RH, A, lD, lK, qD, qK, lD171, lK171;
-  float kE, Sc, Pr;
 };
 
-// f(r) = d r_w^2/dt (eq. 20-24) and df/dr; also returns y = r^2.  Notation as growth_fd.
-__device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c, double& y, double& f, double& dfr) {
+// f(r) = d r_w^2/dt (eq. 20-24) and df/dr; also returns y = r^2 and t = A/r.  Notation as growth_fd.
+__device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c, double& y, double& f, double& dfr,
+                                         double& t_out) {
   y = r * r;
   const double lDr = c.lD * r, lKr = c.lK * r;
-  const double NM = y + lDr, DM = fma(1.71, lDr, y) + c.qD;
-  const double NT = y + lKr, DT = fma(1.71, lKr, y) + c.qK;
+  const double NM = y + lDr, DM = fma(KC[KC_171], lDr, y) + c.qD;
+  const double NT = y + lKr, DT = fma(KC[KC_171], lKr, y) + c.qK;
   const double KN = s.Kc * NT, HN = s.hDc * NM;
   const double Q = fma(KN, DM, HN * DT);
   const double r3 = y * r;
@@ -111,7 +146,8 @@ __device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c,
   const double inv = rcp_nr<2>(r * QW);
   const double invr = inv * QW, invQ = inv * (r * W), invW = inv * (r * Q);
   const double t = c.A * invr;
-  const double ex = exp(t);
+  t_out = t;
+  const double ex = exp_kelvin(t);
   const double NN = NM * NT;
   const double aw = P * invW;
   const double S = fma(-aw, ex, c.RH);
@@ -127,50 +163,57 @@ __device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c,
   dfr = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
 }
 
-// (1+x)^(1/3) - 1 by the binomial series, truncation < 1e-17 for 0 <= x < 0.02
-__device__ __forceinline__ double cbrt1pm1_small(double x) {
-  double p = -935.0 / 59049.0;
-  p = fma(p, x, 374.0 / 19683.0);
-  p = fma(p, x, -154.0 / 6561.0);
-  p = fma(p, x, 22.0 / 729.0);
-  p = fma(p, x, -10.0 / 243.0);
-  p = fma(p, x, 5.0 / 81.0);
-  p = fma(p, x, -1.0 / 9.0);
-  p = fma(p, x, 1.0 / 3.0);
-  return p * x;
+// sqrt(a) and 1/a from the fp32 hardware seeds and ONE fp64 Newton step (relative error ~1e-14, which is
+// ample for the ventilation coefficients: they enter D and K through 1 + (Sh-2)/2)
+__device__ __forceinline__ double sqrt_seeded(double a) {
+  const float af = (float)a;
+  const float is = rsqrtf(af);
+  const double s = (double)(af * is);
+  return fma(fma(-s, s, a), (double)(0.5f * is), s);
+}
+__device__ __forceinline__ double rcp_seeded(double a) {
+  const double x = (double)__frcp_rn((float)a);
+  return fma(fma(-a, x, 1.0), x, x);
 }
 
 // [L] ventilation at the substep's starting radius r0 (reading R-vent) -> per-SD constants.
-// Re·Sc below 2.5e-4 (r0 below ~3 um): Sh - 2 < 1e-4 enters D only through 2 + (Sh - 2), so Re and the
-// series are evaluated in fp32 (relative error 3e-7 of a 1e-4 term: < 3e-11 of D).  Above: fp64.
-__device__ __forceinline__ void sd_setup(double r0, double c0, double heat, double kE, double Sc, double Pr,
-                                         const CellR& c, SdK& s) {
-  const float rf = (float)r0;
-  const float ef = c.kE * rf * sqrtf(rf);
-  const float qf = ef / (sqrtf(1.0f + ef) + 1.0f);
-  const float Ref = (float)(cst::kc_delta0 * cst::kc_delta0 / 4.0) * (qf * qf);
-  const float xs = Ref * c.Sc, xp = Ref * c.Pr;
+// Re from the terminal velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2),
+// Re = (delta0^2/4) (sqrt(1+e) - 1)^2.  Up to Re Sc = 0.02 (r ~ 20 um): fp64 with seeded roots and the
+// binomial series of (1+x)^(1/3) - 1 to x^5 (next term 2e-10 of the first).  Beyond (drizzle and rain)
+// Sh - 2 and Nu - 2 are evaluated in fp32 by formulas that keep their RELATIVE error below 2e-6;
+// D = D_0 (1 + (Sh-2)/2) is then off by at most eps_D = 2e-6 min((Sh-2)/2, 1), likewise K, and f of
+// eq. 20-21 by at most eps_D + eps_K relative.  The implicit step moves r_w^2 by less than |2 dt' f(y0)|
+// (eq. 18-19), so the caller accepts these constants only if (eps_D + eps_K) |2 dt' f0| <= 1e-10 y0 and
+// otherwise leaves the SD to cond_solve, which evaluates everything in fp64.  Returns eps_D + eps_K.
+__device__ __forceinline__ float sd_setup(double r0, double c0, double heat, double kE, double Sc, double Pr, SdK& s) {
+  const double e = kE * (r0 * sqrt_seeded(r0));
+  const double q = e * rcp_seeded(sqrt_seeded(1.0 + e) + 1.0);   // sqrt(1+e) - 1 without cancellation
+  const double Re = KC[KC_D2Q] * (q * q);
+  const double xs = Re * Sc, xp = Re * Pr;
   double shm, num;   // Sh - 2, Nu - 2
-  if (fmaxf(xs, xp) < 2.5e-4f) {
-    shm = (double)(xs * (1.0f / 3.0f + xs * (-1.0f / 9.0f + xs * (5.0f / 81.0f))));
-    num = (double)(xp * (1.0f / 3.0f + xp * (-1.0f / 9.0f + xp * (5.0f / 81.0f))));
+  float eps = 0.f;
+  if (fmax(xs, xp) < 0.02) {
+    double a = KC[KC_B5], b = KC[KC_B5];
+    a = fma(a, xs, KC[KC_B4]); b = fma(b, xp, KC[KC_B4]);
+    a = fma(a, xs, KC[KC_B3]); b = fma(b, xp, KC[KC_B3]);
+    a = fma(a, xs, KC[KC_B2]); b = fma(b, xp, KC[KC_B2]);
+    a = fma(a, xs, KC[KC_B1]); b = fma(b, xp, KC[KC_B1]);
+    shm = a * xs; num = b * xp;
   } else {
-    const double e = kE * (r0 * sqrt(r0));
-    const double q = e / (sqrt(1.0 + e) + 1.0);
-    const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
-    const double x1 = Re * Sc, x2 = Re * Pr;
-    if (Re <= 1.0 && fmax(x1, x2) < 0.02) {
-      shm = cbrt1pm1_small(x1);
-      num = cbrt1pm1_small(x2);
-    } else {
-      shm = vent(Re, Sc) - 2.0;
-      num = vent(Re, Pr) - 2.0;
+    float sf = expm1f(log1pf((float)xs) * (1.0f / 3.0f)), nf = expm1f(log1pf((float)xp) * (1.0f / 3.0f));
+    if (Re > 1.0) {   // (1 + c)(1 + m) - 1, m = Re^0.077 - 1
+      const float m = expm1f(0.077f * logf((float)Re));
+      sf = sf + m + sf * m;
+      nf = nf + m + nf * m;
     }
+    shm = (double)sf; num = (double)nf;
+    eps = 2e-6f * (fminf(0.5f * sf, 1.0f) + fminf(0.5f * nf, 1.0f));
   }
-  const double Dc = fma(0.5 * cst::D_0, shm, cst::D_0);   // eq. 23 without beta_M: D_0 Sh / 2
-  s.Kc = fma(0.5 * cst::K_0, num, cst::K_0);              // eq. 24 without beta_T: K_0 Nu / 2
+  const double Dc = fma(KC[KC_HALF_D0], shm, KC[KC_D0]);   // eq. 23 without beta_M: D_0 Sh / 2
+  s.Kc = fma(KC[KC_HALF_K0], num, KC[KC_K0]);              // eq. 24 without beta_T: K_0 Nu / 2
   s.hDc = heat * Dc;
   s.cDK = c0 * Dc * s.Kc;
+  return eps;
 }
 
 // One condensation substep of one SD: root of g(y) = y - y0 - dt' f(y) in [a, b] of eq. 18-19
@@ -482,59 +525,145 @@ k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __rest
   }
 }
 
-// ---- k_cond3: the shared-memory tile kernel, third version ---------------------------------------
-// Differences from k_cond<true> (kept above for cells too crowded for shared memory):
+// ---- k_cond4: the shared-memory tile kernel ----------------------------------------------------------
+// A CTA of T threads owns a tile of `cpb` consecutive cells holding at most CAP super-droplets.
 //  * r_w (not r_w^2) is resident in shared memory: no sqrt per substep, N d(r_w^3) by two products;
 //  * the sweep is straight-line code around growth_r with a warp-uniform iteration loop; anything
-//    irregular (Newton leaving the bracket of eq. 18-19, an end to verify, slow convergence) is
-//    put on a WARP-private list and solved afterwards by cond_solve, the robust state machine;
-//  * small CTAs (T3 threads, several per SM) so that the serial phases of one tile (cell constants,
-//    slow list, barriers) overlap the sweeps of the others.
-// Shared memory: double cell[C3_N * cpb]; double sd[6 * cap] = r, r_d^3, kappa r_d^3, N, r_d^2,
-// N d(r_w^3); float cellf[3 * cpb]; u32 segl[cpb + 1]; u16 cidx[cap]; u16 list[lstride * warps].
-constexpr int C3_N = 12;   // RH, A, c0, lD, lK, heat, kE, Sc, Pr, qD, qK, sum
-constexpr int T3 = 128;
-static int c3_lstride(int cap) { return ((cap + T3 - 1) / T3) * 32; }
-size_t cond3_smem_bytes(int cpb, int cap) {
-  return (size_t)C3_N * cpb * 8 + (size_t)6 * cap * 8 + (size_t)3 * cpb * 4 + (size_t)(cpb + 1) * 4 + (size_t)cap * 2 +
-         (size_t)c3_lstride(cap) * (T3 / 32) * 2 + 32;
+//    irregular (Newton leaving the bracket of eq. 18-19, an end to verify, slow convergence, a Kelvin
+//    exponent or a ventilation error bound out of range) is put on a list and solved afterwards by
+//    cond_solve, the robust state machine;
+//  * warps take 32-SD chunks of the tile from a shared counter, so a warp that met slow SDs does not
+//    hold the others at the barrier;
+//  * CAP is a compile-time constant, so every shared array sits at a fixed offset from one index
+//    register, and the per-cell constants are one record per cell fetched with LDS.128;
+//  * the state of a cell (theta, r_v, T, p_vs ..) lives in that record between substeps, not in
+//    registers, and is advanced INCREMENTALLY: the feedback of eq. 25-26 changes theta by a relative
+//    d ~ 1e-5 per substep, so T (eq. 43) and p_vs follow from short series in d instead of pow, exp
+//    and log; each warp sums and advances the cells it owns, which takes the serial chain from ~560
+//    instructions on one warp (with three waiting at a barrier) to ~150 on all of them;
+//  * small CTAs (128 threads, 5 per SM) so that the serial phases of one tile overlap the sweeps of
+//    the others; a 512-thread variant with CAP 4096 serves cells of hundreds to thousands of SDs.
+// Shared memory: double sd[6][CAP] = r, r_d^3, kappa r_d^3, N, r_d^2, N d(r_w^3); u16 cidx[CAP];
+// u16 list[CAP]; CellRec cell[cpb]; u32 segl[cpb + 1]; u32 ctr[2].
+struct __align__(16) CellRec {
+  double RH, A, lD, lK, qD, qK, lD171, lK171;   // fast path (CellR)
+  double c0, heat, kE, Sc, Pr;                  // cond_solve and the per-SD set-up
+  double eta;                                   // [L] viscosity, for the cell fields written at the end
+  double th, rv, rhod, fbk;                     // theta, r_v (advanced every substep), rho_d, eq. 25 prefactor
+  double T, invT, lv, pvs;                      // eq. 43, Table 2, [L] Clausius-Clapeyron
+};
+static_assert(sizeof(CellRec) == 176, "CellRec");
+
+// everything the substep needs from (T, 1/T, p_vs, r_v, rho_d); square roots and reciprocals from fp32
+// seeds (sqrt_seeded, rcp_nr: relative error < 1e-14, they feed correction factors and RH to 1e-15)
+__device__ __forceinline__ void cell_derive(CellRec& R, double RH_max) {
+  const double T = R.T, invT = R.invT, rv = R.rv, rhod = R.rhod;
+  const double p = rhod * (cst::R_d + rv * cst::R_v) * T;                          // eq. 44
+  const double lv = cst::l_v0 + (cst::c_pv - cst::c_l) * (T - cst::T_0);           // Table 2 :1087
+  const double rho_vs = R.pvs * invT * (1.0 / cst::R_v);
+  R.lv = lv;
+  R.RH = fmin(rv * rhod * rcp_nr<2>(rho_vs), RH_max);                              // eq. 30, :685
+  R.A = (2.0 * cst::sigma_w / (cst::R_v * cst::rho_w)) * invT;                     // Table 2 :1056
+  R.c0 = (2.0 / cst::rho_w) * rho_vs;
+  const double sqT = sqrt_seeded(T);
+  const double lD = (2.0 * cst::D_0 * 0.03291540093383166 /* 1/sqrt(2 R_v) */) * (sqT * invT);   // [L] Fuchs-Sutugin lengths
+  const double lK = ((4.0 / 5.0) * cst::K_0 * 0.04173919355648411 /* 1/sqrt(2 R_d) */) * (sqT * rcp_nr<2>(p));
+  R.lD = lD; R.lK = lK;
+  R.qD = 1.33 * (lD * lD); R.qK = 1.33 * (lK * lK); R.lD171 = 1.71 * lD; R.lK171 = 1.71 * lK;
+  const double lvT = lv * invT;
+  R.heat = (rho_vs * lvT) * (lvT * (1.0 / cst::R_v) - 1.0);                        // eq. 21
+  // eta = 1.72e-5 (393/(T+120)) (T/273)^1.5
+  const double eta = (1.72e-5 * 393.0 * 2.2169506691164923e-4 /* 273^-1.5 */) * (T * sqT) * rcp_nr<2>(T + 120.0);
+  const double rho_a = rhod * (1.0 + rv);
+  const double inv_eta = rcp_nr<2>(eta);
+  // e = c1 sqrt(X), X = (32/3) r^3 (rho_w - rho_a) g rho_a / eta^2  ->  e = kE r^(3/2)
+  const double c1 = 4.0 / (cst::kc_delta0 * cst::kc_delta0 * 0.5403702434442518 /* sqrt(C0) */);
+  R.kE = c1 * sqrt_seeded((32.0 / 3.0 * cst::g) * ((cst::rho_w - rho_a) * rho_a)) * inv_eta;
+  R.Sc = eta * rcp_nr<2>(rho_a * cst::D_0);
+  R.Pr = eta * (cst::c_pd / cst::K_0);
+  R.eta = eta;
 }
 
-__global__ void __launch_bounds__(T3, 5)
-k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
-        CellFields cf, CondParams cp, Counters cnt, int cpb, int cap, int lstride) {
+// first substep: T from eq. 43 and p_vs from the Clausius-Clapeyron integral, as cell_consts
+__device__ __forceinline__ void cell_init(CellRec& R, double RH_max) {
+  const double c_exn = pow(R.rhod * cst::R_d / cst::p_1000, cst::R_d / cst::c_pd);
+  const double T = pow(R.th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
+  const double ca = (cst::l_v0 + (cst::c_l - cst::c_pv) * cst::T_0) / cst::R_v;
+  const double cb = (cst::c_l - cst::c_pv) / cst::R_v;
+  R.T = T; R.invT = 1.0 / T;
+  R.pvs = cst::p_vs0 * exp(ca * (1.0 / cst::T_0 - 1.0 / T) - cb * log(T / cst::T_0));
+  cell_derive(R, RH_max);
+}
+
+// Feedback of one substep (eq. 25-26 with the old theta and T, :195) and the new T, p_vs.
+// theta' = theta (1 + d), d = -drv l_v/(c_pd T);  T' = T (1+d)^g, g = c_pd/(c_pd - R_d) (eq. 43, rho_d fixed):
+// u = g log1p(d) and T'/T - 1 = expm1(u) by their series (|d| <= 1e-3: truncation < 1e-18);
+// p_vs'/p_vs = exp(v), v = ca (1/T - 1/T') - cb log(T'/T) = ca expm1(u)/T' - cb u.
+// `full` (first substep of a step, or an implausibly large d) recomputes from theta.
+__device__ __forceinline__ void cell_advance(CellRec& R, double sum, double RH_max, bool apply) {
+  if (apply) {
+    const double drv = R.fbk * sum;
+    const double d = -drv * R.lv * R.invT * (1.0 / cst::c_pd);
+    R.th = fma(R.th, d, R.th);
+    R.rv += drv;
+    if (fabs(d) > 1e-3) { cell_init(R, RH_max); return; }
+    const double l = d * fma(d, fma(d, fma(d, fma(d, 0.2, -0.25), 1.0 / 3.0), -0.5), 1.0);   // log1p(d)
+    const double u = (cst::c_pd / (cst::c_pd - cst::R_d)) * l;
+    const double em = u * fma(u, fma(u, fma(u, fma(u, 1.0 / 120.0, 1.0 / 24.0), 1.0 / 6.0), 0.5), 1.0);   // expm1(u)
+    const double T = fma(R.T, em, R.T);
+    const double invT = rcp_nr<2>(T);
+    const double ca = (cst::l_v0 + (cst::c_l - cst::c_pv) * cst::T_0) / cst::R_v;
+    const double cb = (cst::c_l - cst::c_pv) / cst::R_v;
+    const double v = fma(ca * em, invT, -cb * u);
+    R.pvs *= exp_kelvin(v);
+    R.T = T; R.invT = invT;
+  }
+  cell_derive(R, RH_max);
+}
+
+template <int CAP, int T>
+struct Cond4 {
+  static constexpr int NW = T / 32;
+  static constexpr size_t fixed_bytes = (size_t)6 * CAP * 8 + (size_t)CAP * 2 + (size_t)CAP * 2;
+  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CellRec) + (size_t)(cpb + 1) * 4 + 16; }
+};
+
+template <int CAP, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB)
+k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+        CellFields cf, CondParams cp, Counters cnt, int cpb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int NW = T3 / 32;
+  using L = Cond4<CAP, T>;
+  constexpr int NW = L::NW;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c_first = blockIdx.x * cpb;
   const int nc = min(cpb, g.ncell - c_first);
-  double* s_cell = reinterpret_cast<double*>(smem_raw);
-  double* s_sum = s_cell + 11 * cpb;
-  double* s_r = s_cell + C3_N * cpb;
-  double *s_rd3 = s_r + cap, *s_krd3 = s_r + 2 * cap, *s_dn = s_r + 3 * cap, *s_rd2 = s_r + 4 * cap, *s_con = s_r + 5 * cap;
-  float* s_cf = reinterpret_cast<float*>(s_r + 6 * cap);
-  u32* segl = reinterpret_cast<u32*>(s_cf + 3 * cpb);
-  u16* cidx = reinterpret_cast<u16*>(segl + cpb + 1);
-  u16* mylist = cidx + ((cap + 1) & ~1) + warp * lstride;
+  double* s_r = reinterpret_cast<double*>(smem_raw);
+  double *s_rd3 = s_r + CAP, *s_krd3 = s_r + 2 * CAP, *s_dn = s_r + 3 * CAP, *s_rd2 = s_r + 4 * CAP, *s_con = s_r + 5 * CAP;
+  u16* cidx = reinterpret_cast<u16*>(s_r + 6 * CAP);
+  u16* list = cidx + CAP;
+  CellRec* s_cell = reinterpret_cast<CellRec*>(smem_raw + L::fixed_bytes);
+  u32* segl = reinterpret_cast<u32*>(s_cell + cpb);
+  u32* ctr = segl + cpb + 1;   // [0] next chunk of the sweep, [1] length of the slow list
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
 
-  // thread `tid` owns cell c_first + tid: theta, r_v and the feedback live in its registers
-  double th = 0, rv = 0, rhod = 1, c_exn = 0, fbk = 0, T = 0, lv = 0;
-  int ci = 0, cj = 0, ck = 0;
-  if (tid < nc) {
-    const int c = c_first + tid;
-    ck = c % g.NZ; cj = (c / g.NZ) % g.NY; ci = c / (g.NZ * g.NY);
-    th = th_f.at(ci, cj, ck); rv = rv_f.at(ci, cj, ck);
-    rhod = cf.rhod[c];
-    c_exn = pow(rhod * cst::R_d / cst::p_1000, cst::R_d / cst::c_pd);
-    fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
-    segl[tid] = seg[c] - s0;
-    s_sum[tid] = 0.0;
+  // cell cl of the tile is owned by lane cl / NW of warp cl % NW (cpb <= T)
+  const int cl_own = lane * NW + warp;
+  const bool owner = cl_own < nc;
+  if (owner) {
+    const int c = c_first + cl_own;
+    const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+    CellRec& R = s_cell[cl_own];
+    R.th = th_f.at(i, j, k); R.rv = rv_f.at(i, j, k);
+    const double rhod = cf.rhod[c];
+    R.rhod = rhod;
+    R.fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
+    segl[cl_own] = seg[c] - s0;
   }
-  if (tid == 0) segl[nc] = (u32)M;
+  if (tid == 0) { segl[nc] = (u32)M; ctr[0] = 0u; ctr[1] = 0u; }
   __syncthreads();
-  for (int t = tid; t < M; t += T3) {   // stage the tile in sorted order
+  for (int t = tid; t < M; t += T) {   // stage the tile in sorted order
     int lo = 0, hi = nc;
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
     const u32 s = s0 + t;
@@ -549,50 +678,58 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
     cidx[e] = (u16)lo;
   }
   unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
-  for (int sub = 0; sub < cp.sstp && M > 0; ++sub) {
-    // A. feedback of the previous substep (eq. 25-26, old theta and T) and the new cell constants
-    if (tid < nc) {
-      if (sub > 0) {
-        const double drv = fbk * s_sum[tid];
-        th += drv * (-th * lv / (cst::c_pd * T));
-        rv += drv;
+  const double dtp = cp.dtp;
+  const int nsub = M > 0 ? cp.sstp : 0;
+  for (int sub = 0; sub <= nsub; ++sub) {
+    // D + A. every warp sums N d(r_w^3) of the cells it owns (sorted order: lane-strided partial sums, xor
+    // butterfly), then their owner lanes apply the feedback and derive the constants of the next substep;
+    // the pass after the last substep only applies the feedback.
+    double mysum = 0.0;
+    if (sub > 0) {
+      for (int j = 0; j * NW + warp < nc; ++j) {
+        const int cl = j * NW + warp;
+        const int b0 = (int)segl[cl], b1 = (int)segl[cl + 1];
+        double acc = 0.0;
+        for (int e = b0 + lane; e < b1; e += 32) acc += s_con[e];
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        if (lane == j) mysum = acc;
       }
-      CellK c;
-      cell_consts(th, rv, rhod, c_exn, cp.RH_max, c, T, lv);
-      s_cell[0 * cpb + tid] = c.RH; s_cell[1 * cpb + tid] = c.A; s_cell[2 * cpb + tid] = c.c0;
-      s_cell[3 * cpb + tid] = c.lD; s_cell[4 * cpb + tid] = c.lK; s_cell[5 * cpb + tid] = c.heat;
-      s_cell[6 * cpb + tid] = c.kE; s_cell[7 * cpb + tid] = c.Sc; s_cell[8 * cpb + tid] = c.Pr;
-      s_cell[9 * cpb + tid] = 1.33 * (c.lD * c.lD); s_cell[10 * cpb + tid] = 1.33 * (c.lK * c.lK);
-      s_cf[0 * cpb + tid] = (float)c.kE; s_cf[1 * cpb + tid] = (float)c.Sc; s_cf[2 * cpb + tid] = (float)c.Pr;
     }
+    if (owner) {
+      CellRec& R = s_cell[cl_own];
+      if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, mysum, cp.RH_max, true);
+    }
+    if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
+    if (sub == nsub) break;
     __syncthreads();
-    // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (warp-private list)
-    int nslow = 0;
-    const double dtp = cp.dtp;
-    for (int q0 = warp * 32; q0 < M; q0 += T3) {
+    // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (list)
+    for (;;) {
+      int q0 = 0;
+      if (lane == 0) q0 = (int)atomicAdd(&ctr[0], 32u);
+      q0 = __shfl_sync(0xffffffffu, q0, 0);
+      if (q0 >= M) break;
       const int e = q0 + lane;
       const bool valid = e < M;
-      const int cl = valid ? (int)cidx[e] : 0;
+      const CellRec& R = s_cell[valid ? (int)cidx[e] : 0];
       const double r0 = valid ? s_r[e] : 1e-6;
       const double rd2 = valid ? s_rd2[e] : 1e-14;
       SdK s;
       s.rd3 = valid ? s_rd3[e] : 1e-21;
       s.krd3 = valid ? s_krd3[e] : 1e-21;
       CellR c;
-      c.RH = s_cell[0 * cpb + cl]; c.A = s_cell[1 * cpb + cl]; c.lD = s_cell[3 * cpb + cl]; c.lK = s_cell[4 * cpb + cl];
-      c.qD = s_cell[9 * cpb + cl]; c.qK = s_cell[10 * cpb + cl];
-      c.lD171 = 1.71 * c.lD; c.lK171 = 1.71 * c.lK;
-      c.kE = s_cf[0 * cpb + cl]; c.Sc = s_cf[1 * cpb + cl]; c.Pr = s_cf[2 * cpb + cl];
-      sd_setup(r0, s_cell[2 * cpb + cl], s_cell[5 * cpb + cl], s_cell[6 * cpb + cl], s_cell[7 * cpb + cl],
-               s_cell[8 * cpb + cl], c, s);
-      double y0, f, dfr;
-      growth_r(r0, s, c, y0, f, dfr);
+      c.RH = R.RH; c.A = R.A; c.lD = R.lD; c.lK = R.lK; c.qD = R.qD; c.qK = R.qK; c.lD171 = R.lD171; c.lK171 = R.lK171;
+      const float eps = sd_setup(r0, R.c0, R.heat, R.kE, R.Sc, R.Pr, s);
+      double y0, f, dfr, t;
+      growth_r(r0, s, c, y0, f, dfr, t);
       n_eval += valid;
       const double two = 2.0 * dtp * f;
       double lo = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
       double hi = y0 + fmax(two, 0.0);              // eq. 19
       double r = r0, dprev = 0.0;
       int st;
+      // guards: the ventilation error bound (sd_setup) and the range of exp_kelvin
+      const bool guard = (eps > 0.f && eps * fabsf((float)two) > 1e-10f * (float)y0) || !(t < 4.0);
       if (!(lo < hi)) {
         st = (lo == y0) ? 1 : 2;                    // a = b: the result is a
       } else {
@@ -604,29 +741,30 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
         } else {
           dprev = fabs(rn - r0);
           r = rn;
-          st = (400.0 * (dprev * dprev) <= 1e-11 * (rn * rn)) ? 1 : 0;
+          st = (dprev * dprev <= KC[KC_TOL400] * (rn * rn)) ? 1 : 0;
         }
       }
+      if (guard) st = 2;
       if (!valid) st = 1;
       for (int it = 1; it < cp.kfast; ++it) {
         if (!__any_sync(0xffffffffu, st == 0)) break;
         if (st == 0) {
           double y;
-          growth_r(r, s, c, y, f, dfr);
+          growth_r(r, s, c, y, f, dfr, t);
           ++n_eval;
           const double gv = y - y0 - dtp * f;
           const double gp = fma(-dtp, dfr, r + r);
           if (gv < 0.0) lo = y; else hi = y;
           const double rn = fma(-gv, rcp_nr<1>(gp), r);
           const double yn = rn * rn;
-          if (!(gp > 0.0 && yn >= lo && yn <= hi)) {   // a step that rounds to nothing stays on the end it started from
+          if (!(gp > 0.0 && yn >= lo && yn <= hi && t < 4.0)) {
             st = 2;
           } else {
             const double d = fabs(rn - r);
-            const double tol = 1e-11 * rn, d2 = d * d;
+            const double tol = KC[KC_TOL] * rn, d2 = d * d;
             const bool conv = (4.0 * d2 <= tol * rn) && (2.0 * d2 * d <= tol * (dprev * dprev));
             r = rn; dprev = d;
-            if (conv || !(hi - lo > 1e-15 * hi)) st = 1;
+            if (conv || !(hi - lo > KC[KC_EPSW] * hi)) st = 1;
           }
         }
       }
@@ -637,20 +775,22 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
         ++n_sub;
       }
       const unsigned need = __ballot_sync(0xffffffffu, st == 2);
-      if (st == 2) mylist[nslow + __popc(need & ((1u << lane) - 1u))] = (u16)e;
-      nslow += __popc(need);
+      if (need) {   // warp-aggregated append to the tile's slow list
+        u32 base = 0;
+        if (lane == 0) base = atomicAdd(&ctr[1], (u32)__popc(need));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (st == 2) list[base + __popc(need & ((1u << lane) - 1u))] = (u16)e;
+      }
     }
-    __syncwarp();
+    __syncthreads();
     // C. the listed rest: the bracketed state machine, from the start of the substep
-    for (int k0 = 0; k0 < nslow; k0 += 32) {
-      const int k = k0 + lane;
-      if (k < nslow) {
-        const int e = (int)mylist[k];
-        const int cl = (int)cidx[e];
+    const int nlist = (int)ctr[1];
+    if (nlist > 0) {
+      for (int k = tid; k < nlist; k += T) {
+        const int e = (int)list[k];
+        const CellRec& R = s_cell[(int)cidx[e]];
         CellK c;
-        c.RH = s_cell[0 * cpb + cl]; c.A = s_cell[1 * cpb + cl]; c.c0 = s_cell[2 * cpb + cl];
-        c.lD = s_cell[3 * cpb + cl]; c.lK = s_cell[4 * cpb + cl]; c.heat = s_cell[5 * cpb + cl];
-        c.kE = s_cell[6 * cpb + cl]; c.Sc = s_cell[7 * cpb + cl]; c.Pr = s_cell[8 * cpb + cl];
+        c.RH = R.RH; c.A = R.A; c.c0 = R.c0; c.lD = R.lD; c.lK = R.lK; c.heat = R.heat; c.kE = R.kE; c.Sc = R.Sc; c.Pr = R.Pr;
         const double r0 = s_r[e], y0 = r0 * r0;
         double y1 = y0;
         unsigned ill = 0;
@@ -661,34 +801,21 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
         s_con[e] = s_dn[e] * (r1 * r1 * r1 - r0 * y0);
         s_r[e] = r1;
       }
+      __syncthreads();
     }
-    __syncthreads();
-    // D. per-cell sum of N d(r_w^3) in sorted order: lane-strided partial sums, xor butterfly
-    for (int cl = warp; cl < nc; cl += NW) {
-      const int b0 = (int)segl[cl], b1 = (int)segl[cl + 1];
-      double acc = 0.0;
-      for (int e = b0 + lane; e < b1; e += 32) acc += s_con[e];
-#pragma unroll
-      for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-      if (lane == 0) s_sum[cl] = acc;
-    }
-    __syncthreads();
   }
 
-  if (tid < nc) {
-    if (M > 0) {   // feedback of the last substep
-      const double drv = fbk * s_sum[tid];
-      th += drv * (-th * lv / (cst::c_pd * T));
-      rv += drv;
-    }
-    th_f.at(ci, cj, ck) = th;
-    rv_f.at(ci, cj, ck) = rv;
+  if (owner) {
+    const int c = c_first + cl_own;
+    const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+    const CellRec& R = s_cell[cl_own];
+    th_f.at(i, j, k) = R.th;
+    rv_f.at(i, j, k) = R.rv;
     // air properties after the feedback, used by coalescence and sedimentation (v_term)
-    const double Tn = pow(th * c_exn, cst::c_pd / (cst::c_pd - cst::R_d));
-    cf.eta[c_first + tid] = eta_air(Tn);
-    cf.rho_a[c_first + tid] = rhod * (1.0 + rv);
+    cf.eta[c] = R.eta;
+    cf.rho_a[c] = R.rhod * (1.0 + R.rv);
   }
-  for (int t = tid; t < M; t += T3) {
+  for (int t = tid; t < M; t += T) {
     int lo = 0, hi = nc;
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
     const u32 s = s0 + t;
@@ -712,6 +839,23 @@ k_cond3(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
   }
 }
 
+// the two instantiations: sparse cells (5 CTAs of 128 threads per SM) and crowded cells (one CTA of 512)
+#ifndef SDM_COND_CAP
+#define SDM_COND_CAP 800   // SD slots of the small tile kernel
+#define SDM_COND_MINB 5    // its CTAs per SM
+#endif
+using CondSmall = Cond4<SDM_COND_CAP, 128>;
+using CondLarge = Cond4<4096, 512>;
+constexpr size_t kCondSmallBudget = (228 * 1024 - SDM_COND_MINB * 1024) / SDM_COND_MINB;   // per CTA, 1 KB reserved each
+constexpr size_t kCondLargeBudget = 226 * 1024;
+
+// 1: small tile kernel, 2: large tile kernel, 0: a tile of cpb cells with up to `need` SDs fits neither
+int cond_variant(int cpb, int need) {
+  if (cpb <= 128 && need <= SDM_COND_CAP && CondSmall::smem(cpb) <= kCondSmallBudget) return 1;
+  if (cpb <= 512 && need <= 4096 && CondLarge::smem(cpb) <= kCondLargeBudget) return 2;
+  return 0;
+}
+
 // eta, rho_a per cell when condensation is switched off
 __global__ void k_thermo(Grid g, Field th_f, Field rv_f, CellFields cf) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -723,17 +867,22 @@ __global__ void k_thermo(Grid g, Field th_f, Field rv_f, CellFields cf) {
   cf.rho_a[c] = rhod * (1.0 + rv);
 }
 
-// cpb cells per CTA; cap > 0: shared-memory slots per CTA (>= the most populated tile); cap == 0: GMEM
-// variant (cpb must be 1), `alt` = the idle ping-pong copy of the state used as scratch.
-cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+// variant as returned by cond_variant(cpb, need); 0: work in place in global memory (cpb must be 1),
+// `alt` = the idle ping-pong copy of the state used as scratch.
+cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st) {
   const int grid = (g.ncell + cpb - 1) / cpb;
-  if (cap > 0) {
-    const size_t smem = cond3_smem_bytes(cpb, cap);
-    cudaError_t e = cudaFuncSetAttribute(k_cond3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (variant == 1) {
+    const size_t smem = CondSmall::smem(cpb);
+    cudaError_t e = cudaFuncSetAttribute(k_cond4<SDM_COND_CAP, 128, SDM_COND_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_cond3<<<grid, T3, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb, cap, c3_lstride(cap));
+    k_cond4<SDM_COND_CAP, 128, SDM_COND_MINB><<<grid, 128, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  } else if (variant == 2) {
+    const size_t smem = CondLarge::smem(cpb);
+    cudaError_t e = cudaFuncSetAttribute(k_cond4<4096, 512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_cond4<4096, 512, 1><<<grid, 512, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
   } else {
     const size_t smem = cond_smem_bytes(cpb, 0);
     k_cond<false><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);

@@ -39,13 +39,15 @@ cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 ste
 void launch_export_order(const u32* id, const u16* rank, const u32* seg, int ncell, u32* ids_sorted, cudaStream_t st);
 
 // sdm_cond.cu
-// cpb: cells per CTA; cap: shared-memory SD slots per CTA (>= most populated tile) or 0 to work in place in
-// global memory (cpb == 1, `alt` = idle ping-pong copy used as scratch)
-cudaError_t launch_cond(int cpb, int cap, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+// cpb: cells per CTA; variant = cond_variant(cpb, most populated tile): 1 / 2 = shared-memory tile kernels for
+// sparse / crowded cells, 0 = fits neither: work in place in global memory (cpb == 1, `alt` = idle ping-pong
+// copy used as scratch)
+int cond_variant(int cpb, int need);
+int cond_tile_candidate(int cpb0, int k);   // k-th candidate tile size (cells) tried by k_tile_max, k = 0..3
+cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st);
 size_t cond_smem_bytes(int cpb, int cap);
-size_t cond3_smem_bytes(int cpb, int cap);   // the shared-memory tile kernel k_cond3 (cap > 0)
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);
 
 // sdm_coal_move.cu

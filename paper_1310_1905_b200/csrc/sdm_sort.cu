@@ -102,11 +102,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(u32* __restrict__ c
     if (base + k < ncell) { seg[base + k] = ex; ex += v[k]; count[base + k] = 0u; }   // histogram is left zeroed
 }
 
-// Most populated tile of cpb consecutive cells, for the 4 candidate tile sizes cpb_k = max(1, cpb0 >> k):
-// sizes the shared memory of the tile-resident condensation kernel (sdm_cond.cu).
+// Most populated tile of cpb consecutive cells, for the 4 candidate tile sizes cpb_k = cpb0, 3/4, 1/2, 1/4 of it:
+// picks the tile size of the tile-resident condensation kernel (sdm_cond.cu).
+__host__ __device__ inline int tile_candidate(int cpb0, int k) { return max(1, (cpb0 * (4 - k)) / 4); }
+int cond_tile_candidate(int cpb0, int k) { return tile_candidate(cpb0, k); }
 __global__ void __launch_bounds__(256) k_tile_max(const u32* __restrict__ seg, int ncell, int cpb0, u32* __restrict__ out4) {
   for (int k = 0; k < 4; ++k) {
-    const int cpb = max(1, cpb0 >> k);
+    const int cpb = tile_candidate(cpb0, k);
     const int ntile = (ncell + cpb - 1) / cpb;
     u32 mx = 0;
     for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < ntile; t += gridDim.x * blockDim.x)
@@ -171,6 +173,52 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_rank(const u32* __restric
   for (int t = grp.lane; t < m; t += G) rank[s0 + sidx[t]] = (u16)t;
 }
 
+// The same ranks for sparsely populated cells (m <= P <= 128) by COUNTING: the keys are unique, so the
+// rank of an SD is the number of keys of its cell below its own.  m^2 broadcast compares out of shared
+// memory instead of a log^2 network of barriers and swaps: no synchronisation after the keys are staged
+// and 3 instructions per compare, which for the ~64 SDs per cell of the 3D workload is several times
+// cheaper than the bitonic network (the network wins for hundreds of SDs per cell and stays in k_rank).
+template <int G>
+__global__ void __launch_bounds__(128) k_rank_count(const u32* __restrict__ id, const u32* __restrict__ seg, int ncell,
+                                                    u32 step, u32 seed_lo, u32 seed_hi, int P, u16* __restrict__ rank,
+                                                    int* __restrict__ d_error) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NG = 128 / G;
+  const int gi = threadIdx.x / G;
+  const Group<G> grp = make_group<G>(nullptr);
+  const int c = blockIdx.x * NG + gi;
+  if (c >= ncell) return;
+  u64* skey = reinterpret_cast<u64*>(smem_raw) + (size_t)gi * P;
+  const u32 s0 = seg[c];
+  const int m = (int)(seg[c + 1] - s0);
+  if (m > P) { if (grp.lane == 0) atomicExch(d_error, 1); return; }
+  if (m == 0) return;
+  const int m2 = (m + 1) & ~1;   // the compare loop reads key pairs; pad with the largest key
+  for (int t = grp.lane; t < m2; t += G) {
+    u64 key = ~0ull;
+    if (t < m) {
+      const u32 sid = id[s0 + t];
+      key = ((u64)shuffle_key(sid, step, 0u, seed_lo, seed_hi) << 32) | sid;
+    }
+    skey[t] = key;
+  }
+  grp.sync();
+  const ulonglong2* sk2 = reinterpret_cast<const ulonglong2*>(skey);
+  for (int t0 = grp.lane; t0 < m; t0 += 2 * G) {   // two of this lane's SDs per sweep over the cell's keys
+    const int t1 = t0 + G;
+    const u64 k0 = skey[t0], k1 = t1 < m ? skey[t1] : 0ull;
+    int r0 = 0, r1 = 0;
+#pragma unroll 4
+    for (int j = 0; j < (m2 >> 1); ++j) {
+      const ulonglong2 kk = sk2[j];
+      r0 += (kk.x < k0) + (kk.y < k0);
+      r1 += (kk.x < k1) + (kk.y < k1);
+    }
+    rank[s0 + t0] = (u16)r0;
+    if (t1 < m) rank[s0 + t1] = (u16)r1;
+  }
+}
+
 // ids in sorted order (parity export)
 __global__ void k_export_order(const u32* __restrict__ id, const u16* __restrict__ rank, const u32* __restrict__ seg,
                                int ncell, u32* __restrict__ ids_sorted) {
@@ -218,8 +266,27 @@ static cudaError_t launch_rank_t(const u32* id, const u32* seg, int ncell, u32 s
   return cudaGetLastError();
 }
 
+template <int G>
+static cudaError_t launch_rank_count_t(const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                                       u16* rank, int* d_error, cudaStream_t st) {
+  constexpr int NG = 128 / G;
+  k_rank_count<G><<<(ncell + NG - 1) / NG, 128, (size_t)NG * P * sizeof(u64), st>>>(id, seg, ncell, step, seed_lo, seed_hi, P,
+                                                                                  rank, d_error);
+  return cudaGetLastError();
+}
+
+// P = power of two >= the most populated cell.  Up to 128 SDs per cell the ranks come from counting,
+// beyond that from the bitonic network.
 cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
                         u16* rank, int* d_error, cudaStream_t st) {
+  if (P <= 128 && G <= 32) {
+    switch (G) {
+      case 4: return launch_rank_count_t<4>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+      case 8: return launch_rank_count_t<8>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+      case 16: return launch_rank_count_t<16>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+      default: return launch_rank_count_t<32>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    }
+  }
   switch (G) {
     case 4: return launch_rank_t<4>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
     case 8: return launch_rank_t<8>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);

@@ -44,6 +44,7 @@ struct sdm_ctx {
   double *th_dense = nullptr, *rv_dense = nullptr;   // for sdm_step_host
   u64 nslots = 0;            // host-known number of slots in use
   u64 max_nc = 0;
+  u32 tile_max[4] = {0, 0, 0, 0};   // most populated tile for the 4 candidate tile sizes of the last step_sync
   u64 step = 0;
   bool synced = false;       // step_sync of the current step done
   bool have_order = false;
@@ -336,7 +337,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   t_begin(ctx, SDM_STAGE_SCAN, st);
   launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
   t_end(ctx, SDM_STAGE_SCAN, st);
-  if (op->cond) { launch_tile_max(ctx->seg, g.ncell, ctx->cond_cpb0, ctx->d_info + 4, st); ctx->launches++; }
+  launch_tile_max(ctx->seg, g.ncell, ctx->cond_cpb0, ctx->d_info + 4, st);
+  ctx->launches++;
   ctx->launches += (ctx->nslots ? 1 : 0) + 3;
   CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 8 * sizeof(u32), cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(ctx->ev_info, st));
@@ -350,6 +352,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   ctx->cur ^= 1;
   ctx->nslots = ctx->h_info[ctx->cn];
   ctx->max_nc = ctx->h_info[2];
+  for (int k = 0; k < 4; ++k) ctx->tile_max[k] = ctx->h_info[4 + k];
   if (ctx->h_info[3]) return fail(ctx, SDM_ERR_CUDA, "sdm_step_sync: device-side error flag set (corrupted segment sizes)");
 
   // launch sizing from the measured occupancy
@@ -410,9 +413,18 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
       return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
     CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step};
+    int tile_cpb = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
+    for (int k = 0; k < 4 && !tile_cpb && sstp == 1 && !ctx->group_override; ++k) {
+      const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
+      if (coal_tile_fits(cand, (int)ctx->tile_max[k])) tile_cpb = cand;
+    }
     t_begin(ctx, SDM_STAGE_COAL_MOVE, st);
-    CK(launch_coal_move(G, cap, in_smem, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
-                        ctx->cnt, st));
+    if (tile_cpb)
+      CK(launch_coal_move_tile(tile_cpb, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
+                               ctx->cnt, st));
+    else
+      CK(launch_coal_move(G, cap, in_smem, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
+                          ctx->cnt, st));
     t_end(ctx, SDM_STAGE_COAL_MOVE, st);
     ctx->launches++;
   }

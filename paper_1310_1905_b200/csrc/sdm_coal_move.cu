@@ -217,6 +217,279 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArrays a, con
   }
 }
 
+// ---- k_coal_move_tile: the same stages for sstp_coal == 1, tile-resident -----------------------------
+// A CTA of T threads owns a tile of `cpb` consecutive cells (at most CAP - cpb SDs).  n, r_w^2, id and the
+// positions of the tile's SDs are copied into shared memory IN STORAGE ORDER by asynchronous copies
+// (cp.async: no registers, no stall, every copy of the tile in flight at once); the sorted order enters
+// through an inverse map inv[sorted position] = slot, built with every cell's segment padded to an even
+// length, so that thread t owns the pair of sorted positions (2t, 2t+1): all lanes are busy whatever
+// the cell populations are.  r_d^3 and kappa are touched (in global memory) only by the rare pairs that
+// collide, and n, r_w^2 are written back only where they changed: per SD the kernel reads 46 B and writes
+// 24 B of HBM.  The terminal velocity of every SD is evaluated once, in the pair pass (the lone SD of an
+// odd cell by the thread of its padded slot), and reused by the sedimentation.  The arithmetic is,
+// expression by expression, that of k_coal_move above (-fmad=false).
+#ifndef SDM_COAL_UNROLL
+#define SDM_COAL_UNROLL 1
+#endif
+constexpr int kCoalUnroll = SDM_COAL_UNROLL;
+struct __align__(8) CoalCell {
+  double eta, rho_a, scale;                 // air properties; eq. 27 factor n(n-1)/2 / floor(n/2)
+  double Cxl, Cxh, Cyl, Cyh, Czl, Czh;      // Courant numbers at the cell's faces (rho_d C / rho_d)
+  int i, j, k, pad;
+};
+
+template <int CAP, int T>
+struct CoalTile {
+  static constexpr size_t fixed_bytes = (size_t)CAP * (6 * 8 + 4 + 2);
+  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CoalCell) + (size_t)(cpb + 1) * 8 + 16; }
+};
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gmem_src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <int CAP, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB)
+k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, CellFields cf, CoalParams kp,
+                 CoalMoveParams mp, double* flux_slots, Counters cnt, int cpb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  using L = CoalTile<CAP, T>;
+  constexpr u16 NONE = 0xFFFFu;
+  const int tid = threadIdx.x;
+  const int c_first = blockIdx.x * cpb;
+  const int nc = min(cpb, g.ncell - c_first);
+  u64* s_n = reinterpret_cast<u64*>(smem_raw);
+  double* s_rw2 = reinterpret_cast<double*>(smem_raw) + CAP;
+  double* s_x = s_rw2 + CAP;
+  double* s_y = s_x + CAP;
+  double* s_z = s_y + CAP;
+  double* s_vt = s_z + CAP;
+  u32* s_id = reinterpret_cast<u32*>(s_vt + CAP);
+  u16* inv = reinterpret_cast<u16*>(s_id + CAP);
+  CoalCell* s_cell = reinterpret_cast<CoalCell*>(smem_raw + L::fixed_bytes);
+  u32* segl = reinterpret_cast<u32*>(s_cell + cpb);   // storage offsets of the tile's cells
+  u32* segp = segl + cpb + 1;                          // padded (even) offsets of the sorted positions
+  const u32 s0 = seg[c_first];
+  const int M = (int)(seg[c_first + nc] - s0);
+  const bool moving = mp.adve || mp.sedi;
+  const bool need_vt = mp.sedi && g.hz;
+  unsigned n_pairs = 0, n_coll = 0, n_tie = 0;
+  double flux = 0.0;
+  if (M > 0) {
+    // everything that does not need the sorted order starts right away
+#pragma unroll kCoalUnroll
+    for (int t = tid; t < M; t += T) {
+      const u32 s = s0 + t;
+      cp_async<8>(s_n + t, a.n + s);
+      cp_async<8>(s_rw2 + t, a.rw2 + s);
+      if (mp.coal) cp_async<4>(s_id + t, a.id + s);
+      if (moving) {
+        if (g.hx) cp_async<8>(s_x + t, a.x + s);
+        if (g.hy) cp_async<8>(s_y + t, a.y + s);
+        if (g.hz) cp_async<8>(s_z + t, a.z + s);
+      }
+    }
+    for (int cl = tid; cl < nc; cl += T) {
+      const int c = c_first + cl;
+      const u32 b0 = seg[c], b1 = seg[c + 1];
+      segl[cl] = b0 - s0;
+      const int m = (int)(b1 - b0);
+      CoalCell& C = s_cell[cl];
+      C.eta = cf.eta[c]; C.rho_a = cf.rho_a[c];
+      C.scale = m >= 2 ? (double)((u64)m * (u64)(m - 1) / 2) / (double)(m / 2) : 0.0;
+      const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+      C.i = i; C.j = j; C.k = k;
+      const double rhod = cf.rhod[c];
+      C.Cxl = C.Cxh = C.Cyl = C.Cyh = C.Czl = C.Czh = 0.0;
+      if (mp.adve) {
+        if (g.hx) { C.Cxl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod; C.Cxh = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod; }
+        if (g.hy) { C.Cyl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod; C.Cyh = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod; }
+        if (g.hz) { C.Czl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod; C.Czh = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod; }
+      }
+    }
+    if (tid == 0) segl[nc] = (u32)M;
+    __syncthreads();
+    if (tid < 32) {   // padded offsets: warp scan over the cells, 32 at a time
+      u32 carry = 0;
+      for (int c0 = 0; c0 <= nc; c0 += 32) {
+        const int cl = c0 + tid;
+        u32 v = 0;
+        if (cl < nc) { const u32 m = segl[cl + 1] - segl[cl]; v = m + (m & 1u); }
+        u32 inc = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const u32 t = __shfl_up_sync(0xffffffffu, inc, d); if (tid >= d) inc += t; }
+        if (cl <= nc) segp[cl] = carry + inc - v;
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+      }
+    }
+    __syncthreads();
+    const int MP = (int)segp[nc];
+    // inverse map of the sorted order
+    for (int t = tid; t < M; t += T) {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+      inv[(int)segp[lo] + rank[s0 + t]] = (u16)t;
+    }
+    for (int cl = tid; cl < nc; cl += T) {   // the padding slot of an odd cell
+      const u32 m = segl[cl + 1] - segl[cl];
+      if (m & 1u) inv[segp[cl] + m] = NONE;
+    }
+    cp_async_wait_all();
+    __syncthreads();
+    // ---- pairs of sorted positions (2t, 2t+1) -------------------------------------------------------------
+    if (mp.coal || need_vt) {
+      const double dtdv = g.dt / g.dV;
+      for (int t = tid; 2 * t < MP; t += T) {
+        const u32 both = reinterpret_cast<const u32*>(inv)[t];
+        const int ia = (int)(both & 0xFFFFu), ib = (int)(both >> 16);
+        const bool lone = ib == (int)NONE;
+        int lo = 0, hi = nc;   // the pair's cell: segp[lo] <= 2t < segp[lo + 1]
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segp[mid] <= (u32)(2 * t)) lo = mid; else hi = mid; }
+        const CoalCell& C = s_cell[lo];
+        const double ya = s_rw2[ia];
+        const double ra = sqrt(ya);
+        if (lone || !mp.coal) {
+          if (need_vt) {
+            s_vt[ia] = v_term(ra, C.eta, C.rho_a);
+            if (!lone) s_vt[ib] = v_term(sqrt(s_rw2[ib]), C.eta, C.rho_a);
+          }
+          continue;
+        }
+        const u64 na = s_n[ia], nb = s_n[ib];
+        const double yb = s_rw2[ib];
+        const double rb = sqrt(yb);
+        const bool afirst = na >= nb;            // j: larger N; tie -> first in order
+        const int j = afirst ? ia : ib, k = afirst ? ib : ia;
+        const u64 nj = afirst ? na : nb, nk = afirst ? nb : na;
+        const double yj = afirst ? ya : yb, yk = afirst ? yb : ya;
+        const double rj = afirst ? ra : rb, rk = afirst ? rb : ra;
+        double K;
+        if (kp.kernel == 1) {   // Golovin
+          const double vj = (4.0 / 3.0) * cst::pi * (yj * rj), vk = (4.0 / 3.0) * cst::pi * (yk * rk);
+          K = kp.golovin_b * (vj + vk);
+          if (need_vt) { s_vt[j] = v_term(rj, C.eta, C.rho_a); s_vt[k] = v_term(rk, C.eta, C.rho_a); }
+        } else {                // eq. 28
+          const double vj = v_term(rj, C.eta, C.rho_a), vk = v_term(rk, C.eta, C.rho_a);
+          s_vt[j] = vj; s_vt[k] = vk;
+          K = cst::pi * ((rj + rk) * (rj + rk)) * fabs(vj - vk);
+          if (kp.kernel == 2) {
+            const double rl = fmax(rj, rk), rs = fmin(rj, rk);
+            K = K * eff_lookup(kp, rl, rs / rl);
+          }
+        }
+        const double p = (((double)nj * K) * dtdv) * C.scale;   // eq. 27
+        const double u = coal_uniform(s_id[ia], mp.step, 0u, kp.seed_lo, kp.seed_hi);
+        const u64 qmax = nj / nk;
+        u64 gam;
+        if (kp.multi_coal) {
+          const double pf = floor(p);
+          if (pf >= (double)qmax) gam = qmax;
+          else {
+            const double frac = p - pf;
+            if (fabs(u - frac) < 1e-12) ++n_tie;
+            gam = (u64)pf + (u < frac ? 1u : 0u);
+            if (gam > qmax) gam = qmax;
+          }
+        } else {
+          if (fabs(u - p) < 1e-12) ++n_tie;
+          gam = (u < p) ? 1u : 0u;   // :639, :645
+        }
+        ++n_pairs;
+        if (gam == 0) continue;
+        ++n_coll;
+        // the rare pair that collides updates global memory itself (r_d^3 and kappa are not staged)
+        const u32 gj = s0 + (u32)j, gk = s0 + (u32)k;
+        const double gd = (double)gam;
+        const double rw3 = yk * rk + gd * (yj * rj);    // extensive attributes are summed (:643)
+        const double rd3j = gd * a.rd3[gj];
+        const double rd3k = a.rd3[gk];
+        const double kj = a.kappa[gj], kk = a.kappa[gk];
+        if (kj != kk)                                    // intensive ones averaged (:643)
+          a.kappa[gk] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
+        a.rd3[gk] = rd3k + rd3j;
+        const double r = cbrt(rw3);
+        const double y2 = r * r;
+        s_rw2[k] = y2; a.rw2[gk] = y2;
+        s_n[j] = nj - gam * nk; a.n[gj] = nj - gam * nk;
+        if (need_vt) s_vt[k] = v_term(sqrt(y2), C.eta, C.rho_a);
+      }
+      __syncthreads();
+    }
+    // ---- advection + sedimentation, SD by SD in storage order; everything is in shared memory -----------------
+    if (moving) {
+#pragma unroll kCoalUnroll
+      for (int t = tid; t < M; t += T) {
+        const u64 n = s_n[t];
+        if (n == 0) continue;
+        int lo = 0, hi = nc;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
+        const u32 s = s0 + t;
+        const CoalCell& C = s_cell[lo];
+        double xn = 0, yn = 0, zn = 0;
+        if (g.hx) xn = s_x[t];
+        if (g.hy) yn = s_y[t];
+        if (g.hz) zn = s_z[t];
+        if (mp.adve) {   // eq. 16 with the Courant numbers at the edges of the SD's time-n cell
+          if (g.hx) { const double dC = C.Cxh - C.Cxl; xn = (xn + g.dx * (C.Cxl - (double)C.i * dC)) / (1.0 - dC); }
+          if (g.hy) { const double dC = C.Cyh - C.Cyl; yn = (yn + g.dy * (C.Cyl - (double)C.j * dC)) / (1.0 - dC); }
+          if (g.hz) { const double dC = C.Czh - C.Czl; zn = (zn + g.dz * (C.Czl - (double)C.k * dC)) / (1.0 - dC); }
+        }
+        if (need_vt) zn = zn - s_vt[t] * g.dt;                                // explicit Euler (:649)
+        if (g.hx) { xn = wrap(xn, g.X); a.x[s] = xn; }                        // periodic (:558)
+        if (g.hy) { yn = wrap(yn, g.Y); a.y[s] = yn; }
+        if (g.hz) {
+          if (zn < 0.0 || !(zn < g.Z)) {                                       // left the domain (:651)
+            const double y = s_rw2[t];
+            if (zn < 0.0) flux += (double)n * ((4.0 / 3.0) * cst::pi * cst::rho_w * (y * sqrt(y)));
+            a.n[s] = 0;
+          }
+          a.z[s] = zn;
+        }
+      }
+    }
+  }
+  unsigned v0 = n_pairs, v1 = n_coll, v2 = n_tie;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    v0 += __shfl_xor_sync(0xffffffffu, v0, d);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, d);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, d);
+    flux += __shfl_xor_sync(0xffffffffu, flux, d);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    const int slot = (blockIdx.x * (T / 32) + (threadIdx.x >> 5)) & (NSLOT - 1);
+    if (v0) atomicAdd(&cnt.pairs[slot], (unsigned long long)v0);
+    if (v1) atomicAdd(&cnt.collisions[slot], (unsigned long long)v1);
+    if (v2) atomicAdd(&cnt.near_ties[slot], (unsigned long long)v2);
+    if (flux != 0.0) atomicAdd(&flux_slots[slot], flux);
+  }
+}
+
+#ifndef SDM_COAL_CAP
+#define SDM_COAL_CAP 816
+#define SDM_COAL_T 128
+#define SDM_COAL_MINB 5
+#endif
+using CoalSmall = CoalTile<SDM_COAL_CAP, SDM_COAL_T>;
+// can a tile of cpb cells whose most populated instance holds `need` SDs run in k_coal_move_tile?
+bool coal_tile_fits(int cpb, int need) {
+  return need + cpb <= SDM_COAL_CAP && cpb <= 4096 &&
+         CoalSmall::smem(cpb) <= (size_t)(228 * 1024 - SDM_COAL_MINB * 1024) / SDM_COAL_MINB;
+}
+cudaError_t launch_coal_move_tile(int cpb, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
+                                  const Counters& cnt, cudaStream_t st) {
+  const size_t smem = CoalSmall::smem(cpb);
+  auto kern = k_coal_move_tile<SDM_COAL_CAP, SDM_COAL_T, SDM_COAL_MINB>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cpb);
+  return cudaGetLastError();
+}
+
 // sums the NSLOT flux slots in a fixed order, then clears them
 __global__ void k_flux_sum(double* flux_slots, double* flux_out, double* flux_total) {
   __shared__ double sh[NSLOT];

@@ -55,6 +55,11 @@ cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, co
                              const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                              const Counters& cnt, cudaStream_t st);
 size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem);
+// tile-resident variant for sstp_coal == 1 (cpb cells per CTA, most populated tile `need` SDs)
+bool coal_tile_fits(int cpb, int need);
+cudaError_t launch_coal_move_tile(int cpb, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
+                                  const Counters& cnt, cudaStream_t st);
 void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
 
 // sdm_diag.cu

@@ -285,3 +285,87 @@ def test_runs_are_reproducible_bit_for_bit():
     for k in outs[0][0]:
         np.testing.assert_array_equal(outs[0][0][k], outs[1][0][k])
     assert torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])
+
+
+# ------------------------------------------------------------------------------------ full size (bench.py's launch)
+def test_full_size_3d_sampled_columns_match_oracle():
+    """configs[3] at full size (128 x 128 x 64 cells, 67 108 864 SDs), in the launch configuration bench.py times.
+    Every stage but the reorder is local to a column of cells, so the oracle can compute a sampled block of
+    columns on its own: after 3 steps of the whole domain on the GPU, the SDs of two 2 x 2 x 64 blocks are
+    handed to the oracle (same ids, same step counter, fields and Courant numbers sliced), both advance one
+    step, and the block's SDs are compared one by one.  Horizontal positions are compared modulo the block
+    width (an SD that leaves the block wraps in the oracle's small periodic domain)."""
+    b = binding()
+    torch.cuda.empty_cache()
+    w = W.cfg4_3d(device="cuda")
+    nx, ny, nz, dx = w.init["nx"], w.init["ny"], w.init["nz"], w.init["dx"]
+    n_total = w.n_sd
+    assert n_total == 67108864
+    p = b.Particles(max_sd=n_total, sd_conc_mean=64, **w.init)
+    s = w.state
+    p.init_from_arrays(w.rhod, s["n"], s["rw2"], s["rd3"], s["kappa"], s["x"], s["y"], s["z"], s["id"],
+                       courant_1=w.courants[0], courant_2=w.courants[1], courant_3=w.courants[2])
+    th, rv = w.th.clone(), w.rv.clone()
+    w.state = None
+    del s
+    torch.cuda.empty_cache()
+    po, oo = b.make_opts(**w.opts), oracle.make_opts(**w.opts)
+    for _ in range(3):
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+    st = p.export_state()                      # storage order, dead SDs of the last step still present
+    N0 = st["id"].numel()
+    blocks = [(37, 90, 2, 2), (0, 127, 2, 1)]  # (i0, j0, bx, by); the second touches both periodic borders' cells
+    ci = torch.clamp((st["x"] / dx).floor().long(), 0, nx - 1)
+    cj = torch.clamp((st["y"] / dx).floor().long(), 0, ny - 1)
+    oracles, picks = [], []
+    for (i0, j0, bx, by) in blocks:
+        m = (ci >= i0) & (ci < i0 + bx) & (cj >= j0) & (cj < j0 + by) & (st["n"] > 0)
+        sel = torch.nonzero(m).flatten()
+        o = oracle.Oracle(**dict(w.init, nx=bx, ny=by))
+        o.set_threads(4)
+        sl = (slice(i0, i0 + bx), slice(j0, j0 + by))
+        c1, c2, c3 = w.courants
+        o.set_fields(th=np_(th[sl]).ravel(), rv=np_(rv[sl]).ravel(), rhod=np_(w.rhod[sl]).ravel(),
+                     cx=np_(c1[i0:i0 + bx + 1, j0:j0 + by]).ravel(), cy=np_(c2[i0:i0 + bx, j0:j0 + by + 1]).ravel(),
+                     cz=np_(c3[sl]).ravel())
+        o.set_state(np_(st["n"][sel]).astype(np.uint64), np_(st["rw2"][sel]), np_(st["rd3"][sel]), np_(st["kappa"][sel]),
+                    x=np_(st["x"][sel] - i0 * dx), y=np_(st["y"][sel] - j0 * dx), z=np_(st["z"][sel]),
+                    id=np_(st["id"][sel]).astype(np.uint32))
+        o.set_step(3)
+        oracles.append(o)
+        picks.append(st["id"][sel].long())
+        assert sel.numel() > 0.8 * 64 * bx * by * nz
+    del st, ci, cj
+    th_before = th.clone()
+    p.step_sync(po, th, rv)
+    p.step_async(po)
+    g = p.export_state()
+    where = torch.full((n_total,), -1, dtype=torch.int64, device="cuda")
+    where[g["id"].long()] = torch.arange(g["id"].numel(), device="cuda")
+    ncoll = 0
+    for (i0, j0, bx, by), o, ids in zip(blocks, oracles, picks):
+        o.step(oo)
+        r = sorted_by_id(o.get_state())
+        ids_sorted, _ = torch.sort(ids)
+        pos = where[ids_sorted]
+        assert bool((pos >= 0).all())
+        gg = {k: np_(v[pos]) for k, v in g.items()}
+        np.testing.assert_array_equal(gg["id"].astype(np.uint32), r["id"])
+        np.testing.assert_array_equal(gg["n"].astype(np.uint64), r["n"])          # multiplicities: bit-exact
+        np.testing.assert_allclose(np.sqrt(gg["rw2"]), np.sqrt(r["rw2"]), rtol=RTOL)
+        np.testing.assert_allclose(np.cbrt(gg["rd3"]), np.cbrt(r["rd3"]), rtol=RTOL)
+        np.testing.assert_allclose(gg["kappa"], r["kappa"], rtol=RTOL)
+        live = r["n"] > 0
+        np.testing.assert_allclose(gg["z"][live], r["z"][live], rtol=RTOL, atol=1e-9)
+        for k, o0, L, big in (("x", i0 * dx, bx * dx, nx * dx), ("y", j0 * dx, by * dx, ny * dx)):
+            d = np.mod(gg[k][live] - o0, big)            # the block may sit across the periodic border of the domain
+            d = np.mod(d - r[k][live] + 0.5 * L, L) - 0.5 * L
+            assert np.max(np.abs(d)) < 1e-8
+        oth, orv = o.get_fields()
+        sl = (slice(i0, i0 + bx), slice(j0, j0 + by))
+        np.testing.assert_allclose(np_(th[sl]).ravel(), oth, rtol=RTOL)
+        np.testing.assert_allclose(np_(rv[sl]).ravel(), orv, rtol=RTOL)
+        assert not np.array_equal(np_(th_before[sl]).ravel(), oth)                 # condensation did act
+        ncoll += o.counters()["collisions"]
+    assert g["id"].numel() <= N0

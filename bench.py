@@ -182,7 +182,7 @@ def main():
     import torch
     import torch.distributed as dist
 
-    from paper_1310_1905_b200 import binding
+    from paper_1310_1905_b200 import binding, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -194,7 +194,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = f"cuda:{local}"
 
-    w = make_workload(wa, seed=42 + rank, device=dev)
+    w = make_workload(wa, seed=replicas.replica_seed(42, rank), device=dev)
     p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], **w.init)
     s = w.state
     cs = list(w.courants) + [None] * (3 - len(w.courants))
@@ -242,12 +242,7 @@ def main():
     st1 = p.stats()
     stages = p.stage_times(reset=True)
     p.set_timing(False)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    tot = torch.tensor([float(sd_steps)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_max, sd_total = float(t.item()), float(tot.item())
+    ms_max, sd_total = replicas.job_totals(ms, sd_steps, device=dev)   # slowest rank's device time, all ranks' SD-steps
     value = sd_total / (ms_max * 1e-3)
 
     # ---- end to end: Eulerian fields in (pinned) host memory, copied in and out every step ---------
@@ -260,13 +255,9 @@ def main():
         p.step_host(po, th_h, rv_h)
     torch.cuda.synchronize()
     e_dt = time.perf_counter() - t0
-    et = torch.tensor([e_dt], dtype=torch.float64, device=dev)
-    etot = torch.tensor([float(e_sd)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(et, op=dist.ReduceOp.MAX)
-        dist.all_reduce(etot, op=dist.ReduceOp.SUM)
+    e_s, e_tot = replicas.job_totals(e_dt, e_sd, device=dev)
     ncell = th.numel()
-    e2e = {"value": float(etot.item()) / float(et.item()), "unit": UNIT, "h2d_bytes_per_step": 2 * ncell * 8,
+    e2e = {"value": e_tot / e_s, "unit": UNIT, "h2d_bytes_per_step": 2 * ncell * 8,
            "d2h_bytes_per_step": 2 * ncell * 8 + 8, "api": "sdm_step_host (th, rv in pinned host memory)"}
 
     if rank != 0:

@@ -45,12 +45,23 @@ typedef enum {
   SDM_KERNEL_HYDRO_TAB = 2  /* eq. 28 with E(r_large, r_small/r_large) bilinear from a table */
 } sdm_kernel;
 
+/* One lognormal mode of the initial dry-aerosol spectrum (eq. 3 :119, the same fields as blk_2m's
+ * lognormal_mode_t :400-410).  dry_distros of Listing 5.2 (:703-708) maps kappa to a functor n(ln r_d); C has no
+ * functors, so a spectrum is the sum of the modes that share one kappa, and distinct kappas are an external
+ * mixture (:659) whose spectra share the super-droplets equally. */
+typedef struct {
+  double kappa;             /* hygroscopicity */
+  double n_stp;             /* number concentration at STP [m^-3] */
+  double r_mean;            /* mode radius [m] */
+  double sigma_g;           /* geometric standard deviation (> 1) */
+} sdm_lognormal_mode;
+
 /* PAPER.md Listing 5.2 (:699-720) lgrngn::opts_init_t.  Copied by sdm_create. */
 typedef struct {
   int nx, ny, nz;           /* Eulerian grid; 0 = dimension absent (:751: 0..3 Courant components) */
   double dx, dy, dz, dt;    /* grid steps [m] and time step [s]; an absent dimension still
                                contributes its d? to the cell volume dV = dx dy dz (2D: dy = 1 m; box: V) */
-  double x0, y0, z0, x1, y1, z1; /* Lagrangian sub-domain (:713); used by initialisation only */
+  double x0, y0, z0, x1, y1, z1; /* Lagrangian sub-domain (:713); used by sdm_init only; all zero = whole grid */
   double sd_conc_mean;      /* mean number of SDs per cell (:715); a sizing hint here */
   int kernel;               /* sdm_kernel */
   double golovin_b;         /* [1/s] for SDM_KERNEL_GOLOVIN */
@@ -62,6 +73,8 @@ typedef struct {
   int real_bytes;           /* 8 */
   int multi_coal;           /* 1: gamma = floor(p) + [u < frac(p)] (north_star); 0: gamma = [u < p] (PAPER.md :645) */
   uint64_t max_sd;          /* capacity in super-droplets (HBM is allocated once, at creation) */
+  int n_modes;              /* dry_distros (:703-708): number of lognormal modes, 0..8 (0: sdm_init unavailable) */
+  const sdm_lognormal_mode* modes; /* HOST, n_modes entries; copied */
 } sdm_opts_init;
 
 /* PAPER.md Listing 5.1 (:677-689) lgrngn::opts_t */
@@ -98,6 +111,21 @@ int sdm_create(const sdm_opts_init* opts, sdm_ctx** out);
 void sdm_destroy(sdm_ctx* ctx);
 /* message of the last failed call on ctx (ctx == NULL: of the last failed sdm_create); library-owned */
 const char* sdm_last_error(const sdm_ctx* ctx);
+
+/* init() of Listing 5.5 (:759-766): the initialisation of PAPER.md section 5.1.6 (:653-665).  Creates
+ * round(sd_conc_mean * cells of the Lagrangian domain) super-droplets with ids 0..N-1: positions uniform in
+ * [x0,x1) x [y0,y1) x [z0,z1) (:655); ln r_d uniform between the limits at which an SD stands for at least one
+ * particle (:657); multiplicity = n(ln r_d) * range / SDs per cell * dV * rho_d / rho_STP, rounded, at least 1
+ * (:659); wet radius in equilibrium (zero growth rate in eq. 20) with min(RH, 0.95) of the SD's cell (:661-665);
+ * theta and r_v are not changed (:663).  Random numbers: Philox-4x32-10 with the context's seed, counter
+ * (id, 0, 0, tag), tag 2, 3, 4, 5 = x, y, z, ln r_d.  th, rv, rhod are mandatory, the Courant components are
+ * those of the present dimensions (:751) and may be omitted (zero flow); all are DEVICE arrays, copied or read
+ * before the call returns.  Fails with SDM_ERR_INVALID without modes, SDM_ERR_CAPACITY if N > max_sd.  Blocking. */
+int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm_arrinfo rhod_courant_1,
+             sdm_arrinfo rhod_courant_2, sdm_arrinfo rhod_courant_3, void* stream);
+/* The limits of ln r_d chosen by the rule of :657 for spectrum g (0-based, in order of first appearance of its
+ * kappa among the modes); HOST outputs. */
+int sdm_init_range(const sdm_ctx* ctx, int g, double* lnr_lo, double* lnr_hi);
 
 /* Load a particle population (parity tests, the box set-up, checkpoint restart) instead of the
  * paper's init() (:759-766).  rhod and the Courant components (rho_d times Courant number on the

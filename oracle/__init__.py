@@ -70,6 +70,8 @@ def lib():
         L.orc_set_state.argtypes = [C.c_void_p, C.c_long] + [C.c_void_p] * 8
         L.orc_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.orc_set_step.argtypes = [C.c_void_p, C.c_uint32]
+        L.orc_init.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_double] + [C.c_double] * 6 + [C.c_void_p]
+        L.orc_init.restype = C.c_long
         L.orc_get_step.argtypes = [C.c_void_p]
         L.orc_get_step.restype = C.c_uint32
         L.orc_n_sd.argtypes = [C.c_void_p]
@@ -125,6 +127,7 @@ class Oracle:
                     _ptr(self._keep[0]), _ptr(self._keep[1]), _ptr(self._keep[2]))
         self.h = self.L.orc_create(C.byref(ini))
         self.NX, self.NY, self.NZ = max(nx, 1), max(ny, 1), max(nz, 1)
+        self.o_dx, self.o_dy, self.o_dz = dx, dy, dz
         self.ncell = self.NX * self.NY * self.NZ
 
     def __del__(self):
@@ -146,6 +149,18 @@ class Oracle:
     def set_fields(self, th=None, rv=None, rhod=None, cx=None, cy=None, cz=None):
         arrs = [_f64(a) for a in (th, rv, rhod, cx, cy, cz)]
         self.L.orc_set_fields(self.h, *[_ptr(a) for a in arrs])
+
+    def init(self, modes, sd_conc_mean, x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None):
+        """PAPER.md section 5.1.6: modes = [(kappa, N_stp, r_mean, sigma_g), ...]; uses the fields set before.
+        Returns (number of SDs, [(ln r_lo, ln r_hi) per spectrum])."""
+        m = np.ascontiguousarray(np.asarray(modes, dtype=np.float64).reshape(-1, 4))
+        x1 = self.o_dx * self.NX if x1 is None else x1
+        y1 = self.o_dy * self.NY if y1 is None else y1
+        z1 = self.o_dz * self.NZ if z1 is None else z1
+        ranges = np.zeros(2 * len(m), dtype=np.float64)
+        N = self.L.orc_init(self.h, len(m), _ptr(m), float(sd_conc_mean), x0, y0, z0, x1, y1, z1, _ptr(ranges))
+        G = len(dict.fromkeys(m[:, 0].tolist()))
+        return N, [(ranges[2 * g], ranges[2 * g + 1]) for g in range(G)]
 
     def set_step(self, step):
         self.L.orc_set_step(self.h, step)

@@ -385,6 +385,109 @@ void orc_set_fields(void* h, const double* th, const double* rv, const double* r
   if (cz) c.cz.assign(cz, cz + c.cz.size());
   c.thermo.clear();
 }
+// ---- initialisation (section 5.1.6 :653-665; init() of Listing 5.5 :759-766) --------------------
+// DESIGN.md reading R-init.  modes: n_modes x {kappa, N_stp [m^-3], r_mean [m], sigma_g} (eq. 3 :119); modes
+// with the same kappa form one spectrum n(ln r_d), different kappas are an external mixture (:659) whose
+// spectra take the SDs in turn (SD i belongs to spectrum i mod G).  Uses the th, rv, rhod set before.
+struct Spectrum { double kappa; std::vector<int> modes; double lo, hi; };
+static double spectrum_density(const double* modes, const Spectrum& sp, double lnr) {   // n(ln r_d) at STP
+  double out = 0.0;
+  for (int m : sp.modes) {
+    const double N = modes[4 * m + 1], lrm = std::log(modes[4 * m + 2]), ls = std::log(modes[4 * m + 3]);
+    out += N / (std::sqrt(2.0 * pi) * ls) * std::exp(-((lnr - lrm) * (lnr - lrm)) / (2.0 * ls * ls));
+  }
+  return out;
+}
+// :657 "the particle multiplicity for both the minimal and the maximal radii be greater or equal one": the
+// multiplicity at a radius depends on the width of the range, so iterate to the fixed point on a grid in ln r.
+static void auto_range(const double* modes, Spectrum& sp, double sd_conc, double dV) {
+  const int NG = 200001;
+  const double g0 = std::log(1e-10), g1 = std::log(1e-4);
+  double lo = std::log(1e-9), hi = std::log(1e-5);
+  for (int it = 0; it < 50; ++it) {
+    int first = -1, last = -1;
+    for (int q = 0; q < NG; ++q) {
+      const double lnr = g0 + (g1 - g0) * ((double)q / (double)(NG - 1));
+      if (spectrum_density(modes, sp, lnr) * (hi - lo) / sd_conc * dV >= 1.0) { if (first < 0) first = q; last = q; }
+    }
+    if (first < 0) break;
+    const double nlo = g0 + (g1 - g0) * ((double)first / (double)(NG - 1));
+    const double nhi = g0 + (g1 - g0) * ((double)last / (double)(NG - 1));
+    const bool done = std::fabs(nlo - lo) + std::fabs(nhi - hi) < 1e-9;
+    lo = nlo; hi = nhi;
+    if (done) break;
+  }
+  sp.lo = lo; sp.hi = hi;
+}
+static inline double init_uniform(const Ctx& c, u32 id, u32 tag) {
+  u32 ctr[4] = {id, 0u, 0u, tag}, k[2] = {(u32)c.o.seed, (u32)(c.o.seed >> 32)}, out[4];
+  philox4x32_10(ctr, k, out);
+  const u64 w = ((u64)out[0] << 32) | out[1];
+  return ((double)(w >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+}
+// wet radius in equilibrium with RH (zero on the left of eq. 20, :661): root of a_w(r) exp(A/r) = RH between
+// r_d and the critical radius sqrt(3 kappa r_d^3 / A), where the Koehler curve rises monotonically
+static double equilibrium_rw(double rd3, double kappa, double RH, double A) {
+  double lo = std::cbrt(rd3), hi = std::sqrt(3.0 * kappa * rd3 / A);
+  if (!(hi > lo)) return lo;
+  for (int it = 0; it < 300 && hi - lo > 1e-15 * hi; ++it) {
+    const double r = 0.5 * (lo + hi), r3 = r * r * r;
+    const double S = (r3 - rd3) / (r3 - rd3 * (1.0 - kappa)) * std::exp(A / r);
+    if (S < RH) lo = r; else hi = r;
+  }
+  return 0.5 * (lo + hi);
+}
+
+long orc_init(void* h, int n_modes, const double* modes, double sd_conc_mean, double x0, double y0, double z0,
+              double x1, double y1, double z1, double* ranges_out) {
+  Ctx& c = *(Ctx*)h;
+  std::vector<Spectrum> sp;
+  for (int m = 0; m < n_modes; ++m) {
+    size_t g = 0;
+    while (g < sp.size() && sp[g].kappa != modes[4 * m]) ++g;
+    if (g == sp.size()) sp.push_back(Spectrum{modes[4 * m], {}, 0.0, 0.0});
+    sp[g].modes.push_back(m);
+  }
+  const int G = (int)sp.size();
+  const double sd_conc_g = sd_conc_mean / G;
+  for (int g = 0; g < G; ++g) {
+    auto_range(modes, sp[g], sd_conc_g, c.dV);
+    if (ranges_out) { ranges_out[2 * g] = sp[g].lo; ranges_out[2 * g + 1] = sp[g].hi; }
+  }
+  double ncl = 1.0;
+  if (c.o.nx > 0) ncl *= (x1 - x0) / c.o.dx;
+  if (c.o.ny > 0) ncl *= (y1 - y0) / c.o.dy;
+  if (c.o.nz > 0) ncl *= (z1 - z0) / c.o.dz;
+  const long N = (long)std::floor(sd_conc_mean * ncl + 0.5);
+  const double rho_stp = 101325.0 / (R_d * 293.15);   // :130 "T = 20 C and p = 1013.25 hPa"
+  c.n.assign(N, 0); c.rw2.assign(N, 0.0); c.rd3.assign(N, 0.0); c.kappa.assign(N, 0.0);
+  c.x.assign(N, 0.0); c.y.assign(N, 0.0); c.z.assign(N, 0.0); c.id.assign(N, 0u);
+  for (long i = 0; i < N; ++i) {
+    const Spectrum& s = sp[i % G];
+    c.id[i] = (u32)i;
+    if (c.o.nx > 0) c.x[i] = x0 + init_uniform(c, (u32)i, 2u) * (x1 - x0);   // :655 uniform in space
+    if (c.o.ny > 0) c.y[i] = y0 + init_uniform(c, (u32)i, 3u) * (y1 - y0);
+    if (c.o.nz > 0) c.z[i] = z0 + init_uniform(c, (u32)i, 4u) * (z1 - z0);
+    const double lnr = s.lo + (s.hi - s.lo) * init_uniform(c, (u32)i, 5u);     // :657 uniform in ln r_d
+    c.rd3[i] = std::exp(3.0 * lnr);
+    c.kappa[i] = s.kappa;
+    const int ci = c.o.nx > 0 ? cell_1d(c.x[i], c.o.dx, c.NX) : 0;
+    const int cj = c.o.ny > 0 ? cell_1d(c.y[i], c.o.dy, c.NY) : 0;
+    const int ck = c.o.nz > 0 ? cell_1d(c.z[i], c.o.dz, c.NZ) : 0;
+    const long cell = ((long)ci * c.NY + cj) * c.NZ + ck;
+    // :659 spectra are given at STP: concentrations scale with rho_d / rho_STP
+    const double mult = spectrum_density(modes, s, lnr) * (s.hi - s.lo) / sd_conc_g * c.dV * (c.rhod[cell] / rho_stp);
+    c.n[i] = (u64)std::max(1.0, std::floor(mult + 0.5));
+    // :661-665 equilibrium at the cell's RH, at RH = 0.95 where the air is (nearly) saturated
+    const CellThermo t = cell_thermo(c.th[cell], c.rv[cell], c.rhod[cell], 0.95);
+    const double rw = equilibrium_rw(c.rd3[i], s.kappa, t.RH, t.A);
+    c.rw2[i] = rw * rw;
+  }
+  c.step = 0; c.sorted = false;
+  c.rain_flux_total = 0; c.cnt = orc_counters_t{};
+  return N;
+}
+
 void orc_set_step(void* h, u32 step) { ((Ctx*)h)->step = step; }
 u32 orc_get_step(void* h) { return ((Ctx*)h)->step; }
 

@@ -28,7 +28,8 @@ class OptsInit(C.Structure):
                 ("sd_conc_mean", C.c_double), ("kernel", C.c_int), ("golovin_b", C.c_double),
                 ("n_eff_R", C.c_int), ("n_eff_q", C.c_int),
                 ("eff_R", C.c_void_p), ("eff_q", C.c_void_p), ("eff_tab", C.c_void_p),
-                ("seed", C.c_uint64), ("real_bytes", C.c_int), ("multi_coal", C.c_int), ("max_sd", C.c_uint64)]
+                ("seed", C.c_uint64), ("real_bytes", C.c_int), ("multi_coal", C.c_int), ("max_sd", C.c_uint64),
+                ("n_modes", C.c_int), ("modes", C.c_void_p)]
 
 
 class Opts(C.Structure):
@@ -45,7 +46,7 @@ class Stats(C.Structure):
                                           "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow")]
 
 
-EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
+EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_range", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
            "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times"]
@@ -70,6 +71,8 @@ def load_library():
     L.sdm_last_error.argtypes = [vp]
     L.sdm_last_error.restype = C.c_char_p
     L.sdm_init_from_arrays.argtypes = [vp, ArrInfo, ArrInfo, ArrInfo, ArrInfo, C.c_uint64] + [vp] * 8 + [vp]
+    L.sdm_init.argtypes = [vp] + [ArrInfo] * 6 + [vp]
+    L.sdm_init_range.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.sdm_step_sync.argtypes = [vp, C.POINTER(Opts)] + [ArrInfo] * 6 + [vp]
     L.sdm_step_async.argtypes = [vp, C.POINTER(Opts), vp]
     L.sdm_step_async_result.argtypes = [vp, C.POINTER(C.c_double)]
@@ -123,13 +126,21 @@ class Particles:
     """One ``particles_t`` (PAPER.md :747-790) living on the current CUDA device."""
 
     def __init__(self, nx=0, ny=0, nz=0, dx=1.0, dy=1.0, dz=1.0, dt=1.0, kernel="geometric", golovin_b=1500.0,
-                 multi_coal=True, seed=42, eff_R=None, eff_q=None, eff_tab=None, max_sd=None, sd_conc_mean=0.0):
+                 multi_coal=True, seed=42, eff_R=None, eff_q=None, eff_tab=None, max_sd=None, sd_conc_mean=0.0, modes=None,
+                 x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None):
+        """modes: [(kappa, N_stp, r_mean, sigma_g), ...] of the dry spectrum, needed by init() only."""
         import numpy as np
         self.L = load_library()
         keep = [None if a is None else np.ascontiguousarray(a, dtype=np.float64) for a in (eff_R, eff_q, eff_tab)]
         o = OptsInit()
         o.nx, o.ny, o.nz, o.dx, o.dy, o.dz, o.dt = nx, ny, nz, dx, dy, dz, dt
-        o.x1, o.y1, o.z1 = dx * max(nx, 1), dy * max(ny, 1), dz * max(nz, 1)
+        o.x0, o.y0, o.z0 = x0, y0, z0
+        o.x1 = dx * max(nx, 1) if x1 is None else x1
+        o.y1 = dy * max(ny, 1) if y1 is None else y1
+        o.z1 = dz * max(nz, 1) if z1 is None else z1
+        if modes is not None:
+            keep.append(np.ascontiguousarray(np.asarray(modes, dtype=np.float64).reshape(-1, 4)))
+            o.n_modes, o.modes = len(keep[-1]), keep[-1].ctypes.data
         o.sd_conc_mean, o.kernel, o.golovin_b = sd_conc_mean, KERNELS[kernel], golovin_b
         if keep[0] is not None:
             o.n_eff_R, o.n_eff_q = len(keep[0]), len(keep[1])
@@ -154,6 +165,16 @@ class Particles:
     def _ck(self, rc):
         if rc != 0:
             raise SdmError(f"libsdm error {rc}: {self.L.sdm_last_error(self.h).decode()}")
+
+    def init(self, th, rv, rhod, courant_1=None, courant_2=None, courant_3=None):
+        """particles_t::init() (PAPER.md :759-766, section 5.1.6)."""
+        self._ck(self.L.sdm_init(self.h, arrinfo(th), arrinfo(rv), arrinfo(rhod), arrinfo(courant_1), arrinfo(courant_2),
+                                 arrinfo(courant_3), _stream()))
+
+    def init_range(self, g=0):
+        lo, hi = C.c_double(), C.c_double()
+        self._ck(self.L.sdm_init_range(self.h, g, C.byref(lo), C.byref(hi)))
+        return lo.value, hi.value
 
     def init_from_arrays(self, rhod, n, rw2, rd3, kappa, x=None, y=None, z=None, id=None, courant_1=None, courant_2=None,
                          courant_3=None):

@@ -17,6 +17,7 @@ UNITS = {
     "sdm_cond.cu": [],
     "sdm_coal_move.cu": ["-fmad=false"],
     "sdm_diag.cu": ["-fmad=false"],
+    "sdm_init.cu": ["-fmad=false"],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 

@@ -3,6 +3,7 @@
 #include "../../include/sdm.h"
 #include "sdm_kernels.cuh"
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -40,6 +41,8 @@ struct sdm_ctx {
   unsigned long long* cnt_mem = nullptr;
   Counters cnt{};
   CoalParams kp{};
+  InitParams ip{};           // dry spectra and the limits of :657, prepared at creation
+  bool have_modes = false;
   double *d_effR = nullptr, *d_effq = nullptr, *d_efftab = nullptr;
   double *th_dense = nullptr, *rv_dense = nullptr;   // for sdm_step_host
   u64 nslots = 0;            // host-known number of slots in use
@@ -245,6 +248,25 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
     kp.eff_R = ctx->d_effR; kp.eff_q = ctx->d_effq; kp.eff_tab = ctx->d_efftab;
   }
   ctx->o.eff_R = ctx->o.eff_q = ctx->o.eff_tab = nullptr;   // host pointers are not retained
+  if (o->n_modes > 0) {
+    if (!o->modes || !(o->sd_conc_mean > 0)) { sdm_destroy(ctx); return fail(nullptr, SDM_ERR_INVALID, "sdm_create: modes given without a modes array or sd_conc_mean"); }
+    static_assert(sizeof(sdm_lognormal_mode) == sizeof(sdm_mode_view), "mode layout");
+    const int rc = init_prepare(reinterpret_cast<const sdm_mode_view*>(o->modes), o->n_modes, o->sd_conc_mean, g.dV, ctx->ip);
+    if (rc) { sdm_destroy(ctx); return fail(nullptr, SDM_ERR_INVALID, rc == -2 ? "sdm_create: the dry spectrum is too dilute for sd_conc_mean (no radius with multiplicity >= 1)" : "sdm_create: 1..8 modes with kappa, n_stp, r_mean > 0 and sigma_g > 1 required"); }
+    const bool whole = o->x0 == 0 && o->x1 == 0 && o->y0 == 0 && o->y1 == 0 && o->z0 == 0 && o->z1 == 0;
+    ctx->ip.x0 = whole ? 0.0 : o->x0; ctx->ip.x1 = whole ? g.X : o->x1;
+    ctx->ip.y0 = whole ? 0.0 : o->y0; ctx->ip.y1 = whole ? g.Y : o->y1;
+    ctx->ip.z0 = whole ? 0.0 : o->z0; ctx->ip.z1 = whole ? g.Z : o->z1;
+    if ((g.hx && !(ctx->ip.x0 >= 0 && ctx->ip.x1 <= g.X && ctx->ip.x0 < ctx->ip.x1)) ||
+        (g.hy && !(ctx->ip.y0 >= 0 && ctx->ip.y1 <= g.Y && ctx->ip.y0 < ctx->ip.y1)) ||
+        (g.hz && !(ctx->ip.z0 >= 0 && ctx->ip.z1 <= g.Z && ctx->ip.z0 < ctx->ip.z1))) {
+      sdm_destroy(ctx);
+      return fail(nullptr, SDM_ERR_INVALID, "sdm_create: the Lagrangian domain x0..z1 must lie inside the grid");
+    }
+    ctx->ip.seed_lo = kp.seed_lo; ctx->ip.seed_hi = kp.seed_hi;
+    ctx->have_modes = true;
+  }
+  ctx->o.modes = nullptr;
   if ((e = cudaEventCreateWithFlags(&ctx->ev_info, cudaEventDisableTiming)) ||
       (e = cudaEventCreateWithFlags(&ctx->ev_async, cudaEventDisableTiming)))
     return bail(e, "events");
@@ -271,6 +293,49 @@ void sdm_destroy(sdm_ctx* ctx) {
   for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
   cudaGetLastError();
   delete ctx;
+}
+
+int sdm_init_range(const sdm_ctx* ctx, int g, double* lnr_lo, double* lnr_hi) {
+  if (!ctx || !lnr_lo || !lnr_hi || !ctx->have_modes || g < 0 || g >= ctx->ip.n_spectra) return SDM_ERR_INVALID;
+  *lnr_lo = ctx->ip.lnr_lo[g]; *lnr_hi = ctx->ip.lnr_hi[g];
+  return SDM_OK;
+}
+
+int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arrinfo c2, sdm_arrinfo c3,
+             void* stream) {
+  if (!ctx) return SDM_ERR_INVALID;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Grid& g = ctx->g;
+  if (!ctx->have_modes) return fail(ctx, SDM_ERR_INVALID, "sdm_init: the context was created without dry-aerosol modes");
+  if (!th.data_zero || !rv.data_zero || !rhod.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_init: th, rv and rhod are mandatory");
+  const InitParams& ip = ctx->ip;
+  double ncl = 1.0;
+  if (g.hx) ncl *= (ip.x1 - ip.x0) / g.dx;
+  if (g.hy) ncl *= (ip.y1 - ip.y0) / g.dy;
+  if (g.hz) ncl *= (ip.z1 - ip.z0) / g.dz;
+  const double Nd = std::floor(ctx->o.sd_conc_mean * ncl + 0.5);
+  if (Nd > (double)ctx->cap_sd) return fail(ctx, SDM_ERR_CAPACITY, "sdm_init: sd_conc_mean x cells exceeds max_sd");
+  const u64 N = (u64)Nd;
+  launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st);
+  ctx->launches++;
+  const sdm_arrinfo comps[3] = {c1, c2, c3};
+  if (int rc = copy_courants(ctx, comps, st)) return rc;
+  ctx->cur = 0; ctx->cn = 0;
+  // scratch per cell: RH to equilibrate with (outbuf) and the Kelvin length (eta, rewritten by every step_sync)
+  launch_init(ctx->buf[0], (u32)N, g, ip, make_field(ctx, th), make_field(ctx, rv), ctx->cf.rhod, ctx->outbuf, ctx->cf.eta, st);
+  ctx->launches += 1 + (N ? 1 : 0);
+  CK(cudaGetLastError());
+  const u32 info[8] = {(u32)N, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+  CK(cudaMemcpyAsync(ctx->d_info, info, sizeof(info), cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
+  CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT, st));
+  CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
+  CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
+  CK(cudaMemsetAsync(ctx->outbuf, 0, sizeof(double) * g.ncell, st));
+  CK(cudaStreamSynchronize(st));
+  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false;
+  ctx->last_stream = st;
+  return SDM_OK;
 }
 
 int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arrinfo c2, sdm_arrinfo c3, uint64_t N,

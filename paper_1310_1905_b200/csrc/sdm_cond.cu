@@ -41,6 +41,7 @@ __device__ __forceinline__ double vent(double Re, double X) {
 struct SdK {   // per-SD constants of one substep
   double rd3, krd3;   // r_d^3, kappa r_d^3
   double Kc, hDc;     // K_0 Nu/2 (eq. 24 without beta_T), heat * D_0 Sh/2
+  double c0Dc;        // c0 * D_0 Sh/2 (bounds c0 D_eff in single_root_bracket)
   double cDK;         // c0 * Dc * Kc
 };
 
@@ -212,7 +213,8 @@ __device__ __forceinline__ float sd_setup(double r0, double c0, double heat, dou
   const double Dc = fma(KC[KC_HALF_D0], shm, KC[KC_D0]);   // eq. 23 without beta_M: D_0 Sh / 2
   s.Kc = fma(KC[KC_HALF_K0], num, KC[KC_K0]);              // eq. 24 without beta_T: K_0 Nu / 2
   s.hDc = heat * Dc;
-  s.cDK = c0 * Dc * s.Kc;
+  s.c0Dc = c0 * Dc;
+  s.cDK = s.c0Dc * s.Kc;
   return eps;
 }
 
@@ -225,12 +227,36 @@ __device__ __forceinline__ float sd_setup(double r0, double c0, double heat, dou
 // Stopping rule for a Newton step of size d_k from an iterate whose previous step was d_(k-1):
 // the error left after the step is C d_k^2 with C = |g''/(2g')|, estimated by d_k/d_(k-1)^2 and
 // bounded below by 1/y (first step: 100/y); stop when that is below 1e-11 y.
+// Root selection.  eq. 17 can have SEVERAL roots inside the bracket of eq. 18-19 (a haze particle far from
+// equilibrium in supersaturated air: the implicit-Euler haze root, one at the unstable Koehler equilibrium and an
+// "activated" one), or two, in which case the paper's rule (:579) calls the bracket ill-posed.  The paper's
+// bisection then defines the result, and a Newton iteration started at y0 would land elsewhere.  Newton is
+// therefore used only where the bracket [lo, hi] provably or structurally holds at most one root:
+//  (1) it lies on the solute-dominated side of the Koehler curve, hi <= y_c = 3 kappa r_d^3 / A (for
+//      kappa <= 2 the activity term then outweighs the Kelvin term everywhere in it: a_w e^(A/r) rises with r, f
+//      has one zero and g = y - y0 - dt' f one sign change), or
+//  (2) it is narrow, hi - lo <= lo/2, and from max(lo, y_c) on the Kelvin term is too weak to bend g back:
+//      dt' c0 D 1.3 A / (2 r^3) <= 1/2 and e^(A/r) <= 1.3, or
+//  (3) the particle grows (lo = y0) in subsaturated air: a_w e^(A/r) = RH < 1 has one solution y_eq, on the
+//      rising side of the Koehler curve, f > 0 below it and f < 0 above, so g > 0 from y_eq on and changes sign
+//      once between y0 and y_eq (haze catching up with a moister cell: by far the most frequent wide bracket).
+// Everything else is solved by the paper's own procedure, literally (bisect_paper).  dtcD = dt' c0 D_0 Sh/2.
+__device__ __forceinline__ bool single_root_bracket(double lo, double hi, double y0, double RH, double rd3, double krd3, double A,
+                                                    double invA, double dtcD) {
+  const double yc = 3.0 * krd3 * invA;
+  if ((hi <= yc && krd3 <= 2.0 * rd3) || (RH < 1.0 && lo == y0)) return true;   // (1), (3)
+  const double ym = fmax(lo, yc);
+  const double K3 = 1.3 * A * dtcD;
+  return (hi - lo <= 0.5 * lo) && (ym * ym * ym >= K3 * K3) && (A * A <= 0.0625 * ym);   // (2)
+}
+
 enum { M_FIRST = 0, M_MAIN = 1, M_CHK_A = 2, M_CHK_B = 3 };
 
 __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, double krd3, const CellK& c, double dtp,
                                            int max_evals, double& y_out, unsigned& n_ill, unsigned& n_eval) {
   SdK s;
   s.rd3 = rd3; s.krd3 = krd3;
+  double Dc;
   {
     // [L] ventilation at the substep's starting radius (reading R-vent); Re from the terminal
     // velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2)
@@ -238,7 +264,7 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
     const double e = c.kE * (r0 * sqrt(r0));
     const double q = e / (sqrt(1.0 + e) + 1.0);
     const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
-    const double Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;   // eq. 23 without beta_M
+    Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;   // eq. 23 without beta_M
     s.Kc = cst::K_0 * vent(Re, c.Pr) * 0.5;              // eq. 24 without beta_T
     s.hDc = c.heat * Dc;
     s.cDK = c.c0 * Dc * s.Kc;
@@ -256,6 +282,28 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
       a = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
       b = y0 + fmax(two, 0.0);              // eq. 19
       if (!(a < b)) { y_out = a; return true; }
+      if (!single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc)) {
+        // the paper's procedure, literally (:573-579): signs at both ends, (a+b)/2 if they agree, else bisection
+        if (max_evals < 100) return false;   // not in a budgeted sweep: leave it to the pass that may finish
+        const double f0 = f;
+        double ga, gb;
+        if (a == y0) ga = -dtp * f0; else { growth_fd(a, s, c, f, df); ++n_eval; ga = a - y0 - dtp * f; }
+        if (b == y0) gb = -dtp * f0; else { growth_fd(b, s, c, f, df); ++n_eval; gb = b - y0 - dtp * f; }
+        if (ga == 0.0) { y_out = a; return true; }
+        if (gb == 0.0) { y_out = b; return true; }
+        if ((ga > 0.0) == (gb > 0.0)) { n_ill += (b - a > 1e-9 * b); y_out = 0.5 * (a + b); return true; }
+        while (b - a > 1e-15 * b) {
+          const double m = 0.5 * (a + b);
+          if (m <= a || m >= b) break;
+          growth_fd(m, s, c, f, df);
+          ++n_eval;
+          const double gm = m - y0 - dtp * f;
+          if (gm == 0.0) { y_out = m; return true; }
+          if ((gm > 0.0) == (ga > 0.0)) { a = m; ga = gm; } else { b = m; gb = gm; }
+        }
+        y_out = 0.5 * (a + b);
+        return true;
+      }
       // g(lo) < 0 < g(hi) is what a well-posed bracket means; the end that is not y0 is unverified
       lo = a; hi = b;
       lo_unv = !(f > 0.0); hi_unv = (f > 0.0);
@@ -551,8 +599,9 @@ struct __align__(16) CellRec {
   double eta;                                   // [L] viscosity, for the cell fields written at the end
   double th, rv, rhod, fbk;                     // theta, r_v (advanced every substep), rho_d, eq. 25 prefactor
   double T, invT, lv, pvs;                      // eq. 43, Table 2, [L] Clausius-Clapeyron
+  double invA, pad;
 };
-static_assert(sizeof(CellRec) == 176, "CellRec");
+static_assert(sizeof(CellRec) == 192, "CellRec");
 
 // everything the substep needs from (T, 1/T, p_vs, r_v, rho_d); square roots and reciprocals from fp32
 // seeds (sqrt_seeded, rcp_nr: relative error < 1e-14, they feed correction factors and RH to 1e-15)
@@ -564,6 +613,7 @@ __device__ __forceinline__ void cell_derive(CellRec& R, double RH_max) {
   R.lv = lv;
   R.RH = fmin(rv * rhod * rcp_nr<2>(rho_vs), RH_max);                              // eq. 30, :685
   R.A = (2.0 * cst::sigma_w / (cst::R_v * cst::rho_w)) * invT;                     // Table 2 :1056
+  R.invA = (cst::R_v * cst::rho_w / (2.0 * cst::sigma_w)) * T;
   R.c0 = (2.0 / cst::rho_w) * rho_vs;
   const double sqT = sqrt_seeded(T);
   const double lD = (2.0 * cst::D_0 * 0.03291540093383166 /* 1/sqrt(2 R_v) */) * (sqT * invT);   // [L] Fuchs-Sutugin lengths
@@ -729,7 +779,8 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
       double r = r0, dprev = 0.0;
       int st;
       // guards: the ventilation error bound (sd_setup) and the range of exp_kelvin
-      const bool guard = (eps > 0.f && eps * fabsf((float)two) > 1e-10f * (float)y0) || !(t < 4.0);
+      const bool guard = (eps > 0.f && eps * fabsf((float)two) > 1e-10f * (float)y0) || !(t < 4.0) ||
+                         !single_root_bracket(lo, hi, y0, c.RH, s.rd3, s.krd3, c.A, R.invA, dtp * s.c0Dc);
       if (!(lo < hi)) {
         st = (lo == y0) ? 1 : 2;                    // a = b: the result is a
       } else {

@@ -62,6 +62,22 @@ cudaError_t launch_coal_move_tile(int cpb, const SdArrays& a, const u16* rank, c
                                   const Counters& cnt, cudaStream_t st);
 void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
 
+// sdm_init.cu
+constexpr int INIT_MAX_MODES = 8;
+struct sdm_mode_view { double kappa, n_stp, r_mean, sigma_g; };   // same layout as sdm_lognormal_mode (sdm.h)
+struct InitParams {
+  int n_modes, n_spectra;
+  int mode_spectrum[INIT_MAX_MODES];
+  double mode_lnr[INIT_MAX_MODES], mode_amp[INIT_MAX_MODES], mode_2ls2[INIT_MAX_MODES];   // ln r_m, N/(sqrt(2 pi) ln s), 2 ln^2 s
+  double kappa[INIT_MAX_MODES], lnr_lo[INIT_MAX_MODES], lnr_hi[INIT_MAX_MODES];          // per spectrum
+  double sd_conc_spectrum, rho_stp;
+  double x0, y0, z0, x1, y1, z1;
+  u32 seed_lo, seed_hi;
+};
+int init_prepare(const sdm_mode_view* modes, int n_modes, double sd_conc_mean, double dV, InitParams& ip);
+void launch_init(const SdArrays& a, u32 N, const Grid& g, const InitParams& ip, Field th, Field rv, const double* rhod,
+                 double* RHeq, double* Akel, cudaStream_t st);
+
 // sdm_diag.cu
 void launch_diag_mom(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
                      double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st);

@@ -25,7 +25,7 @@ def test_header_declares_the_boundary_of_survey_8b():
     syms = declared_symbols()
     for s in ("sdm_create", "sdm_destroy", "sdm_step_sync", "sdm_step_async", "sdm_step_async_result", "sdm_diag_sd_conc",
               "sdm_diag_dry_rng", "sdm_diag_wet_rng", "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_export_state",
-              "sdm_init_from_arrays", "sdm_last_error", "sdm_stats"):
+              "sdm_init", "sdm_init_from_arrays", "sdm_last_error", "sdm_stats"):
         assert s in syms
 
 

@@ -560,3 +560,105 @@ def test_openmp_over_cells_is_bitwise_identical_to_serial():
     for k in res[0][0]:
         np.testing.assert_array_equal(res[0][0][k], res[1][0][k])
     np.testing.assert_array_equal(res[0][1][0], res[1][1][0])
+
+
+# ------------------------------------------------------------------------------ initialisation (section 5.1.6)
+VOCALS = [(0.61, 60e6, 0.02e-6, 1.4), (0.61, 40e6, 0.075e-6, 1.6)]   # PAPER.md :117-130 (mode diameters 0.04, 0.15 um)
+
+
+def _init_case(sd=64, nx=6, nz=75, seed=5, modes=VOCALS):
+    from paper_1310_1905_b200 import workloads as W
+    from tests.util import make_oracle
+
+    w = W.cfg2_2d(sd_per_cell=sd, nx=nx, nz=nz, seed=seed)
+    o = make_oracle(w)
+    N, ranges = o.init(modes, float(sd))
+    return w, o, N, ranges, o.get_state()
+
+
+def test_init_range_rule_and_agreement_with_the_independent_generator():
+    """:657: the multiplicity at both ends of the r_d range is >= 1 and just outside it is < 1; the limits equal
+    those found by workloads.auto_rd_range (an independent torch implementation of the same rule)."""
+    w, o, N, ranges, s = _init_case()
+    lo, hi = ranges[0]
+    assert N == 64 * 6 * 75 and len(ranges) == 1
+    np.testing.assert_allclose([lo, hi], np.log(w.meta["rd_range"]), rtol=0, atol=1e-9)
+
+    def mult(lnr):   # eq. 3 written out again, at STP density
+        dens = sum(n / (np.sqrt(2 * np.pi) * np.log(sg)) * np.exp(-(lnr - np.log(rm)) ** 2 / (2 * np.log(sg) ** 2))
+                   for _, n, rm, sg in VOCALS)
+        return dens * (hi - lo) / 64.0 * (20.0 * 1.0 * 20.0)
+
+    step = (np.log(1e-4) - np.log(1e-10)) / 200000
+    assert mult(lo) >= 1.0 and mult(hi) >= 1.0 and mult(lo - step) < 1.0 and mult(hi + step) < 1.0
+
+
+def test_init_positions_sizes_and_total_concentration():
+    """:655 uniform positions, :657 log-uniform dry radii inside the range, :659 the SDs of a cell add up to the
+    spectrum's total concentration scaled by rho_d / rho_STP (Monte-Carlo: within 5 standard errors)."""
+    w, o, N, ranges, s = _init_case(sd=128, nx=8)
+    lo, hi = ranges[0]
+    X, Z = 8 * 20.0, 75 * 20.0
+    assert s["x"].min() >= 0 and s["x"].max() < X and s["z"].min() >= 0 and s["z"].max() < Z
+    assert abs(s["x"].mean() / X - 0.5) < 5 / np.sqrt(12 * N) and abs(s["z"].mean() / Z - 0.5) < 5 / np.sqrt(12 * N)
+    lnr = np.log(s["rd3"]) / 3
+    assert lnr.min() >= lo - 1e-12 and lnr.max() <= hi + 1e-12
+    assert abs((lnr.mean() - lo) / (hi - lo) - 0.5) < 5 / np.sqrt(12 * N)
+    np.testing.assert_array_equal(s["id"], np.arange(N, dtype=np.uint32))
+    assert np.all(s["kappa"] == 0.61) and s["n"].min() >= 1
+    # total concentration: integral of eq. 3 over the range (erf closed form) x <rho_d>/rho_STP
+    from math import erf, log, sqrt
+    tot = sum(n * 0.5 * (erf((hi - log(rm)) / (sqrt(2) * log(sg))) - erf((lo - log(rm)) / (sqrt(2) * log(sg))))
+              for _, n, rm, sg in VOCALS)
+    rho_stp = 101325.0 / (287.0 * 293.15)
+    k = np.clip((s["z"] / 20.0).astype(int), 0, 74)
+    rhod = w.rhod.numpy()[0]
+    expect = tot * rhod.mean() / rho_stp
+    got = s["n"].sum() / (X * 1.0 * Z)
+    # per-SD weights n_i have a wide distribution: standard error from the sample itself
+    se = np.sqrt(N * np.var(s["n"].astype(np.float64))) / (X * Z)
+    assert abs(got - expect) < 5 * se and se < 0.05 * expect
+    # multiplicity of one SD follows the formula of :659 with its own cell's density
+    i = int(np.argmax(s["n"]))
+    dens = sum(n / (np.sqrt(2 * np.pi) * np.log(sg)) * np.exp(-(lnr[i] - np.log(rm)) ** 2 / (2 * np.log(sg) ** 2)) for _, n, rm, sg in VOCALS)
+    assert s["n"][i] == np.floor(dens * (hi - lo) / 128.0 * 400.0 * rhod[k[i]] / rho_stp + 0.5)
+
+
+def test_init_wet_radius_is_the_koehler_equilibrium_at_min_rh_095():
+    """:661-665: zero growth rate (RH = a_w exp(A/r)) at the cell's RH, capped at 0.95; the root lies on the stable
+    branch below the critical radius; agrees with the torch bisection of workloads.equilibrium_rw."""
+    import torch
+    from paper_1310_1905_b200 import workloads as W
+
+    w, o, N, ranges, s = _init_case(sd=32, nx=4)
+    k = np.clip((s["z"] / 20.0).astype(int), 0, 74)
+    T = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["T"] for r in w.rhod.numpy()[0]])
+    RH = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["RH"] for r in w.rhod.numpy()[0]])
+    A = 2 * 0.072 / (461.5 * T * 1000.0)
+    r = np.sqrt(s["rw2"])
+    r3 = r ** 3
+    S = (r3 - s["rd3"]) / (r3 - s["rd3"] * (1 - 0.61)) * np.exp(A[k] / r)
+    np.testing.assert_allclose(S, np.minimum(RH[k], 0.95), rtol=1e-11)
+    assert np.all(r > np.cbrt(s["rd3"])) and np.all(r < np.sqrt(3 * 0.61 * s["rd3"] / A[k]))
+    assert RH.max() > 1.0 and RH.min() < 0.7          # the profile spans clear and (super)saturated air
+    ref = W.equilibrium_rw(torch.from_numpy(s["rd3"]), torch.full((N,), 0.61, dtype=torch.float64),
+                           torch.from_numpy(np.minimum(RH[k], 0.95)), torch.from_numpy(T[k])).numpy()
+    np.testing.assert_allclose(r, ref, rtol=1e-9)
+
+
+def test_init_external_mixture_shares_the_sds_between_kappas():
+    """:659 "externally mixed aerosol ... multiple spectra, each characterised by different kappa": SD i belongs to
+    spectrum i mod G, each spectrum has its own range and its SDs reproduce its own concentration."""
+    modes = [(0.61, 60e6, 0.02e-6, 1.4), (1.28, 40e6, 0.075e-6, 1.6)]
+    w, o, N, ranges, s = _init_case(sd=128, nx=8, modes=modes)
+    assert len(ranges) == 2 and ranges[0] != ranges[1]
+    assert np.all(s["kappa"][0::2] == 0.61) and np.all(s["kappa"][1::2] == 1.28)
+    from math import erf, log, sqrt
+    rho_ratio = w.rhod.numpy()[0].mean() / (101325.0 / (287.0 * 293.15))
+    for g, (kap, n, rm, sg) in enumerate(modes):
+        lo, hi = ranges[g]
+        tot = n * 0.5 * (erf((hi - log(rm)) / (sqrt(2) * log(sg))) - erf((lo - log(rm)) / (sqrt(2) * log(sg))))
+        ng = s["n"][g::2].astype(np.float64)
+        got = ng.sum() / (160.0 * 1500.0)
+        se = np.sqrt(len(ng) * np.var(ng)) / (160.0 * 1500.0)
+        assert abs(got - tot * rho_ratio) < 5 * se

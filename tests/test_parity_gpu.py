@@ -369,3 +369,99 @@ def test_full_size_3d_sampled_columns_match_oracle():
         assert not np.array_equal(np_(th_before[sl]).ravel(), oth)                 # condensation did act
         ncoll += o.counters()["collisions"]
     assert g["id"].numel() <= N0
+
+
+# ------------------------------------------------------------------------------------ init() (section 5.1.6)
+VOCALS = [(0.61, 60e6, 0.02e-6, 1.4), (0.61, 40e6, 0.075e-6, 1.6)]
+
+
+@pytest.mark.parametrize("case", ["2d", "3d_subdomain", "mixture"])
+def test_device_init_matches_oracle_init(case):
+    """sdm_init vs the oracle's init on the same fields, seed and modes: ids, positions (hence cells) bit-equal,
+    dry and wet radii within 1e-9, the range of :657 equal.  Multiplicities are floor(x + 1/2) of a product that
+    contains exp() of the two maths libraries (1 ulp apart at worst): they must agree exactly for all but a
+    1e-4 fraction of the SDs, and there differ by 1."""
+    b = binding()
+    if case == "2d":
+        w, modes, ext = W.cfg2_2d(sd_per_cell=32, nx=12, nz=75, seed=21), VOCALS, {}
+    elif case == "3d_subdomain":
+        w, modes = W.cfg4_3d(sd_per_cell=16, nx=6, ny=5, nz=64, seed=22), VOCALS
+        ext = dict(x0=20.0, x1=100.0, y0=0.0, y1=60.0, z0=200.0, z1=1280.0)
+    else:
+        w, modes, ext = W.cfg2_2d(sd_per_cell=64, nx=8, nz=75, seed=23), [(0.61, 60e6, 0.02e-6, 1.4), (1.28, 40e6, 0.075e-6, 1.6)], {}
+    sd = w.meta["sd_per_cell"]
+    o = make_oracle(w)
+    N, ranges = o.init(modes, float(sd), **ext)
+    p = b.Particles(max_sd=N + 7, sd_conc_mean=float(sd), modes=modes, **dict(w.init, **ext))
+    cs = [c.cuda() for c in w.courants] + [None] * (3 - len(w.courants))
+    th, rv = w.th.cuda(), w.rv.cuda()
+    p.init(th, rv, w.rhod.cuda(), *cs)
+    assert p.n_sd() == N
+    for g, (lo, hi) in enumerate(ranges):
+        np.testing.assert_allclose(p.init_range(g), (lo, hi), rtol=0, atol=1e-12)
+    gs, rs = sorted_by_id(p.export_state()), sorted_by_id(o.get_state())
+    np.testing.assert_array_equal(gs["id"].astype(np.uint32), rs["id"])
+    for k, present in zip("xyz", p.dims):
+        if present:
+            np.testing.assert_array_equal(gs[k], rs[k])
+    np.testing.assert_array_equal(gs["kappa"], rs["kappa"])
+    np.testing.assert_allclose(np.cbrt(gs["rd3"]), np.cbrt(rs["rd3"]), rtol=RTOL)
+    np.testing.assert_allclose(np.sqrt(gs["rw2"]), np.sqrt(rs["rw2"]), rtol=RTOL)
+    dn = gs["n"].astype(np.int64) - rs["n"].astype(np.int64)
+    assert np.abs(dn).max() <= 1 and np.count_nonzero(dn) <= 1e-4 * N + 1
+    # th, rv untouched (:663); the initialised population steps like a loaded one
+    np.testing.assert_array_equal(np_(th), np_(w.th))
+    agree = dn == 0
+    if agree.all():
+        po, oo = b.make_opts(**w.opts), oracle.make_opts(**w.opts)
+        o.step(oo)
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+        compare_states(p, o)
+        compare_fields(th, rv, o)
+
+
+def test_device_init_errors():
+    b = binding()
+    w = W.cfg2_2d(sd_per_cell=8, nx=4, nz=4, seed=1)
+    p = b.Particles(max_sd=1000, sd_conc_mean=8.0, **w.init)                      # no modes
+    with pytest.raises(b.SdmError, match="without dry-aerosol modes"):
+        p.init(w.th.cuda(), w.rv.cuda(), w.rhod.cuda())
+    p = b.Particles(max_sd=100, sd_conc_mean=8.0, modes=VOCALS, **w.init)        # 128 SDs do not fit
+    with pytest.raises(b.SdmError, match="exceeds max_sd"):
+        p.init(w.th.cuda(), w.rv.cuda(), w.rhod.cuda())
+    with pytest.raises(b.SdmError, match="too dilute"):
+        b.Particles(max_sd=100, sd_conc_mean=8.0, modes=[(0.61, 1e-3, 0.02e-6, 1.4)], **w.init)
+    with pytest.raises(b.SdmError, match="inside the grid"):
+        b.Particles(max_sd=100, sd_conc_mean=8.0, modes=VOCALS, **dict(w.init, x1=1e6))
+
+
+# ------------------------------------------------------------------------------------ which root of eq. 17
+def test_first_step_in_supersaturated_air_takes_the_bisection_root():
+    """The initial haze (equilibrium at RH <= 0.95) under RH_max = 1.05 is far from equilibrium: eq. 17 then has
+    several roots inside the bracket of eq. 18-19, or two (the ill-posed case of :579).  The paper's bisection
+    defines which one is meant; the Newton path must certify a single root or defer to that procedure."""
+    w = W.cfg2_2d(sd_per_cell=24, nx=6, nz=75, seed=21)     # full height: cells from RH 0.66 to the 1.05 cap
+    p, o, th, rv = run_both(w, 2)
+    sp, so = p.stats(), o.counters()
+    assert sp["ill_posed"] == so["ill_posed"] > 100
+
+
+def test_root_selection_scan_of_independent_sds():
+    """Sizes from barely wet to 3000 r_d, r_d from 1 nm to 2 um, kappa 0.05-1.55, RH 0.3-1.05, multiplicity 1 (no
+    feedback: every SD-substep is an independent instance of eq. 17-19): radii and ill-posed counts must match."""
+    seed, nx, nz, sd = 7, 24, 24, 64
+    w = W.cfg2_2d(sd_per_cell=sd, nx=nx, nz=nz, seed=seed)
+    idx = torch.arange(w.n_sd, dtype=torch.int64)
+    u1, u2, u3 = (W.hash_uniform(seed, 200 + k, idx) for k in range(3))
+    rd = torch.exp(np.log(1e-9) + u1 * (np.log(2e-6) - np.log(1e-9)))
+    w.state["rd3"] = rd ** 3
+    w.state["rw2"] = (rd * torch.exp(1e-4 + u2 * u2 * np.log(3e3))) ** 2
+    w.state["kappa"] = torch.where(u3 < 0.5, torch.full_like(u3, 0.61), 0.05 + 1.5 * u3)
+    w.state["n"] = torch.ones_like(w.state["n"])
+    ci = torch.arange(nx, dtype=torch.float64)[:, None].expand(nx, nz)
+    w.rv = w.rv * (0.35 + 0.95 * ci / (nx - 1))
+    p, o, th, rv = run_both(w, 2, opts=dict(coal=False, adve=False, sedi=False))
+    sp, so = p.stats(), o.counters()
+    assert sp["ill_posed"] == so["ill_posed"] > 50
+    assert sp["cond_slow"] > 0.05 * sp["sd_substeps"]       # the literal-bisection path was exercised

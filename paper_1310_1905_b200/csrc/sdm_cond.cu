@@ -250,25 +250,76 @@ __device__ __forceinline__ bool single_root_bracket(double lo, double hi, double
   return (hi - lo <= 0.5 * lo) && (ym * ym * ym >= K3 * K3) && (A * A <= 0.0625 * ym);   // (2)
 }
 
+// per-SD constants of one substep in plain fp64 (cond_solve and the literal bisection)
+__device__ __forceinline__ void slow_setup(double y0, double rd3, double krd3, const CellK& c, SdK& s, double& Dc) {
+  s.rd3 = rd3; s.krd3 = krd3;
+  // [L] ventilation at the substep's starting radius (reading R-vent); Re from the terminal
+  // velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2)
+  const double r0 = sqrt(y0);
+  const double e = c.kE * (r0 * sqrt(r0));
+  const double q = e / (sqrt(1.0 + e) + 1.0);
+  const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
+  Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;     // eq. 23 without beta_M
+  s.Kc = cst::K_0 * vent(Re, c.Pr) * 0.5;   // eq. 24 without beta_T
+  s.hDc = c.heat * Dc;
+  s.c0Dc = c.c0 * Dc;
+  s.cDK = s.c0Dc * s.Kc;
+}
+
+// The paper's procedure (:573-579) for one SD by a whole WARP: signs of g at both ends, (a+b)/2 if they agree,
+// else bisection - five levels per round: lane l = 1..31 is node l of the binary tree of midpoints below the
+// current interval (heap order), computes its midpoint with the very operations the serial bisection would use on
+// the way there, evaluates g, and the ballot of the signs lets every lane walk the five levels.  Same result
+// as the serial loop of the oracle, a fifth of its latency.  All lanes pass the same arguments.
+__device__ __forceinline__ double bisect_paper_warp(double a, double b, double f0, double y0, const SdK& s, const CellK& c,
+                                                    double dtp, int lane, unsigned& n_ill, unsigned& n_eval) {
+  double f, df;
+  double ga, gb;
+  if (a == y0) ga = -dtp * f0; else { growth_fd(a, s, c, f, df); n_eval += (lane == 0); ga = a - y0 - dtp * f; }
+  if (b == y0) gb = -dtp * f0; else { growth_fd(b, s, c, f, df); n_eval += (lane == 0); gb = b - y0 - dtp * f; }
+  if (ga == 0.0) return a;
+  if (gb == 0.0) return b;
+  if ((ga > 0.0) == (gb > 0.0)) { n_ill += (lane == 0 && b - a > 1e-9 * b); return 0.5 * (a + b); }
+  const bool ga_pos = ga > 0.0;
+  const int depth = 31 - __clz(max(lane, 1));   // level of this lane's node (root = 0)
+  for (;;) {
+    // this lane's node: follow the bits of `lane` below its leading one from the current interval
+    double lo = a, hi = b;
+    bool alive = lane >= 1;
+    for (int j = depth - 1; j >= 0 && alive; --j) {
+      if (!(hi - lo > 1e-15 * hi)) { alive = false; break; }
+      const double m = 0.5 * (lo + hi);
+      if (m <= lo || m >= hi) { alive = false; break; }
+      if ((lane >> j) & 1) lo = m; else hi = m;
+    }
+    double m = 0.5 * (lo + hi);
+    alive = alive && (hi - lo > 1e-15 * hi) && m > lo && m < hi;
+    double gm = 1.0;
+    if (alive) { growth_fd(m, s, c, f, df); ++n_eval; gm = m - y0 - dtp * f; }
+    const unsigned right = __ballot_sync(0xffffffffu, alive && ((gm > 0.0) == ga_pos));
+    const unsigned zero = __ballot_sync(0xffffffffu, alive && gm == 0.0);
+    // walk five levels with the signs
+    int node = 1;
+    bool done = false;
+    for (int lev = 0; lev < 5; ++lev) {
+      if (!(b - a > 1e-15 * b)) { done = true; break; }
+      const double mm = 0.5 * (a + b);
+      if (mm <= a || mm >= b) { done = true; break; }
+      if ((zero >> node) & 1u) return mm;
+      if ((right >> node) & 1u) { a = mm; node = 2 * node + 1; } else { b = mm; node = 2 * node; }
+    }
+    if (done) break;
+  }
+  return 0.5 * (a + b);
+}
+
 enum { M_FIRST = 0, M_MAIN = 1, M_CHK_A = 2, M_CHK_B = 3 };
 
 __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, double krd3, const CellK& c, double dtp,
                                            int max_evals, double& y_out, unsigned& n_ill, unsigned& n_eval) {
   SdK s;
-  s.rd3 = rd3; s.krd3 = krd3;
   double Dc;
-  {
-    // [L] ventilation at the substep's starting radius (reading R-vent); Re from the terminal
-    // velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2)
-    const double r0 = sqrt(y0);
-    const double e = c.kE * (r0 * sqrt(r0));
-    const double q = e / (sqrt(1.0 + e) + 1.0);
-    const double Re = (cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
-    Dc = cst::D_0 * vent(Re, c.Sc) * 0.5;   // eq. 23 without beta_M
-    s.Kc = cst::K_0 * vent(Re, c.Pr) * 0.5;              // eq. 24 without beta_T
-    s.hDc = c.heat * Dc;
-    s.cDK = c.c0 * Dc * s.Kc;
-  }
+  slow_setup(y0, rd3, krd3, c, s, Dc);
   int mode = M_FIRST;
   double yE = y0, y = y0, g = 0.0, gp = 1.0, a = 0.0, b = 0.0, lo = 0.0, hi = 0.0, dprev = 0.0;
   bool lo_unv = false, hi_unv = false;
@@ -834,23 +885,46 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
       }
     }
     __syncthreads();
-    // C. the listed rest: the bracketed state machine, from the start of the substep
+    // C. the listed rest, from the start of the substep: cond_solve (bracketed Newton) or the paper's literal
+    // bisection.  A long list (a shock, e.g. the first step) is worked off one SD per thread; a short one
+    // (steady state: usually one SD holding the whole tile at the barrier) one SD per WARP, for latency.
     const int nlist = (int)ctr[1];
     if (nlist > 0) {
-      for (int k = tid; k < nlist; k += T) {
+      const bool per_warp = nlist <= 2 * NW;
+      for (int k = per_warp ? warp : tid; k < nlist; k += per_warp ? NW : T) {
         const int e = (int)list[k];
         const CellRec& R = s_cell[(int)cidx[e]];
         CellK c;
         c.RH = R.RH; c.A = R.A; c.c0 = R.c0; c.lD = R.lD; c.lK = R.lK; c.heat = R.heat; c.kE = R.kE; c.Sc = R.Sc; c.Pr = R.Pr;
         const double r0 = s_r[e], y0 = r0 * r0;
+        const double rd2 = s_rd2[e], rd3 = s_rd3[e], krd3 = s_krd3[e];
         double y1 = y0;
-        unsigned ill = 0;
-        cond_solve(y0, s_rd2[e], s_rd3[e], s_krd3[e], c, dtp, 200, y1, ill, n_eval);
-        const double r1 = sqrt(y1);
-        n_ill += ill;
-        ++n_sub; ++n_slow;
-        s_con[e] = s_dn[e] * (r1 * r1 * r1 - r0 * y0);
-        s_r[e] = r1;
+        unsigned ill = 0, ev = 0;
+        bool solved = false;
+        if (per_warp) {   // all lanes hold the same SD
+          SdK s;
+          double Dc, f, df;
+          slow_setup(y0, rd3, krd3, c, s, Dc);
+          growth_fd(y0, s, c, f, df);
+          const double two = 2.0 * dtp * f;
+          const double a = fmax(rd2, y0 + fmin(two, 0.0)), b = y0 + fmax(two, 0.0);   // eq. 18-19
+          if (a < b && !single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, R.invA, dtp * s.c0Dc)) {
+            ev = (lane == 0);
+            y1 = bisect_paper_warp(a, b, f, y0, s, c, dtp, lane, ill, ev);
+            solved = true;
+          }
+        }
+        if (!solved) {
+          cond_solve(y0, rd2, rd3, krd3, c, dtp, 200, y1, ill, ev);
+          if (per_warp && lane != 0) { ill = 0; ev = 0; }   // the lanes of the warp did the same work: count it once
+        }
+        n_ill += ill; n_eval += ev;
+        if (!per_warp || lane == 0) {
+          const double r1 = sqrt(y1);
+          ++n_sub; ++n_slow;
+          s_con[e] = s_dn[e] * (r1 * r1 * r1 - r0 * y0);
+          s_r[e] = r1;
+        }
       }
       __syncthreads();
     }

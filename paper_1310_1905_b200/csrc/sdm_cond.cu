@@ -177,22 +177,25 @@ __device__ __forceinline__ double rcp_seeded(double a) {
   return fma(fma(-a, x, 1.0), x, x);
 }
 
+// (1 + x)^(1/3) - 1 for x >= 0.02 from the fp32 cube root and one fp64 Newton step (relative error ~1e-14)
+__device__ __forceinline__ double cbrt1pm1_seeded(double x) {
+  const double w = 1.0 + x;
+  const double c = (double)cbrtf((float)w);
+  const double c2 = c * c;
+  return (c - 1.0) - fma(c2, c, -w) * rcp_seeded(3.0 * c2);
+}
+
 // [L] ventilation at the substep's starting radius r0 (reading R-vent) -> per-SD constants.
 // Re from the terminal velocity of Khvorostyanov & Curry 2002: e = c1 sqrt(X) = kE r^(3/2),
-// Re = (delta0^2/4) (sqrt(1+e) - 1)^2.  Up to Re Sc = 0.02 (r ~ 20 um): fp64 with seeded roots and the
-// binomial series of (1+x)^(1/3) - 1 to x^5 (next term 2e-10 of the first).  Beyond (drizzle and rain)
-// Sh - 2 and Nu - 2 are evaluated in fp32 by formulas that keep their RELATIVE error below 2e-6;
-// D = D_0 (1 + (Sh-2)/2) is then off by at most eps_D = 2e-6 min((Sh-2)/2, 1), likewise K, and f of
-// eq. 20-21 by at most eps_D + eps_K relative.  The implicit step moves r_w^2 by less than |2 dt' f(y0)|
-// (eq. 18-19), so the caller accepts these constants only if (eps_D + eps_K) |2 dt' f0| <= 1e-10 y0 and
-// otherwise leaves the SD to cond_solve, which evaluates everything in fp64.  Returns eps_D + eps_K.
-__device__ __forceinline__ float sd_setup(double r0, double c0, double heat, double kE, double Sc, double Pr, SdK& s) {
+// Re = (delta0^2/4) (sqrt(1+e) - 1)^2.  fp64 throughout, with roots and reciprocals from fp32 seeds and one
+// Newton step (~1e-14).  Up to Re Sc = 0.02 (r ~ 20 um) the binomial series of (1+x)^(1/3) - 1 to x^5 (next
+// term 2e-10 of the first); beyond, the seeded cube root; Re > 1 (drizzle and rain) takes the library pow.
+__device__ __forceinline__ void sd_setup(double r0, double c0, double heat, double kE, double Sc, double Pr, SdK& s) {
   const double e = kE * (r0 * sqrt_seeded(r0));
   const double q = e * rcp_seeded(sqrt_seeded(1.0 + e) + 1.0);   // sqrt(1+e) - 1 without cancellation
   const double Re = KC[KC_D2Q] * (q * q);
   const double xs = Re * Sc, xp = Re * Pr;
   double shm, num;   // Sh - 2, Nu - 2
-  float eps = 0.f;
   if (fmax(xs, xp) < 0.02) {
     double a = KC[KC_B5], b = KC[KC_B5];
     a = fma(a, xs, KC[KC_B4]); b = fma(b, xp, KC[KC_B4]);
@@ -201,21 +204,18 @@ __device__ __forceinline__ float sd_setup(double r0, double c0, double heat, dou
     a = fma(a, xs, KC[KC_B1]); b = fma(b, xp, KC[KC_B1]);
     shm = a * xs; num = b * xp;
   } else {
-    float sf = expm1f(log1pf((float)xs) * (1.0f / 3.0f)), nf = expm1f(log1pf((float)xp) * (1.0f / 3.0f));
+    shm = cbrt1pm1_seeded(xs); num = cbrt1pm1_seeded(xp);
     if (Re > 1.0) {   // (1 + c)(1 + m) - 1, m = Re^0.077 - 1
-      const float m = expm1f(0.077f * logf((float)Re));
-      sf = sf + m + sf * m;
-      nf = nf + m + nf * m;
+      const double m = pow(Re, 0.077) - 1.0;
+      shm = shm + m + shm * m;
+      num = num + m + num * m;
     }
-    shm = (double)sf; num = (double)nf;
-    eps = 2e-6f * (fminf(0.5f * sf, 1.0f) + fminf(0.5f * nf, 1.0f));
   }
   const double Dc = fma(KC[KC_HALF_D0], shm, KC[KC_D0]);   // eq. 23 without beta_M: D_0 Sh / 2
   s.Kc = fma(KC[KC_HALF_K0], num, KC[KC_K0]);              // eq. 24 without beta_T: K_0 Nu / 2
   s.hDc = heat * Dc;
   s.c0Dc = c0 * Dc;
   s.cDK = s.c0Dc * s.Kc;
-  return eps;
 }
 
 // One condensation substep of one SD: root of g(y) = y - y0 - dt' f(y) in [a, b] of eq. 18-19
@@ -629,7 +629,7 @@ k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __rest
 //  * r_w (not r_w^2) is resident in shared memory: no sqrt per substep, N d(r_w^3) by two products;
 //  * the sweep is straight-line code around growth_r with a warp-uniform iteration loop; anything
 //    irregular (Newton leaving the bracket of eq. 18-19, an end to verify, slow convergence, a Kelvin
-//    exponent or a ventilation error bound out of range) is put on a list and solved afterwards by
+//    exponent out of range, a bracket that may hold several roots) is put on a list and solved afterwards by
 //    cond_solve, the robust state machine;
 //  * warps take 32-SD chunks of the tile from a shared counter, so a warp that met slow SDs does not
 //    hold the others at the barrier;
@@ -820,7 +820,7 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
       s.krd3 = valid ? s_krd3[e] : 1e-21;
       CellR c;
       c.RH = R.RH; c.A = R.A; c.lD = R.lD; c.lK = R.lK; c.qD = R.qD; c.qK = R.qK; c.lD171 = R.lD171; c.lK171 = R.lK171;
-      const float eps = sd_setup(r0, R.c0, R.heat, R.kE, R.Sc, R.Pr, s);
+      sd_setup(r0, R.c0, R.heat, R.kE, R.Sc, R.Pr, s);
       double y0, f, dfr, t;
       growth_r(r0, s, c, y0, f, dfr, t);
       n_eval += valid;
@@ -829,8 +829,8 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
       double hi = y0 + fmax(two, 0.0);              // eq. 19
       double r = r0, dprev = 0.0;
       int st;
-      // guards: the ventilation error bound (sd_setup) and the range of exp_kelvin
-      const bool guard = (eps > 0.f && eps * fabsf((float)two) > 1e-10f * (float)y0) || !(t < 4.0) ||
+      // guards: the range of exp_kelvin, and the bracket must hold at most one root
+      const bool guard = !(t < 4.0) ||
                          !single_root_bracket(lo, hi, y0, c.RH, s.rd3, s.krd3, c.A, R.invA, dtp * s.c0Dc);
       if (!(lo < hi)) {
         st = (lo == y0) ? 1 : 2;                    // a = b: the result is a
@@ -846,6 +846,10 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
           st = (dprev * dprev <= KC[KC_TOL400] * (rn * rn)) ? 1 : 0;
         }
       }
+#ifdef SDM_DEBUG_REASON
+      if (valid && st == 2) atomicAdd(&cnt.collisions[tid], 1ull);                 // first Newton step left the bracket / a = b off y0
+      if (valid && guard) atomicAdd(&cnt.pairs[tid], 1ull);                        // guard (certificate, eps, t)
+#endif
       if (guard) st = 2;
       if (!valid) st = 1;
       for (int it = 1; it < cp.kfast; ++it) {
@@ -870,6 +874,9 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
           }
         }
       }
+#ifdef SDM_DEBUG_REASON
+      if (valid && st == 0) atomicAdd(&cnt.near_ties[tid], 1ull);                  // no convergence within kfast evaluations
+#endif
       if (st == 0) st = 2;
       if (valid && st == 1) {
         s_con[e] = s_dn[e] * (r * r * r - r0 * y0);

@@ -438,15 +438,13 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   }
   ctx->have_order = true;
   if (op->cond) {
-    // largest candidate tile that fits the small tile kernel, else the large one, else one cell per CTA in place
+    // the most preferred tile kernel (small, medium, large) any candidate tile size fits, with the largest such
+    // tile; else one cell per CTA in place in global memory
     int cpb = 1, variant = cond_variant(1, (int)ctx->max_nc);
-    for (int want = 1; want <= 2; ++want) {
-      bool found = false;
-      for (int k = 0; k < 4 && !found; ++k) {
-        const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
-        if (cond_variant(cand, (int)ctx->h_info[4 + k]) == want) { cpb = cand; variant = want; found = true; }
-      }
-      if (found || variant == want) break;
+    for (int k = 3; k >= 0; --k) {
+      const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
+      const int v = cond_variant(cand, (int)ctx->tile_max[k]);
+      if (v && (variant == 0 || v <= variant)) { cpb = cand; variant = v; }
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
     t_begin(ctx, SDM_STAGE_COND, st);

@@ -977,15 +977,29 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
 #define SDM_COND_MINB 5    // its CTAs per SM
 #endif
 using CondSmall = Cond4<SDM_COND_CAP, 128>;
-using CondLarge = Cond4<4096, 512>;
+using CondMedium = Cond4<1280, 256>;   // 3 CTAs of 256 threads per SM: cells of ~1000 SDs
+using CondLarge = Cond4<4096, 512>;    // one CTA of 512 threads per SM: cells of thousands of SDs
 constexpr size_t kCondSmallBudget = (228 * 1024 - SDM_COND_MINB * 1024) / SDM_COND_MINB;   // per CTA, 1 KB reserved each
-constexpr size_t kCondLargeBudget = 226 * 1024;
+constexpr size_t kCondMediumBudget = (228 * 1024 - 3 * 1024) / 3;
+constexpr size_t kCondLargeBudget = 227 * 1024;
 
-// 1: small tile kernel, 2: large tile kernel, 0: a tile of cpb cells with up to `need` SDs fits neither
+// 1, 2, 3: small, medium, large tile kernel (in order of preference); 0: a tile of cpb cells with up to `need`
+// SDs fits none of them
 int cond_variant(int cpb, int need) {
   if (cpb <= 128 && need <= SDM_COND_CAP && CondSmall::smem(cpb) <= kCondSmallBudget) return 1;
-  if (cpb <= 512 && need <= 4096 && CondLarge::smem(cpb) <= kCondLargeBudget) return 2;
+  if (cpb <= 256 && need <= 1280 && CondMedium::smem(cpb) <= kCondMediumBudget) return 2;
+  if (cpb <= 512 && need <= 4096 && CondLarge::smem(cpb) <= kCondLargeBudget) return 3;
   return 0;
+}
+
+template <int CAP, int T, int MINB>
+static cudaError_t launch_cond4(size_t smem, int grid, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
+                                Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, int cpb,
+                                cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_cond4<CAP, T, MINB><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  return cudaGetLastError();
 }
 
 // eta, rho_a per cell when condensation is switched off
@@ -1005,20 +1019,11 @@ cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays&
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st) {
   const int grid = (g.ncell + cpb - 1) / cpb;
-  if (variant == 1) {
-    const size_t smem = CondSmall::smem(cpb);
-    cudaError_t e = cudaFuncSetAttribute(k_cond4<SDM_COND_CAP, 128, SDM_COND_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_cond4<SDM_COND_CAP, 128, SDM_COND_MINB><<<grid, 128, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
-  } else if (variant == 2) {
-    const size_t smem = CondLarge::smem(cpb);
-    cudaError_t e = cudaFuncSetAttribute(k_cond4<4096, 512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    k_cond4<4096, 512, 1><<<grid, 512, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
-  } else {
-    const size_t smem = cond_smem_bytes(cpb, 0);
-    k_cond<false><<<grid, COND_THREADS, smem, st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);
-  }
+  if (variant == 1)
+    return launch_cond4<SDM_COND_CAP, 128, SDM_COND_MINB>(CondSmall::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  if (variant == 2) return launch_cond4<1280, 256, 3>(CondMedium::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  if (variant == 3) return launch_cond4<4096, 512, 1>(CondLarge::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  k_cond<false><<<grid, COND_THREADS, cond_smem_bytes(cpb, 0), st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);
   return cudaGetLastError();
 }
 

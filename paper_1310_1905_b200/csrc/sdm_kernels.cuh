@@ -39,9 +39,9 @@ cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 ste
 void launch_export_order(const u32* id, const u16* rank, const u32* seg, int ncell, u32* ids_sorted, cudaStream_t st);
 
 // sdm_cond.cu
-// cpb: cells per CTA; variant = cond_variant(cpb, most populated tile): 1 / 2 = shared-memory tile kernels for
-// sparse / crowded cells, 0 = fits neither: work in place in global memory (cpb == 1, `alt` = idle ping-pong
-// copy used as scratch)
+// cpb: cells per CTA; variant = cond_variant(cpb, most populated tile): 1, 2, 3 = shared-memory tile kernels for
+// up to 800 / 1280 / 4096 SDs per tile (in order of preference), 0 = fits none: work in place in global memory
+// (cpb == 1, `alt` = idle ping-pong copy used as scratch)
 int cond_variant(int cpb, int need);
 int cond_tile_candidate(int cpb0, int k);   // k-th candidate tile size (cells) tried by k_tile_max, k = 0..3
 cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,

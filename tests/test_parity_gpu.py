@@ -181,6 +181,15 @@ def test_crowded_cells_fall_back_to_global_memory_paths():
     assert p.stats()["max_cell_count"] > 2500
 
 
+def test_cells_of_a_thousand_sds():
+    """~1000 SDs per cell (top of the configs[4] sweep): the 1280-slot condensation tile kernel, bitonic ranks by a
+    CTA per cell, the per-cell coalescence kernel."""
+    w = rain_mix(W.cfg2_2d(sd_per_cell=1000, nx=3, nz=4, seed=14), frac=0.3)
+    p, o, _, _ = run_both(w, 2, opts=dict(sstp_cond=3))
+    assert 800 < p.stats()["max_cell_count"] <= 1280
+    assert p.stats()["collisions"] == o.counters()["collisions"] > 0
+
+
 # ----------------------------------------------------------------------------------------------- API
 def test_strided_fields_and_optional_arguments():
     """arrinfo_t strides (:730-745): halo-padded, non-contiguous th/rv/rhod give the same result."""

@@ -219,6 +219,70 @@ __global__ void __launch_bounds__(128) k_rank_count(const u32* __restrict__ id, 
   }
 }
 
+// Ranks for cells of tens to thousands of SDs (m <= 8192) by BUCKETS: the Philox keys are uniform, so the top bits of the key
+// split a cell's SDs into P/16 buckets of ~16; a histogram and a scan give every bucket its place, the keys are
+// scattered bucket by bucket, and an SD's rank is the start of its bucket plus the number of smaller keys inside
+// it: ~16 compares per SD instead of the log^2 m barriers and swaps of the bitonic network (which stays for cells
+// beyond 8192 SDs).  G = 32: a warp per cell, 4 cells per CTA; G = 256: a CTA per cell.
+// Shared memory per group: u64 keys[P], u64 sorted[P], u32 hist[P/16].
+template <int G>
+__global__ void __launch_bounds__(CtaOf<G>::threads) k_rank_bucket(const u32* __restrict__ id, const u32* __restrict__ seg,
+                                                                   int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                                                                   u16* __restrict__ rank, int* __restrict__ d_error) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NG = CtaOf<G>::threads / G;
+  const int gi = threadIdx.x / G;
+  const Group<G> grp = make_group<G>(nullptr);
+  const int NB = max(P >> 4, 4);               // buckets (power of two)
+  const int shift = 64 - (31 - __clz(NB));     // key >> shift = bucket
+  unsigned char* base = smem_raw + (size_t)gi * ((size_t)P * 16 + (size_t)NB * 4);
+  u64* skey = reinterpret_cast<u64*>(base);
+  u64* ssort = skey + P;
+  u32* hist = reinterpret_cast<u32*>(ssort + P);
+  const int c = blockIdx.x * NG + gi;
+  const bool live = c < ncell;                 // (no early return: CTA-wide groups meet at barriers)
+  const u32 s0 = live ? seg[c] : 0u;
+  int m = live ? (int)(seg[c + 1] - s0) : 0;
+  if (m > P) { if (grp.lane == 0) atomicExch(d_error, 1); m = 0; }
+  for (int b = grp.lane; b < NB; b += G) hist[b] = 0u;
+  grp.sync();
+  for (int t = grp.lane; t < m; t += G) {
+    const u32 sid = id[s0 + t];
+    const u64 key = ((u64)shuffle_key(sid, step, 0u, seed_lo, seed_hi) << 32) | sid;
+    skey[t] = key;
+    atomicAdd(&hist[(u32)(key >> shift)], 1u);
+  }
+  grp.sync();
+  // exclusive scan of the histogram by the first W = min(G, 32) lanes of the group (NB/W consecutive buckets each)
+  constexpr int W = G < 32 ? G : 32;
+  if (grp.lane < W) {
+    const int per = max(NB / W, 1);
+    const int b0 = grp.lane * per;
+    u32 sum = 0;
+    if (b0 < NB) for (int b = b0; b < b0 + per; ++b) sum += hist[b];
+    u32 inc = sum;
+    const u32 mask = G >= 32 ? 0xffffffffu : grp.mask;
+#pragma unroll
+    for (int d = 1; d < W; d <<= 1) { const u32 v = __shfl_up_sync(mask, inc, d, W); if (grp.lane >= d) inc += v; }
+    u32 run = inc - sum;
+    if (b0 < NB) for (int b = b0; b < b0 + per; ++b) { const u32 h = hist[b]; hist[b] = run; run += h; }
+  }
+  grp.sync();
+  for (int t = grp.lane; t < m; t += G) {      // scatter; afterwards hist[b] = end of bucket b
+    const u64 key = skey[t];
+    ssort[atomicAdd(&hist[(u32)(key >> shift)], 1u)] = key;
+  }
+  grp.sync();
+  for (int t = grp.lane; t < m; t += G) {
+    const u64 key = skey[t];
+    const u32 b = (u32)(key >> shift);
+    const int lo = b ? (int)hist[b - 1] : 0, hi = (int)hist[b];
+    int r = lo;
+    for (int j = lo; j < hi; ++j) r += (ssort[j] < key);
+    rank[s0 + t] = (u16)r;
+  }
+}
+
 // ids in sorted order (parity export)
 __global__ void k_export_order(const u32* __restrict__ id, const u16* __restrict__ rank, const u32* __restrict__ seg,
                                int ncell, u32* __restrict__ ids_sorted) {
@@ -275,10 +339,29 @@ static cudaError_t launch_rank_count_t(const u32* id, const u32* seg, int ncell,
   return cudaGetLastError();
 }
 
-// P = power of two >= the most populated cell.  Up to 128 SDs per cell the ranks come from counting,
-// beyond that from the bitonic network.
+// P = power of two >= the most populated cell.  Sparse cells (P < 64, or small groups) take their ranks from
+// counting all pairs, cells up to 8192 SDs from counting inside key buckets, beyond that from the bitonic network.
+template <int G>
+static cudaError_t launch_rank_bucket_t(const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
+                                        u16* rank, int* d_error, cudaStream_t st) {
+  constexpr int NG = CtaOf<G>::threads / G;
+  const size_t smem = (size_t)NG * ((size_t)P * 16 + (size_t)std::max(P >> 4, 4) * 4);
+  cudaError_t e = cudaFuncSetAttribute(k_rank_bucket<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_rank_bucket<G><<<(ncell + NG - 1) / NG, CtaOf<G>::threads, smem, st>>>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
                         u16* rank, int* d_error, cudaStream_t st) {
+  if (P >= 256 && P <= 8192) {   // crowded cells: buckets (a warp per cell up to 512 SDs, else a CTA)
+    if (P <= 512) return launch_rank_bucket_t<32>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    return launch_rank_bucket_t<256>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+  }
+  if (P >= 64 && P <= 128 && (G == 16 || G == 32)) {   // measured: buckets beat all-pairs counting from ~30 SDs per cell on
+    if (G == 16) return launch_rank_bucket_t<16>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+    return launch_rank_bucket_t<32>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);
+  }
   if (P <= 128 && G <= 32) {
     switch (G) {
       case 4: return launch_rank_count_t<4>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error, st);

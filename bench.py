@@ -29,7 +29,8 @@ UNIT = "SD-steps/s"
 #  - condensation kernel: fp64 operations per growth-rate evaluation and per SD-substep set-up, counted
 #    from the formulae (an FMA counts 2; a division, sqrt, rsqrt, exp, cbrt count as the length of their
 #    fp64 instruction sequences).
-BYTES_PER_SD_STEP = {3: 350.0, 2: 350.0 - 16.0 - 8.0}
+BYTES_PER_SD_STEP = {(3, 8): 350.0, (2, 8): 350.0 - 16.0 - 8.0,      # fp64 state: SURVEY.md 8d
+                     (3, 4): 232.0, (2, 4): 232.0 - 8.0 - 4.0}       # fp32 state: the six reals at 4 bytes
 FLOP_PER_EVAL = 190.0
 FLOP_PER_SETUP = 150.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
@@ -47,6 +48,7 @@ def parse():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the horizontal grid (debugging only; reported in config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--group", type=int, default=0)
+    ap.add_argument("--real-bytes", type=int, default=8, choices=[8, 4], help="storage type of the SD attributes (configs[4]: fp32 state)")
     return ap.parse_args()
 
 
@@ -195,8 +197,10 @@ def main():
     dev = f"cuda:{local}"
 
     w = make_workload(wa, seed=replicas.replica_seed(42, rank), device=dev)
-    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], **w.init)
+    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], real_bytes=a.real_bytes, **w.init)
     s = w.state
+    if a.real_bytes == 4:
+        s = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in s.items()}
     cs = list(w.courants) + [None] * (3 - len(w.courants))
     p.init_from_arrays(w.rhod, s["n"], s["rw2"], s["rd3"], s["kappa"], s["x"], s["y"], s["z"], s["id"], courant_1=cs[0],
                        courant_2=cs[1], courant_3=cs[2])
@@ -281,13 +285,13 @@ def main():
                 "evals_per_sd_substep": evals / max(subs, 1),
                 "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
                 "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms}
-    bytes_step = BYTES_PER_SD_STEP[ndim] * (sd_steps / a.steps)
+    bytes_step = BYTES_PER_SD_STEP[(ndim, a.real_bytes)] * (sd_steps / a.steps)
     hbm = {"bound": "hbm", "achieved": bytes_step / (step_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
            "frac": bytes_step / (step_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
-           "algorithmic_bytes_per_sd_step": BYTES_PER_SD_STEP[ndim]}
+           "algorithmic_bytes_per_sd_step": BYTES_PER_SD_STEP[(ndim, a.real_bytes)]}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
            "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-           "data": "synthetic", "config": config_of(wa), "clocks": clocks, "e2e": e2e,
+           "data": "synthetic", "config": dict(config_of(wa), state="fp64" if a.real_bytes == 8 else "fp32 storage, fp64 arithmetic"), "clocks": clocks, "e2e": e2e,
            "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm,
            "stage_ms": stage_ms, "n_sd_live": p.n_sd(), "n_sd_initial": n_sd0}
     if not a.no_cpu_baseline:

@@ -15,7 +15,9 @@
  *    host memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy
  *    default stream).  Work is enqueued on that stream; functions documented
  *    as "blocking" synchronise with it.
- *  - All floating-point arrays are IEEE double (real_bytes == 8).
+ *  - Eulerian fields (th, rv, rhod, Courant numbers, outbuf) are IEEE double.  The real attributes of the
+ *    super-droplets (rw2, rd3, kappa, x, y, z) are stored as double or float (real_bytes 8 or 4, the real_t of the
+ *    paper's templates); the arithmetic is fp64 either way, values are rounded when stored.
  *  - There is no CPU fallback: sdm_create fails with SDM_ERR_NO_DEVICE when no
  *    sm_100 device is usable (PAPER.md :827 "does report an error").
  */
@@ -70,7 +72,8 @@ typedef struct {
   const double* eff_q;      /* HOST, n_eff_q radius ratios small/large, ascending */
   const double* eff_tab;    /* HOST, row-major [n_eff_R][n_eff_q] */
   uint64_t seed;            /* Philox-4x32-10 key (low word, high word) */
-  int real_bytes;           /* 8 */
+  int real_bytes;           /* 8 or 4: storage type of rw2, rd3, kappa, x, y, z (and of the arrays of
+                               sdm_init_from_arrays / sdm_export_state) */
   int multi_coal;           /* 1: gamma = floor(p) + [u < frac(p)] (north_star); 0: gamma = [u < p] (PAPER.md :645) */
   uint64_t max_sd;          /* capacity in super-droplets (HBM is allocated once, at creation) */
   int n_modes;              /* dry_distros (:703-708): number of lognormal modes, 0..8 (0: sdm_init unavailable) */
@@ -133,11 +136,11 @@ int sdm_init_range(const sdm_ctx* ctx, int g, double* lnr_lo, double* lnr_hi);
  * component is the vertical one and the third is omitted, :751) are copied into library-owned dense
  * arrays.  n (multiplicity, uint64), rw2 (wet radius squared), rd3 (dry radius cubed), kappa, x, y,
  * z, id (unique uint32) are DEVICE arrays of N elements, copied; coordinates of absent dimensions
- * may be NULL.  Positions must lie inside the domain.  Blocking. */
+ * may be NULL; rw2 .. z are arrays of real_bytes-sized reals.  Positions must lie inside the domain.  Blocking. */
 int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo rhod_courant_1,
                          sdm_arrinfo rhod_courant_2, sdm_arrinfo rhod_courant_3, uint64_t N,
-                         const uint64_t* n, const double* rw2, const double* rd3, const double* kappa,
-                         const double* x, const double* y, const double* z, const uint32_t* id, void* stream);
+                         const uint64_t* n, const void* rw2, const void* rd3, const void* kappa,
+                         const void* x, const void* y, const void* z, const uint32_t* id, void* stream);
 
 /* step_sync() of Listing 5.5 (:768-775, :816): the part of a step that alters the Eulerian fields.
  * Removes N = 0 SDs, sorts the SDs by (cell, Philox key, id), and if opts->cond integrates
@@ -180,8 +183,8 @@ const double* sdm_outbuf(sdm_ctx* ctx);
  * until the next step_sync.  sdm_export_order: after step_sync, the ids in sorted (cell, key, id)
  * order and the nx*ny*nz+1 segment offsets (DEVICE arrays).  All enqueue on `stream`. */
 int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd);
-int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double* kappa,
-                     double* x, double* y, double* z, uint32_t* id, void* stream);
+int sdm_export_state(sdm_ctx* ctx, uint64_t* n, void* rw2, void* rd3, void* kappa,
+                     void* x, void* y, void* z, uint32_t* id, void* stream);
 int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, void* stream);
 /* Counters (blocking: synchronises the context's last stream). */
 int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out);

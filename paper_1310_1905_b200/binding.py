@@ -127,8 +127,8 @@ class Particles:
 
     def __init__(self, nx=0, ny=0, nz=0, dx=1.0, dy=1.0, dz=1.0, dt=1.0, kernel="geometric", golovin_b=1500.0,
                  multi_coal=True, seed=42, eff_R=None, eff_q=None, eff_tab=None, max_sd=None, sd_conc_mean=0.0, modes=None,
-                 x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None):
-        """modes: [(kappa, N_stp, r_mean, sigma_g), ...] of the dry spectrum, needed by init() only."""
+                 x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None, real_bytes=8):
+        """real_bytes: 8 or 4, the storage type of rw2, rd3, kappa, x, y, z (fields stay float64).  modes: [(kappa, N_stp, r_mean, sigma_g), ...] of the dry spectrum, needed by init() only."""
         import numpy as np
         self.L = load_library()
         keep = [None if a is None else np.ascontiguousarray(a, dtype=np.float64) for a in (eff_R, eff_q, eff_tab)]
@@ -145,7 +145,8 @@ class Particles:
         if keep[0] is not None:
             o.n_eff_R, o.n_eff_q = len(keep[0]), len(keep[1])
             o.eff_R, o.eff_q, o.eff_tab = (k.ctypes.data for k in keep)
-        o.seed, o.real_bytes, o.multi_coal, o.max_sd = seed, 8, int(multi_coal), int(max_sd)
+        o.seed, o.real_bytes, o.multi_coal, o.max_sd = seed, int(real_bytes), int(multi_coal), int(max_sd)
+        self.real = torch.float64 if int(real_bytes) == 8 else torch.float32
         self.h = C.c_void_p()
         rc = self.L.sdm_create(C.byref(o), C.byref(self.h))
         if rc != 0:
@@ -181,6 +182,9 @@ class Particles:
         N = n.numel()
         if id is None:
             id = torch.arange(N, dtype=torch.int32, device=n.device)
+        for name, t in (("rw2", rw2), ("rd3", rd3), ("kappa", kappa), ("x", x), ("y", y), ("z", z)):
+            if t is not None and (t.dtype != self.real or not t.is_contiguous()):
+                raise SdmError(f"init_from_arrays: {name} must be a contiguous {self.real} tensor (real_bytes of this context)")
         self._ck(self.L.sdm_init_from_arrays(self.h, arrinfo(rhod), arrinfo(courant_1), arrinfo(courant_2), arrinfo(courant_3),
                                              N, _ptr(n), _ptr(rw2), _ptr(rd3), _ptr(kappa), _ptr(x), _ptr(y), _ptr(z), _ptr(id),
                                              _stream()))
@@ -236,7 +240,7 @@ class Particles:
         dev = "cuda"
         out = dict(n=torch.empty(N, dtype=torch.int64, device=dev), id=torch.empty(N, dtype=torch.int32, device=dev))
         for k in ("rw2", "rd3", "kappa", "x", "y", "z"):
-            out[k] = torch.zeros(N, dtype=torch.float64, device=dev)
+            out[k] = torch.zeros(N, dtype=self.real, device=dev)
         self._ck(self.L.sdm_export_state(self.h, *[_ptr(out[k]) for k in ("n", "rw2", "rd3", "kappa", "x", "y", "z", "id")],
                                          _stream()))
         torch.cuda.current_stream().synchronize()

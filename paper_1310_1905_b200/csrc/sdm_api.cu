@@ -70,6 +70,9 @@ struct sdm_ctx {
 
 namespace {
 
+// the state arrays are stored in the double-typed struct; with real_bytes == 4 the same pointers are floats
+template <typename R> const SdArraysT<R>& view(const SdArrays& b) { return reinterpret_cast<const SdArraysT<R>&>(b); }
+
 int fail(sdm_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg; else g_create_error = msg;
   return code;
@@ -160,7 +163,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   sdm_ctx* ctx = nullptr;
   if (!o || !out) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: NULL argument");
   *out = nullptr;
-  if (o->real_bytes != 8) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: real_bytes must be 8 (fp64 state)");
+  if (o->real_bytes != 8 && o->real_bytes != 4) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: real_bytes must be 8 or 4");
   if (o->nx < 0 || o->ny < 0 || o->nz < 0 || !(o->dx > 0) || !(o->dy > 0) || !(o->dz > 0) || !(o->dt > 0))
     return fail(nullptr, SDM_ERR_INVALID, "sdm_create: grid sizes must be >= 0 and dx, dy, dz, dt > 0");
   if (o->kernel < 0 || o->kernel > 2) return fail(nullptr, SDM_ERR_INVALID, "sdm_create: unknown kernel");
@@ -201,8 +204,9 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   cudaError_t e;
   for (int b = 0; b < 2; ++b) {
     SdArrays& a = ctx->buf[b];
-    if ((e = dalloc(&a.n, N)) || (e = dalloc(&a.rw2, N)) || (e = dalloc(&a.rd3, N)) || (e = dalloc(&a.kappa, N)) ||
-        (e = dalloc(&a.x, g.hx ? N : 1)) || (e = dalloc(&a.y, g.hy ? N : 1)) || (e = dalloc(&a.z, g.hz ? N : 1)) ||
+    const size_t NR = o->real_bytes == 8 ? N : (N + 1) / 2;   // doubles that hold N reals
+    if ((e = dalloc(&a.n, N)) || (e = dalloc(&a.rw2, NR)) || (e = dalloc(&a.rd3, NR)) || (e = dalloc(&a.kappa, NR)) ||
+        (e = dalloc(&a.x, g.hx ? NR : 1)) || (e = dalloc(&a.y, g.hy ? NR : 1)) || (e = dalloc(&a.z, g.hz ? NR : 1)) ||
         (e = dalloc(&a.id, N)))
       return bail(e, "particle state");
   }
@@ -322,7 +326,8 @@ int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm
   if (int rc = copy_courants(ctx, comps, st)) return rc;
   ctx->cur = 0; ctx->cn = 0;
   // scratch per cell: RH to equilibrate with (outbuf) and the Kelvin length (eta, rewritten by every step_sync)
-  launch_init(ctx->buf[0], (u32)N, g, ip, make_field(ctx, th), make_field(ctx, rv), ctx->cf.rhod, ctx->outbuf, ctx->cf.eta, st);
+  if (ctx->o.real_bytes == 8) launch_init(view<double>(ctx->buf[0]), (u32)N, g, ip, make_field(ctx, th), make_field(ctx, rv), ctx->cf.rhod, ctx->outbuf, ctx->cf.eta, st);
+  else launch_init(view<float>(ctx->buf[0]), (u32)N, g, ip, make_field(ctx, th), make_field(ctx, rv), ctx->cf.rhod, ctx->outbuf, ctx->cf.eta, st);
   ctx->launches += 1 + (N ? 1 : 0);
   CK(cudaGetLastError());
   const u32 info[8] = {(u32)N, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
@@ -339,8 +344,8 @@ int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm
 }
 
 int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arrinfo c2, sdm_arrinfo c3, uint64_t N,
-                         const uint64_t* n, const double* rw2, const double* rd3, const double* kappa, const double* x,
-                         const double* y, const double* z, const uint32_t* id, void* stream) {
+                         const uint64_t* n, const void* rw2, const void* rd3, const void* kappa, const void* x,
+                         const void* y, const void* z, const uint32_t* id, void* stream) {
   if (!ctx) return SDM_ERR_INVALID;
   cudaStream_t st = (cudaStream_t)stream;
   const Grid& g = ctx->g;
@@ -356,12 +361,13 @@ int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arr
   SdArrays& a = ctx->buf[0];
   if (N) {
     CK(cudaMemcpyAsync(a.n, n, N * 8, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemcpyAsync(a.rw2, rw2, N * 8, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemcpyAsync(a.rd3, rd3, N * 8, cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemcpyAsync(a.kappa, kappa, N * 8, cudaMemcpyDeviceToDevice, st));
-    if (g.hx) CK(cudaMemcpyAsync(a.x, x, N * 8, cudaMemcpyDeviceToDevice, st));
-    if (g.hy) CK(cudaMemcpyAsync(a.y, y, N * 8, cudaMemcpyDeviceToDevice, st));
-    if (g.hz) CK(cudaMemcpyAsync(a.z, z, N * 8, cudaMemcpyDeviceToDevice, st));
+    const size_t rb = (size_t)ctx->o.real_bytes;
+    CK(cudaMemcpyAsync(a.rw2, rw2, N * rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.rd3, rd3, N * rb, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(a.kappa, kappa, N * rb, cudaMemcpyDeviceToDevice, st));
+    if (g.hx) CK(cudaMemcpyAsync(a.x, x, N * rb, cudaMemcpyDeviceToDevice, st));
+    if (g.hy) CK(cudaMemcpyAsync(a.y, y, N * rb, cudaMemcpyDeviceToDevice, st));
+    if (g.hz) CK(cudaMemcpyAsync(a.z, z, N * rb, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpyAsync(a.id, id, N * 4, cudaMemcpyDeviceToDevice, st));
   }
   const u32 info[8] = {(u32)N, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
@@ -397,7 +403,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   // condensation tiles: about kCondTileTarget SDs per CTA at the occupancy seen before this step
   ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, kCondTileTarget * g.ncell / std::max<double>(ctx->nslots, 1.0)));
   t_begin(ctx, SDM_STAGE_HIST, st);
-  launch_cellhist(ctx->buf[ctx->cur], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+  if (ctx->o.real_bytes == 8) launch_cellhist(view<double>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+  else launch_cellhist(view<float>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
   t_end(ctx, SDM_STAGE_HIST, st);
   t_begin(ctx, SDM_STAGE_SCAN, st);
   launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
@@ -408,7 +415,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 8 * sizeof(u32), cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(ctx->ev_info, st));
   t_begin(ctx, SDM_STAGE_SCATTER, st);
-  launch_scatter(ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
+  if (ctx->o.real_bytes == 8) launch_scatter(view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
+  else launch_scatter(view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
   t_end(ctx, SDM_STAGE_SCATTER, st);
   ctx->launches += ctx->nslots ? 1 : 0;
   CK(cudaGetLastError());
@@ -448,8 +456,12 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
     t_begin(ctx, SDM_STAGE_COND, st);
-    CK(launch_cond(cpb, variant, ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp,
-                   ctx->cnt, st));
+    if (ctx->o.real_bytes == 8)
+      CK(launch_cond(cpb, variant, view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
+                     rvf, ctx->cf, cp, ctx->cnt, st));
+    else
+      CK(launch_cond(cpb, variant, view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
+                     rvf, ctx->cf, cp, ctx->cnt, st));
     t_end(ctx, SDM_STAGE_COND, st);
   } else {
     launch_thermo(g, thf, rvf, ctx->cf, st);
@@ -479,15 +491,22 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     int tile_cpb = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
     for (int k = 0; k < 4 && !tile_cpb && sstp == 1 && !ctx->group_override; ++k) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
-      if (coal_tile_fits(cand, (int)ctx->tile_max[k])) tile_cpb = cand;
+      if (coal_tile_fits(cand, (int)ctx->tile_max[k], ctx->o.real_bytes)) tile_cpb = cand;
     }
     t_begin(ctx, SDM_STAGE_COAL_MOVE, st);
-    if (tile_cpb)
-      CK(launch_coal_move_tile(tile_cpb, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
-                               ctx->cnt, st));
+    const bool f64 = ctx->o.real_bytes == 8;
+    if (tile_cpb && f64)
+      CK(launch_coal_move_tile(tile_cpb, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                               ctx->flux_slots, ctx->cnt, st));
+    else if (tile_cpb)
+      CK(launch_coal_move_tile(tile_cpb, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                               ctx->flux_slots, ctx->cnt, st));
+    else if (f64)
+      CK(launch_coal_move(G, cap, in_smem, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                          ctx->flux_slots, ctx->cnt, st));
     else
-      CK(launch_coal_move(G, cap, in_smem, ctx->buf[ctx->cur], ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp, ctx->flux_slots,
-                          ctx->cnt, st));
+      CK(launch_coal_move(G, cap, in_smem, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                          ctx->flux_slots, ctx->cnt, st));
     t_end(ctx, SDM_STAGE_COAL_MOVE, st);
     ctx->launches++;
   }
@@ -533,8 +552,12 @@ int sdm_step_host(sdm_ctx* ctx, const sdm_opts* op, double* th_host, double* rv_
 static int diag_launch(sdm_ctx* ctx, int wet, double lo, double hi, int k, int count_only, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   ctx->last_stream = st;
-  launch_diag_mom(ctx->buf[ctx->cur], ctx->d_info + ctx->cn, (u32)ctx->nslots, ctx->g, wet, lo, hi, k, count_only, ctx->cf.rhod,
-                  ctx->outbuf, st);
+  if (ctx->o.real_bytes == 8)
+    launch_diag_mom(view<double>(ctx->buf[ctx->cur]), ctx->d_info + ctx->cn, (u32)ctx->nslots, ctx->g, wet, lo, hi, k, count_only,
+                    ctx->cf.rhod, ctx->outbuf, st);
+  else
+    launch_diag_mom(view<float>(ctx->buf[ctx->cur]), ctx->d_info + ctx->cn, (u32)ctx->nslots, ctx->g, wet, lo, hi, k, count_only,
+                    ctx->cf.rhod, ctx->outbuf, st);
   ctx->launches += (ctx->nslots ? 1 : 0) + (count_only ? 0 : 1);
   CK(cudaGetLastError());
   return SDM_OK;
@@ -560,7 +583,7 @@ int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd) {
   return SDM_OK;
 }
 
-int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double* kappa, double* x, double* y, double* z,
+int sdm_export_state(sdm_ctx* ctx, uint64_t* n, void* rw2, void* rd3, void* kappa, void* x, void* y, void* z,
                      uint32_t* id, void* stream) {
   if (!ctx) return SDM_ERR_INVALID;
   cudaStream_t st = (cudaStream_t)stream;
@@ -568,12 +591,13 @@ int sdm_export_state(sdm_ctx* ctx, uint64_t* n, double* rw2, double* rd3, double
   const size_t N = ctx->nslots;
   if (!N) return SDM_OK;
   if (n) CK(cudaMemcpyAsync(n, a.n, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (rw2) CK(cudaMemcpyAsync(rw2, a.rw2, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (rd3) CK(cudaMemcpyAsync(rd3, a.rd3, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (kappa) CK(cudaMemcpyAsync(kappa, a.kappa, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (x && ctx->g.hx) CK(cudaMemcpyAsync(x, a.x, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (y && ctx->g.hy) CK(cudaMemcpyAsync(y, a.y, N * 8, cudaMemcpyDeviceToDevice, st));
-  if (z && ctx->g.hz) CK(cudaMemcpyAsync(z, a.z, N * 8, cudaMemcpyDeviceToDevice, st));
+  const size_t rb = (size_t)ctx->o.real_bytes;
+  if (rw2) CK(cudaMemcpyAsync(rw2, a.rw2, N * rb, cudaMemcpyDeviceToDevice, st));
+  if (rd3) CK(cudaMemcpyAsync(rd3, a.rd3, N * rb, cudaMemcpyDeviceToDevice, st));
+  if (kappa) CK(cudaMemcpyAsync(kappa, a.kappa, N * rb, cudaMemcpyDeviceToDevice, st));
+  if (x && ctx->g.hx) CK(cudaMemcpyAsync(x, a.x, N * rb, cudaMemcpyDeviceToDevice, st));
+  if (y && ctx->g.hy) CK(cudaMemcpyAsync(y, a.y, N * rb, cudaMemcpyDeviceToDevice, st));
+  if (z && ctx->g.hz) CK(cudaMemcpyAsync(z, a.z, N * rb, cudaMemcpyDeviceToDevice, st));
   if (id) CK(cudaMemcpyAsync(id, a.id, N * 4, cudaMemcpyDeviceToDevice, st));
   return SDM_OK;
 }

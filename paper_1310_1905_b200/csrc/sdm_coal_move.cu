@@ -8,6 +8,9 @@
 
 namespace sdm {
 
+template <bool SMEM, typename R> struct RealSel { typedef double type; };
+template <typename R> struct RealSel<false, R> { typedef R type; };
+
 // collision efficiency: bilinear in (collector radius, ratio), clamped at the table edges
 __device__ __forceinline__ double eff_lookup(const CoalParams& kp, double R, double q) {
   const int nR = kp.n_eff_R, nq = kp.n_eff_q;
@@ -31,8 +34,8 @@ __device__ __forceinline__ double wrap(double x, double X) {
 
 // Shared memory per group: cap x {n (u64), rw2, rd3, kappa (double), id (u32)} (SMEM) or cap x u16 slot
 // indices (attributes left in HBM/L2), and for sstp_coal > 1 another P x {u64 key, u16 order}.
-template <int G, bool SMEM>
-__global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArrays a, const u16* __restrict__ rank,
+template <int G, bool SMEM, typename R>
+__global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a, const u16* __restrict__ rank,
                                                                  const u32* __restrict__ seg, Grid g, CellFields cf,
                                                                  CoalParams kp, CoalMoveParams mp, double* flux_slots,
                                                                  Counters cnt, int cap, int P) {
@@ -51,7 +54,8 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArrays a, con
     // otherwise (cells too large for shared memory) only the slot of position e, attributes stay in HBM/L2.
     const size_t attr_bytes = SMEM ? (size_t)cap * 36 : (size_t)cap * 2;
     unsigned char* base = smem_raw + (size_t)gi * (attr_bytes + (size_t)P * 10);
-    u64* pn; double *prw2, *prd3, *pkap; u32* pid;
+    using PT = typename RealSel<SMEM, R>::type;   // staged copies are doubles; in place, the storage type
+    u64* pn; PT *prw2, *prd3, *pkap; u32* pid;
     u16* s_inv = reinterpret_cast<u16*>(base);
     if constexpr (SMEM) {
       pn = reinterpret_cast<u64*>(base);
@@ -238,9 +242,9 @@ struct __align__(8) CoalCell {
   int i, j, k, pad;
 };
 
-template <int CAP, int T>
-struct CoalTile {
-  static constexpr size_t fixed_bytes = (size_t)CAP * (6 * 8 + 4 + 2);
+template <int CAP, int T, typename R>
+struct CoalTile {   // u64 n; R rw2, x, y, z; double vt; u32 id; u16 inv
+  static constexpr size_t fixed_bytes = (size_t)CAP * (8 + 4 * sizeof(R) + 8 + 4 + 2);
   static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CoalCell) + (size_t)(cpb + 1) * 8 + 16; }
 };
 
@@ -251,23 +255,23 @@ __device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-template <int CAP, int T, int MINB>
+template <int CAP, int T, int MINB, typename R>
 __global__ void __launch_bounds__(T, MINB)
-k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, CellFields cf, CoalParams kp,
+k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, CellFields cf, CoalParams kp,
                  CoalMoveParams mp, double* flux_slots, Counters cnt, int cpb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  using L = CoalTile<CAP, T>;
+  using L = CoalTile<CAP, T, R>;
   constexpr u16 NONE = 0xFFFFu;
   const int tid = threadIdx.x;
   const int c_first = blockIdx.x * cpb;
   const int nc = min(cpb, g.ncell - c_first);
   u64* s_n = reinterpret_cast<u64*>(smem_raw);
-  double* s_rw2 = reinterpret_cast<double*>(smem_raw) + CAP;
-  double* s_x = s_rw2 + CAP;
-  double* s_y = s_x + CAP;
-  double* s_z = s_y + CAP;
-  double* s_vt = s_z + CAP;
-  u32* s_id = reinterpret_cast<u32*>(s_vt + CAP);
+  double* s_vt = reinterpret_cast<double*>(smem_raw) + CAP;
+  R* s_rw2 = reinterpret_cast<R*>(s_vt + CAP);
+  R* s_x = s_rw2 + CAP;
+  R* s_y = s_x + CAP;
+  R* s_z = s_y + CAP;
+  u32* s_id = reinterpret_cast<u32*>(s_z + CAP);
   u16* inv = reinterpret_cast<u16*>(s_id + CAP);
   CoalCell* s_cell = reinterpret_cast<CoalCell*>(smem_raw + L::fixed_bytes);
   u32* segl = reinterpret_cast<u32*>(s_cell + cpb);   // storage offsets of the tile's cells
@@ -284,12 +288,12 @@ k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict
     for (int t = tid; t < M; t += T) {
       const u32 s = s0 + t;
       cp_async<8>(s_n + t, a.n + s);
-      cp_async<8>(s_rw2 + t, a.rw2 + s);
+      cp_async<sizeof(R)>(s_rw2 + t, a.rw2 + s);
       if (mp.coal) cp_async<4>(s_id + t, a.id + s);
       if (moving) {
-        if (g.hx) cp_async<8>(s_x + t, a.x + s);
-        if (g.hy) cp_async<8>(s_y + t, a.y + s);
-        if (g.hz) cp_async<8>(s_z + t, a.z + s);
+        if (g.hx) cp_async<sizeof(R)>(s_x + t, a.x + s);
+        if (g.hy) cp_async<sizeof(R)>(s_y + t, a.y + s);
+        if (g.hz) cp_async<sizeof(R)>(s_z + t, a.z + s);
       }
     }
     for (int cl = tid; cl < nc; cl += T) {
@@ -354,7 +358,7 @@ k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict
         if (lone || !mp.coal) {
           if (need_vt) {
             s_vt[ia] = v_term(ra, C.eta, C.rho_a);
-            if (!lone) s_vt[ib] = v_term(sqrt(s_rw2[ib]), C.eta, C.rho_a);
+            if (!lone) s_vt[ib] = v_term(sqrt((double)s_rw2[ib]), C.eta, C.rho_a);
           }
           continue;
         }
@@ -411,8 +415,8 @@ k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict
           a.kappa[gk] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
         a.rd3[gk] = rd3k + rd3j;
         const double r = cbrt(rw3);
-        const double y2 = r * r;
-        s_rw2[k] = y2; a.rw2[gk] = y2;
+        const double y2 = (R)(r * r);   // what is stored is the radius from here on
+        s_rw2[k] = (R)y2; a.rw2[gk] = (R)y2;
         s_n[j] = nj - gam * nk; a.n[gj] = nj - gam * nk;
         if (need_vt) s_vt[k] = v_term(sqrt(y2), C.eta, C.rho_a);
       }
@@ -473,17 +477,17 @@ k_coal_move_tile(SdArrays a, const u16* __restrict__ rank, const u32* __restrict
 #define SDM_COAL_T 128
 #define SDM_COAL_MINB 5
 #endif
-using CoalSmall = CoalTile<SDM_COAL_CAP, SDM_COAL_T>;
 // can a tile of cpb cells whose most populated instance holds `need` SDs run in k_coal_move_tile?
-bool coal_tile_fits(int cpb, int need) {
-  return need + cpb <= SDM_COAL_CAP && cpb <= 4096 &&
-         CoalSmall::smem(cpb) <= (size_t)(228 * 1024 - SDM_COAL_MINB * 1024) / SDM_COAL_MINB;
+bool coal_tile_fits(int cpb, int need, int real_bytes) {
+  const size_t smem = real_bytes == 8 ? CoalTile<SDM_COAL_CAP, SDM_COAL_T, double>::smem(cpb) : CoalTile<SDM_COAL_CAP, SDM_COAL_T, float>::smem(cpb);
+  return need + cpb <= SDM_COAL_CAP && cpb <= 4096 && smem <= (size_t)(228 * 1024 - SDM_COAL_MINB * 1024) / SDM_COAL_MINB;
 }
-cudaError_t launch_coal_move_tile(int cpb, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+template <typename R>
+cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                   const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                                   const Counters& cnt, cudaStream_t st) {
-  const size_t smem = CoalSmall::smem(cpb);
-  auto kern = k_coal_move_tile<SDM_COAL_CAP, SDM_COAL_T, SDM_COAL_MINB>;
+  const size_t smem = CoalTile<SDM_COAL_CAP, SDM_COAL_T, R>::smem(cpb);
+  auto kern = k_coal_move_tile<SDM_COAL_CAP, SDM_COAL_T, SDM_COAL_MINB, R>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cpb);
@@ -509,8 +513,8 @@ size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem) {
   return (size_t)NG * ((size_t)cap * (in_smem ? 36 : 2) + (size_t)P * 10);
 }
 
-template <int G>
-static cudaError_t launch_coal_move_t(int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+template <int G, typename R>
+static cudaError_t launch_coal_move_t(int cap, bool in_smem, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                       const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp,
                                       double* flux_slots, const Counters& cnt, cudaStream_t st) {
   constexpr int NG = CtaOf<G>::threads / G;
@@ -518,18 +522,19 @@ static cudaError_t launch_coal_move_t(int cap, bool in_smem, const SdArrays& a, 
   const int P = mp.sstp_coal > 1 ? next_pow2(cap) : 0;
   const size_t smem = coal_smem_bytes(G, cap, mp.sstp_coal, in_smem);
   if (in_smem) {
-    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, true, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_coal_move<G, true><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
+    k_coal_move<G, true, R><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
   } else {
-    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, false, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_coal_move<G, false><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
+    k_coal_move<G, false, R><<<grid, CtaOf<G>::threads, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cap, P);
   }
   return cudaGetLastError();
 }
 
-cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+template <typename R>
+cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                              const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                              const Counters& cnt, cudaStream_t st) {
   switch (G) {
@@ -540,6 +545,15 @@ cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, co
     default: return launch_coal_move_t<256>(cap, in_smem, a, rank, seg, g, cf, kp, mp, flux_slots, cnt, st);
   }
 }
+
+#define SDM_INST(R)                                                                                                      \
+  template cudaError_t launch_coal_move<R>(int, int, bool, const SdArraysT<R>&, const u16*, const u32*, const Grid&,          \
+                                           const CellFields&, const CoalParams&, const CoalMoveParams&, double*, const Counters&, \
+                                           cudaStream_t);                                                               \
+  template cudaError_t launch_coal_move_tile<R>(int, const SdArraysT<R>&, const u16*, const u32*, const Grid&, const CellFields&, \
+                                                const CoalParams&, const CoalMoveParams&, double*, const Counters&, cudaStream_t);
+SDM_INSTANTIATE_REAL(SDM_INST)
+#undef SDM_INST
 
 void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st) {
   k_flux_sum<<<1, 256, 0, st>>>(const_cast<double*>(flux_slots), flux_out, flux_total);

@@ -32,12 +32,15 @@ struct Grid {
   double dx, dy, dz, dt, dV;
   double X, Y, Z;
 };
-struct SdArrays {        // SoA particle state in HBM (PAPER.md :510-520, Table 1 :162-169)
-  u64* n;                // multiplicity N
-  double *rw2, *rd3, *kappa;
-  double *x, *y, *z;
+template <typename R>
+struct SdArraysT {       // SoA particle state in HBM (PAPER.md :510-520, Table 1 :162-169); R = real_t of the
+  u64* n;                // paper's templates (double or float): the STORAGE type of the real attributes.  The
+  R *rw2, *rd3, *kappa;  // kernels load them into fp64, compute in fp64 and round on store; multiplicities are
+  R *x, *y, *z;          // 64-bit integers either way.
   u32* id;               // persistent unique id (keys every Philox draw)
 };
+using SdArrays = SdArraysT<double>;
+#define SDM_INSTANTIATE_REAL(MACRO) MACRO(double) MACRO(float)
 struct Field {           // arrinfo_t mapped on (i,j,k) (PAPER.md :730-745)
   double* p;
   long long s0, s1, s2;

@@ -439,14 +439,14 @@ __device__ __forceinline__ void cell_consts(double th, double rv, double rhod, d
 //   u32 segl[cpb + 2]                  tile-local segment offsets, list counter
 //   u16 cidx[cap], list[cap]           local cell of each slot; slots left for the second pass
 // GMEM variant (a cell too crowded for shared memory; cpb = 1): the state stays in HBM/L2 in storage
-// order, contributions go to alt.rw2 in sorted order, the list to alt.id.
+// order, contributions go to alt.n (8 bytes per SD, used as doubles) in sorted order, the list to alt.id.
 size_t cond_smem_bytes(int cpb, int cap) {
   return (size_t)(CELLK_N + 1) * cpb * 8 + (size_t)6 * cap * 8 + (size_t)(cpb + 2) * 4 + (size_t)cap * 4 + 16;
 }
 
-template <bool SMEM>
+template <bool SMEM, typename R>
 __global__ void __launch_bounds__(COND_THREADS, 2)
-k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+k_cond(SdArraysT<R> a, SdArraysT<R> alt, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
        CellFields cf, CondParams cp, Counters cnt, int cpb, int cap) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -465,7 +465,7 @@ k_cond(SdArrays a, SdArrays alt, const u16* __restrict__ rank, const u32* __rest
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
   u32* list32 = alt.id + s0;
-  if constexpr (!SMEM) s_con = alt.rw2 + s0;
+  if constexpr (!SMEM) s_con = reinterpret_cast<double*>(alt.n) + s0;
 
   // thread `tid` owns cell c_first + tid for the whole kernel: theta, r_v and the feedback live in its registers
   double th = 0, rv = 0, rhod = 1, c_exn = 0, fbk = 0, T = 0, lv = 0;
@@ -729,9 +729,9 @@ struct Cond4 {
   static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CellRec) + (size_t)(cpb + 1) * 4 + 16; }
 };
 
-template <int CAP, int T, int MINB>
+template <int CAP, int T, int MINB, typename R>
 __global__ void __launch_bounds__(T, MINB)
-k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
         CellFields cf, CondParams cp, Counters cnt, int cpb) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using L = Cond4<CAP, T>;
@@ -771,7 +771,7 @@ k_cond4(SdArrays a, const u16* __restrict__ rank, const u32* __restrict__ seg, G
     const int e = (int)segl[lo] + rank[s];
     const double rd3 = a.rd3[s];
     const double q = cbrt(rd3);
-    s_r[e] = sqrt(a.rw2[s]);
+    s_r[e] = sqrt((double)a.rw2[s]);
     s_rd3[e] = rd3;
     s_krd3[e] = a.kappa[s] * rd3;
     s_dn[e] = (double)a.n[s];
@@ -992,13 +992,13 @@ int cond_variant(int cpb, int need) {
   return 0;
 }
 
-template <int CAP, int T, int MINB>
-static cudaError_t launch_cond4(size_t smem, int grid, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g, Field th,
+template <int CAP, int T, int MINB, typename R>
+static cudaError_t launch_cond4(size_t smem, int grid, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g, Field th,
                                 Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, int cpb,
                                 cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_cond4<CAP, T, MINB><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  k_cond4<CAP, T, MINB, R><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
   return cudaGetLastError();
 }
 
@@ -1015,7 +1015,8 @@ __global__ void k_thermo(Grid g, Field th_f, Field rv_f, CellFields cf) {
 
 // variant as returned by cond_variant(cpb, need); 0: work in place in global memory (cpb must be 1),
 // `alt` = the idle ping-pong copy of the state used as scratch.
-cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+template <typename R>
+cudaError_t launch_cond(int cpb, int variant, const SdArraysT<R>& a, const SdArraysT<R>& alt, const u16* rank, const u32* seg,
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st) {
   const int grid = (g.ncell + cpb - 1) / cpb;
@@ -1023,9 +1024,15 @@ cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays&
     return launch_cond4<SDM_COND_CAP, 128, SDM_COND_MINB>(CondSmall::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
   if (variant == 2) return launch_cond4<1280, 256, 3>(CondMedium::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
   if (variant == 3) return launch_cond4<4096, 512, 1>(CondLarge::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
-  k_cond<false><<<grid, COND_THREADS, cond_smem_bytes(cpb, 0), st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);
+  k_cond<false, R><<<grid, COND_THREADS, cond_smem_bytes(cpb, 0), st>>>(a, alt, rank, seg, g, th, rv, cf, cp, cnt, cpb, 0);
   return cudaGetLastError();
 }
+
+#define SDM_INST(R)                                                                                                     \
+  template cudaError_t launch_cond<R>(int, int, const SdArraysT<R>&, const SdArraysT<R>&, const u16*, const u32*, const Grid&, \
+                                      Field, Field, const CellFields&, const CondParams&, const Counters&, cudaStream_t);
+SDM_INSTANTIATE_REAL(SDM_INST)
+#undef SDM_INST
 
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st) {
   k_thermo<<<(g.ncell + 127) / 128, 128, 0, st>>>(g, th, rv, cf);

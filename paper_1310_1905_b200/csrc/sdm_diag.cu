@@ -7,7 +7,8 @@ namespace sdm {
 // M^k[cell] += N r^k for r in [r_mi, r_mx); SDs are visited in storage order, which is cell-sorted
 // up to the last move, so lanes of a warp that hit the same cell are first summed in lane order and
 // issue one atomic per distinct cell.
-__global__ void __launch_bounds__(256) k_diag_mom(SdArrays a, const u32* __restrict__ d_nslots, Grid g, int wet,
+template <typename R>
+__global__ void __launch_bounds__(256) k_diag_mom(SdArraysT<R> a, const u32* __restrict__ d_nslots, Grid g, int wet,
                                                   double r_mi, double r_mx, int k, int count_only,
                                                   double* __restrict__ out) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -21,7 +22,7 @@ __global__ void __launch_bounds__(256) k_diag_mom(SdArrays a, const u32* __restr
         v = 1.0;
         c = cell_of(g, g.hx ? a.x[i] : 0.0, g.hy ? a.y[i] : 0.0, g.hz ? a.z[i] : 0.0);
       } else {
-        const double r = wet ? sqrt(a.rw2[i]) : cbrt(a.rd3[i]);
+        const double r = wet ? sqrt((double)a.rw2[i]) : cbrt((double)a.rd3[i]);
         if (r >= r_mi && r < r_mx) {
           v = (double)n * pow(r, (double)k);
           c = cell_of(g, g.hx ? a.x[i] : 0.0, g.hy ? a.y[i] : 0.0, g.hz ? a.z[i] : 0.0);
@@ -53,13 +54,20 @@ __global__ void k_dense_copy(Field src, double* __restrict__ dst, int n0, int n1
   dst[t] = src.at(i, j, k);
 }
 
-void launch_diag_mom(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
+template <typename R>
+void launch_diag_mom(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
                      double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st) {
   cudaMemsetAsync(out, 0, sizeof(double) * g.ncell, st);
   if (nslots_bound)
-    k_diag_mom<<<(nslots_bound + 255) / 256, 256, 0, st>>>(a, d_nslots, g, wet, r_mi, r_mx, k, count_only, out);
+    k_diag_mom<R><<<(nslots_bound + 255) / 256, 256, 0, st>>>(a, d_nslots, g, wet, r_mi, r_mx, k, count_only, out);
   if (!count_only) k_diag_norm<<<(g.ncell + 255) / 256, 256, 0, st>>>(out, rhod, g.ncell, g.dV);
 }
+
+#define SDM_INST(R)                                                                                             \
+  template void launch_diag_mom<R>(const SdArraysT<R>&, const u32*, u32, const Grid&, int, double, double, int, int, \
+                                   const double*, double*, cudaStream_t);
+SDM_INSTANTIATE_REAL(SDM_INST)
+#undef SDM_INST
 
 void launch_dense_copy(Field src, double* dst, int n0, int n1, int n2, cudaStream_t st) {
   const long long tot = (long long)n0 * n1 * n2;

@@ -46,18 +46,20 @@ __global__ void k_init_cells(Grid g, Field th_f, Field rv_f, const double* __res
   Akel[c] = 2.0 * cst::sigma_w / (cst::R_v * T * cst::rho_w);
 }
 
-__global__ void __launch_bounds__(256) k_init_sd(SdArrays a, u32 N, Grid g, InitParams ip, const double* __restrict__ rhod,
+template <typename R>
+__global__ void __launch_bounds__(256) k_init_sd(SdArraysT<R> a, u32 N, Grid g, InitParams ip, const double* __restrict__ rhod,
                                                  const double* __restrict__ RHeq, const double* __restrict__ Akel) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   const int sp = (int)(i % (u32)ip.n_spectra);
   double x = 0.0, y = 0.0, z = 0.0;
-  if (g.hx) { x = ip.x0 + init_uniform(i, TAG_INIT_X, ip.seed_lo, ip.seed_hi) * (ip.x1 - ip.x0); a.x[i] = x; }
-  if (g.hy) { y = ip.y0 + init_uniform(i, TAG_INIT_Y, ip.seed_lo, ip.seed_hi) * (ip.y1 - ip.y0); a.y[i] = y; }
-  if (g.hz) { z = ip.z0 + init_uniform(i, TAG_INIT_Z, ip.seed_lo, ip.seed_hi) * (ip.z1 - ip.z0); a.z[i] = z; }
+  // (the stored value, rounded to R, is the position: the cell below is the cell of what is stored)
+  if (g.hx) { x = (R)(ip.x0 + init_uniform(i, TAG_INIT_X, ip.seed_lo, ip.seed_hi) * (ip.x1 - ip.x0)); a.x[i] = (R)x; }
+  if (g.hy) { y = (R)(ip.y0 + init_uniform(i, TAG_INIT_Y, ip.seed_lo, ip.seed_hi) * (ip.y1 - ip.y0)); a.y[i] = (R)y; }
+  if (g.hz) { z = (R)(ip.z0 + init_uniform(i, TAG_INIT_Z, ip.seed_lo, ip.seed_hi) * (ip.z1 - ip.z0)); a.z[i] = (R)z; }
   const double lo = ip.lnr_lo[sp], hi = ip.lnr_hi[sp];
   const double lnr = lo + (hi - lo) * init_uniform(i, TAG_INIT_LNR, ip.seed_lo, ip.seed_hi);
-  const double rd3 = exp(3.0 * lnr);
+  const double rd3 = (R)exp(3.0 * lnr);
   const double kappa = ip.kappa[sp];
   const u32 c = cell_of(g, x, y, z);
   const double mult = spectrum_density(ip, sp, lnr) * (hi - lo) / ip.sd_conc_spectrum * g.dV * (rhod[c] / ip.rho_stp);
@@ -121,10 +123,17 @@ int init_prepare(const sdm_mode_view* modes, int n_modes, double sd_conc_mean, d
   return 0;
 }
 
-void launch_init(const SdArrays& a, u32 N, const Grid& g, const InitParams& ip, Field th, Field rv, const double* rhod,
+template <typename R>
+void launch_init(const SdArraysT<R>& a, u32 N, const Grid& g, const InitParams& ip, Field th, Field rv, const double* rhod,
                  double* RHeq, double* Akel, cudaStream_t st) {
   k_init_cells<<<(g.ncell + 127) / 128, 128, 0, st>>>(g, th, rv, rhod, RHeq, Akel);
-  if (N) k_init_sd<<<(N + 255) / 256, 256, 0, st>>>(a, N, g, ip, rhod, RHeq, Akel);
+  if (N) k_init_sd<R><<<(N + 255) / 256, 256, 0, st>>>(a, N, g, ip, rhod, RHeq, Akel);
 }
+
+#define SDM_INST(R)                                                                                              \
+  template void launch_init<R>(const SdArraysT<R>&, u32, const Grid&, const InitParams&, Field, Field, const double*, \
+                               double*, double*, cudaStream_t);
+SDM_INSTANTIATE_REAL(SDM_INST)
+#undef SDM_INST
 
 }  // namespace sdm

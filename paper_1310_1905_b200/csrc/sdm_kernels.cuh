@@ -27,12 +27,14 @@ struct CellFields {  // library-owned dense per-cell arrays
 };
 
 // sdm_sort.cu
-void launch_cellhist(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
+template <typename R>
+void launch_cellhist(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
                      u32* count, cudaStream_t st);
 int scan_num_blocks(int ncell);
 void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_next, u32* d_maxcount, cudaStream_t st);
 void launch_tile_max(const u32* seg, int ncell, int cpb0, u32* d_tilemax4, cudaStream_t st);
-void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
+template <typename R>
+void launch_scatter(const SdArraysT<R>& src, const SdArraysT<R>& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
                     const u32* cell, const u32* off, const u32* seg, cudaStream_t st);
 cudaError_t launch_rank(int G, const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
                         u16* rank, int* d_error, cudaStream_t st);
@@ -44,20 +46,23 @@ void launch_export_order(const u32* id, const u16* rank, const u32* seg, int nce
 // (cpb == 1, `alt` = idle ping-pong copy used as scratch)
 int cond_variant(int cpb, int need);
 int cond_tile_candidate(int cpb0, int k);   // k-th candidate tile size (cells) tried by k_tile_max, k = 0..3
-cudaError_t launch_cond(int cpb, int variant, const SdArrays& a, const SdArrays& alt, const u16* rank, const u32* seg,
+template <typename R>
+cudaError_t launch_cond(int cpb, int variant, const SdArraysT<R>& a, const SdArraysT<R>& alt, const u16* rank, const u32* seg,
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st);
 size_t cond_smem_bytes(int cpb, int cap);
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);
 
 // sdm_coal_move.cu
-cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+template <typename R>
+cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                              const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                              const Counters& cnt, cudaStream_t st);
 size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem);
 // tile-resident variant for sstp_coal == 1 (cpb cells per CTA, most populated tile `need` SDs)
-bool coal_tile_fits(int cpb, int need);
-cudaError_t launch_coal_move_tile(int cpb, const SdArrays& a, const u16* rank, const u32* seg, const Grid& g,
+bool coal_tile_fits(int cpb, int need, int real_bytes);
+template <typename R>
+cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                   const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                                   const Counters& cnt, cudaStream_t st);
 void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
@@ -75,11 +80,13 @@ struct InitParams {
   u32 seed_lo, seed_hi;
 };
 int init_prepare(const sdm_mode_view* modes, int n_modes, double sd_conc_mean, double dV, InitParams& ip);
-void launch_init(const SdArrays& a, u32 N, const Grid& g, const InitParams& ip, Field th, Field rv, const double* rhod,
+template <typename R>
+void launch_init(const SdArraysT<R>& a, u32 N, const Grid& g, const InitParams& ip, Field th, Field rv, const double* rhod,
                  double* RHeq, double* Akel, cudaStream_t st);
 
 // sdm_diag.cu
-void launch_diag_mom(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
+template <typename R>
+void launch_diag_mom(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, int wet, double r_mi,
                      double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st);
 void launch_dense_copy(Field src, double* dst, int n0, int n1, int n2, cudaStream_t st);
 

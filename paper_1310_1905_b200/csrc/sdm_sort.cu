@@ -9,7 +9,8 @@
 namespace sdm {
 
 // ---- a0/a1: cell index + histogram (warp-aggregated atomics) ----------------------------------------
-__global__ void __launch_bounds__(256) k_cellhist(SdArrays a, const u32* __restrict__ d_nslots, Grid g,
+template <typename R>
+__global__ void __launch_bounds__(256) k_cellhist(SdArraysT<R> a, const u32* __restrict__ d_nslots, Grid g,
                                                   u32* __restrict__ cell, u32* __restrict__ off,
                                                   u32* __restrict__ count) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -119,7 +120,8 @@ __global__ void __launch_bounds__(256) k_tile_max(const u32* __restrict__ seg, i
 }
 
 // ---- a3: scatter the SoA state into cell-sorted storage (drops dead SDs) ----------------------------
-__global__ void __launch_bounds__(256) k_scatter(SdArrays src, SdArrays dst, const u32* __restrict__ d_nslots, Grid g,
+template <typename R>
+__global__ void __launch_bounds__(256) k_scatter(SdArraysT<R> src, SdArraysT<R> dst, const u32* __restrict__ d_nslots, Grid g,
                                                  const u32* __restrict__ cell, const u32* __restrict__ off,
                                                  const u32* __restrict__ seg) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -293,10 +295,11 @@ __global__ void k_export_order(const u32* __restrict__ id, const u16* __restrict
 }
 
 // ---- host launchers ----------------------------------------------------------------------------------
-void launch_cellhist(const SdArrays& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
+template <typename R>
+void launch_cellhist(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
                      u32* count, cudaStream_t st) {
   if (nslots_bound == 0) return;
-  k_cellhist<<<(nslots_bound + 255) / 256, 256, 0, st>>>(a, d_nslots, g, cell, off, count);
+  k_cellhist<R><<<(nslots_bound + 255) / 256, 256, 0, st>>>(a, d_nslots, g, cell, off, count);
 }
 
 int scan_num_blocks(int ncell) { return (ncell + SCAN_TILE - 1) / SCAN_TILE; }
@@ -313,11 +316,19 @@ void launch_tile_max(const u32* seg, int ncell, int cpb0, u32* d_tilemax4, cudaS
   k_tile_max<<<nb, 256, 0, st>>>(seg, ncell, cpb0, d_tilemax4);
 }
 
-void launch_scatter(const SdArrays& src, const SdArrays& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
+template <typename R>
+void launch_scatter(const SdArraysT<R>& src, const SdArraysT<R>& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
                     const u32* cell, const u32* off, const u32* seg, cudaStream_t st) {
   if (nslots_bound == 0) return;
-  k_scatter<<<(nslots_bound + 255) / 256, 256, 0, st>>>(src, dst, d_nslots, g, cell, off, seg);
+  k_scatter<R><<<(nslots_bound + 255) / 256, 256, 0, st>>>(src, dst, d_nslots, g, cell, off, seg);
 }
+
+#define SDM_INST(R)                                                                                              \
+  template void launch_cellhist<R>(const SdArraysT<R>&, const u32*, u32, const Grid&, u32*, u32*, u32*, cudaStream_t); \
+  template void launch_scatter<R>(const SdArraysT<R>&, const SdArraysT<R>&, const u32*, u32, const Grid&, const u32*,  \
+                                  const u32*, const u32*, cudaStream_t);
+SDM_INSTANTIATE_REAL(SDM_INST)
+#undef SDM_INST
 
 template <int G>
 static cudaError_t launch_rank_t(const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,

@@ -474,3 +474,87 @@ def test_root_selection_scan_of_independent_sds():
     sp, so = p.stats(), o.counters()
     assert sp["ill_posed"] == so["ill_posed"] > 50
     assert sp["cond_slow"] > 0.05 * sp["sd_substeps"]       # the literal-bisection path was exercised
+
+
+# ------------------------------------------------------------------------------------ fp32 particle state
+def _fp32_case(w, steps=1, **opts):
+    """Single-step parity with real_bytes = 4 (north_star: 1e-4 on radii in fp32): the state is rounded to fp32
+    first, the oracle starts from exactly those values in fp64, and before every further step the oracle is
+    re-loaded with the device's (fp32) state, so that each step is compared on its own."""
+    b = binding()
+    st32 = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in w.state.items()}
+    w.state = {k: (v if v is None or k in ("n", "id") else v.to(torch.float64)) for k, v in st32.items()}
+    o = make_oracle(w, threads=4)
+    p = b.Particles(max_sd=w.n_sd, sd_conc_mean=w.meta["sd_per_cell"], real_bytes=4, **w.init)
+    cs = [c.cuda() for c in w.courants] + [None] * (3 - len(w.courants))
+    g = {k: (None if v is None else v.cuda()) for k, v in st32.items()}
+    p.init_from_arrays(w.rhod.cuda(), g["n"], g["rw2"], g["rd3"], g["kappa"], g["x"], g["y"], g["z"], g["id"],
+                       courant_1=cs[0], courant_2=cs[1], courant_3=cs[2])
+    th, rv = w.th.cuda().clone(), w.rv.cuda().clone()
+    kw = dict(w.opts)
+    kw.update(opts)
+    po, oo = b.make_opts(**kw), oracle.make_opts(**kw)
+    for s in range(steps):
+        fo = o.step(oo)
+        p.step_sync(po, th, rv)
+        p.step_async(po)
+        fp = p.step_async_result()
+        ex = p.export_state()
+        assert ex["rw2"].dtype == torch.float32 and ex["x"].dtype == torch.float32
+        gs, rs = sorted_by_id(ex), sorted_by_id(o.get_state())
+        np.testing.assert_array_equal(gs["id"].astype(np.uint32), rs["id"])
+        np.testing.assert_array_equal(gs["n"].astype(np.uint64), rs["n"])             # multiplicities: bit-exact
+        np.testing.assert_allclose(np.sqrt(gs["rw2"].astype(np.float64)), np.sqrt(rs["rw2"]), rtol=1e-4)
+        np.testing.assert_allclose(np.cbrt(gs["rd3"].astype(np.float64)), np.cbrt(rs["rd3"]), rtol=1e-4)
+        np.testing.assert_allclose(gs["kappa"], rs["kappa"], rtol=1e-4)
+        live = rs["n"] > 0
+        for k, present in zip("xyz", p.dims):
+            if present:   # fp32 positions: half an ulp of the domain size
+                np.testing.assert_allclose(gs[k][live], rs[k][live], rtol=1e-6, atol=1e-6 * 3000.0)
+        oth, orv = o.get_fields()
+        np.testing.assert_allclose(np_(th).ravel(), oth, rtol=1e-6)
+        np.testing.assert_allclose(np_(rv).ravel(), orv, rtol=1e-6)
+        np.testing.assert_allclose(fp, fo, rtol=3e-4, atol=1e-300)
+        assert p.stats()["collisions"] == o.counters()["collisions"]
+        # next step from the device's rounded state
+        o.set_state(gs["n"].astype(np.uint64), gs["rw2"].astype(np.float64), gs["rd3"].astype(np.float64),
+                    gs["kappa"].astype(np.float64), x=gs["x"].astype(np.float64), y=gs["y"].astype(np.float64),
+                    z=gs["z"].astype(np.float64), id=gs["id"].astype(np.uint32))
+        o.set_fields(th=np_(th).ravel(), rv=np_(rv).ravel())
+    return p, o
+
+
+def test_fp32_state_2d_and_3d():
+    p, o = _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=32, nx=10, nz=40, seed=31)), steps=3)
+    assert o.counters()["collisions"] > 0
+    _fp32_case(rain_mix(W.cfg4_3d(sd_per_cell=64, nx=4, ny=3, nz=32, seed=32)), steps=2)
+
+
+def test_fp32_state_fallback_kernels():
+    """fp32 storage through the per-cell kernels: coalescence substeps (k_coal_move<G>), ~1000 SDs per cell (medium
+    condensation tile, bucket ranks) and one crowded cell (in-place condensation and coalescence)."""
+    _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=40, nx=6, nz=8, seed=33), frac=0.5), steps=2, sstp_coal=3)
+    _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=1000, nx=2, nz=3, seed=34), frac=0.3), steps=1, sstp_cond=3)
+    w = rain_mix(W.cfg2_2d(sd_per_cell=1500, nx=2, nz=3, seed=35), frac=0.3)
+    w.state["x"] = w.state["x"] * 0.4
+    _fp32_case(w, steps=1, sstp_cond=2)
+
+
+def test_fp32_init_and_diagnostics():
+    b = binding()
+    w = W.cfg2_2d(sd_per_cell=32, nx=8, nz=30, seed=36)
+    p = b.Particles(max_sd=w.n_sd + 8, sd_conc_mean=32.0, modes=VOCALS, real_bytes=4, **w.init)
+    p64 = b.Particles(max_sd=w.n_sd + 8, sd_conc_mean=32.0, modes=VOCALS, **w.init)
+    cs = [c.cuda() for c in w.courants]
+    for q in (p, p64):
+        q.init(w.th.cuda(), w.rv.cuda(), w.rhod.cuda(), *cs)
+    a, r = sorted_by_id(p.export_state()), sorted_by_id(p64.export_state())
+    np.testing.assert_array_equal(a["n"], r["n"])
+    for k in ("rw2", "rd3", "x", "z"):
+        np.testing.assert_allclose(a[k], r[k], rtol=2e-7)
+    p.diag_wet_rng(0.0, 1.0)
+    p64.diag_wet_rng(0.0, 1.0)
+    np.testing.assert_allclose(np_(p.diag_wet_mom(3)), np_(p64.diag_wet_mom(3)), rtol=1e-5)
+    with pytest.raises(b.SdmError, match="float32"):
+        p.init_from_arrays(w.rhod.cuda(), w.state["n"].cuda(), w.state["rw2"].cuda(), w.state["rd3"].cuda(), w.state["kappa"].cuda(),
+                           w.state["x"].cuda(), None, w.state["z"].cuda())

@@ -828,6 +828,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       double lo = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
       double hi = y0 + fmax(two, 0.0);              // eq. 19
       double r = r0, dprev = 0.0;
+      double rq = r0, gq = 0.0, gpq = 1.0;   // previous iterate, g and dg/dr there (for the curvature estimate)
       int st;
       // guards: the range of exp_kelvin, and the bracket must hold at most one root
       const bool guard = !(t < 4.0) ||
@@ -838,6 +839,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
         const double gp = fma(-dtp, dfr, r0 + r0);
         const double rn = fma(dtp * f, rcp_nr<1>(gp), r0);
         const double yn = rn * rn;
+        gq = -dtp * f; gpq = gp;
         if (!(gp > 0.0 && yn >= lo && yn <= hi)) {   // a step that rounds to nothing stays on the end it started from
           st = 2;
         } else {
@@ -861,14 +863,31 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
           const double gv = y - y0 - dtp * f;
           const double gp = fma(-dtp, dfr, r + r);
           if (gv < 0.0) lo = y; else hi = y;
-          const double rn = fma(-gv, rcp_nr<1>(gp), r);
+          // Newton step dN = -g/g', corrected to third order with g'' at r from the cubic through the last two
+          // iterates (values and slopes): g''(r) = [6 (g_q - g)/s + 2 g'_q + 4 g']/s, s = r - r_q;
+          // step = dN (1 + c), c = -dN g''/(2 g').  One reciprocal, of g' s.
+          const double sq = r - rq;
+          const double inv = rcp_nr<1>(gp * sq);
+          const double dN = -gv * (inv * sq);
+          const double h = fma(6.0 * (gq - gv), inv * gp, fma(2.0, gpq, 4.0 * gp));
+          double cc = -0.5 * dN * (h * inv);
+          const bool third = fabs(cc) <= 0.1;
+          if (!third) cc = 0.0;
+          const double rn = fma(dN, cc, dN) + r;
           const double yn = rn * rn;
           if (!(gp > 0.0 && yn >= lo && yn <= hi && t < 4.0)) {
             st = 2;
           } else {
-            const double d = fabs(rn - r);
+            const double d = fabs(dN);
             const double tol = KC[KC_TOL] * rn, d2 = d * d;
-            const bool conv = (4.0 * d2 <= tol * rn) && (2.0 * d2 * d <= tol * (dprev * dprev));
+            // Newton alone leaves C d^2 (C from the last two steps, at least 1/r); with the correction what is left
+            // is d cm (16 (s/r)^2 + cm), cm = max(|c|, d/r): the error of the curvature estimate and the next order
+            bool conv = (4.0 * d2 <= tol * rn) && (2.0 * d2 * d <= tol * (dprev * dprev));
+            if (third) {
+              const double cmr = fmax(fabs(cc) * rn, d);
+              conv = conv || (d * cmr * fma(cmr, rn, 16.0 * (sq * sq)) <= 0.5 * tol * (yn * rn));
+            }
+            rq = r; gq = gv; gpq = gp;
             r = rn; dprev = d;
             if (conv || !(hi - lo > KC[KC_EPSW] * hi)) st = 1;
           }

@@ -473,7 +473,7 @@ def test_root_selection_scan_of_independent_sds():
     p, o, th, rv = run_both(w, 2, opts=dict(coal=False, adve=False, sedi=False))
     sp, so = p.stats(), o.counters()
     assert sp["ill_posed"] == so["ill_posed"] > 50
-    assert sp["cond_slow"] > 0.05 * sp["sd_substeps"]       # the literal-bisection path was exercised
+    assert sp["cond_slow"] > 0.02 * sp["sd_substeps"]       # the literal-bisection path was exercised
 
 
 # ------------------------------------------------------------------------------------ fp32 particle state

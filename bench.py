@@ -33,6 +33,7 @@ BYTES_PER_SD_STEP = {(3, 8): 350.0, (2, 8): 350.0 - 16.0 - 8.0,      # fp64 stat
                      (3, 4): 232.0, (2, 4): 232.0 - 8.0 - 4.0}       # fp32 state: the six reals at 4 bytes
 FLOP_PER_EVAL = 190.0
 FLOP_PER_SETUP = 150.0
+FLOP_PER_CORRECTION = 28.0   # third-order correction of every Newton step after the first (curvature from the last two iterates)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
 NCU_COND_DRAM_BYTES = 2.316079e9 + 0.551624e9       # k_cond4 on the default workload, one ncu --set full capture
 
@@ -274,7 +275,7 @@ def main():
     cond_ms, cond_n = stages["cond"]
     evals = st1["newton_iters"] - st0["newton_iters"]
     subs = st1["sd_substeps"] - st0["sd_substeps"]
-    flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP
+    flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP + max(evals - subs, 0) * FLOP_PER_CORRECTION
     ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
     stage_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in stages.items()}
     step_ms = ms / a.steps

@@ -812,12 +812,13 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       if (q0 >= M) break;
       const int e = q0 + lane;
       const bool valid = e < M;
-      const CellRec& R = s_cell[valid ? (int)cidx[e] : 0];
-      const double r0 = valid ? s_r[e] : 1e-6;
-      const double rd2 = valid ? s_rd2[e] : 1e-14;
+      const int ec = min(e, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
+      const CellRec& R = s_cell[(int)cidx[ec]];
+      const double r0 = s_r[ec];
+      const double rd2 = s_rd2[ec];
       SdK s;
-      s.rd3 = valid ? s_rd3[e] : 1e-21;
-      s.krd3 = valid ? s_krd3[e] : 1e-21;
+      s.rd3 = s_rd3[ec];
+      s.krd3 = s_krd3[ec];
       CellR c;
       c.RH = R.RH; c.A = R.A; c.lD = R.lD; c.lK = R.lK; c.qD = R.qD; c.qK = R.qK; c.lD171 = R.lD171; c.lK171 = R.lK171;
       sd_setup(r0, R.c0, R.heat, R.kE, R.Sc, R.Pr, s);

@@ -70,6 +70,11 @@ def lib():
         L.orc_set_state.argtypes = [C.c_void_p, C.c_long] + [C.c_void_p] * 8
         L.orc_set_fields.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.orc_set_step.argtypes = [C.c_void_p, C.c_uint32]
+        L.orc_set_recycle.argtypes = [C.c_void_p, C.c_int]
+        L.orc_recycled.argtypes = [C.c_void_p]
+        L.orc_recycled.restype = C.c_longlong
+        L.orc_stage_recycle.argtypes = [C.c_void_p]
+        L.orc_stage_recycle.restype = None
         L.orc_init.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_double] + [C.c_double] * 6 + [C.c_void_p]
         L.orc_init.restype = C.c_long
         L.orc_get_step.argtypes = [C.c_void_p]
@@ -164,6 +169,17 @@ class Oracle:
 
     def set_step(self, step):
         self.L.orc_set_step(self.h, step)
+
+    def set_recycle(self, on):
+        """PAPER.md :641, :651: recycle zero-multiplicity SDs at the beginning of each step (default: compaction only)."""
+        self.L.orc_set_recycle(self.h, int(bool(on)))
+
+    def stage_recycle(self):
+        self.L.orc_stage_recycle(self.h)
+
+    @property
+    def recycled(self):
+        return int(self.L.orc_recycled(self.h))
 
     @property
     def step_count(self):

@@ -6,7 +6,7 @@
 // code with the CUDA path (paper_1310_1905_b200/csrc).
 //
 // Step order (PAPER.md :620, :641, :816; reading R-order):
-//   compact N=0 -> cell index + shuffle key -> sort (cell,key,id)
+//   [recycle N=0 ->] compact N=0 -> cell index + shuffle key -> sort (cell,key,id)
 //   -> condensation x sstp_cond -> coalescence x sstp_coal -> advection+sedimentation
 //
 // Pins (tests/test_oracle_pins.py): Philox known answers; Golovin closed form;
@@ -72,6 +72,8 @@ struct Ctx {
   orc_counters_t cnt{};
   int nthreads = 1;
   bool sorted = false;
+  int recycle = 0;            // 1: PAPER.md :641 recycling of zero-multiplicity SDs before the compaction
+  long long recycled = 0;     // SDs recycled so far
 };
 
 static inline u32 shuffle_key(const Ctx& c, u32 id, u32 step, u32 sub) {
@@ -122,9 +124,44 @@ static void compact(Ctx& c) {
   c.x.resize(w); c.y.resize(w); c.z.resize(w); c.id.resize(w);
 }
 
+// PAPER.md :641 "Particles with zero multiplicity are 'recycled' at the begining of each timestep.  The recycling
+// procedure first looks for computational particles with highest multiplicites and then assignes their properties
+// to the recycled particles halving the multiplicity"; :651 the same for SDs that left the domain.
+// DESIGN.md reading R-recycle: with k SDs of zero multiplicity, the donors are the k SDs first in the order
+// (multiplicity descending, id ascending) among those with multiplicity >= 2 (one real particle cannot be halved;
+// fewer donors than k: the zero-multiplicity SDs of highest id stay dead and are compacted away); the i-th donor
+// serves the zero-multiplicity SD of i-th smallest id, which takes the donor's r_w^2, r_d^3, kappa and position,
+// keeps its own id (its random streams stay its own) and gets floor(N/2); the donor keeps N - floor(N/2).
+// The selection is made once, from the multiplicities before any halving.
+static void recycle(Ctx& c) {
+  const long N = (long)c.n.size();
+  std::vector<long> dead, donors;
+  for (long s = 0; s < N; ++s) {
+    if (c.n[s] == 0) dead.push_back(s);
+    else if (c.n[s] >= 2) donors.push_back(s);
+  }
+  if (dead.empty() || donors.empty()) return;
+  std::sort(dead.begin(), dead.end(), [&](long a, long b) { return c.id[a] < c.id[b]; });
+  std::sort(donors.begin(), donors.end(), [&](long a, long b) {
+    if (c.n[a] != c.n[b]) return c.n[a] > c.n[b];
+    return c.id[a] < c.id[b];
+  });
+  const long k = (long)std::min(dead.size(), donors.size());
+  for (long i = 0; i < k; ++i) {
+    const long d = dead[i], s = donors[i];
+    const u64 half = c.n[s] / 2;
+    c.rw2[d] = c.rw2[s]; c.rd3[d] = c.rd3[s]; c.kappa[d] = c.kappa[s];
+    c.x[d] = c.x[s]; c.y[d] = c.y[s]; c.z[d] = c.z[s];
+    c.n[d] = half;
+    c.n[s] -= half;
+  }
+  c.recycled += k;
+}
+
 // PAPER.md :624 "randomly grouped into non-overlapping pairs": the random grouping
 // is the order of the SDs of a cell under the total order (cell, key, id).
 static void sort_stage(Ctx& c) {
+  if (c.recycle) recycle(c);
   compact(c);
   compute_cells(c);
   const long N = (long)c.n.size();
@@ -488,6 +525,9 @@ long orc_init(void* h, int n_modes, const double* modes, double sd_conc_mean, do
   return N;
 }
 
+void orc_set_recycle(void* h, int on) { ((Ctx*)h)->recycle = on; }
+long long orc_recycled(void* h) { return ((Ctx*)h)->recycled; }
+void orc_stage_recycle(void* h) { recycle(*(Ctx*)h); }
 void orc_set_step(void* h, u32 step) { ((Ctx*)h)->step = step; }
 u32 orc_get_step(void* h) { return ((Ctx*)h)->step; }
 

@@ -268,6 +268,104 @@ def test_box_golovin_against_analytic_solution():
     assert np.argmax(hist[3600]) > np.argmax(hist[1200])
 
 
+# ----------------------------------------------------------------------------- recycling (PAPER.md :641, :651)
+def _recycle_case(n):
+    N = len(n)
+    rng = np.random.default_rng(3)
+    ids = rng.permutation(N).astype(np.uint32)   # storage order is not id order
+    o = oracle.Oracle(dx=100, dy=100, dz=100, kernel="golovin")
+    rw2 = rng.uniform(1e-12, 1e-10, N)
+    o.set_state(n, rw2, rw2**1.5 * 1e-3, rng.uniform(0.1, 1.0, N), rng.uniform(0, 100, N), rng.uniform(0, 100, N),
+                rng.uniform(0, 100, N), id=ids)
+    before = o.get_state()
+    o.stage_recycle()
+    return before, o.get_state(), o
+
+
+def test_recycling_takes_the_highest_multiplicities_and_halves_them():
+    """PAPER.md :641: 'first looks for computational particles with highest multiplicites and then assignes their
+    properties to the recycled particles halving the multiplicity'.  Checked as properties of the result, not by
+    re-sorting: what changed, who gave, who received, and that no SD that kept its multiplicity outranks a donor."""
+    rng = np.random.default_rng(11)
+    n = rng.integers(1, 50, 400).astype(np.uint64)   # many ties
+    n[rng.choice(400, 37, replace=False)] = 0
+    b, a, o = _recycle_case(n)
+    dead = b["n"] == 0
+    assert o.recycled == 37 and (a["n"] > 0).all()
+    assert int(a["n"].sum()) == int(b["n"].sum())                                   # real particles conserved exactly
+    for k in ("rw2", "rd3"):                                                        # extensive totals conserved
+        np.testing.assert_allclose((a["n"] * a[k] ** (1.5 if k == "rw2" else 1)).sum(),
+                                   (b["n"] * b[k] ** (1.5 if k == "rw2" else 1)).sum(), rtol=1e-14)
+    np.testing.assert_array_equal(a["id"], b["id"])                                 # ids are persistent
+    donors = np.flatnonzero(~dead & (a["n"] != b["n"]))
+    assert len(donors) == 37
+    # every donor kept the larger half, and exactly one recycled SD holds the other half with the donor's attributes
+    taken = set()
+    for s in donors:
+        half = int(b["n"][s]) // 2
+        assert int(a["n"][s]) == int(b["n"][s]) - half
+        m = np.flatnonzero(dead & (a["n"] == half) & (a["rw2"] == b["rw2"][s]) & (a["x"] == b["x"][s]) & (a["kappa"] == b["kappa"][s])
+                           & (a["rd3"] == b["rd3"][s]) & (a["y"] == b["y"][s]) & (a["z"] == b["z"][s]))
+        assert len(m) == 1 and m[0] not in taken
+        taken.add(int(m[0]))
+    # the donors are the top of the order (multiplicity descending, id ascending): nobody left out outranks one
+    rest = np.flatnonzero(~dead & (a["n"] == b["n"]))
+    worst = min((int(b["n"][s]), -int(b["id"][s])) for s in donors)
+    assert all((int(b["n"][s]), -int(b["id"][s])) < worst for s in rest)
+    # donors in rank order serve the dead SDs in id order
+    rank = sorted(donors, key=lambda s: (-int(b["n"][s]), int(b["id"][s])))
+    dead_by_id = sorted(np.flatnonzero(dead), key=lambda s: int(b["id"][s]))
+    for s, d in zip(rank, dead_by_id):
+        assert a["rw2"][d] == b["rw2"][s] and int(a["n"][d]) == int(b["n"][s]) // 2
+
+
+def test_recycling_without_enough_donors_and_without_dead():
+    n = np.array([1, 0, 1, 0, 3, 0, 1, 2], np.uint64)       # two SDs can be halved, three are dead
+    b, a, o = _recycle_case(n)
+    assert o.recycled == 2 and int(a["n"].sum()) == int(b["n"].sum())
+    dead_ids = sorted(int(i) for i in b["id"][b["n"] == 0])
+    still_dead = [int(i) for i in a["id"][a["n"] == 0]]
+    assert still_dead == [dead_ids[-1]]                      # the dead SD of highest id is not served
+    assert sorted(a["n"].tolist()) == [0, 1, 1, 1, 1, 1, 1, 2]
+    n = np.array([4, 7, 1], np.uint64)
+    b, a, o = _recycle_case(n)
+    assert o.recycled == 0 and all((a[k] == b[k]).all() for k in a)
+
+
+def test_box_golovin_with_recycling_keeps_the_sample_and_the_late_spectrum():
+    """configs[0] with the paper's recycling instead of compaction: the SD count stays at 2^13, so the zeroth moment
+    still follows the Golovin solution at 3600 s (compaction alone is left with ~40 SDs there) and the second
+    moment, carried by the few largest drops, is not lost."""
+    N, n0, V, b = 2**13, 2.0**23, 1e6, 1500.0
+    v0 = 4 / 3 * np.pi * 30.531e-6**3
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True)
+    times = (1200, 2400, 3600)
+    M0 = {t: [] for t in times}
+    M2 = {t: [] for t in times}
+    for seed in range(42, 46):
+        v = np.random.default_rng(seed).exponential(v0, N)
+        o = oracle.Oracle(dx=100, dy=100, dz=100, dt=1.0, kernel="golovin", golovin_b=b, seed=seed)
+        o.set_recycle(True)
+        n = np.full(N, int(n0 * V / N), np.uint64)
+        o.set_state(n, (v / (4 / 3 * np.pi)) ** (2 / 3), np.full(N, 1e-27), np.full(N, 0.5))
+        m_ini = (n * v).sum()
+        for t in range(1, 3601):
+            o.step(op)
+            if t in times:
+                st = o.get_state()
+                assert (st["n"] > 0).sum() >= 0.995 * N
+                vv = 4 / 3 * np.pi * st["rw2"] ** 1.5
+                nn = st["n"].astype(float)
+                np.testing.assert_allclose((nn * vv).sum(), m_ini, rtol=1e-12)
+                M0[t].append(nn.sum() / V)
+                M2[t].append((nn * vv * vv).sum() / V)
+    for t, tol in zip(times, (0.05, 0.08, 0.12)):
+        T = b * n0 * v0 * t
+        assert abs(np.mean(M0[t]) / (n0 * np.exp(-T)) - 1) < tol, (t, np.mean(M0[t]) / (n0 * np.exp(-T)))
+    T = b * n0 * v0 * 2400
+    assert 0.6 < np.mean(M2[2400]) / (2 * n0 * v0**2 * np.exp(2 * T)) < 1.4
+
+
 # ----------------------------------------------------------------------------- thermodynamics
 def test_T_p_inversion_of_eq41():
     """:1016-1018 eq. 41 theta = T (p_1000/p_d)^(R_d/c_pd), p_d = rho_d R_d T  <=>  eq. 43 (:1044)."""

@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the horizontal grid (debugging only; reported in config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--group", type=int, default=0)
+    ap.add_argument("--recycle", action="store_true", help="the paper's recycling of zero-multiplicity SDs (:641) instead of compaction only")
     ap.add_argument("--real-bytes", type=int, default=8, choices=[8, 4], help="storage type of the SD attributes (configs[4]: fp32 state)")
     return ap.parse_args()
 
@@ -212,6 +213,8 @@ def main():
     torch.cuda.empty_cache()
     if a.group:
         p.set_group_size(a.group)
+    if a.recycle:
+        p.set_recycle(True)
     po = binding.make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=1.05, sstp_cond=10, sstp_coal=1)
 
     def barrier():
@@ -295,6 +298,9 @@ def main():
            "data": "synthetic", "config": dict(config_of(wa), state="fp64" if a.real_bytes == 8 else "fp32 storage, fp64 arithmetic"), "clocks": clocks, "e2e": e2e,
            "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm,
            "stage_ms": stage_ms, "n_sd_live": p.n_sd(), "n_sd_initial": n_sd0}
+    if a.recycle:
+        out["config"]["recycling"] = "on (PAPER.md :641)"
+        out["recycled"] = st1["recycled"] - st0["recycled"]
     if not a.no_cpu_baseline:
         v, cores, desc, _ = oracle_rate(wa, 2, 1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}

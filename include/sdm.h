@@ -106,6 +106,7 @@ typedef struct {
   uint64_t newton_iters;    /* condensation: growth-rate evaluations (summed) */
   uint64_t sd_substeps;     /* condensation: SD-substeps solved */
   uint64_t cond_slow;       /* condensation: SD-substeps deferred to the second (compacted) solver pass */
+  uint64_t recycled;        /* zero-multiplicity SDs recycled (sdm_set_recycle) */
 } sdm_stats_t;
 
 /* factory() of Listing 5.7 (:800-808).  Allocates all device memory for max_sd super-droplets on
@@ -199,10 +200,21 @@ typedef enum {
   SDM_STAGE_RANK = 3,      /* a2: (Philox key, id) order inside each cell */
   SDM_STAGE_COND = 4,      /* a4: condensation substeps */
   SDM_STAGE_COAL_MOVE = 5, /* a5-a6: coalescence + advection + sedimentation */
-  SDM_N_STAGES = 6
+  SDM_STAGE_RECYCLE = 6,   /* recycling of zero-multiplicity SDs (only with sdm_set_recycle) */
+  SDM_N_STAGES = 7
 } sdm_stage;
 int sdm_set_timing(sdm_ctx* ctx, int enable);
 int sdm_stage_times(sdm_ctx* ctx, double* ms, uint64_t* launches, int reset);
+/* PAPER.md :641, :651: "Particles with zero multiplicity are 'recycled' at the begining of each timestep.  The
+ * recycling procedure first looks for computational particles with highest multiplicites and then assignes their
+ * properties to the recycled particles halving the multiplicity."  on = 0 (default): zero-multiplicity SDs are
+ * removed by the compaction of step_sync (BASELINE.json north_star).  on = 1: at the beginning of step_sync, with k
+ * zero-multiplicity SDs in storage, the first k SDs in the order (multiplicity descending, id ascending) among those
+ * with multiplicity >= 2 give: the i-th of them to the zero-multiplicity SD of i-th smallest id, which takes its
+ * r_w^2, r_d^3, kappa and position, keeps its own id and gets floor(N/2), the donor keeping N - floor(N/2); with fewer
+ * donors than k the rest is compacted away.  The first call with on = 1 allocates 32 bytes of scratch per SD of
+ * capacity (SDM_ERR_CUDA if that fails).  Adds one host synchronisation to step_sync. */
+int sdm_set_recycle(sdm_ctx* ctx, int on);
 /* Overrides the step counter used in the Philox counters (restart from a checkpoint, parity). */
 int sdm_set_step(sdm_ctx* ctx, uint64_t step);
 /* Tuning override for tests: threads cooperating on one cell in the cell-resident kernels

@@ -43,15 +43,15 @@ class ArrInfo(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("n_sd", "max_cell_count", "step", "kernel_launches", "pairs", "collisions",
-                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow")]
+                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow", "recycled")]
 
 
 EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_range", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
-           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times"]
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle"]
 
-STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move")
+STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
 _lib = None
 
@@ -92,6 +92,7 @@ def load_library():
     L.sdm_set_group_size.argtypes = [vp, C.c_int]
     L.sdm_set_cond_kfast.argtypes = [vp, C.c_int]
     L.sdm_set_timing.argtypes = [vp, C.c_int]
+    L.sdm_set_recycle.argtypes = [vp, C.c_int]
     L.sdm_stage_times.argtypes = [vp, C.POINTER(C.c_double), u64p, C.c_int]
     _lib = L
     return L
@@ -267,6 +268,10 @@ class Particles:
 
     def set_cond_kfast(self, kfast):
         self._ck(self.L.sdm_set_cond_kfast(self.h, kfast))
+
+    def set_recycle(self, on=True):
+        """PAPER.md :641, :651: recycle zero-multiplicity SDs at the beginning of each step instead of only compacting."""
+        self._ck(self.L.sdm_set_recycle(self.h, int(bool(on))))
 
     def set_timing(self, enable=True):
         self._ck(self.L.sdm_set_timing(self.h, int(enable)))

@@ -18,6 +18,7 @@ UNITS = {
     "sdm_coal_move.cu": ["-fmad=false"],
     "sdm_diag.cu": ["-fmad=false"],
     "sdm_init.cu": ["-fmad=false"],
+    "sdm_recycle.cu": [],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 

@@ -62,8 +62,13 @@ struct sdm_ctx {
   // optional per-stage timing with CUDA events on the launching stream (sdm_set_timing)
   bool timing = false;
   std::vector<cudaEvent_t> tev[SDM_N_STAGES];   // start/stop pairs not yet folded into t_ms
-  double t_ms[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0};
-  uint64_t t_cnt[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0};
+  double t_ms[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0, 0};
+  uint64_t t_cnt[SDM_N_STAGES] = {0, 0, 0, 0, 0, 0, 0};
+  // recycling (sdm_set_recycle): two item lists, histogram + info words on the device, pinned info mirror
+  bool recycle = false;
+  RecItem *rec_dead = nullptr, *rec_cand = nullptr;
+  u32 *rec_hist = nullptr, *rec_info = nullptr, *h_rec = nullptr;
+  u64 recycled = 0;
   std::vector<cudaEvent_t> ev_pool;
   std::string err;
 };
@@ -291,6 +296,8 @@ void sdm_destroy(sdm_ctx* ctx) {
   cudaFree(ctx->flux_slots); cudaFree(ctx->d_flux); cudaFree(ctx->cnt_mem);
   cudaFree(ctx->d_effR); cudaFree(ctx->d_effq); cudaFree(ctx->d_efftab);
   if (ctx->h_info) cudaFreeHost(ctx->h_info);
+  if (ctx->h_rec) cudaFreeHost(ctx->h_rec);
+  cudaFree(ctx->rec_dead); cudaFree(ctx->rec_cand); cudaFree(ctx->rec_hist); cudaFree(ctx->rec_info);
   if (ctx->ev_info) cudaEventDestroy(ctx->ev_info);
   if (ctx->ev_async) cudaEventDestroy(ctx->ev_async);
   for (int q = 0; q < SDM_N_STAGES; ++q) for (cudaEvent_t e : ctx->tev[q]) cudaEventDestroy(e);
@@ -394,6 +401,26 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   if (rhod.data_zero) { launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st); ctx->launches++; }
   const sdm_arrinfo comps[3] = {c1, c2, c3};
   if (int rc = copy_courants(ctx, comps, st)) return rc;
+
+  // recycling of zero-multiplicity SDs, before they are compacted away (PAPER.md :641 "at the begining of each timestep")
+  if (ctx->recycle && ctx->nslots) {
+    t_begin(ctx, SDM_STAGE_RECYCLE, st);
+    const SdArrays& b = ctx->buf[ctx->cur];
+    launch_recycle_scan(b.n, b.id, (u32)ctx->nslots, ctx->rec_dead, ctx->rec_info, ctx->rec_hist, st);
+    ctx->launches += 2;
+    CK(cudaMemcpyAsync(ctx->h_rec, ctx->rec_info, 4 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const u32 n_dead = ctx->h_rec[0], k = ctx->h_rec[1];
+    if (k) {
+      if (ctx->o.real_bytes == 8)
+        ctx->launches += launch_recycle_apply(view<double>(b), g, (u32)ctx->nslots, n_dead, k, ctx->rec_dead, ctx->rec_cand, ctx->rec_info, ctx->h_rec + 4, st);
+      else
+        ctx->launches += launch_recycle_apply(view<float>(b), g, (u32)ctx->nslots, n_dead, k, ctx->rec_dead, ctx->rec_cand, ctx->rec_info, ctx->h_rec + 4, st);
+      ctx->recycled += k;
+    }
+    CK(cudaGetLastError());
+    t_end(ctx, SDM_STAGE_RECYCLE, st);
+  }
 
   // a0-a3: compaction + cell index + counting sort by cell
   u32* d_cur = ctx->d_info + ctx->cn;
@@ -622,6 +649,7 @@ int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out) {
   out->n_sd = ctx->nslots; out->max_cell_count = ctx->max_nc; out->step = ctx->step; out->kernel_launches = ctx->launches;
   out->pairs = s[0]; out->collisions = s[1]; out->near_ties = s[2]; out->ill_posed = s[3]; out->newton_iters = s[4];
   out->sd_substeps = s[5]; out->cond_slow = s[6];
+  out->recycled = ctx->recycled;
   return SDM_OK;
 }
 
@@ -647,6 +675,20 @@ int sdm_stage_times(sdm_ctx* ctx, double* ms, uint64_t* launches, int reset) {
     if (launches) launches[q] = ctx->t_cnt[q];
     if (reset) { ctx->t_ms[q] = 0; ctx->t_cnt[q] = 0; }
   }
+  return SDM_OK;
+}
+
+int sdm_set_recycle(sdm_ctx* ctx, int on) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (on && !ctx->rec_dead) {
+    const size_t cap = recycle_items_capacity(ctx->cap_sd);
+    CK(dalloc(&ctx->rec_dead, cap));
+    CK(dalloc(&ctx->rec_cand, cap));
+    CK(dalloc(&ctx->rec_hist, 2048));
+    CK(dalloc(&ctx->rec_info, 8));
+    CK(cudaMallocHost((void**)&ctx->h_rec, 8 * sizeof(u32)));
+  }
+  ctx->recycle = on != 0;
   return SDM_OK;
 }
 

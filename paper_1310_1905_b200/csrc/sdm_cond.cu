@@ -107,11 +107,17 @@ __device__ __forceinline__ double exp_kelvin(double t) {
   const double fn = z - KC[KC_MAGIC];
   double s = fma(-fn, KC[KC_LN2_HI], t);
   s = fma(-fn, KC[KC_LN2_LO], s);
-  double p = KC[KC_E13];
-  p = fma(p, s, KC[KC_E12]); p = fma(p, s, KC[KC_E11]); p = fma(p, s, KC[KC_E10]); p = fma(p, s, KC[KC_E9]);
-  p = fma(p, s, KC[KC_E8]); p = fma(p, s, KC[KC_E7]); p = fma(p, s, KC[KC_E6]); p = fma(p, s, KC[KC_E5]);
-  p = fma(p, s, KC[KC_E4]); p = fma(p, s, KC[KC_E3]); p = fma(p, s, KC[KC_E2]);
-  p = fma(p, s, 1.0); p = fma(p, s, 1.0);
+  // even and odd part as two Horner chains in s^2 (same 14 operations as one chain of 13, half the depth:
+  // a dependent DFMA issues every ~9 cycles on sm_100; measured)
+  const double s2 = s * s;
+  double pe = KC[KC_E12], po = KC[KC_E13];
+  pe = fma(pe, s2, KC[KC_E10]); po = fma(po, s2, KC[KC_E11]);
+  pe = fma(pe, s2, KC[KC_E8]); po = fma(po, s2, KC[KC_E9]);
+  pe = fma(pe, s2, KC[KC_E6]); po = fma(po, s2, KC[KC_E7]);
+  pe = fma(pe, s2, KC[KC_E4]); po = fma(po, s2, KC[KC_E5]);
+  pe = fma(pe, s2, KC[KC_E2]); po = fma(po, s2, KC[KC_E3]);
+  pe = fma(pe, s2, 1.0); po = fma(po, s2, 1.0);
+  const double p = fma(po, s, pe);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 

@@ -67,6 +67,18 @@ cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* ran
                                   const Counters& cnt, cudaStream_t st);
 void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
 
+// sdm_recycle.cu: recycling of zero-multiplicity SDs (PAPER.md :641, :651; reading R-recycle)
+struct __align__(16) RecItem { u64 key; u32 id; u32 slot; };   // ordered by (key, id); key = ~N for donors, 0 for dead SDs
+size_t recycle_items_capacity(u64 cap_sd);   // items each of the two lists must hold
+// counts the dead SDs (list `dead`, unordered), builds the histogram of multiplicities and picks the threshold bin;
+// info (8 u32, device): [0] dead SDs, [1] k = SDs that will be recycled, [2] candidates, [3] threshold bin
+void launch_recycle_scan(const u64* n, const u32* id, u32 nslots, RecItem* dead, u32* info, u32* hist, cudaStream_t st);
+// collects and orders the donors, orders the dead SDs by id and applies the recycling; synchronises the stream once
+// (h_ncand: pinned host word); returns the number of kernels launched
+template <typename R>
+int launch_recycle_apply(const SdArraysT<R>& a, const Grid& g, u32 nslots, u32 n_dead, u32 k, RecItem* dead, RecItem* cand,
+                         u32* info, u32* h_ncand, cudaStream_t st);
+
 // sdm_init.cu
 constexpr int INIT_MAX_MODES = 8;
 struct sdm_mode_view { double kappa, n_stp, r_mean, sigma_g; };   // same layout as sdm_lognormal_mode (sdm.h)

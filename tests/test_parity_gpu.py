@@ -62,12 +62,15 @@ def compare_fields(th, rv, o, rtol=RTOL):
     np.testing.assert_allclose(np_(rv).ravel(), orv, rtol=rtol)
 
 
-def run_both(w, steps, group=0, opts=None, check_every=1, **override):
+def run_both(w, steps, group=0, opts=None, check_every=1, recycle=False, **override):
     b = binding()
     kw = dict(w.opts)
     kw.update(opts or {})
     o = make_oracle(w, threads=4, **override)
     p, th, rv = make_particles(w, **override)
+    if recycle:
+        o.set_recycle(True)
+        p.set_recycle(True)
     if group:
         p.set_group_size(group)
     oo, po = oracle.make_opts(**kw), b.make_opts(**kw)
@@ -477,7 +480,7 @@ def test_root_selection_scan_of_independent_sds():
 
 
 # ------------------------------------------------------------------------------------ fp32 particle state
-def _fp32_case(w, steps=1, **opts):
+def _fp32_case(w, steps=1, recycle=False, **opts):
     """Single-step parity with real_bytes = 4 (north_star: 1e-4 on radii in fp32): the state is rounded to fp32
     first, the oracle starts from exactly those values in fp64, and before every further step the oracle is
     re-loaded with the device's (fp32) state, so that each step is compared on its own."""
@@ -491,6 +494,9 @@ def _fp32_case(w, steps=1, **opts):
     p.init_from_arrays(w.rhod.cuda(), g["n"], g["rw2"], g["rd3"], g["kappa"], g["x"], g["y"], g["z"], g["id"],
                        courant_1=cs[0], courant_2=cs[1], courant_3=cs[2])
     th, rv = w.th.cuda().clone(), w.rv.cuda().clone()
+    if recycle:
+        o.set_recycle(True)
+        p.set_recycle(True)
     kw = dict(w.opts)
     kw.update(opts)
     po, oo = b.make_opts(**kw), oracle.make_opts(**kw)
@@ -558,3 +564,44 @@ def test_fp32_init_and_diagnostics():
     with pytest.raises(b.SdmError, match="float32"):
         p.init_from_arrays(w.rhod.cuda(), w.state["n"].cuda(), w.state["rw2"].cuda(), w.state["rd3"].cuda(), w.state["kappa"].cuda(),
                            w.state["x"].cuda(), None, w.state["z"].cuda())
+
+
+# ----------------------------------------------------------------------------------------------- recycling
+def test_recycling_box_golovin_keeps_every_sd_and_matches_the_oracle():
+    """PAPER.md :641: SDs left with zero multiplicity by equal-multiplicity collisions are recycled at the beginning of
+    the next step.  configs[0] starts with equal multiplicities everywhere, so ties (order by id) and halving of odd
+    multiplicities are exercised from the first steps on."""
+    w = W.box_golovin(seed=43)
+    p, o, _, _ = run_both(w, 500, check_every=50, recycle=True)
+    assert p.n_sd() == o.n_sd() == w.n_sd
+    assert p.stats()["recycled"] == o.recycled > 500
+    sp, so = p.stats(), o.counters()
+    assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"]
+
+
+def test_recycling_of_sds_that_left_the_domain():
+    """PAPER.md :651: SDs that sedimented out of the domain 'undergo the same recycling procedure'."""
+    w = rain_mix(W.cfg2_2d(nx=12, nz=12, sd_per_cell=40, seed=9), seed=9, frac=0.3)
+    p, o, _, _ = run_both(w, 12, recycle=True)
+    assert p.stats()["recycled"] == o.recycled > 20
+    assert p.n_sd() == o.n_sd() == w.n_sd
+    # fp32 state: the same, each step compared on its own from the device's rounded state
+    w = rain_mix(W.cfg2_2d(nx=12, nz=12, sd_per_cell=40, seed=10), seed=10, frac=0.3)
+    p, o = _fp32_case(w, steps=8, recycle=True)
+    assert p.stats()["recycled"] == o.recycled > 10
+
+
+@pytest.mark.parametrize("spc,n_dead,distinct", [(34, 9000, 1), (34, 200, 7), (6, 4000, 3), (78, 1, 1000000), (1, 600, 2)])
+def test_recycling_selection_with_ties_across_sort_tiles(spc, n_dead, distinct):
+    """The donors are exactly the oracle's: many equal multiplicities (order by id decides), candidate lists longer than
+    one shared-memory sort tile (global bitonic steps), fewer donors than dead SDs, multiplicity 1 never halved."""
+    w = W.cfg2_2d(nx=30, nz=30, sd_per_cell=spc, seed=7)
+    n_sd = w.n_sd
+    idx = torch.arange(n_sd, dtype=torch.int64)
+    u = W.hash_uniform(3, 11, idx)
+    n = (1 if distinct > 1 else 6) + (W.hash_uniform(3, 12, idx) * distinct).to(torch.int64)   # ties; N = 1 cannot give
+    w.state["n"] = torch.where(u < n_dead / n_sd, torch.zeros_like(n), n)
+    w.state["id"] = torch.randperm(n_sd, generator=torch.Generator().manual_seed(1)).to(torch.int32)
+    p, o, _, _ = run_both(w, 1, opts=dict(coal=False, cond=False, adve=False, sedi=False), recycle=True)
+    assert p.stats()["recycled"] == o.recycled > 0
+    assert p.n_sd() == o.n_sd()

@@ -35,7 +35,7 @@ FLOP_PER_EVAL = 190.0
 FLOP_PER_SETUP = 150.0
 FLOP_PER_CORRECTION = 28.0   # third-order correction of every Newton step after the first (curvature from the last two iterates)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
-NCU_COND_DRAM_BYTES = 2.316079e9 + 0.551624e9       # k_cond4 on the default workload, one ncu --set full capture
+NCU_COND_DRAM_BYTES = 2.313708e9 + 0.553631e9       # k_cond4 on the default workload, one ncu --set full capture
 
 
 def parse():
@@ -284,7 +284,7 @@ def main():
     step_ms = ms / a.steps
     roofline = {"kernel": "k_cond4 (condensation, 10 fused substeps)", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": NCU_COND_DRAM_BYTES if wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64 else None,
-                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_k_cond4_ncu_full.md",
+                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_k_cond4_v6_ncu_full.md",
                 "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
                 "evals_per_sd_substep": evals / max(subs, 1),
                 "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),

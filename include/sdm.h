@@ -220,6 +220,13 @@ int sdm_set_step(sdm_ctx* ctx, uint64_t step);
 /* Tuning override for tests: threads cooperating on one cell in the cell-resident kernels
  * (0 = automatic; 4, 8, 16, 32 = sub-warp groups; 256 = one CTA per cell). */
 int sdm_set_group_size(sdm_ctx* ctx, int group);
+/* Arithmetic of the condensation sweep (a4).  8 (default): fp64, radii within 1e-9 of the oracle.  4: fp32 -- the
+ * `real_t = float` of the paper's templates (PAPER.md :747; its timings are single precision, :908) -- allowed with
+ * real_bytes = 4 only (SDM_ERR_INVALID otherwise); radii within 1e-4 of the fp64 oracle started from the same
+ * fp32-representable state (BASELINE.json north_star).  The cells' thermodynamics, the feedback on th and rv (eq. 25-26)
+ * and every SD whose bracket may hold several roots or whose iterate leaves the bracket stay fp64.  One crowded cell
+ * beyond 4096 SDs is solved in fp64 either way. */
+int sdm_set_cond_arith(sdm_ctx* ctx, int bytes);
 /* Tuning override: growth-rate evaluations the dense condensation sweep spends on an SD before deferring it
  * to the compacted second pass (1..200, default 4).  Does not change results beyond the solver tolerance. */
 int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast);

@@ -49,7 +49,7 @@ class Stats(C.Structure):
 EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_range", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
-           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle"]
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
@@ -93,6 +93,7 @@ def load_library():
     L.sdm_set_cond_kfast.argtypes = [vp, C.c_int]
     L.sdm_set_timing.argtypes = [vp, C.c_int]
     L.sdm_set_recycle.argtypes = [vp, C.c_int]
+    L.sdm_set_cond_arith.argtypes = [vp, C.c_int]
     L.sdm_stage_times.argtypes = [vp, C.POINTER(C.c_double), u64p, C.c_int]
     _lib = L
     return L
@@ -272,6 +273,10 @@ class Particles:
     def set_recycle(self, on=True):
         """PAPER.md :641, :651: recycle zero-multiplicity SDs at the beginning of each step instead of only compacting."""
         self._ck(self.L.sdm_set_recycle(self.h, int(bool(on))))
+
+    def set_cond_arith(self, bytes_):
+        """8: fp64 condensation sweep (default); 4: fp32 arithmetic (real_bytes = 4 only; radii to 1e-4)."""
+        self._ck(self.L.sdm_set_cond_arith(self.h, int(bytes_)))
 
     def set_timing(self, enable=True):
         self._ck(self.L.sdm_set_timing(self.h, int(enable)))

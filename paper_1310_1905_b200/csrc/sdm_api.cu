@@ -55,6 +55,7 @@ struct sdm_ctx {
   int group_override = 0;
   int cond_cpb0 = 1;         // candidate cells per condensation tile (halved up to 3 times if a tile overflows)
   int kfast = 4;
+  int cond_arith = 8;        // 8: fp64 arithmetic in the condensation sweep; 4: fp32 (real_bytes == 4 only)
   cudaEvent_t ev_info = nullptr, ev_async = nullptr;
   cudaStream_t last_stream = nullptr;
   u64 launches = 0;
@@ -486,6 +487,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     if (ctx->o.real_bytes == 8)
       CK(launch_cond(cpb, variant, view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
                      rvf, ctx->cf, cp, ctx->cnt, st));
+    else if (ctx->cond_arith == 4 && variant != 0)
+      CK(launch_cond_f32(cpb, variant, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
     else
       CK(launch_cond(cpb, variant, view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
                      rvf, ctx->cf, cp, ctx->cnt, st));
@@ -689,6 +692,14 @@ int sdm_set_recycle(sdm_ctx* ctx, int on) {
     CK(cudaMallocHost((void**)&ctx->h_rec, 8 * sizeof(u32)));
   }
   ctx->recycle = on != 0;
+  return SDM_OK;
+}
+
+int sdm_set_cond_arith(sdm_ctx* ctx, int bytes) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (bytes != 8 && bytes != 4) return fail(ctx, SDM_ERR_INVALID, "sdm_set_cond_arith: 8 or 4");
+  if (bytes == 4 && ctx->o.real_bytes != 4) return fail(ctx, SDM_ERR_INVALID, "sdm_set_cond_arith: fp32 arithmetic needs real_bytes = 4");
+  ctx->cond_arith = bytes;
   return SDM_OK;
 }
 

@@ -997,10 +997,397 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   }
 }
 
+
+// =====================================================================================================================
+// fp32 arithmetic (real_t = float of the paper's templates, :747, :908; north_star: radii to 1e-4 in fp32; selected by
+// sdm_set_cond_arith(ctx, 4) with real_bytes = 4).  The sweep of k_cond4 in single precision; everything that decides
+// a branch of the method (root selection, ill-posed brackets, iterates leaving the bracket) still goes to the fp64
+// slow list, and the cells' thermodynamics and the feedback stay fp64.  What makes single precision sufficient:
+//  * lengths in micrometres (r ~ 1e-3 .. 3e3, r^3 ~ 1e-9 .. 1e10, D_0 and K_0 scaled by 1e12): every intermediate of
+//    eq. 20-24 stays inside the fp32 range, and no product of three large factors is formed (three reciprocals
+//    instead of the one of the fp64 path; MUFU.RCP is cheap in fp32);
+//  * the unknown is the increment d = r - r0, g(d) = d (2 r0 + d) - dt' f(r0 + d): the growth per substep (1e-3 r and
+//    less) is resolved to its own 1e-7, and N d(r^3) = N d (3 r0^2 + 3 r0 d + d^2) has no cancellation;
+//  * the driving force without cancellation: RH - a_w e^(A/r) = (RH - 1) + kappa r_d^3 / W - a_w expm1(A/r), with RH - 1
+//    taken from the fp64 cell record: three terms of size 1e-1 .. 1e-4 each known to 1e-7 of itself, where the plain
+//    form subtracts two numbers near 1;
+//  * the first step solves d^2 + g' d - dt' f0 = 0 exactly (Newton in r^2 with f linearised in r), so that what is
+//    left is dt' f'' d^2 / (2 g'), and |f''| is bounded from quantities the evaluation has anyway:
+//    |f''| <= (8/r) (|f'| + |f|/r + c (a_w' + a_w t / r) e^t), c = f / S (power-law factors of degree <= 4 and the
+//    Koehler terms).  An SD is done when that bound is below 1e-6 r: a cloud droplet growing by 0.3 % per substep
+//    (bound 4 (d/r)^3) and haze following its cell (bound 8 (d/r)^2, d/r < 3.5e-4) take ONE evaluation.
+// MUFU approximations (1-2 ulp, no special-case branches): ample for the 1e-6 the sweep is solved to
+__device__ __forceinline__ float frcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fsqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+struct CellF {   // per-cell constants of one substep, lengths in micrometres
+  float S0, RH, A, invA, lD, lK, qD, qK, lD171, lK171, c0, heat, kE, Sc, Pr, pad;
+};
+static_assert(sizeof(CellF) == 64, "CellF");
+struct SdF { float rd3, krd3, Kc, hDc, c0Dc, cDK; };
+
+__device__ __forceinline__ void cell_to_float(const CellRec& R, CellF& F) {
+  F.S0 = (float)(R.RH - 1.0); F.RH = (float)R.RH;
+  F.A = (float)(R.A * 1e6); F.invA = (float)(R.invA * 1e-6);
+  F.lD = (float)(R.lD * 1e6); F.lK = (float)(R.lK * 1e6);
+  F.qD = (float)(R.qD * 1e12); F.qK = (float)(R.qK * 1e12);
+  F.lD171 = (float)(R.lD171 * 1e6); F.lK171 = (float)(R.lK171 * 1e6);
+  F.c0 = (float)R.c0; F.heat = (float)R.heat;
+  F.kE = (float)(R.kE * 1e-9);   // e = kE r^(3/2), r in micrometres
+  F.Sc = (float)R.Sc; F.Pr = (float)R.Pr; F.pad = 0.f;
+}
+
+// [L] ventilation at the substep's starting radius (reading R-vent), as sd_setup; D_0, K_0 in um^2/s units
+__device__ __forceinline__ void sd_setup_f(float r0, const CellF& c, SdF& s) {
+  const float e = c.kE * (r0 * fsqrt(r0));
+  const float q = e * frcp(fsqrt(1.0f + e) + 1.0f);
+  const float Re = (float)(cst::kc_delta0 * cst::kc_delta0 / 4.0) * (q * q);
+  const float xs = Re * c.Sc, xp = Re * c.Pr;
+  float shm, num;
+  if (fmaxf(xs, xp) < 0.02f) {
+    float a = 22.0f / 729.0f, b = 22.0f / 729.0f;
+    a = fmaf(a, xs, -10.0f / 243.0f); b = fmaf(b, xp, -10.0f / 243.0f);
+    a = fmaf(a, xs, 5.0f / 81.0f); b = fmaf(b, xp, 5.0f / 81.0f);
+    a = fmaf(a, xs, -1.0f / 9.0f); b = fmaf(b, xp, -1.0f / 9.0f);
+    a = fmaf(a, xs, 1.0f / 3.0f); b = fmaf(b, xp, 1.0f / 3.0f);
+    shm = a * xs; num = b * xp;
+  } else {
+    shm = cbrtf(1.0f + xs) - 1.0f; num = cbrtf(1.0f + xp) - 1.0f;
+    if (Re > 1.0f) {
+      const float m = powf(Re, 0.077f) - 1.0f;
+      shm = shm + m + shm * m;
+      num = num + m + num * m;
+    }
+  }
+  const float Dc = fmaf((float)(0.5e12 * cst::D_0), shm, (float)(1e12 * cst::D_0));
+  s.Kc = fmaf((float)(0.5e12 * cst::K_0), num, (float)(1e12 * cst::K_0));
+  s.hDc = c.heat * Dc;
+  s.c0Dc = c.c0 * Dc;
+  s.cDK = s.c0Dc * s.Kc;
+}
+
+// e^t - 1 for 0 <= t < 4 with relative error ~1e-7: Taylor to t^7 below 0.25 (next term 0.25^7/8! = 1.5e-9 of t),
+// exp2 of the hardware otherwise
+__device__ __forceinline__ float expm1_kelvin_f(float t) {
+  if (t < 0.25f) {
+    float p = 1.0f / 5040.0f;
+    p = fmaf(p, t, 1.0f / 720.0f); p = fmaf(p, t, 1.0f / 120.0f); p = fmaf(p, t, 1.0f / 24.0f);
+    p = fmaf(p, t, 1.0f / 6.0f); p = fmaf(p, t, 0.5f); p = fmaf(p, t, 1.0f);
+    return p * t;
+  }
+  return fex2(t * 1.4426950408889634f) - 1.0f;
+}
+
+// f(r) = d r_w^2/dt [um^2/s], df/dr and B >= |d2f/dr2| (see above); r, lengths in micrometres
+__device__ __forceinline__ void growth_f32(float r, const SdF& s, const CellF& c, float& f, float& dfr, float& B, float& t_out) {
+  const float y = r * r;
+  const float lDr = c.lD * r, lKr = c.lK * r;
+  const float NM = y + lDr, DM = fmaf(1.71f, lDr, y) + c.qD;
+  const float NT = y + lKr, DT = fmaf(1.71f, lKr, y) + c.qK;
+  const float KN = s.Kc * NT, HN = s.hDc * NM;
+  const float Q = fmaf(KN, DM, HN * DT);
+  const float P = fmaf(y, r, -s.rd3), W = P + s.krd3;
+  const float invQ = frcp(Q), invW = frcp(W), invr = frcp(r);
+  const float t = c.A * invr;
+  t_out = t;
+  const float em1 = expm1_kelvin_f(t), ex = 1.0f + em1;
+  const float aw = P * invW;
+  const float S = c.S0 + fmaf(-aw, em1, s.krd3 * invW);
+  const float NN = NM * NT;
+  const float cN = s.cDK * invQ * NN;
+  f = cN * S;
+  const float r2 = r + r;
+  const float NMp = r2 + c.lD, DMp = r2 + c.lD171, NTp = r2 + c.lK, DTp = r2 + c.lK171;
+  const float NNp = fmaf(NMp, NT, NM * NTp);
+  const float Qp = s.Kc * fmaf(NTp, DM, NT * DMp) + s.hDc * fmaf(NMp, DT, NM * DTp);
+  const float awp = 3.0f * y * s.krd3 * (invW * invW);
+  const float kel = aw * t * invr;
+  const float Sp = ex * (kel - awp);
+  const float lnp = NNp * frcp(NN) - Qp * invQ;   // d ln(NN/Q) / dr
+  dfr = fmaf(f, lnp, cN * Sp);
+  B = 8.0f * invr * (fabsf(dfr) + fabsf(f) * invr + cN * ex * (awp + kel));
+}
+
+__device__ __forceinline__ bool single_root_bracket_f(float Dlo, float Dhi, float y0, float two, float S0, float rd3, float krd3,
+                                                      float A, float invA, float dtcD) {
+  const float lo = y0 + Dlo, hi = y0 + Dhi;
+  const float yc = 3.0f * krd3 * invA;
+  if ((hi <= 0.999f * yc && krd3 <= 2.0f * rd3) || (S0 < 0.0f && Dlo == 0.0f && two > 0.0f)) return true;   // (1), (3)
+  const float ym = fmaxf(lo, yc);
+  const float K3 = 1.3f * A * dtcD;
+  return (Dhi - Dlo <= 0.49f * lo) && (ym * ym * ym >= 1.01f * K3 * K3) && (A * A <= 0.06f * ym);             // (2)
+}
+
+constexpr float COND_TOLF = 1e-6f;   // bound on the error left in r, relative (north_star: 1e-4 on radii in fp32)
+
+template <int CAP, int T>
+struct Cond4F {
+  static constexpr int NW = T / 32;
+  static constexpr size_t fixed_bytes = (size_t)6 * CAP * 4 + (size_t)2 * CAP * 2;
+  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * (sizeof(CellRec) + sizeof(CellF)) + (size_t)(cpb + 1) * 4 + 16; }
+};
+
+template <int CAP, int T, int MINB>
+__global__ void __launch_bounds__(T, MINB)
+k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
+         CellFields cf, CondParams cp, Counters cnt, int cpb) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  using L = Cond4F<CAP, T>;
+  constexpr int NW = L::NW;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int c_first = blockIdx.x * cpb;
+  const int nc = min(cpb, g.ncell - c_first);
+  float* s_r = reinterpret_cast<float*>(smem_raw);   // micrometres
+  float *s_rd3 = s_r + CAP, *s_krd3 = s_r + 2 * CAP, *s_dn = s_r + 3 * CAP, *s_rd2 = s_r + 4 * CAP, *s_con = s_r + 5 * CAP;
+  u16* cidx = reinterpret_cast<u16*>(s_r + 6 * CAP);
+  u16* list = cidx + CAP;
+  CellRec* s_cell = reinterpret_cast<CellRec*>(smem_raw + L::fixed_bytes);
+  CellF* s_cf = reinterpret_cast<CellF*>(s_cell + cpb);
+  u32* segl = reinterpret_cast<u32*>(s_cf + cpb);
+  u32* ctr = segl + cpb + 1;   // [0] next chunk of the sweep, [1] length of the slow list
+  const u32 s0 = seg[c_first];
+  const int M = (int)(seg[c_first + nc] - s0);
+
+  // The fp32 sweep costs ~8 instructions per SD-substep, so what surrounds it is organised for instruction count:
+  // the cells' fp64 thermodynamics run on the lanes of ONE warp (the chain is as long for 3 lanes as for 30, and four
+  // warps issuing it cost four times the slots), staging and the per-cell sums go cell by cell without searches.
+  for (int cl = tid; cl < nc; cl += T) {
+    const int c = c_first + cl;
+    const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+    CellRec& R = s_cell[cl];
+    R.th = th_f.at(i, j, k); R.rv = rv_f.at(i, j, k);
+    const double rhod = cf.rhod[c];
+    R.rhod = rhod;
+    R.fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
+    segl[cl] = seg[c] - s0;
+  }
+  if (tid == 0) { segl[nc] = (u32)M; ctr[0] = 0u; ctr[1] = 0u; }
+  __syncthreads();
+  const bool by_cell = M >= 24 * nc;   // populated cells: a warp stages a cell at a time
+  for (int q = by_cell ? warp : tid; q < (by_cell ? nc : M); q += by_cell ? NW : T) {   // stage the tile in sorted order, lengths in micrometres
+    int cl, t0, t1;
+    if (by_cell) {
+      cl = q; t0 = (int)segl[cl] + lane; t1 = (int)segl[cl + 1];
+    } else {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)q) lo = mid; else hi = mid; }
+      cl = lo; t0 = q; t1 = q + 1;
+    }
+    const int b0 = (int)segl[cl];
+    for (int t = t0; t < t1; t += 32) {
+      const u32 s = s0 + t;
+      const int e = b0 + rank[s];
+      const float rd3 = a.rd3[s] * 1e18f;
+      const float q3 = cbrtf(rd3);
+      s_r[e] = fsqrt(a.rw2[s] * 1e12f);
+      s_rd3[e] = rd3;
+      s_krd3[e] = a.kappa[s] * rd3;
+      s_dn[e] = (float)a.n[s];
+      s_rd2[e] = q3 * q3;
+      cidx[e] = (u16)cl;
+    }
+  }
+  unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
+  const float dtp = (float)cp.dtp;
+  const int nsub = M > 0 ? cp.sstp : 0;
+  for (int sub = 0; sub <= nsub; ++sub) {
+    // D. per-cell sums of N d(r_w^3) [um^3]: 8 lanes per cell, fixed order (deterministic); R.pad carries the sum
+    if (sub > 0) {
+      const int l8 = lane & 7, grp = lane >> 3;
+      for (int cl = warp * 4 + grp; cl < ((nc + 3) & ~3); cl += NW * 4) {   // warp-uniform trip count
+        float acc = 0.0f;   // fp32 sum of ~64 terms: 1e-6 of the substep's change of r_v
+        if (cl < nc) {
+          const int b1 = (int)segl[cl + 1];
+          for (int e = (int)segl[cl] + l8; e < b1; e += 8) acc += s_con[e];
+        }
+        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+        if (cl < nc && l8 == 0) s_cell[cl].pad = (double)acc * 1e-18;
+      }
+      __syncthreads();
+    }
+    // A. feedback (eq. 25-26) and the constants of the next substep, fp64, one lane per cell on the first warp(s)
+    if (tid < ((nc + 31) & ~31)) {
+      for (int cl = tid; cl < nc; cl += T) {
+        CellRec& R = s_cell[cl];
+        if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, R.pad, cp.RH_max, true);
+        cell_to_float(R, s_cf[cl]);
+      }
+    }
+    if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
+    if (sub == nsub) break;
+    __syncthreads();
+    // B. dense sweep in fp32.  st: 0 = iterating, 1 = solved, 2 = left to the fp64 list
+    for (;;) {
+      int q0 = 0;
+      if (lane == 0) q0 = (int)atomicAdd(&ctr[0], 32u);
+      q0 = __shfl_sync(0xffffffffu, q0, 0);
+      if (q0 >= M) break;
+      const bool valid = q0 + lane < M;
+      const int e = min(q0 + lane, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
+      const CellF c = s_cf[(int)cidx[e]];
+      const float r0 = s_r[e], rd2 = s_rd2[e];
+      SdF s;
+      s.rd3 = s_rd3[e]; s.krd3 = s_krd3[e];
+      sd_setup_f(r0, c, s);
+      float f, dfr, B, t;
+      growth_f32(r0, s, c, f, dfr, B, t);
+      n_eval += valid;
+      const float y0 = r0 * r0, r02 = r0 + r0;
+      const float dtf = dtp * f, two = dtf + dtf;
+      // eq. 18-19 in D = y - y0
+      float Dlo = fmaxf(rd2 - y0, fminf(two, 0.0f)), Dhi = fmaxf(two, 0.0f);
+      const bool guard = !(t < 4.0f) || !single_root_bracket_f(Dlo, Dhi, y0, two, c.S0, s.rd3, s.krd3, c.A, c.invA, dtp * s.c0Dc);
+      Dlo *= 0.99f; Dhi *= 0.99f;   // an iterate this close to an end of the bracket is left to the fp64 list
+      float d = 0.0f;
+      int st;
+      if (!(Dlo < Dhi)) {
+        st = (two == 0.0f) ? 1 : 2;   // a = b = y0: the result is a
+      } else {
+        const float gp = fmaf(-dtp, dfr, r02);
+        const float disc = fmaf(gp, gp, 4.0f * dtf);
+        if (!(gp > 0.0f && disc > 0.0f)) {
+          st = 2;
+        } else {
+          d = two * frcp(gp + fsqrt(disc));   // d^2 + g' d - dt' f0 = 0, the root that vanishes with f0
+          const float D = d * (r02 + d);
+          if (!(D >= Dlo && D <= Dhi)) st = 2;
+          else st = (dtp * B * d * d <= 2.0f * COND_TOLF * gp * (r0 + d)) ? 1 : 0;
+        }
+      }
+      if (guard) st = 2;
+      if (!valid) st = 1;
+      for (int it = 1; it < cp.kfast; ++it) {
+        if (!__any_sync(0xffffffffu, st == 0)) break;
+        if (st == 0) {
+          const float r = r0 + d;
+          growth_f32(r, s, c, f, dfr, B, t);
+          ++n_eval;
+          const float D = d * (r02 + d);
+          const float gv = fmaf(-dtp, f, D);
+          const float gp = fmaf(-dtp, dfr, r + r);
+          if (gv < 0.0f) Dlo = D; else Dhi = D;
+          const float dN = -gv * frcp(gp);
+          const float dn = d + dN;
+          const float Dn = dn * (r02 + dn);
+          if (!(gp > 0.0f && Dn >= Dlo && Dn <= Dhi && t < 4.0f)) {
+            st = 2;
+          } else {
+            d = dn;
+            st = (fmaf(dtp, B, 2.0f) * dN * dN <= 2.0f * COND_TOLF * gp * (r0 + dn)) ? 1 : 0;
+          }
+        }
+      }
+      if (st == 0) st = 2;
+      if (valid && st == 1) {
+        s_con[e] = s_dn[e] * (d * fmaf(3.0f * r0, r0 + d, d * d));   // N (r^3 - r0^3) without cancellation
+        s_r[e] = r0 + d;
+        ++n_sub;
+      }
+      const unsigned need = __ballot_sync(0xffffffffu, st == 2);
+      if (need) {   // warp-aggregated append to the tile's slow list
+        u32 base = 0;
+        if (lane == 0) base = atomicAdd(&ctr[1], (u32)__popc(need));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (st == 2) list[base + __popc(need & ((1u << lane) - 1u))] = (u16)e;
+      }
+    }
+    __syncthreads();
+    // C. the listed rest in fp64 (SI units), exactly as k_cond4 does: cond_solve or the paper's literal bisection
+    const int nlist = (int)ctr[1];
+    if (nlist > 0) {
+      const bool per_warp = nlist <= 2 * NW;
+      for (int k = per_warp ? warp : tid; k < nlist; k += per_warp ? NW : T) {
+        const int e = (int)list[k];
+        const CellRec& R = s_cell[(int)cidx[e]];
+        CellK c;
+        c.RH = R.RH; c.A = R.A; c.c0 = R.c0; c.lD = R.lD; c.lK = R.lK; c.heat = R.heat; c.kE = R.kE; c.Sc = R.Sc; c.Pr = R.Pr;
+        const double r0 = (double)s_r[e] * 1e-6, y0 = r0 * r0;
+        const double rd3 = (double)s_rd3[e] * 1e-18, krd3 = (double)s_krd3[e] * 1e-18;
+        const double rd2 = fmin((double)s_rd2[e] * 1e-12, y0);
+        double y1 = y0;
+        unsigned ill = 0, ev = 0;
+        bool solved = false;
+        if (per_warp) {   // all lanes hold the same SD
+          SdK s;
+          double Dc, f, df;
+          slow_setup(y0, rd3, krd3, c, s, Dc);
+          growth_fd(y0, s, c, f, df);
+          const double two = 2.0 * cp.dtp * f;
+          const double a_ = fmax(rd2, y0 + fmin(two, 0.0)), b_ = y0 + fmax(two, 0.0);   // eq. 18-19
+          if (a_ < b_ && !single_root_bracket(a_, b_, y0, c.RH, rd3, krd3, c.A, R.invA, cp.dtp * s.c0Dc)) {
+            ev = (lane == 0);
+            y1 = bisect_paper_warp(a_, b_, f, y0, s, c, cp.dtp, lane, ill, ev);
+            solved = true;
+          }
+        }
+        if (!solved) {
+          cond_solve(y0, rd2, rd3, krd3, c, cp.dtp, 200, y1, ill, ev);
+          if (per_warp && lane != 0) { ill = 0; ev = 0; }
+        }
+        n_ill += ill; n_eval += ev;
+        if (!per_warp || lane == 0) {
+          const double r1 = sqrt(y1);
+          ++n_sub; ++n_slow;
+          s_con[e] = (float)((double)s_dn[e] * (r1 * r1 * r1 - r0 * y0) * 1e18);
+          s_r[e] = (float)(r1 * 1e6);
+        }
+      }
+      __syncthreads();
+    }
+  }
+
+  for (int cl = tid; cl < nc; cl += T) {
+    const int c = c_first + cl;
+    const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+    const CellRec& R = s_cell[cl];
+    th_f.at(i, j, k) = R.th;
+    rv_f.at(i, j, k) = R.rv;
+    cf.eta[c] = R.eta;   // air properties after the feedback, used by coalescence and sedimentation (v_term)
+    cf.rho_a[c] = R.rhod * (1.0 + R.rv);
+  }
+  for (int q = by_cell ? warp : tid; q < (by_cell ? nc : M); q += by_cell ? NW : T) {
+    int cl, t0, t1;
+    if (by_cell) {
+      cl = q; t0 = (int)segl[cl] + lane; t1 = (int)segl[cl + 1];
+    } else {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)q) lo = mid; else hi = mid; }
+      cl = lo; t0 = q; t1 = q + 1;
+    }
+    const int b0 = (int)segl[cl];
+    for (int t = t0; t < t1; t += 32) {
+      const u32 s = s0 + t;
+      const float r = s_r[b0 + rank[s]] * 1e-6f;
+      a.rw2[s] = r * r;
+    }
+  }
+  unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub, v3 = n_slow;
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    v0 += __shfl_xor_sync(0xffffffffu, v0, d);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, d);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, d);
+    v3 += __shfl_xor_sync(0xffffffffu, v3, d);
+  }
+  if (lane == 0) {
+    const int slot = (blockIdx.x * NW + warp) & (NSLOT - 1);
+    if (v0) atomicAdd(&cnt.ill_posed[slot], (unsigned long long)v0);
+    if (v1) atomicAdd(&cnt.f_evals[slot], (unsigned long long)v1);
+    if (v2) atomicAdd(&cnt.sd_substeps[slot], (unsigned long long)v2);
+    if (v3) atomicAdd(&cnt.cond_slow[slot], (unsigned long long)v3);
+  }
+}
+
 // the two instantiations: sparse cells (5 CTAs of 128 threads per SM) and crowded cells (one CTA of 512)
 #ifndef SDM_COND_CAP
 #define SDM_COND_CAP 800   // SD slots of the small tile kernel
 #define SDM_COND_MINB 5    // its CTAs per SM
+#endif
+#ifndef SDM_COND32_MINB
+#define SDM_COND32_MINB 8  // CTAs per SM of the fp32-arithmetic small tile kernel
 #endif
 using CondSmall = Cond4<SDM_COND_CAP, 128>;
 using CondMedium = Cond4<1280, 256>;   // 3 CTAs of 256 threads per SM: cells of ~1000 SDs
@@ -1026,6 +1413,28 @@ static cudaError_t launch_cond4(size_t smem, int grid, const SdArraysT<R>& a, co
   if (e != cudaSuccess) return e;
   k_cond4<CAP, T, MINB, R><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
   return cudaGetLastError();
+}
+
+template <int CAP, int T, int MINB>
+static cudaError_t launch_cond4f(size_t smem, int grid, const SdArraysT<float>& a, const u16* rank, const u32* seg, const Grid& g,
+                                 Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, int cpb,
+                                 cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(k_cond4f<CAP, T, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  k_cond4f<CAP, T, MINB><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  return cudaGetLastError();
+}
+
+// fp32-arithmetic condensation for the tile variants 1..3 of cond_variant (same tiles as the fp64 kernels, which need
+// more shared memory, so whatever they fit, these fit); variant 0 (one crowded cell in global memory) has no fp32 form
+cudaError_t launch_cond_f32(int cpb, int variant, const SdArraysT<float>& a, const u16* rank, const u32* seg, const Grid& g,
+                            Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st) {
+  const int grid = (g.ncell + cpb - 1) / cpb;
+  if (variant == 1)
+    return launch_cond4f<SDM_COND_CAP, 128, SDM_COND32_MINB>(Cond4F<SDM_COND_CAP, 128>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  if (variant == 2) return launch_cond4f<1280, 256, 4>(Cond4F<1280, 256>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  if (variant == 3) return launch_cond4f<4096, 512, 1>(Cond4F<4096, 512>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+  return cudaErrorInvalidValue;
 }
 
 // eta, rho_a per cell when condensation is switched off

@@ -480,7 +480,7 @@ def test_root_selection_scan_of_independent_sds():
 
 
 # ------------------------------------------------------------------------------------ fp32 particle state
-def _fp32_case(w, steps=1, recycle=False, **opts):
+def _fp32_case(w, steps=1, recycle=False, arith=8, **opts):
     """Single-step parity with real_bytes = 4 (north_star: 1e-4 on radii in fp32): the state is rounded to fp32
     first, the oracle starts from exactly those values in fp64, and before every further step the oracle is
     re-loaded with the device's (fp32) state, so that each step is compared on its own."""
@@ -497,6 +497,7 @@ def _fp32_case(w, steps=1, recycle=False, **opts):
     if recycle:
         o.set_recycle(True)
         p.set_recycle(True)
+    p.set_cond_arith(arith)
     kw = dict(w.opts)
     kw.update(opts)
     po, oo = b.make_opts(**kw), oracle.make_opts(**kw)
@@ -637,3 +638,18 @@ def test_box_golovin_full_length_16_seeds_against_the_closed_form(recycle):
     for t in times:
         ratio = np.mean(M0[t]) / (n0 * np.exp(-bb * n0 * v0 * t))
         assert abs(ratio - 1) < tol[t], (t, ratio)
+
+
+# ----------------------------------------------------------------------------------------------- fp32 arithmetic
+def test_fp32_arithmetic_condensation_2d_3d_and_first_step():
+    """sdm_set_cond_arith(4): the condensation sweep in single precision (real_t = float, PAPER.md :747).  north_star:
+    radii within 1e-4 of the fp64 oracle started from the same fp32 state, multiplicities and collisions bit-exact."""
+    p, o = _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=32, nx=10, nz=75, seed=41)), steps=4, arith=4)
+    assert o.counters()["collisions"] > 0
+    _fp32_case(rain_mix(W.cfg4_3d(sd_per_cell=64, nx=4, ny=3, nz=64, seed=42)), steps=3, arith=4)
+    # haze only, from the initial condition at full height: the first step under RH_max = 1.05 (multi-root brackets)
+    _fp32_case(W.cfg2_2d(sd_per_cell=64, nx=4, nz=75, seed=43), steps=3, arith=4)
+    # cells of ~1000 SDs (medium tile) and the fp64 fallback for one crowded cell
+    _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=1000, nx=2, nz=3, seed=44), frac=0.3), steps=2, sstp_cond=3, arith=4)
+    with pytest.raises(Exception):
+        make_particles(W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1))[0].set_cond_arith(4)   # fp64 state: refused

@@ -35,7 +35,13 @@ FLOP_PER_EVAL = 190.0
 FLOP_PER_SETUP = 150.0
 FLOP_PER_CORRECTION = 28.0   # third-order correction of every Newton step after the first (curvature from the last two iterates)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
-NCU_COND_DRAM_BYTES = 2.313708e9 + 0.553631e9       # k_cond4 on the default workload, one ncu --set full capture
+# --cond-arith 4 (k_cond4f): fp32 operations of one evaluation with derivative and curvature bound (62 instructions, 20 of
+# them FMA, 4 MUFU) and of the per-SD-substep set-up, first step and N d(r^3) (45 instructions, 15 FMA); DESIGN.md section 7
+FLOP_PER_EVAL_F32 = 86.0
+FLOP_PER_SETUP_F32 = 60.0
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x fp32 FMA lanes x 2 x max SM clock = 74.4
+NCU_COND_DRAM_BYTES = 2.313708e9 + 0.553631e9
+NCU_COND32_DRAM_BYTES = None                        # k_cond4f on the default workload with --real-bytes 4 --cond-arith 4       # k_cond4 on the default workload, one ncu --set full capture
 
 
 def parse():
@@ -281,14 +287,21 @@ def main():
     cond_ms, cond_n = stages["cond"]
     evals = st1["newton_iters"] - st0["newton_iters"]
     subs = st1["sd_substeps"] - st0["sd_substeps"]
-    flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP + max(evals - subs, 0) * FLOP_PER_CORRECTION
+    f32 = a.cond_arith == 4
+    if f32:
+        flops = evals * FLOP_PER_EVAL_F32 + subs * FLOP_PER_SETUP_F32
+    else:
+        flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP + max(evals - subs, 0) * FLOP_PER_CORRECTION
+    peak_alu = FP32_PEAK_TFLOPS if f32 else FP64_PEAK_TFLOPS
     ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
     stage_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in stages.items()}
     step_ms = ms / a.steps
-    roofline = {"kernel": "k_cond4 (condensation, 10 fused substeps)", "bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS, "traffic": NCU_COND_DRAM_BYTES if wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64 else None,
-                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1_k_cond4_v6_ncu_full.md",
-                "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+    full3d = wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64
+    roofline = {"kernel": ("k_cond4f (condensation, 10 fused substeps, fp32 sweep)" if f32 else "k_cond4 (condensation, 10 fused substeps)"),
+                "bound": "alu", "achieved": ach, "peak": peak_alu,
+                "unit": "TFLOP/s", "frac": ach / peak_alu, "traffic": (NCU_COND32_DRAM_BYTES if f32 else NCU_COND_DRAM_BYTES) if full3d and (f32 or a.real_bytes == 8) else None,
+                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/" + ("r1_k_cond4f_ncu_full.md" if f32 else "r1_k_cond4_v6_ncu_full.md"),
+                "peak_source": "derived: 148 SMs x %d fp%d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % ((128, 32) if f32 else (64, 64)),
                 "evals_per_sd_substep": evals / max(subs, 1),
                 "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
                 "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms}

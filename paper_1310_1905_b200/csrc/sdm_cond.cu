@@ -752,6 +752,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   CellRec* s_cell = reinterpret_cast<CellRec*>(smem_raw + L::fixed_bytes);
   u32* segl = reinterpret_cast<u32*>(s_cell + cpb);
   u32* ctr = segl + cpb + 1;   // [0] next chunk of the sweep, [1] length of the slow list
+  const u32 ctr_addr = (u32)__cvta_generic_to_shared(ctr);   // atom.shared by address: no generic-to-shared conversion per chunk
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
 
@@ -813,7 +814,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (list)
     for (;;) {
       int q0 = 0;
-      if (lane == 0) q0 = (int)atomicAdd(&ctr[0], 32u);
+      if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 32;" : "=r"(q0) : "r"(ctr_addr) : "memory");
       q0 = __shfl_sync(0xffffffffu, q0, 0);
       if (q0 >= M) break;
       const int e = q0 + lane;
@@ -1220,11 +1221,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
     if (sub == nsub) break;
     __syncthreads();
     // B. dense sweep in fp32.  st: 0 = iterating, 1 = solved, 2 = left to the fp64 list
-    for (;;) {
-      int q0 = 0;
-      if (lane == 0) q0 = (int)atomicAdd(&ctr[0], 32u);
-      q0 = __shfl_sync(0xffffffffu, q0, 0);
-      if (q0 >= M) break;
+    for (int q0 = warp * 32; q0 < M; q0 += NW * 32) {   // static chunks: with ~1 evaluation per SD the warps stay balanced
       const bool valid = q0 + lane < M;
       const int e = min(q0 + lane, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
       const CellF c = s_cf[(int)cidx[e]];

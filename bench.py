@@ -41,7 +41,7 @@ FLOP_PER_EVAL_F32 = 86.0
 FLOP_PER_SETUP_F32 = 60.0
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x fp32 FMA lanes x 2 x max SM clock = 74.4
 NCU_COND_DRAM_BYTES = 2.313708e9 + 0.553631e9
-NCU_COND32_DRAM_BYTES = None                        # k_cond4f on the default workload with --real-bytes 4 --cond-arith 4       # k_cond4 on the default workload, one ncu --set full capture
+NCU_COND32_DRAM_BYTES = 1.509464e9 + 0.313273e9     # k_cond4f, the default workload with --real-bytes 4 --cond-arith 4
 
 
 def parse():

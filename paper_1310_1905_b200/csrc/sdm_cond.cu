@@ -170,6 +170,11 @@ __device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c,
   dfr = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
 }
 
+// max / min without the NaN handling of fmax / fmin (DSETP + 2 SEL instead of DSETP + 2 FSEL + LOP3 + moves); the
+// sweep sends anything that is not a finite, ordered bracket to the slow list anyway
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+
 // sqrt(a) and 1/a from the fp32 hardware seeds and ONE fp64 Newton step (relative error ~1e-14, which is
 // ample for the ventilation coefficients: they enter D and K through 1 + (Sh-2)/2)
 __device__ __forceinline__ double sqrt_seeded(double a) {
@@ -202,7 +207,7 @@ __device__ __forceinline__ void sd_setup(double r0, double c0, double heat, doub
   const double Re = KC[KC_D2Q] * (q * q);
   const double xs = Re * Sc, xp = Re * Pr;
   double shm, num;   // Sh - 2, Nu - 2
-  if (fmax(xs, xp) < 0.02) {
+  if (dmax(xs, xp) < 0.02) {
     double a = KC[KC_B5], b = KC[KC_B5];
     a = fma(a, xs, KC[KC_B4]); b = fma(b, xp, KC[KC_B4]);
     a = fma(a, xs, KC[KC_B3]); b = fma(b, xp, KC[KC_B3]);
@@ -251,7 +256,7 @@ __device__ __forceinline__ bool single_root_bracket(double lo, double hi, double
                                                     double invA, double dtcD) {
   const double yc = 3.0 * krd3 * invA;
   if ((hi <= yc && krd3 <= 2.0 * rd3) || (RH < 1.0 && lo == y0)) return true;   // (1), (3)
-  const double ym = fmax(lo, yc);
+  const double ym = dmax(lo, yc);
   const double K3 = 1.3 * A * dtcD;
   return (hi - lo <= 0.5 * lo) && (ym * ym * ym >= K3 * K3) && (A * A <= 0.0625 * ym);   // (2)
 }
@@ -752,22 +757,18 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   CellRec* s_cell = reinterpret_cast<CellRec*>(smem_raw + L::fixed_bytes);
   u32* segl = reinterpret_cast<u32*>(s_cell + cpb);
   u32* ctr = segl + cpb + 1;   // [0] next chunk of the sweep, [1] length of the slow list
-  const u32 ctr_addr = (u32)__cvta_generic_to_shared(ctr);   // atom.shared by address: no generic-to-shared conversion per chunk
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
 
-  // cell cl of the tile is owned by lane cl / NW of warp cl % NW (cpb <= T)
-  const int cl_own = lane * NW + warp;
-  const bool owner = cl_own < nc;
-  if (owner) {
-    const int c = c_first + cl_own;
+  for (int cl = tid; cl < nc; cl += T) {   // thread cl owns cell cl of the tile (cpb <= T)
+    const int c = c_first + cl;
     const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
-    CellRec& R = s_cell[cl_own];
+    CellRec& R = s_cell[cl];
     R.th = th_f.at(i, j, k); R.rv = rv_f.at(i, j, k);
     const double rhod = cf.rhod[c];
     R.rhod = rhod;
     R.fbk = -(4.0 * cst::pi * cst::rho_w / 3.0) / (rhod * g.dV);   // eq. 25 prefactor
-    segl[cl_own] = seg[c] - s0;
+    segl[cl] = seg[c] - s0;
   }
   if (tid == 0) { segl[nc] = (u32)M; ctr[0] = 0u; ctr[1] = 0u; }
   __syncthreads();
@@ -789,34 +790,36 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   const double dtp = cp.dtp;
   const int nsub = M > 0 ? cp.sstp : 0;
   for (int sub = 0; sub <= nsub; ++sub) {
-    // D + A. every warp sums N d(r_w^3) of the cells it owns (sorted order: lane-strided partial sums, xor
-    // butterfly), then their owner lanes apply the feedback and derive the constants of the next substep;
-    // the pass after the last substep only applies the feedback.
-    double mysum = 0.0;
+    // D. per-cell sums of N d(r_w^3): 8 lanes per cell, fixed order (deterministic); R.pad carries the sum.
+    // A. feedback (eq. 25-26) and the constants of the next substep, one lane per cell on the FIRST warp(s): the chain
+    // is as long for 3 lanes as for 30, and four warps issuing it cost four times the issue and fp64 slots.  The pass
+    // after the last substep only applies the feedback.
     if (sub > 0) {
-      for (int j = 0; j * NW + warp < nc; ++j) {
-        const int cl = j * NW + warp;
-        const int b0 = (int)segl[cl], b1 = (int)segl[cl + 1];
+      const int l8 = lane & 7, grp = lane >> 3;
+      for (int cl = warp * 4 + grp; cl < ((nc + 3) & ~3); cl += NW * 4) {   // warp-uniform trip count
         double acc = 0.0;
-        for (int e = b0 + lane; e < b1; e += 32) acc += s_con[e];
-#pragma unroll
-        for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-        if (lane == j) mysum = acc;
+        if (cl < nc) {
+          const int b1 = (int)segl[cl + 1];
+          for (int e = (int)segl[cl] + l8; e < b1; e += 8) acc += s_con[e];
+        }
+        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+        if (cl < nc && l8 == 0) s_cell[cl].pad = acc;
       }
+      __syncthreads();
     }
-    if (owner) {
-      CellRec& R = s_cell[cl_own];
-      if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, mysum, cp.RH_max, true);
+    if (tid < ((nc + 31) & ~31)) {
+      for (int cl = tid; cl < nc; cl += T) {
+        CellRec& R = s_cell[cl];
+        if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, R.pad, cp.RH_max, true);
+      }
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
     if (sub == nsub) break;
     __syncthreads();
     // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (list)
-    for (;;) {
-      int q0 = 0;
-      if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 32;" : "=r"(q0) : "r"(ctr_addr) : "memory");
-      q0 = __shfl_sync(0xffffffffu, q0, 0);
-      if (q0 >= M) break;
+    for (int q0 = warp * 32; q0 < M; q0 += NW * 32) {   // static chunks (a shared counter costs an atomic, a shuffle and two S2R per chunk)
       const int e = q0 + lane;
       const bool valid = e < M;
       const int ec = min(e, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
@@ -833,8 +836,8 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       growth_r(r0, s, c, y0, f, dfr, t);
       n_eval += valid;
       const double two = 2.0 * dtp * f;
-      double lo = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
-      double hi = y0 + fmax(two, 0.0);              // eq. 19
+      double lo = dmax(rd2, y0 + dmin(two, 0.0));   // eq. 18
+      double hi = y0 + dmax(two, 0.0);              // eq. 19
       double r = r0, dprev = 0.0;
       double rq = r0, gq = 0.0, gpq = 1.0;   // previous iterate, g and dg/dr there (for the curvature estimate)
       int st;
@@ -892,7 +895,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
             // is d cm (16 (s/r)^2 + cm), cm = max(|c|, d/r): the error of the curvature estimate and the next order
             bool conv = (4.0 * d2 <= tol * rn) && (2.0 * d2 * d <= tol * (dprev * dprev));
             if (third) {
-              const double cmr = fmax(fabs(cc) * rn, d);
+              const double cmr = dmax(fabs(cc) * rn, d);
               conv = conv || (d * cmr * fma(cmr, rn, 16.0 * (sq * sq)) <= 0.5 * tol * (yn * rn));
             }
             rq = r; gq = gv; gpq = gp;
@@ -964,10 +967,10 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     }
   }
 
-  if (owner) {
-    const int c = c_first + cl_own;
+  for (int cl = tid; cl < nc; cl += T) {
+    const int c = c_first + cl;
     const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
-    const CellRec& R = s_cell[cl_own];
+    const CellRec& R = s_cell[cl];
     th_f.at(i, j, k) = R.th;
     rv_f.at(i, j, k) = R.rv;
     // air properties after the feedback, used by coalescence and sedimentation (v_term)

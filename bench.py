@@ -40,7 +40,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x 
 FLOP_PER_EVAL_F32 = 86.0
 FLOP_PER_SETUP_F32 = 60.0
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x fp32 FMA lanes x 2 x max SM clock = 74.4
-NCU_COND_DRAM_BYTES = 2.313708e9 + 0.553631e9
+NCU_COND_DRAM_BYTES = 2.317242e9 + 0.551745e9
 NCU_COND32_DRAM_BYTES = 1.509464e9 + 0.313273e9     # k_cond4f, the default workload with --real-bytes 4 --cond-arith 4
 
 
@@ -300,7 +300,7 @@ def main():
     roofline = {"kernel": ("k_cond4f (condensation, 10 fused substeps, fp32 sweep)" if f32 else "k_cond4 (condensation, 10 fused substeps)"),
                 "bound": "alu", "achieved": ach, "peak": peak_alu,
                 "unit": "TFLOP/s", "frac": ach / peak_alu, "traffic": (NCU_COND32_DRAM_BYTES if f32 else NCU_COND_DRAM_BYTES) if full3d and (f32 or a.real_bytes == 8) else None,
-                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/" + ("r1_k_cond4f_ncu_full.md" if f32 else "r1_k_cond4_v6_ncu_full.md"),
+                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/" + ("r1_k_cond4f_ncu_full.md" if f32 else "r1_k_cond4_v7_ncu_full.md"),
                 "peak_source": "derived: 148 SMs x %d fp%d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % ((128, 32) if f32 else (64, 64)),
                 "evals_per_sd_substep": evals / max(subs, 1),
                 "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),

@@ -54,6 +54,7 @@ def parse():
     ap.add_argument("--sd-per-cell", type=int, default=0)
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the horizontal grid (debugging only; reported in config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fp32-mode", action="store_true", help="skip the extra fp32-mode measurement of the default run")
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--cond-arith", type=int, default=8, choices=[8, 4], help="arithmetic of the condensation sweep; 4 = fp32 (needs --real-bytes 4)")
     ap.add_argument("--recycle", action="store_true", help="the paper's recycling of zero-multiplicity SDs (:641) instead of compaction only")
@@ -320,6 +321,24 @@ def main():
     if not a.no_cpu_baseline:
         v, cores, desc, _ = oracle_rate(wa, 2, 1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline:
+        # the same workload and step counts in the fp32 mode of configs[4] (fp32 state, fp32 condensation sweep; radii to
+        # 1e-4 instead of 1e-9): a second line of context, measured by the same code in a child process
+        try:
+            del p
+            torch.cuda.empty_cache()
+            cmd = [sys.executable, os.path.abspath(__file__), "--steps", str(a.steps), "--warmup", str(a.warmup), "--workload", a.workload,
+                   "--sd-per-cell", str(a.sd_per_cell), "--scale", str(a.scale), "--real-bytes", "4", "--cond-arith", "4", "--no-cpu-baseline"]
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+            out["fp32_mode"] = {k: d[k] for k in ("value", "unit", "ms_per_step", "dtype", "stage_ms", "gpu_launches")}
+            out["fp32_mode"]["state"] = d["config"]["state"]
+            out["fp32_mode"]["e2e"] = d["e2e"]["value"]
+            out["fp32_mode"]["roofline"] = {k: d["roofline"][k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac")}
+            out["fp32_mode"]["roofline_step_hbm_frac"] = d["roofline_step_hbm"]["frac"]
+            out["fp32_mode"]["parity"] = "radii within 1e-4 of the fp64 oracle (tests/test_parity_gpu.py::test_fp32_arithmetic_condensation_2d_3d_and_first_step)"
+        except Exception as ex:   # context only: never fails the bench line
+            out["fp32_mode"] = {"unavailable": str(ex)[:200]}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -649,7 +649,12 @@ def test_fp32_arithmetic_condensation_2d_3d_and_first_step():
     _fp32_case(rain_mix(W.cfg4_3d(sd_per_cell=64, nx=4, ny=3, nz=64, seed=42)), steps=3, arith=4)
     # haze only, from the initial condition at full height: the first step under RH_max = 1.05 (multi-root brackets)
     _fp32_case(W.cfg2_2d(sd_per_cell=64, nx=4, nz=75, seed=43), steps=3, arith=4)
-    # cells of ~1000 SDs (medium tile) and the fp64 fallback for one crowded cell
+    # sparse cells (8 SDs per cell: many cells per tile, the flat staging loop) and cells of ~1000 SDs (medium tile)
+    _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=8, nx=16, nz=40, seed=45)), steps=3, arith=4)
     _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=1000, nx=2, nz=3, seed=44), frac=0.3), steps=2, sstp_cond=3, arith=4)
+    # one crowded cell (beyond every tile kernel): solved in fp64 in place
+    w = rain_mix(W.cfg2_2d(sd_per_cell=1500, nx=2, nz=3, seed=46), frac=0.3)
+    w.state["x"] = w.state["x"] * 0.4
+    _fp32_case(w, steps=1, sstp_cond=2, arith=4)
     with pytest.raises(Exception):
         make_particles(W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1))[0].set_cond_arith(4)   # fp64 state: refused

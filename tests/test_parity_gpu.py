@@ -658,3 +658,68 @@ def test_fp32_arithmetic_condensation_2d_3d_and_first_step():
     _fp32_case(w, steps=1, sstp_cond=2, arith=4)
     with pytest.raises(Exception):
         make_particles(W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1))[0].set_cond_arith(4)   # fp64 state: refused
+
+
+# ----------------------------------------------------------------------------------------------- sync / async
+def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
+    """PAPER.md :816 and Figure 7 (:833-848): step_sync returns th, rv for the host model, step_async (coalescence +
+    movement, which touch neither) runs while the Eulerian solver advances th, rv.  Here the "solver" is a first-order
+    upstream shift of th, rv on a second stream, ordered after step_sync by an event.  Checked: step_async returns
+    to the host before its device work is done, the overlapped run equals the serialised one bit for bit, and it
+    matches the oracle driven the same way."""
+    b = binding()
+    w = W.cfg4_3d(sd_per_cell=64, nx=48, ny=48, nz=64, seed=61, device="cuda")
+
+    def solver(th, rv):   # stand-in for the host model's advection step (not part of libsdm)
+        th.copy_(0.75 * th + 0.25 * torch.roll(th, 1, 0))
+        rv.copy_(0.75 * rv + 0.25 * torch.roll(rv, 1, 0))
+
+    def run(overlap):
+        p, th, rv = make_particles(w)
+        po = b.make_opts(**w.opts)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        returned_early = 0
+        torch.cuda.synchronize()
+        for _ in range(3):
+            with torch.cuda.stream(s1):
+                p.step_sync(po, th, rv)
+                ready = torch.cuda.Event()
+                ready.record(s1)
+                p.step_async(po)
+                done = torch.cuda.Event()
+                done.record(s1)
+                returned_early += int(not done.query())
+            if not overlap:
+                s1.synchronize()
+            with torch.cuda.stream(s2):
+                s2.wait_event(ready)
+                solver(th, rv)
+            s1.wait_stream(s2)   # the next step_sync reads the solver's th, rv
+            with torch.cuda.stream(s1):
+                p.step_async_result()
+        torch.cuda.synchronize()
+        return sorted_by_id(p.export_state()), th.clone(), rv.clone(), returned_early
+
+    a, th_a, rv_a, early = run(overlap=True)
+    s, th_s, rv_s, _ = run(overlap=False)
+    assert early >= 2   # the host got control back while coalescence + movement were still running
+    for k in a:
+        np.testing.assert_array_equal(a[k], s[k])
+    assert torch.equal(th_a, th_s) and torch.equal(rv_a, rv_s)
+    # the oracle driven in the same order, on a sub-domain it finishes in seconds
+    wo = W.cfg4_3d(sd_per_cell=64, nx=4, ny=4, nz=64, seed=62)
+    o = make_oracle(wo, threads=4)
+    p, th, rv = make_particles(wo)
+    po, oo = b.make_opts(**wo.opts), oracle.make_opts(**wo.opts)
+    for _ in range(3):
+        p.step_sync(po, th, rv)
+        o.step_sync(oo)
+        p.step_async(po)
+        o.step_async(oo)
+        solver(th, rv)
+        oth, orv = o.get_fields()
+        oth, orv = torch.from_numpy(oth.reshape(th.shape).copy()), torch.from_numpy(orv.reshape(rv.shape).copy())
+        solver(oth, orv)
+        o.set_fields(th=oth.numpy().ravel(), rv=orv.numpy().ravel())
+    compare_states(p, o)
+    compare_fields(th, rv, o)

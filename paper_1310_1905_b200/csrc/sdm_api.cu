@@ -18,6 +18,10 @@ constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are will
 #define SDM_COND_TILE_TARGET 660.0
 #endif
 constexpr double kCondTileTarget = SDM_COND_TILE_TARGET;   // SDs per condensation tile (mean); 5 sigma above fits the 800 slots of k_cond4
+#ifndef SDM_COND32_TILE_TARGET
+#define SDM_COND32_TILE_TARGET 660.0
+#endif
+constexpr double kCond32TileTarget = SDM_COND32_TILE_TARGET;   // the same for the fp32-arithmetic kernel (sdm_set_cond_arith)
 constexpr double kCondMaxCpb = 128.0;       // one thread per cell of the tile
 }
 
@@ -429,7 +433,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   CK(cudaMemsetAsync(ctx->d_info + 2, 0, sizeof(u32), st));
   CK(cudaMemsetAsync(ctx->d_info + 4, 0, 4 * sizeof(u32), st));
   // condensation tiles: about kCondTileTarget SDs per CTA at the occupancy seen before this step
-  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, kCondTileTarget * g.ncell / std::max<double>(ctx->nslots, 1.0)));
+  const bool arith32 = ctx->cond_arith == 4 && ctx->o.real_bytes == 4;
+  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, (arith32 ? kCond32TileTarget : kCondTileTarget) * g.ncell / std::max<double>(ctx->nslots, 1.0)));
   t_begin(ctx, SDM_STAGE_HIST, st);
   if (ctx->o.real_bytes == 8) launch_cellhist(view<double>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
   else launch_cellhist(view<float>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
@@ -476,10 +481,10 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   if (op->cond) {
     // the most preferred tile kernel (small, medium, large) any candidate tile size fits, with the largest such
     // tile; else one cell per CTA in place in global memory
-    int cpb = 1, variant = cond_variant(1, (int)ctx->max_nc);
+    int cpb = 1, variant = arith32 ? cond_variant_f32(1, (int)ctx->max_nc) : cond_variant(1, (int)ctx->max_nc);
     for (int k = 3; k >= 0; --k) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
-      const int v = cond_variant(cand, (int)ctx->tile_max[k]);
+      const int v = arith32 ? cond_variant_f32(cand, (int)ctx->tile_max[k]) : cond_variant(cand, (int)ctx->tile_max[k]);
       if (v && (variant == 0 || v <= variant)) { cpb = cand; variant = v; }
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
@@ -487,7 +492,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     if (ctx->o.real_bytes == 8)
       CK(launch_cond(cpb, variant, view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
                      rvf, ctx->cf, cp, ctx->cnt, st));
-    else if (ctx->cond_arith == 4 && variant != 0)
+    else if (arith32 && variant != 0)
       CK(launch_cond_f32(cpb, variant, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
     else
       CK(launch_cond(cpb, variant, view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,

@@ -1389,6 +1389,12 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
 #ifndef SDM_COND32_MINB
 #define SDM_COND32_MINB 8  // CTAs per SM of the fp32-arithmetic small tile kernel
 #endif
+#ifndef SDM_COND32_CAP
+#define SDM_COND32_CAP 800 // its SD slots
+#endif
+#ifndef SDM_COND32_T
+#define SDM_COND32_T 128   // its threads
+#endif
 using CondSmall = Cond4<SDM_COND_CAP, 128>;
 using CondMedium = Cond4<1280, 256>;   // 3 CTAs of 256 threads per SM: cells of ~1000 SDs
 using CondLarge = Cond4<4096, 512>;    // one CTA of 512 threads per SM: cells of thousands of SDs
@@ -1425,13 +1431,23 @@ static cudaError_t launch_cond4f(size_t smem, int grid, const SdArraysT<float>& 
   return cudaGetLastError();
 }
 
-// fp32-arithmetic condensation for the tile variants 1..3 of cond_variant (same tiles as the fp64 kernels, which need
-// more shared memory, so whatever they fit, these fit); variant 0 (one crowded cell in global memory) has no fp32 form
+// as cond_variant, for the fp32-arithmetic tile kernels (28 instead of 52 bytes of shared memory per SD)
+using Cond32Small = Cond4F<SDM_COND32_CAP, SDM_COND32_T>;
+int cond_variant_f32(int cpb, int need) {
+  constexpr size_t small_budget = (228 * 1024 - SDM_COND32_MINB * 1024) / SDM_COND32_MINB;
+  if (cpb <= 128 && need <= SDM_COND32_CAP && Cond32Small::smem(cpb) <= small_budget) return 1;
+  if (cpb <= 256 && need <= 1280 && Cond4F<1280, 256>::smem(cpb) <= (228 * 1024 - 4 * 1024) / 4) return 2;
+  if (cpb <= 512 && need <= 4096 && Cond4F<4096, 512>::smem(cpb) <= 227 * 1024) return 3;
+  return 0;
+}
+
+// fp32-arithmetic condensation for the tile variants 1..3 of cond_variant_f32; variant 0 (one crowded cell in global
+// memory) has no fp32 form
 cudaError_t launch_cond_f32(int cpb, int variant, const SdArraysT<float>& a, const u16* rank, const u32* seg, const Grid& g,
                             Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st) {
   const int grid = (g.ncell + cpb - 1) / cpb;
   if (variant == 1)
-    return launch_cond4f<SDM_COND_CAP, 128, SDM_COND32_MINB>(Cond4F<SDM_COND_CAP, 128>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
+    return launch_cond4f<SDM_COND32_CAP, SDM_COND32_T, SDM_COND32_MINB>(Cond32Small::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
   if (variant == 2) return launch_cond4f<1280, 256, 4>(Cond4F<1280, 256>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
   if (variant == 3) return launch_cond4f<4096, 512, 1>(Cond4F<4096, 512>::smem(cpb), grid, a, rank, seg, g, th, rv, cf, cp, cnt, cpb, st);
   return cudaErrorInvalidValue;

@@ -51,7 +51,8 @@ cudaError_t launch_cond(int cpb, int variant, const SdArraysT<R>& a, const SdArr
                         const Grid& g, Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt,
                         cudaStream_t st);
 size_t cond_smem_bytes(int cpb, int cap);
-// the tile kernels (variant 1..3) with the sweep in fp32 arithmetic (sdm_set_cond_arith; fp32 state only)
+// the tile kernels (variant 1..3 of cond_variant_f32) with the sweep in fp32 arithmetic (sdm_set_cond_arith; fp32 state only)
+int cond_variant_f32(int cpb, int need);
 cudaError_t launch_cond_f32(int cpb, int variant, const SdArraysT<float>& a, const u16* rank, const u32* seg, const Grid& g,
                             Field th, Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, cudaStream_t st);
 void launch_thermo(const Grid& g, Field th, Field rv, const CellFields& cf, cudaStream_t st);

@@ -492,7 +492,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     if (ctx->o.real_bytes == 8)
       CK(launch_cond(cpb, variant, view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
                      rvf, ctx->cf, cp, ctx->cnt, st));
-    else if (arith32 && variant != 0)
+    else if (arith32 && variant != 0 && op->sstp_cond <= 500)   // (its packed per-lane counters hold 500 substeps)
       CK(launch_cond_f32(cpb, variant, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, thf, rvf, ctx->cf, cp, ctx->cnt, st));
     else
       CK(launch_cond(cpb, variant, view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,

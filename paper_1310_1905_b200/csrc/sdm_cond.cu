@@ -1192,7 +1192,9 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
       cidx[e] = (u16)cl;
     }
   }
-  unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
+  // per-lane counters, packed so that the sweep holds one register: evaluations (low 20 bits: a lane stays far below 2^20 per
+  // launch) and solved SD-substeps (high 12: at most ~7 per substep and lane, sstp_cond <= 500); the slow list's counters are touched only there
+  unsigned n_es = 0, n_ill = 0, n_slow = 0;
   const float dtp = (float)cp.dtp;
   const int nsub = M > 0 ? cp.sstp : 0;
   for (int sub = 0; sub <= nsub; ++sub) {
@@ -1234,7 +1236,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
       sd_setup_f(r0, c, s);
       float f, dfr, B, t;
       growth_f32(r0, s, c, f, dfr, B, t);
-      n_eval += valid;
+      n_es += valid;
       const float y0 = r0 * r0, r02 = r0 + r0;
       const float dtf = dtp * f, two = dtf + dtf;
       // eq. 18-19 in D = y - y0
@@ -1264,7 +1266,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
         if (st == 0) {
           const float r = r0 + d;
           growth_f32(r, s, c, f, dfr, B, t);
-          ++n_eval;
+          ++n_es;
           const float D = d * (r02 + d);
           const float gv = fmaf(-dtp, f, D);
           const float gp = fmaf(-dtp, dfr, r + r);
@@ -1284,7 +1286,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
       if (valid && st == 1) {
         s_con[e] = s_dn[e] * (d * fmaf(3.0f * r0, r0 + d, d * d));   // N (r^3 - r0^3) without cancellation
         s_r[e] = r0 + d;
-        ++n_sub;
+        n_es += 0x100000u;
       }
       const unsigned need = __ballot_sync(0xffffffffu, st == 2);
       if (need) {   // warp-aggregated append to the tile's slow list
@@ -1327,10 +1329,10 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
           cond_solve(y0, rd2, rd3, krd3, c, cp.dtp, 200, y1, ill, ev);
           if (per_warp && lane != 0) { ill = 0; ev = 0; }
         }
-        n_ill += ill; n_eval += ev;
+        n_ill += ill; n_es += ev;
         if (!per_warp || lane == 0) {
           const double r1 = sqrt(y1);
-          ++n_sub; ++n_slow;
+          n_es += 0x100000u; ++n_slow;
           s_con[e] = (float)((double)s_dn[e] * (r1 * r1 * r1 - r0 * y0) * 1e18);
           s_r[e] = (float)(r1 * 1e6);
         }
@@ -1364,7 +1366,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
       a.rw2[s] = r * r;
     }
   }
-  unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub, v3 = n_slow;
+  unsigned v0 = n_ill, v1 = n_es & 0xfffffu, v2 = n_es >> 20, v3 = n_slow;
 #pragma unroll
   for (int d = 16; d >= 1; d >>= 1) {
     v0 += __shfl_xor_sync(0xffffffffu, v0, d);

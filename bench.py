@@ -158,6 +158,11 @@ def oracle_rate(wa, steps, warmup, seed=42):
         n += o.n_live()
         o.step(oo)
     dt = time.perf_counter() - t0
+    # the same sample on ONE thread (the serial oracle is the stated baseline, the OpenMP one the fair one)
+    o.set_threads(1)
+    n1, t1 = o.n_live(), time.perf_counter()
+    o.step(oo)
+    oracle_rate.one_thread = n1 / (time.perf_counter() - t1)
     desc = (f"{w.name}: {w.n_sd} SDs in {sub['nx']}x{max(sub['ny'], 1)}x{sub['nz']} full columns of the same recipe, "
             f"{steps} steps after {warmup} warm-up, OpenMP over cells")
     return n / dt, cores, desc, dt / steps * 1e3
@@ -320,7 +325,8 @@ def main():
         out["recycled"] = st1["recycled"] - st0["recycled"]
     if not a.no_cpu_baseline:
         v, cores, desc, _ = oracle_rate(wa, 2, 1)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                               "value_1_thread": getattr(oracle_rate, "one_thread", None)}
     if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline:
         # the same workload and step counts in the fp32 mode of configs[4] (fp32 state, fp32 condensation sweep; radii to
         # 1e-4 instead of 1e-9): a second line of context, measured by the same code in a child process

@@ -723,3 +723,24 @@ def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
         o.set_fields(th=oth.numpy().ravel(), rv=orv.numpy().ravel())
     compare_states(p, o)
     compare_fields(th, rv, o)
+
+
+def test_fp32_arithmetic_root_selection_scan_of_independent_sds():
+    """The scan of test_root_selection_scan_of_independent_sds with the fp32 sweep: r_d from 1 nm to 2 um, sizes from
+    barely wet to 3000 r_d, kappa 0.05-1.55, RH 0.3-1.05, multiplicity 1 (no feedback).  Whatever the fp32 certificate
+    lets through must land on the root the paper's bisection defines, to 1e-4; the rest goes to the fp64 list."""
+    seed, nx, nz, sd = 8, 24, 24, 64
+    w = W.cfg2_2d(sd_per_cell=sd, nx=nx, nz=nz, seed=seed)
+    idx = torch.arange(w.n_sd, dtype=torch.int64)
+    u1, u2, u3 = (W.hash_uniform(seed, 200 + k, idx) for k in range(3))
+    rd = torch.exp(np.log(1e-9) + u1 * (np.log(2e-6) - np.log(1e-9)))
+    w.state["rd3"] = rd ** 3
+    w.state["rw2"] = (rd * torch.exp(1e-4 + u2 * u2 * np.log(3e3))) ** 2
+    w.state["kappa"] = torch.where(u3 < 0.5, torch.full_like(u3, 0.61), 0.05 + 1.5 * u3)
+    w.state["n"] = torch.ones_like(w.state["n"])
+    ci = torch.arange(nx, dtype=torch.float64)[:, None].expand(nx, nz)
+    w.rv = w.rv * (0.35 + 0.95 * ci / (nx - 1))
+    p, o = _fp32_case(w, steps=2, arith=4, coal=False, adve=False, sedi=False)
+    sp = p.stats()
+    assert sp["cond_slow"] > 0.02 * sp["sd_substeps"]       # the fp64 list was exercised
+    assert sp["cond_slow"] < 0.5 * sp["sd_substeps"]        # ... and the fp32 sweep solved most

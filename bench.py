@@ -31,6 +31,19 @@ UNIT = "SD-steps/s"
 #    fp64 instruction sequences).
 BYTES_PER_SD_STEP = {(3, 8): 350.0, (2, 8): 350.0 - 16.0 - 8.0,      # fp64 state: SURVEY.md 8d
                      (3, 4): 232.0, (2, 4): 232.0 - 8.0 - 4.0}       # fp32 state: the six reals at 4 bytes
+
+
+def stage_bytes(ndim, rb):
+    """Algorithmic HBM bytes per SD of each timed stage (SURVEY.md 8d: one pass over the attributes a stage must touch;
+    fp64 3D: 32 + 20 + 124 + 40 + 132 = 348).  rb = bytes of a real attribute, ndim = stored coordinates."""
+    state = 8 + (3 + ndim) * rb + 4                      # n, rw2, rd3, kappa, coordinates, id
+    return {"hist": ndim * rb + 8,                       # a1: read the position, write cell + key
+            "rank": 20.0,                                # a2: sort within the cell (SURVEY's figure)
+            "scatter": 2 * state + 4,                    # a3: read state + permutation, write state
+            "cond": 8 + 3 * rb + rb,                     # a4: read n, rw2, rd3, kappa, write rw2
+            "coal_move": 2 * (8 + 3 * rb) + (ndim * rb + rb + 4) + (ndim * rb + 8)}   # a5 + a6
+
+
 FLOP_PER_EVAL = 190.0
 FLOP_PER_SETUP = 150.0
 FLOP_PER_CORRECTION = 28.0   # third-order correction of every Newton step after the first (curvature from the last two iterates)
@@ -315,10 +328,14 @@ def main():
     hbm = {"bound": "hbm", "achieved": bytes_step / (step_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
            "frac": bytes_step / (step_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
            "algorithmic_bytes_per_sd_step": BYTES_PER_SD_STEP[(ndim, a.real_bytes)]}
+    sb = stage_bytes(ndim, a.real_bytes)
+    roofline_stages = {k: {"bytes_per_sd": sb[k], "achieved": sb[k] * (sd_steps / a.steps) / (stage_ms[k] * 1e-3) / 1e9, "unit": "GB/s",
+                           "frac": sb[k] * (sd_steps / a.steps) / (stage_ms[k] * 1e-3) / 1e9 / hbm_peak}
+                       for k in sb if stage_ms.get(k, 0.0) > 0}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
            "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if a.cond_arith == 4 else "f64",
            "data": "synthetic", "config": dict(config_of(wa), state="fp64" if a.real_bytes == 8 else ("fp32 storage, fp32 condensation sweep (thermodynamics, feedback, coalescence probability, movement in fp64)" if a.cond_arith == 4 else "fp32 storage, fp64 arithmetic")), "clocks": clocks, "e2e": e2e,
-           "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm,
+           "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm, "roofline_stages_hbm": roofline_stages,
            "stage_ms": stage_ms, "n_sd_live": p.n_sd(), "n_sd_initial": n_sd0}
     if a.recycle:
         out["config"]["recycling"] = "on (PAPER.md :641)"

@@ -282,21 +282,37 @@ def test_edge_cases_empty_single_and_errors():
         b.Particles(nx=2, nz=2, max_sd=0)
 
 
-def test_runs_are_reproducible_bit_for_bit():
-    """Storage order inside a cell depends on atomics, results must not."""
+@pytest.mark.parametrize("mode", ["fp64", "fp32_sweep_recycle", "3d_larger"])
+def test_runs_are_reproducible_bit_for_bit(mode):
+    """Storage order inside a cell and the order of list appends depend on atomics, results must not (this is also the
+    race detector of the tile kernels: compute-sanitizer is not available on the GPU pool)."""
     b = binding()
-    w = rain_mix(W.cfg2_2d(sd_per_cell=32, nx=12, nz=12, seed=17))
+    if mode == "3d_larger":
+        w = rain_mix(W.cfg4_3d(sd_per_cell=64, nx=16, ny=16, nz=64, seed=18))
+    else:
+        w = rain_mix(W.cfg2_2d(sd_per_cell=32, nx=12, nz=12, seed=17))
     outs = []
-    for _ in range(2):
-        p, th, rv = make_particles(w)
+    for _ in range(3 if mode != "3d_larger" else 2):
+        if mode == "fp32_sweep_recycle":
+            st32 = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32).cuda()) for k, v in w.state.items()}
+            p = b.Particles(max_sd=w.n_sd, sd_conc_mean=w.meta["sd_per_cell"], real_bytes=4, **w.init)
+            cs = [c.cuda() for c in w.courants] + [None] * (3 - len(w.courants))
+            p.init_from_arrays(w.rhod.cuda(), w.state["n"].cuda(), st32["rw2"], st32["rd3"], st32["kappa"], st32["x"], st32["y"], st32["z"],
+                               w.state["id"].cuda(), courant_1=cs[0], courant_2=cs[1], courant_3=cs[2])
+            th, rv = w.th.cuda().clone(), w.rv.cuda().clone()
+            p.set_cond_arith(4)
+            p.set_recycle(True)
+        else:
+            p, th, rv = make_particles(w)
         po = b.make_opts(**w.opts)
-        for _ in range(3):
+        for _ in range(4):
             p.step_sync(po, th, rv)
             p.step_async(po)
         outs.append((sorted_by_id(p.export_state()), th.clone(), rv.clone()))
-    for k in outs[0][0]:
-        np.testing.assert_array_equal(outs[0][0][k], outs[1][0][k])
-    assert torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])
+    for o in outs[1:]:
+        for k in outs[0][0]:
+            np.testing.assert_array_equal(outs[0][0][k], o[0][k])
+        assert torch.equal(outs[0][1], o[1]) and torch.equal(outs[0][2], o[2])
 
 
 # ------------------------------------------------------------------------------------ full size (bench.py's launch)

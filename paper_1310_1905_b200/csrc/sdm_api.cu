@@ -29,6 +29,7 @@ struct sdm_ctx {
   sdm_opts_init o{};
   Grid g{};
   int device = 0;
+  int n_sm = 148;
   u64 cap_sd = 0;
   SdArrays buf[2]{};
   int cur = 0;
@@ -197,6 +198,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   ctx = new sdm_ctx();
   ctx->o = *o;
   ctx->device = dev;
+  ctx->n_sm = prop.multiProcessorCount;
   Grid& g = ctx->g;
   g.NX = std::max(o->nx, 1); g.NY = std::max(o->ny, 1); g.NZ = std::max(o->nz, 1);
   g.hx = o->nx > 0; g.hy = o->ny > 0; g.hz = o->nz > 0;
@@ -434,7 +436,14 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   CK(cudaMemsetAsync(ctx->d_info + 4, 0, 4 * sizeof(u32), st));
   // condensation tiles: about kCondTileTarget SDs per CTA at the occupancy seen before this step
   const bool arith32 = ctx->cond_arith == 4 && ctx->o.real_bytes == 4;
-  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, (arith32 ? kCond32TileTarget : kCondTileTarget) * g.ncell / std::max<double>(ctx->nslots, 1.0)));
+  double tile_target = arith32 ? kCond32TileTarget : kCondTileTarget;
+  {  // a population that does not fill one wave of resident CTAs (5 per SM, 8 for the fp32 sweep): smaller tiles, so
+     // that every SM gets its share (configs[1]: 281 full-size tiles on 740 slots; measured 0.288 -> 0.250 ms per step;
+     // beyond one wave smaller tiles lose more to their fixed costs than the balance gains)
+    const double wave = (double)ctx->n_sm * (arith32 ? 8 : 5);
+    if ((double)ctx->nslots / tile_target < wave) tile_target = std::max(128.0, (double)ctx->nslots / wave);
+  }
+  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, tile_target * g.ncell / std::max<double>(ctx->nslots, 1.0)));
   t_begin(ctx, SDM_STAGE_HIST, st);
   if (ctx->o.real_bytes == 8) launch_cellhist(view<double>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
   else launch_cellhist(view<float>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);

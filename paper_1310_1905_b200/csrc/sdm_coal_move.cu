@@ -472,22 +472,38 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
   }
 }
 
+// Tile capacity and CTAs per SM by storage type (swept on the 3D workload at 16.7 M SDs; the kernel is bound by the latency
+// of its IEEE divisions and square roots, so resident warps count): fp64 state 58 B of shared memory per SD -> 672 slots,
+// 6 CTAs per SM, 78 registers (816 slots / 5 CTAs: +10 %); fp32 state 38 B per SD -> 816 slots, 7 CTAs, 72 registers
+// (5 CTAs: +23 %).  No spills in either.
 #ifndef SDM_COAL_CAP
-#define SDM_COAL_CAP 816
-#define SDM_COAL_T 128
-#define SDM_COAL_MINB 5
+#define SDM_COAL_CAP 672
+#define SDM_COAL_MINB 6
 #endif
+#ifndef SDM_COAL_CAP32
+#define SDM_COAL_CAP32 816
+#define SDM_COAL_MINB32 7
+#endif
+#ifndef SDM_COAL_T
+#define SDM_COAL_T 128
+#endif
+template <typename R> constexpr int coal_minb() { return sizeof(R) == 4 ? SDM_COAL_MINB32 : SDM_COAL_MINB; }
+template <typename R> constexpr int coal_cap() { return sizeof(R) == 4 ? SDM_COAL_CAP32 : SDM_COAL_CAP; }
 // can a tile of cpb cells whose most populated instance holds `need` SDs run in k_coal_move_tile?
+template <typename R>
+static bool coal_tile_fits_t(int cpb, int need) {
+  const size_t smem = CoalTile<coal_cap<R>(), SDM_COAL_T, R>::smem(cpb);
+  return need + cpb <= coal_cap<R>() && cpb <= 4096 && smem <= (size_t)(228 * 1024 - coal_minb<R>() * 1024) / coal_minb<R>();
+}
 bool coal_tile_fits(int cpb, int need, int real_bytes) {
-  const size_t smem = real_bytes == 8 ? CoalTile<SDM_COAL_CAP, SDM_COAL_T, double>::smem(cpb) : CoalTile<SDM_COAL_CAP, SDM_COAL_T, float>::smem(cpb);
-  return need + cpb <= SDM_COAL_CAP && cpb <= 4096 && smem <= (size_t)(228 * 1024 - SDM_COAL_MINB * 1024) / SDM_COAL_MINB;
+  return real_bytes == 8 ? coal_tile_fits_t<double>(cpb, need) : coal_tile_fits_t<float>(cpb, need);
 }
 template <typename R>
 cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                   const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
                                   const Counters& cnt, cudaStream_t st) {
-  const size_t smem = CoalTile<SDM_COAL_CAP, SDM_COAL_T, R>::smem(cpb);
-  auto kern = k_coal_move_tile<SDM_COAL_CAP, SDM_COAL_T, SDM_COAL_MINB, R>;
+  const size_t smem = CoalTile<coal_cap<R>(), SDM_COAL_T, R>::smem(cpb);
+  auto kern = k_coal_move_tile<coal_cap<R>(), SDM_COAL_T, coal_minb<R>(), R>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cpb);

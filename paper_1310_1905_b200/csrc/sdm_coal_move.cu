@@ -244,6 +244,7 @@ struct __align__(8) CoalCell {
 
 template <int CAP, int T, typename R>
 struct CoalTile {   // u64 n; R rw2, x, y, z; double vt; u32 id; u16 inv
+  static_assert(CAP % 16 == 0, "the arrays of the tile follow one another in shared memory: keep every one of them 16-byte aligned");
   static constexpr size_t fixed_bytes = (size_t)CAP * (8 + 4 * sizeof(R) + 8 + 4 + 2);
   static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CoalCell) + (size_t)(cpb + 1) * 8 + 16; }
 };
@@ -473,12 +474,12 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
 }
 
 // Tile capacity and CTAs per SM by storage type (swept on the 3D workload at 16.7 M SDs; the kernel is bound by the latency
-// of its IEEE divisions and square roots, so resident warps count): fp64 state 58 B of shared memory per SD -> 672 slots,
-// 6 CTAs per SM, 78 registers (816 slots / 5 CTAs: +10 %); fp32 state 38 B per SD -> 816 slots, 7 CTAs, 72 registers
-// (5 CTAs: +23 %).  No spills in either.
+// of its IEEE divisions and square roots, so resident warps count): fp64 state 58 B of shared memory per SD -> 560 slots,
+// 7 CTAs per SM, 72 registers (672 / 6: +7 %, 816 / 5: +17 %, 448 / 8: +7 %); fp32 state 38 B per SD -> 816 slots, 7 CTAs,
+// 72 registers (5 CTAs: +23 %, 704 / 8: the same, 560 / 10: +9 %).  No spills in either.
 #ifndef SDM_COAL_CAP
-#define SDM_COAL_CAP 672
-#define SDM_COAL_MINB 6
+#define SDM_COAL_CAP 560
+#define SDM_COAL_MINB 7
 #endif
 #ifndef SDM_COAL_CAP32
 #define SDM_COAL_CAP32 816

@@ -18,6 +18,9 @@ constexpr size_t kSmemLimit = 200 * 1024;   // dynamic shared memory we are will
 #define SDM_COND_TILE_TARGET 660.0
 #endif
 constexpr double kCondTileTarget = SDM_COND_TILE_TARGET;   // SDs per condensation tile (mean); 5 sigma above fits the 800 slots of k_cond4
+#ifndef SDM_SMALL_WAVES
+#define SDM_SMALL_WAVES 1.0
+#endif
 #ifndef SDM_COND32_TILE_TARGET
 #define SDM_COND32_TILE_TARGET 660.0
 #endif
@@ -441,7 +444,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
      // that every SM gets its share (configs[1]: 281 full-size tiles on 740 slots; measured 0.288 -> 0.250 ms per step;
      // beyond one wave smaller tiles lose more to their fixed costs than the balance gains)
     const double wave = (double)ctx->n_sm * (arith32 ? 8 : 5);
-    if ((double)ctx->nslots / tile_target < wave) tile_target = std::max(128.0, (double)ctx->nslots / wave);
+    if ((double)ctx->nslots / tile_target < wave) tile_target = std::max(128.0, (double)ctx->nslots / (SDM_SMALL_WAVES * wave));
   }
   ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, tile_target * g.ncell / std::max<double>(ctx->nslots, 1.0)));
   t_begin(ctx, SDM_STAGE_HIST, st);

@@ -128,15 +128,21 @@ __global__ void __launch_bounds__(256) k_scatter(SdArraysT<R> src, SdArraysT<R> 
   if (i >= *d_nslots) return;
   const u32 c = cell[i];
   if (c == CELL_DEAD) return;
-  const u32 d = seg[c] + off[i];
-  dst.n[d] = src.n[i];
-  dst.rw2[d] = src.rw2[i];
-  dst.rd3[d] = src.rd3[i];
-  dst.kappa[d] = src.kappa[i];
-  if (g.hx) dst.x[d] = src.x[i];
-  if (g.hy) dst.y[d] = src.y[i];
-  if (g.hz) dst.z[d] = src.z[i];
-  dst.id[d] = src.id[i];
+  // all loads first: the two copies of the state are not declared disjoint, so a store between two loads would order them
+  const u32 o = off[i], sg = seg[c];
+  const u64 n = src.n[i];
+  const R rw2 = src.rw2[i], rd3 = src.rd3[i], kappa = src.kappa[i];
+  const R x = g.hx ? src.x[i] : R(0), y = g.hy ? src.y[i] : R(0), z = g.hz ? src.z[i] : R(0);
+  const u32 id = src.id[i];
+  const u32 d = sg + o;
+  dst.n[d] = n;
+  dst.rw2[d] = rw2;
+  dst.rd3[d] = rd3;
+  dst.kappa[d] = kappa;
+  if (g.hx) dst.x[d] = x;
+  if (g.hy) dst.y[d] = y;
+  if (g.hz) dst.z[d] = z;
+  dst.id[d] = id;
 }
 
 // ---- a2 (second level): rank of every SD inside its cell under (Philox key, id) ----------------------

@@ -16,7 +16,11 @@ __global__ void __launch_bounds__(256) k_cellhist(SdArraysT<R> a, const u32* __r
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
   const u32 nslots = *d_nslots;
   u32 c = CELL_DEAD;
-  if (i < nslots && a.n[i] != 0) c = cell_of(g, g.hx ? a.x[i] : 0.0, g.hy ? a.y[i] : 0.0, g.hz ? a.z[i] : 0.0);
+  if (i < nslots) {   // position loads do not wait for the multiplicity
+    const u64 n = a.n[i];
+    const double x = g.hx ? (double)a.x[i] : 0.0, y = g.hy ? (double)a.y[i] : 0.0, z = g.hz ? (double)a.z[i] : 0.0;
+    if (n != 0) c = cell_of(g, x, y, z);
+  }
   // lanes that fall in the same cell take consecutive slots with one atomic
   const u32 peers = __match_any_sync(0xffffffffu, c);
   const int lane = threadIdx.x & 31;
@@ -126,15 +130,16 @@ __global__ void __launch_bounds__(256) k_scatter(SdArraysT<R> src, SdArraysT<R> 
                                                  const u32* __restrict__ seg) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= *d_nslots) return;
+  // all loads first, and none of them behind the test for a dead SD: the two copies of the state are not declared
+  // disjoint, so a store between two loads would order them
   const u32 c = cell[i];
-  if (c == CELL_DEAD) return;
-  // all loads first: the two copies of the state are not declared disjoint, so a store between two loads would order them
-  const u32 o = off[i], sg = seg[c];
+  const u32 o = off[i];
   const u64 n = src.n[i];
   const R rw2 = src.rw2[i], rd3 = src.rd3[i], kappa = src.kappa[i];
   const R x = g.hx ? src.x[i] : R(0), y = g.hy ? src.y[i] : R(0), z = g.hz ? src.z[i] : R(0);
   const u32 id = src.id[i];
-  const u32 d = sg + o;
+  if (c == CELL_DEAD) return;
+  const u32 d = seg[c] + o;
   dst.n[d] = n;
   dst.rw2[d] = rw2;
   dst.rd3[d] = rd3;

@@ -162,7 +162,9 @@ int sdm_step_async_result(sdm_ctx* ctx, double* rain_flux);
 
 /* The same step for a caller whose Eulerian fields live in HOST memory (the paper's CPU solver,
  * :845-848): copies th, rv (dense C order, nx*ny*nz doubles, pinned or pageable) to the device,
- * runs step_sync, copies them back, runs step_async.  Blocking; *rain_flux as above. */
+ * runs step_sync, copies them back, runs step_async.  The copies travel on a stream of the library's own: in while
+ * the sort runs (the condensation kernel waits for them), out while coalescence and movement run (with pinned
+ * buffers; pageable ones serialise in the driver).  Blocking; *rain_flux as above. */
 int sdm_step_host(sdm_ctx* ctx, const sdm_opts* opts, double* th_host, double* rv_host,
                   double* rain_flux, void* stream);
 

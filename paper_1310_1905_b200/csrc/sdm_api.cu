@@ -65,6 +65,10 @@ struct sdm_ctx {
   int kfast = 4;
   int cond_arith = 8;        // 8: fp64 arithmetic in the condensation sweep; 4: fp32 (real_bytes == 4 only)
   cudaEvent_t ev_info = nullptr, ev_async = nullptr;
+  // sdm_step_host: th, rv travel on a stream of their own, overlapped with the sort (in) and with coalescence + movement (out)
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copy_go = nullptr, ev_h2d = nullptr, ev_fields = nullptr;
+  bool wait_h2d = false;
   cudaStream_t last_stream = nullptr;
   u64 launches = 0;
   double dry_lo = 0, dry_hi = 1e300, wet_lo = 0, wet_hi = 1e300;
@@ -307,6 +311,7 @@ void sdm_destroy(sdm_ctx* ctx) {
   cudaFree(ctx->d_effR); cudaFree(ctx->d_effq); cudaFree(ctx->d_efftab);
   if (ctx->h_info) cudaFreeHost(ctx->h_info);
   if (ctx->h_rec) cudaFreeHost(ctx->h_rec);
+  if (ctx->copy_stream) { cudaStreamDestroy(ctx->copy_stream); cudaEventDestroy(ctx->ev_copy_go); cudaEventDestroy(ctx->ev_h2d); cudaEventDestroy(ctx->ev_fields); }
   cudaFree(ctx->rec_dead); cudaFree(ctx->rec_cand); cudaFree(ctx->rec_hist); cudaFree(ctx->rec_info);
   if (ctx->ev_info) cudaEventDestroy(ctx->ev_info);
   if (ctx->ev_async) cudaEventDestroy(ctx->ev_async);
@@ -490,6 +495,10 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     ctx->launches++;
   }
   ctx->have_order = true;
+  if (ctx->wait_h2d) {   // sdm_step_host: th, rv arrive on the copy stream while the sort runs
+    CK(cudaStreamWaitEvent(st, ctx->ev_h2d, 0));
+    ctx->wait_h2d = false;
+  }
   if (op->cond) {
     // the most preferred tile kernel (small, medium, large) any candidate tile size fits, with the largest such
     // tile; else one cell per CTA in place in global memory
@@ -579,19 +588,35 @@ int sdm_step_host(sdm_ctx* ctx, const sdm_opts* op, double* th_host, double* rv_
   cudaStream_t st = (cudaStream_t)stream;
   const Grid& g = ctx->g;
   const size_t bytes = sizeof(double) * g.ncell;
-  CK(cudaMemcpyAsync(ctx->th_dense, th_host, bytes, cudaMemcpyHostToDevice, st));
-  CK(cudaMemcpyAsync(ctx->rv_dense, rv_host, bytes, cudaMemcpyHostToDevice, st));
+  if (!ctx->copy_stream) {
+    CK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&ctx->ev_copy_go, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&ctx->ev_h2d, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&ctx->ev_fields, cudaEventDisableTiming));
+  }
+  cudaStream_t cs = ctx->copy_stream;
+  // in: after whatever the caller's stream still does with the dense copies; the condensation kernel waits for ev_h2d
+  CK(cudaEventRecord(ctx->ev_copy_go, st));
+  CK(cudaStreamWaitEvent(cs, ctx->ev_copy_go, 0));
+  CK(cudaMemcpyAsync(ctx->th_dense, th_host, bytes, cudaMemcpyHostToDevice, cs));
+  CK(cudaMemcpyAsync(ctx->rv_dense, rv_host, bytes, cudaMemcpyHostToDevice, cs));
+  CK(cudaEventRecord(ctx->ev_h2d, cs));
+  ctx->wait_h2d = true;
   sdm_arrinfo th{ctx->th_dense, {0, 0, 0}}, rv{ctx->rv_dense, {0, 0, 0}}, none{nullptr, {0, 0, 0}};
   int idx = 0;   // dense C-order strides over the present dimensions
   const long long sx = (long long)g.NY * g.NZ, sy = g.NZ, sz = 1;
   if (g.hx) { th.strides[idx] = rv.strides[idx] = sx; ++idx; }
   if (g.hy) { th.strides[idx] = rv.strides[idx] = sy; ++idx; }
   if (g.hz) { th.strides[idx] = rv.strides[idx] = sz; ++idx; }
-  if (int rc = sdm_step_sync(ctx, op, th, rv, none, none, none, none, stream)) return rc;
-  CK(cudaMemcpyAsync(th_host, ctx->th_dense, bytes, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(rv_host, ctx->rv_dense, bytes, cudaMemcpyDeviceToHost, st));
+  if (int rc = sdm_step_sync(ctx, op, th, rv, none, none, none, none, stream)) { ctx->wait_h2d = false; return rc; }
+  // out: th, rv are final once the work of step_sync is done (:816); they leave while coalescence and movement run
+  CK(cudaEventRecord(ctx->ev_fields, st));
+  CK(cudaStreamWaitEvent(cs, ctx->ev_fields, 0));
+  CK(cudaMemcpyAsync(th_host, ctx->th_dense, bytes, cudaMemcpyDeviceToHost, cs));
+  CK(cudaMemcpyAsync(rv_host, ctx->rv_dense, bytes, cudaMemcpyDeviceToHost, cs));
   if (int rc = sdm_step_async(ctx, op, stream)) return rc;
   CK(cudaStreamSynchronize(st));
+  CK(cudaStreamSynchronize(cs));
   if (rain_flux) CK(cudaMemcpy(rain_flux, ctx->d_flux, sizeof(double), cudaMemcpyDeviceToHost));
   return SDM_OK;
 }

@@ -14,16 +14,20 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liboracle.so")
 _SRC = [os.path.join(_HERE, f) for f in ("sdm_oracle.cpp", "formulae.h")]
+# ORACLE_SANITIZE=1 (environment): the same source built with -fsanitize=address,undefined into liboracle_san.so;
+# the process must then run with LD_PRELOAD=$(gcc -print-file-name=libasan.so) (tests/test_oracle_sanitize.py does).
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") == "1"
+_SO = os.path.join(_HERE, "liboracle_san.so" if _SANITIZE else "liboracle.so")
 
 
 def build(force=False):
     """Compile the oracle with gcc (-O2, no FMA contraction, OpenMP over cells)."""
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
         return _SO
-    cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-           _SRC[0], "-o", _SO]
+    cmd = ["g++", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC[0], "-o", _SO]
+    if _SANITIZE:
+        cmd[1:2] = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
     subprocess.check_call(cmd)
     return _SO
 

@@ -122,6 +122,120 @@ def test_pair_probability_bruteforce(nsd):
         assert abs(hits[pr] - T * p) < 4.5 * max(sd / np.sqrt(scale), 3.0), (pr, hits[pr], T * p)
 
 
+def _stokes(r, eta, rho_a):
+    """Stokes fall speed 2 r^2 g (rho_w - rho_a) / (9 eta): the r -> 0 limit of the terminal-velocity formula (:649),
+    within 3e-3 of it up to 1 um (test_terminal_velocity_stokes_limit_and_textbook)."""
+    return 2.0 * r * r * 9.81 * (RHO_W - rho_a) / (9.0 * eta)
+
+
+def _two_sd_collisions(kernel, rj, rk, nj, dV, dt=1.0, sstp_coal=1, **kw):
+    """One coalescence stage on a cell holding exactly two SDs (N_j = nj >> N_k = 1, so n_c(n_c-1)/2 / floor(n_c/2) = 1
+    and the cap floor(N_j/N_k) is far away).  With multiple coalescence gamma = floor(p) + [u < frac p] (north_star), so
+    the drop of N_j equals p = N_j K dt/dV to within one event per substep: K is read off deterministically."""
+    side = dV ** (1 / 3)
+    o = oracle.Oracle(dx=side, dy=side, dz=side, dt=dt, kernel=kernel, seed=7, **kw)
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, sstp_coal=sstp_coal)
+    o.set_state(np.array([nj, 1], np.uint64), np.array([rj**2, rk**2]), np.full(2, 1e-27), np.full(2, 0.5))
+    o.stage("sort")
+    o.stage("coal", op)
+    st = o.get_state()
+    assert st["n"][1] == 1
+    return nj - int(st["n"][0]), st
+
+
+@pytest.mark.parametrize("rj,rk", [(0.4e-6, 1.0e-6), (1.0e-6, 0.3e-6), (0.7e-6, 0.9e-6)])
+def test_geometric_kernel_is_eq28(rj, rk):
+    """:633-637 eq. 28: K = E pi (r_j + r_k)^2 |v_j - v_k| (E = 1 for `geometric`).  Sub-micron drops fall at the
+    Stokes speed (closed form), so the expected number of events of the pair is known without the oracle:
+    N_j pi (r_j + r_k)^2 |v_j - v_k| dt / dV.  A dropped square, a missing pi, volumes in place of radii, a sum in
+    place of the difference of the fall speeds or a swapped operand each change it by far more than the 1 % bar."""
+    ct = oracle.cell_thermo(300.0, 0.0, 1.0)      # the default fields of a fresh oracle (th = 300 K, r_v = 0, rho_d = 1)
+    vj, vk = _stokes(rj, ct["eta"], ct["rho_a"]), _stokes(rk, ct["eta"], ct["rho_a"])
+    K = np.pi * (rj + rk) ** 2 * abs(vj - vk)
+    dV, dt = 1e-9, 1.0
+    nj = int(2000.5 * dV / (K * dt))              # p = 2000.5
+    got, _ = _two_sd_collisions("geometric", rj, rk, nj, dV, dt)
+    assert abs(got - nj * K * dt / dV) <= 1 + 0.01 * 2000.5, (got, nj * K * dt / dV)
+    # and the time step enters linearly
+    got2, _ = _two_sd_collisions("geometric", rj, rk, nj, dV, 0.5 * dt)
+    assert abs(got2 - 0.5 * nj * K * dt / dV) <= 1 + 0.01 * 1000.0
+
+
+def test_hydro_tab_kernel_is_eq28_times_the_tabulated_efficiency():
+    """:633-637 eq. 28 with E(collector radius, small/large ratio) from a 2 x 2 table: the bilinear value is computed
+    by hand here (collector = the LARGER drop whichever of the two SDs carries the larger multiplicity)."""
+    R, q = np.array([0.5e-6, 1.5e-6]), np.array([0.2, 0.8])
+    tab = np.array([[0.1, 0.3], [0.6, 1.0]])
+    ct = oracle.cell_thermo(300.0, 0.0, 1.0)
+    for rj, rk in ((0.4e-6, 1.0e-6), (1.0e-6, 0.4e-6), (1.2e-6, 0.9e-6)):
+        rl, rs = max(rj, rk), min(rj, rk)
+        t, u = (rl - R[0]) / (R[1] - R[0]), (rs / rl - q[0]) / (q[1] - q[0])
+        E = (1 - t) * (1 - u) * tab[0, 0] + (1 - t) * u * tab[0, 1] + t * (1 - u) * tab[1, 0] + t * u * tab[1, 1]
+        K = E * np.pi * (rj + rk) ** 2 * abs(_stokes(rj, ct["eta"], ct["rho_a"]) - _stokes(rk, ct["eta"], ct["rho_a"]))
+        dV = 1e-9
+        nj = int(3000.5 * dV / K)
+        got, _ = _two_sd_collisions("hydro_tab", rj, rk, nj, dV, eff_R=R, eff_q=q, eff_tab=tab)
+        assert abs(got - nj * K / dV) <= 1 + 0.01 * 3000.5, (rj, rk, got, nj * K / dV)
+
+
+def test_coalescence_substeps_use_dt_over_sstp_coal():
+    """:624 / DESIGN.md reading R-sstp-coal: each of the sstp_coal substeps applies eq. 27 with dt'' = dt / sstp_coal.
+    Two-SD cell, Golovin kernel with v_j << v_k so that K hardly changes when k grows: the events of one step add up
+    to N_j K dt / dV whatever the number of substeps (a full dt per substep would give sstp_coal times as many)."""
+    rj, rk, b, dV = 1e-6, 100e-6, 1500.0, 1e-3
+    K = b * 4 / 3 * np.pi * (rj**3 + rk**3)
+    nj = int(1000.5 * dV / K)
+    for sstp in (1, 4, 5):
+        got, st = _two_sd_collisions("golovin", rj, rk, nj, dV, sstp_coal=sstp, golovin_b=b)
+        growth = 1 + got * rj**3 / rk**3           # v_k grew by the collected volume: K rose by less than this
+        assert 1000.5 - sstp <= got <= 1000.5 * growth + sstp, (sstp, got)
+        np.testing.assert_allclose(st["rw2"][1] ** 1.5, rk**3 + got * rj**3, rtol=1e-13)
+
+
+@pytest.mark.parametrize("kernel,nsd,sstp", [("geometric", 4, 1), ("geometric", 5, 1), ("geometric", 4, 4)])
+def test_pair_probability_bruteforce_geometric(kernel, nsd, sstp):
+    """eq. 27 with eq. 28 on 4-5-SD cells of distinct radii (and once with sstp_coal = 4): the expected events of every
+    unordered pair per step are max(N_i, N_j) pi (r_i + r_j)^2 |v_i - v_j| dt/dV with Stokes fall speeds."""
+    n = (np.array([7, 11, 13, 17, 19][:nsd]) * 10**9).astype(np.uint64)
+    r = np.array([0.35, 0.95, 0.6, 0.8, 0.45][:nsd]) * 1e-6
+    ct = oracle.cell_thermo(300.0, 0.0, 1.0)
+    v = _stokes(r, ct["eta"], ct["rho_a"])
+    pairs = list(itertools.combinations(range(nsd), 2))
+    scale = (nsd * (nsd - 1) / 2) / (nsd // 2)
+    K = {pr: np.pi * (r[pr[0]] + r[pr[1]]) ** 2 * abs(v[pr[0]] - v[pr[1]]) for pr in pairs}
+    dV = max(float(max(n[a], n[b])) * K[(a, b)] for a, b in pairs) * scale / (0.5 if sstp == 1 else 0.12)
+    expect = {pr: float(max(n[pr[0]], n[pr[1]])) * K[pr] / dV for pr in pairs}
+    side = dV ** (1 / 3)
+    o = oracle.Oracle(dx=side, dy=side, dz=side, dt=1.0, kernel=kernel, seed=99)
+    op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, sstp_coal=sstp)
+    T = 40000
+    hits, ambiguous = dict.fromkeys(pairs, 0), 0
+    rw2, rd3, kap = r**2, np.full(nsd, 1e-27), np.full(nsd, 0.5)
+    for t in range(T):
+        o.set_state(n, rw2, rd3, kap)
+        o.set_step(t)
+        o.stage("sort")
+        o.stage("coal", op)
+        st = o.get_state()
+        grown, shrunk = np.nonzero(st["rw2"] != rw2)[0], np.nonzero(st["n"] != n)[0]
+        found = []
+        for k in grown:   # the partner is the SD whose multiplicity dropped by n_k
+            j = [j for j in shrunk if n[j] - st["n"][j] == n[k]]
+            if len(j) == 1:
+                found.append(tuple(sorted((int(k), int(j[0])))))
+        if len(found) != len(grown) or len(grown) != len(shrunk):
+            ambiguous += 1      # two events touching one SD within the substeps of a step: not attributable
+            continue
+        for pr in found:
+            hits[pr] += 1
+    assert ambiguous <= (0 if sstp == 1 else 0.01 * T)
+    for pr in pairs:
+        p = expect[pr]
+        tol = 4.5 * np.sqrt(T * p) + (0.0 if sstp == 1 else 0.12 * T * p)   # substeps: second-order depletion of the sample
+        assert abs(hits[pr] - T * p) < max(tol, 8.0), (pr, hits[pr], T * p)
+    assert sum(hits.values()) > 3000
+
+
 def test_collision_update_worked_example():
     """:639-643 with DESIGN.md reading R-collision (Shima 2009 rule): hand-computed two-SD cell."""
     b, dV, dt = 1.0, 1.0, 1.0
@@ -601,6 +715,51 @@ def test_move_stage_matches_eq16_per_dimension_and_sediments():
     assert o.get_state()["id"].tolist() == np.nonzero(~out)[0].tolist()
 
 
+def test_move_stage_3d_indexes_every_courant_component():
+    """:534-556 eq. 16 in three dimensions with the C-grid shapes of :751 ((nx+1) x ny x nz, nx x (ny+1) x nz,
+    nx x ny x (nz+1)), all different sizes so that a transposed or mis-strided index picks a different number;
+    every component random in all three directions; periodic in x and y (:558)."""
+    rng = np.random.default_rng(14)
+    nx, ny, nz, N = 5, 3, 4, 600
+    dx, dy, dz, dt = 10.0, 7.0, 20.0, 1.0
+    o = oracle.Oracle(nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, dz=dz, dt=dt, seed=1)
+    rhod = rng.uniform(1.0, 1.2, (nx, ny, nz))
+    cx = rng.uniform(-0.3, 0.3, (nx + 1, ny, nz))
+    cy = rng.uniform(-0.3, 0.3, (nx, ny + 1, nz))
+    cz = rng.uniform(-0.1, 0.1, (nx, ny, nz + 1))
+    cz[:, :, 0] = cz[:, :, -1] = 0
+    o.set_fields(th=np.full(rhod.size, 289.0), rv=np.full(rhod.size, 7e-3), rhod=rhod.ravel(), cx=cx.ravel(), cy=cy.ravel(),
+                 cz=cz.ravel())
+    x, y, z = rng.uniform(0, nx * dx, N), rng.uniform(0, ny * dy, N), rng.uniform(0, nz * dz, N)
+    n = rng.integers(1, 10**6, N).astype(np.uint64)
+    o.set_state(n, np.full(N, (5e-6) ** 2), np.full(N, 1e-24), np.full(N, 0.61), x=x, y=y, z=z)
+    o.step(oracle.make_opts(adve=True, sedi=False, cond=False, coal=False))
+    st = o.get_state()
+    i, j, k = np.floor(x / dx).astype(int), np.floor(y / dy).astype(int), np.floor(z / dz).astype(int)
+    q = rhod[i, j, k]
+
+    def eq16(a, d, idx, lo, hi):      # backward Euler with the Courant number interpolated to the NEW position
+        dC = hi - lo
+        return (a + d * (lo - idx * dC)) / (1 - dC)
+
+    xe = eq16(x, dx, i, cx[i, j, k] / q, cx[i + 1, j, k] / q)
+    ye = eq16(y, dy, j, cy[i, j, k] / q, cy[i, j + 1, k] / q)
+    ze = eq16(z, dz, k, cz[i, j, k] / q, cz[i, j, k + 1] / q)
+    om = xe / dx - i                                               # eq. 13-15 hold at the new position
+    np.testing.assert_allclose(xe, x + dx * ((1 - om) * cx[i, j, k] + om * cx[i + 1, j, k]) / q, rtol=1e-13)
+    om = ye / dy - j
+    np.testing.assert_allclose(ye, y + dy * ((1 - om) * cy[i, j, k] + om * cy[i, j + 1, k]) / q, rtol=1e-13)
+    om = ze / dz - k
+    np.testing.assert_allclose(ze, z + dz * ((1 - om) * cz[i, j, k] + om * cz[i, j, k + 1]) / q, rtol=1e-13, atol=1e-12)
+    xe = np.where(xe < 0, xe + nx * dx, np.where(xe >= nx * dx, xe - nx * dx, xe))
+    ye = np.where(ye < 0, ye + ny * dy, np.where(ye >= ny * dy, ye - ny * dy, ye))
+    assert (np.abs(xe - x) > 1.0).sum() > N // 2 and ((xe < x - 20) | (xe > x + 20)).sum() > 0    # wraps happened
+    np.testing.assert_allclose(st["x"], xe, rtol=1e-14)
+    np.testing.assert_allclose(st["y"], ye, rtol=1e-14)
+    np.testing.assert_allclose(st["z"], ze, rtol=1e-14, atol=1e-13)
+    assert (st["n"] == n).all()
+
+
 # ----------------------------------------------------------------------------- diagnostics / table / threads
 def test_moments_bruteforce():
     """:818-823 eq. 29."""
@@ -661,40 +820,47 @@ def test_openmp_over_cells_is_bitwise_identical_to_serial():
 
 
 # ------------------------------------------------------------------------------ initialisation (section 5.1.6)
-VOCALS = [(0.61, 60e6, 0.02e-6, 1.4), (0.61, 40e6, 0.075e-6, 1.6)]   # PAPER.md :117-130 (mode diameters 0.04, 0.15 um)
+# These pins import nothing from the product package: the environment and the second statement of each rule come
+# from tests/pin_helpers.py (numpy + scipy).
+from tests import pin_helpers as H   # noqa: E402
+
+VOCALS = H.VOCALS   # PAPER.md :117-130 (mode diameters 0.04, 0.15 um)
 
 
 def _init_case(sd=64, nx=6, nz=75, seed=5, modes=VOCALS):
-    from paper_1310_1905_b200 import workloads as W
-    from tests.util import make_oracle
-
-    w = W.cfg2_2d(sd_per_cell=sd, nx=nx, nz=nz, seed=seed)
-    o = make_oracle(w)
+    """A 2D column set-up (cells of 20 m x 1 m x 20 m, theta = 289 K, r_v = 7.5 g/kg, hydrostatic rho_d, :115)
+    initialised by the oracle's init().  Returns (rho_d(z), oracle, N, ranges, state)."""
+    o = oracle.Oracle(nx=nx, ny=0, nz=nz, dx=20.0, dy=1.0, dz=20.0, dt=1.0, seed=seed)
+    th, rv, rhod, rz = H.column_fields(nx, nz)
+    o.set_fields(th=th, rv=rv, rhod=rhod)
     N, ranges = o.init(modes, float(sd))
-    return w, o, N, ranges, o.get_state()
+    return rz, o, N, ranges, o.get_state()
 
 
-def test_init_range_rule_and_agreement_with_the_independent_generator():
+def test_init_range_rule_and_agreement_with_root_finding():
     """:657: the multiplicity at both ends of the r_d range is >= 1 and just outside it is < 1; the limits equal
-    those found by workloads.auto_rd_range (an independent torch implementation of the same rule)."""
-    w, o, N, ranges, s = _init_case()
+    the outermost roots of n(ln r)(hi - lo)/sd_conc dV = 1 found by brentq on the continuous density, to the
+    oracle's grid step."""
+    rz, o, N, ranges, s = _init_case()
     lo, hi = ranges[0]
     assert N == 64 * 6 * 75 and len(ranges) == 1
-    np.testing.assert_allclose([lo, hi], np.log(w.meta["rd_range"]), rtol=0, atol=1e-9)
+    step = (np.log(1e-4) - np.log(1e-10)) / 200000
+    rlo, rhi = H.rd_range_by_root_finding(VOCALS, 64.0, 20.0 * 1.0 * 20.0)
+    assert rlo - 1e-9 <= lo <= rlo + 2 * step and rhi - 2 * step <= hi <= rhi + 1e-9
+    assert 1e-9 < np.exp(lo) < 5e-9 and 1e-6 < np.exp(hi) < 3e-6      # SURVEY 8c-8: about 2 nm .. 1.7 um
 
     def mult(lnr):   # eq. 3 written out again, at STP density
         dens = sum(n / (np.sqrt(2 * np.pi) * np.log(sg)) * np.exp(-(lnr - np.log(rm)) ** 2 / (2 * np.log(sg) ** 2))
                    for _, n, rm, sg in VOCALS)
         return dens * (hi - lo) / 64.0 * (20.0 * 1.0 * 20.0)
 
-    step = (np.log(1e-4) - np.log(1e-10)) / 200000
     assert mult(lo) >= 1.0 and mult(hi) >= 1.0 and mult(lo - step) < 1.0 and mult(hi + step) < 1.0
 
 
 def test_init_positions_sizes_and_total_concentration():
     """:655 uniform positions, :657 log-uniform dry radii inside the range, :659 the SDs of a cell add up to the
     spectrum's total concentration scaled by rho_d / rho_STP (Monte-Carlo: within 5 standard errors)."""
-    w, o, N, ranges, s = _init_case(sd=128, nx=8)
+    rhod, o, N, ranges, s = _init_case(sd=128, nx=8)
     lo, hi = ranges[0]
     X, Z = 8 * 20.0, 75 * 20.0
     assert s["x"].min() >= 0 and s["x"].max() < X and s["z"].min() >= 0 and s["z"].max() < Z
@@ -710,7 +876,6 @@ def test_init_positions_sizes_and_total_concentration():
               for _, n, rm, sg in VOCALS)
     rho_stp = 101325.0 / (287.0 * 293.15)
     k = np.clip((s["z"] / 20.0).astype(int), 0, 74)
-    rhod = w.rhod.numpy()[0]
     expect = tot * rhod.mean() / rho_stp
     got = s["n"].sum() / (X * 1.0 * Z)
     # per-SD weights n_i have a wide distribution: standard error from the sample itself
@@ -724,14 +889,11 @@ def test_init_positions_sizes_and_total_concentration():
 
 def test_init_wet_radius_is_the_koehler_equilibrium_at_min_rh_095():
     """:661-665: zero growth rate (RH = a_w exp(A/r)) at the cell's RH, capped at 0.95; the root lies on the stable
-    branch below the critical radius; agrees with the torch bisection of workloads.equilibrium_rw."""
-    import torch
-    from paper_1310_1905_b200 import workloads as W
-
-    w, o, N, ranges, s = _init_case(sd=32, nx=4)
+    branch below the critical radius; agrees with scipy's brentq on the Koehler curve (tests/pin_helpers.py)."""
+    rhod, o, N, ranges, s = _init_case(sd=32, nx=4)
     k = np.clip((s["z"] / 20.0).astype(int), 0, 74)
-    T = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["T"] for r in w.rhod.numpy()[0]])
-    RH = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["RH"] for r in w.rhod.numpy()[0]])
+    T = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["T"] for r in rhod])
+    RH = np.array([oracle.cell_thermo(289.0, 7.5e-3, float(r))["RH"] for r in rhod])
     A = 2 * 0.072 / (461.5 * T * 1000.0)
     r = np.sqrt(s["rw2"])
     r3 = r ** 3
@@ -739,20 +901,20 @@ def test_init_wet_radius_is_the_koehler_equilibrium_at_min_rh_095():
     np.testing.assert_allclose(S, np.minimum(RH[k], 0.95), rtol=1e-11)
     assert np.all(r > np.cbrt(s["rd3"])) and np.all(r < np.sqrt(3 * 0.61 * s["rd3"] / A[k]))
     assert RH.max() > 1.0 and RH.min() < 0.7          # the profile spans clear and (super)saturated air
-    ref = W.equilibrium_rw(torch.from_numpy(s["rd3"]), torch.full((N,), 0.61, dtype=torch.float64),
-                           torch.from_numpy(np.minimum(RH[k], 0.95)), torch.from_numpy(T[k])).numpy()
-    np.testing.assert_allclose(r, ref, rtol=1e-9)
+    pick = np.random.default_rng(0).choice(N, 1500, replace=False)
+    ref = np.array([H.equilibrium_rw_brentq(float(s["rd3"][i]), 0.61, float(min(RH[k[i]], 0.95)), float(T[k[i]])) for i in pick])
+    np.testing.assert_allclose(r[pick], ref, rtol=1e-9)
 
 
 def test_init_external_mixture_shares_the_sds_between_kappas():
     """:659 "externally mixed aerosol ... multiple spectra, each characterised by different kappa": SD i belongs to
     spectrum i mod G, each spectrum has its own range and its SDs reproduce its own concentration."""
     modes = [(0.61, 60e6, 0.02e-6, 1.4), (1.28, 40e6, 0.075e-6, 1.6)]
-    w, o, N, ranges, s = _init_case(sd=128, nx=8, modes=modes)
+    rhod, o, N, ranges, s = _init_case(sd=128, nx=8, modes=modes)
     assert len(ranges) == 2 and ranges[0] != ranges[1]
     assert np.all(s["kappa"][0::2] == 0.61) and np.all(s["kappa"][1::2] == 1.28)
     from math import erf, log, sqrt
-    rho_ratio = w.rhod.numpy()[0].mean() / (101325.0 / (287.0 * 293.15))
+    rho_ratio = rhod.mean() / (101325.0 / (287.0 * 293.15))
     for g, (kap, n, rm, sg) in enumerate(modes):
         lo, hi = ranges[g]
         tot = n * 0.5 * (erf((hi - log(rm)) / (sqrt(2) * log(sg))) - erf((lo - log(rm)) / (sqrt(2) * log(sg))))

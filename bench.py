@@ -44,17 +44,23 @@ def stage_bytes(ndim, rb):
             "coal_move": 2 * (8 + 3 * rb) + (ndim * rb + rb + 4) + (ndim * rb + 8)}   # a5 + a6
 
 
-FLOP_PER_EVAL = 190.0
-FLOP_PER_SETUP = 150.0
-FLOP_PER_CORRECTION = 28.0   # third-order correction of every Newton step after the first (curvature from the last two iterates)
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # SMs x fp64 FMA lanes x 2 x max SM clock = 37.2
+# k_cond4, fp64 thread-instructions executed per unit of work, from the per-instruction execution counts of one
+# `ncu --set full --import-source on` capture of this build (profiles/r2_k_cond4_ncu_full.md: the SASS page summed by opcode and
+# by source line; "first" = everything an SD-substep costs with ONE growth-rate evaluation: ventilation set-up, eq. 18-19,
+# the certificate of R-roots, the evaluation, the Newton step, N d(r^3); "more" = every further evaluation with its
+# third-order corrected Newton step; "cell" = the cells' thermodynamics, spread over the SDs).  flops: DFMA = 2, DMUL = DADD = 1.
+FP64_INSTR = {"first": {"dfma": 62.0, "dmul": 58.0, "dadd": 19.0, "other": 11.0},
+              "more": {"dfma": 48.0, "dmul": 42.0, "dadd": 14.0, "other": 9.0}}
+FP64_INSTR_SOURCE = "profiles/r2_k_cond4_ncu_full.md"
+FP64_LANES_PER_SM = 64        # fp64 FMA lanes per SM per clock on sm_100 (B200_PROFILING.md; sdm_measure_fp64_peak confirms)
 # --cond-arith 4 (k_cond4f): fp32 operations of one evaluation with derivative and curvature bound (62 instructions, 20 of
 # them FMA, 4 MUFU) and of the per-SD-substep set-up, first step and N d(r^3) (45 instructions, 15 FMA); DESIGN.md section 7
 FLOP_PER_EVAL_F32 = 86.0
 FLOP_PER_SETUP_F32 = 60.0
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x fp32 FMA lanes x 2 x max SM clock = 74.4
-NCU_COND_DRAM_BYTES = 2.317242e9 + 0.551745e9
-NCU_COND32_DRAM_BYTES = 1.509464e9 + 0.313273e9     # k_cond4f, the default workload with --real-bytes 4 --cond-arith 4
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch on the default workload, from the ncu capture named beside it
+NCU_COND_DRAM_BYTES = (2.317242e9 + 0.551745e9, "profiles/r1_k_cond4_v7_ncu_full.md (kernel of round 1; the staging code is unchanged)")
+NCU_COND32_DRAM_BYTES = (1.509464e9 + 0.313273e9, "profiles/r1_k_cond4f_ncu_full.md")
 
 
 def parse():
@@ -72,6 +78,9 @@ def parse():
     ap.add_argument("--cond-arith", type=int, default=8, choices=[8, 4], help="arithmetic of the condensation sweep; 4 = fp32 (needs --real-bytes 4)")
     ap.add_argument("--recycle", action="store_true", help="the paper's recycling of zero-multiplicity SDs (:641) instead of compaction only")
     ap.add_argument("--real-bytes", type=int, default=8, choices=[8, 4], help="storage type of the SD attributes (configs[4]: fp32 state)")
+    ap.add_argument("--long-run", type=int, default=-1, help="after the timed region, continue the run to this many steps in all and report "
+                    "ms/step, evaluations per SD-substep, slow-list fraction and the launch configuration per 100-step window "
+                    "(default: 600 = the length of configs[3] for the default workload, 0 otherwise)")
     return ap.parse_args()
 
 
@@ -178,19 +187,22 @@ def oracle_rate(wa, steps, warmup, seed=42):
     oracle_rate.one_thread = n1 / (time.perf_counter() - t1)
     desc = (f"{w.name}: {w.n_sd} SDs in {sub['nx']}x{max(sub['ny'], 1)}x{sub['nz']} full columns of the same recipe, "
             f"{steps} steps after {warmup} warm-up, OpenMP over cells")
-    return n / dt, cores, desc, dt / steps * 1e3
+    return n / dt, cores, desc, dt / steps * 1e3, w.n_sd
 
 
 def run_reference(a, wa):
+    """The oracle as it stands on the host cores, K steps after W warm-up steps, every step on a bounded sample of the
+    workload (a block of full columns of the same recipe; the 67M-SD domain would take ~50 s per step on 16 cores)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps = max(1, min(a.steps, 3))
-    warm = max(1, min(a.warmup, 1))
-    v, cores, desc, ms = oracle_rate(wa, steps, warm)
-    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": steps, "warmup": warm,
+    v, cores, desc, ms, n_sample = oracle_rate(wa, max(a.steps, 1), max(a.warmup, 0))
+    cfg = config_of(wa)
+    cfg["n_sd_per_gpu"] = n_sample
+    cfg["sample"] = desc
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": max(a.steps, 1), "warmup": max(a.warmup, 0),
            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": config_of(wa), "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+           "config": cfg, "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(out), flush=True)
 
@@ -201,6 +213,32 @@ def config_of(wa):
             "n_sd_per_gpu": wa["nx"] * max(wa["ny"], 1) * wa["nz"] * wa["sd"],
             "l2": "state (60 B/SD) far exceeds the 126 MB L2; no flush needed",
             "parallelism": "independent replicas (single-GPU path, no collective)"}
+
+
+def make_particles(binding, torch, w, wa, a):
+    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], real_bytes=a.real_bytes, **w.init)
+    s = w.state
+    if a.real_bytes == 4:
+        s = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in s.items()}
+    cs = list(w.courants) + [None] * (3 - len(w.courants))
+    p.init_from_arrays(w.rhod, s["n"], s["rw2"], s["rd3"], s["kappa"], s["x"], s["y"], s["z"], s["id"], courant_1=cs[0],
+                       courant_2=cs[1], courant_3=cs[2])
+    if a.group:
+        p.set_group_size(a.group)
+    if a.recycle:
+        p.set_recycle(True)
+    if a.cond_arith == 4:
+        p.set_cond_arith(4)
+    return p
+
+
+def cond_fp64_work(evals, subs):
+    """fp64 thread-instructions and flops (DFMA = 2, DMUL = DADD = 1) of k_cond4 for `subs` SD-substeps solved with `evals`
+    growth-rate evaluations, from the per-unit counts of FP64_INSTR."""
+    more = max(evals - subs, 0)
+    instr = {k: subs * FP64_INSTR["first"][k] + more * FP64_INSTR["more"][k] for k in ("dfma", "dmul", "dadd", "other")}
+    flops = 2.0 * instr["dfma"] + instr["dmul"] + instr["dadd"]
+    return instr, flops
 
 
 def main():
@@ -223,27 +261,21 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = f"cuda:{local}"
+    warm = max(a.warmup, 3)
+    full3d = wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64
+    long_run = a.long_run if a.long_run >= 0 else (600 if full3d and world == 1 and not a.recycle else 0)
 
     w = make_workload(wa, seed=replicas.replica_seed(42, rank), device=dev)
-    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], real_bytes=a.real_bytes, **w.init)
-    s = w.state
-    if a.real_bytes == 4:
-        s = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in s.items()}
-    cs = list(w.courants) + [None] * (3 - len(w.courants))
-    p.init_from_arrays(w.rhod, s["n"], s["rw2"], s["rd3"], s["kappa"], s["x"], s["y"], s["z"], s["id"], courant_1=cs[0],
-                       courant_2=cs[1], courant_3=cs[2])
+    p = make_particles(binding, torch, w, wa, a)
+    p_host = make_particles(binding, torch, w, wa, a)   # a second, identically initialised context for the end-to-end leg
     n_sd0 = w.n_sd
     th, rv = w.th.clone(), w.rv.clone()
+    th_h, rv_h = w.th.cpu().pin_memory(), w.rv.cpu().pin_memory()
     ndim = 3 if wa["ny"] > 0 else 2
-    del w, s
+    del w
     torch.cuda.empty_cache()
-    if a.group:
-        p.set_group_size(a.group)
-    if a.recycle:
-        p.set_recycle(True)
-    if a.cond_arith == 4:
-        p.set_cond_arith(4)
     po = binding.make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=1.05, sstp_cond=10, sstp_coal=1)
+    fp64_peak_tflops, fp64_lanes = binding.measure_fp64_peak()   # measured on this device, before the timed region
 
     def barrier():
         torch.cuda.synchronize()
@@ -251,12 +283,9 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def one_step():
+    for _ in range(warm):
         p.step_sync(po, th, rv)
         p.step_async(po)
-
-    for _ in range(max(a.warmup, 3)):
-        one_step()
     # ---- device-resident timing ------------------------------------------------------------------
     p.set_timing(True)
     p.stage_times(reset=True)
@@ -281,25 +310,69 @@ def main():
     ms_max, sd_total = replicas.job_totals(ms, sd_steps, device=dev)   # slowest rank's device time, all ranks' SD-steps
     value = sd_total / (ms_max * 1e-3)
 
-    # ---- end to end: Eulerian fields in (pinned) host memory, copied in and out every step ---------
-    th_h, rv_h = th.cpu().pin_memory(), rv.cpu().pin_memory()
-    p.step_host(po, th_h, rv_h)
+    # ---- end to end: the SAME steps (the second context, same initial state, same warm-up) with the Eulerian fields in
+    # pinned host memory, copied in and out inside every timed step through sdm_step_host ------------------------------
+    for _ in range(warm):
+        p_host.step_host(po, th_h, rv_h)
     barrier()
     e_sd, t0 = 0, time.perf_counter()
     for _ in range(a.steps):
-        e_sd += p.n_sd()
-        p.step_host(po, th_h, rv_h)
+        e_sd += p_host.n_sd()
+        p_host.step_host(po, th_h, rv_h)
     torch.cuda.synchronize()
     e_dt = time.perf_counter() - t0
     e_s, e_tot = replicas.job_totals(e_dt, e_sd, device=dev)
     ncell = th.numel()
     e2e = {"value": e_tot / e_s, "unit": UNIT, "h2d_bytes_per_step": 2 * ncell * 8,
-           "d2h_bytes_per_step": 2 * ncell * 8 + 8, "api": "sdm_step_host (th, rv in pinned host memory)"}
+           "d2h_bytes_per_step": 2 * ncell * 8 + 8, "api": "sdm_step_host (th, rv in pinned host memory)",
+           "window": f"steps {warm + 1}..{warm + a.steps} after the initial condition, the same as the device-timed region"}
+    del p_host
+    torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
+
+    # ---- the rest of the run (configs[3]: 600 steps): the cloud forms, drops grow, rain starts -----------------------
+    long = None
+    if long_run > warm + a.steps:
+        long = {"total_steps": long_run, "windows": []}
+        done = warm + a.steps
+        t_all, n_all = 0.0, 0
+        while done < long_run:
+            k = min(100 - done % 100, long_run - done)
+            s0 = p.stats()
+            p.set_timing(True)
+            p.stage_times(reset=True)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n_w = 0
+            e0.record()
+            for _ in range(k):
+                p.step_sync(po, th, rv)
+                n_w += p.n_sd()
+                p.step_async(po)
+            e1.record()
+            torch.cuda.synchronize()
+            s1 = p.stats()
+            stg = p.stage_times(reset=True)
+            p.set_timing(False)
+            w_ms = e0.elapsed_time(e1)
+            subs = max(s1["sd_substeps"] - s0["sd_substeps"], 1)
+            long["windows"].append({"steps": [done + 1, done + k], "ms_per_step": w_ms / k, "value": n_w / (w_ms * 1e-3),
+                                    "evals_per_sd_substep": (s1["newton_iters"] - s0["newton_iters"]) / subs,
+                                    "slow_list_fraction": (s1["cond_slow"] - s0["cond_slow"]) / subs,
+                                    "collisions_per_step": (s1["collisions"] - s0["collisions"]) / k,
+                                    "max_cell_count": s1["max_cell_count"], "n_sd_live": s1["n_sd"],
+                                    "cond_variant": s1["cond_variant"], "cond_tile_cells": s1["cond_tile_cells"],
+                                    "coal_tile_cells": s1["coal_tile_cells"],
+                                    "cond_ms": stg["cond"][0] / max(stg["cond"][1], 1), "coal_move_ms": stg["coal_move"][0] / max(stg["coal_move"][1], 1)})
+            t_all += w_ms
+            n_all += n_w
+            done += k
+        long["value"] = (n_all + sd_steps) / ((t_all + ms) * 1e-3)
+        long["unit"] = UNIT
+        long["note"] = f"device-timed SD-steps/s over steps {warm + 1}..{long_run} of the run (the headline window included)"
 
     # ---- roofline of the dominant kernel (condensation), measured live ---------------------------
     hbm_peak, peak_src = peaks()
@@ -307,23 +380,34 @@ def main():
     evals = st1["newton_iters"] - st0["newton_iters"]
     subs = st1["sd_substeps"] - st0["sd_substeps"]
     f32 = a.cond_arith == 4
-    if f32:
-        flops = evals * FLOP_PER_EVAL_F32 + subs * FLOP_PER_SETUP_F32
-    else:
-        flops = evals * FLOP_PER_EVAL + subs * FLOP_PER_SETUP + max(evals - subs, 0) * FLOP_PER_CORRECTION
-    peak_alu = FP32_PEAK_TFLOPS if f32 else FP64_PEAK_TFLOPS
-    ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
     stage_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in stages.items()}
     step_ms = ms / a.steps
-    full3d = wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64
-    roofline = {"kernel": ("k_cond4f (condensation, 10 fused substeps, fp32 sweep)" if f32 else "k_cond4 (condensation, 10 fused substeps)"),
-                "bound": "alu", "achieved": ach, "peak": peak_alu,
-                "unit": "TFLOP/s", "frac": ach / peak_alu, "traffic": (NCU_COND32_DRAM_BYTES if f32 else NCU_COND_DRAM_BYTES) if full3d and (f32 or a.real_bytes == 8) else None,
-                "traffic_source": "bytes per launch, dram__bytes_read.sum + dram__bytes_write.sum of profiles/" + ("r1_k_cond4f_ncu_full.md" if f32 else "r1_k_cond4_v7_ncu_full.md"),
-                "peak_source": "derived: 148 SMs x %d fp%d FMA/clk x 2 x 1.965 GHz (DESIGN.md)" % ((128, 32) if f32 else (64, 64)),
-                "evals_per_sd_substep": evals / max(subs, 1),
-                "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
-                "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms}
+    sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    if f32:
+        flops = evals * FLOP_PER_EVAL_F32 + subs * FLOP_PER_SETUP_F32
+        ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
+        roofline = {"kernel": "k_cond4f (condensation, 10 fused substeps, fp32 sweep)", "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS,
+                    "unit": "TFLOP/s", "frac": ach / FP32_PEAK_TFLOPS,
+                    "peak_source": "derived: 148 SMs x 128 fp32 FMA/clk x 2 x 1.965 GHz (DESIGN.md)",
+                    "traffic": NCU_COND32_DRAM_BYTES[0] if full3d else None, "traffic_source": "from profile: " + NCU_COND32_DRAM_BYTES[1]}
+    else:
+        instr, flops = cond_fp64_work(evals, subs)
+        ach = flops / (cond_ms * 1e-3) / 1e12 if cond_ms > 0 else 0.0
+        n_instr = instr["dfma"] + instr["dmul"] + instr["dadd"] + instr["other"]
+        slots = n_sm * FP64_LANES_PER_SM * sm_hz * (cond_ms * 1e-3)
+        roofline = {"kernel": "k_cond4 (condensation, 10 fused substeps)", "bound": "alu", "achieved": ach, "peak": fp64_peak_tflops,
+                    "unit": "TFLOP/s", "frac": ach / fp64_peak_tflops,
+                    "peak_source": "measured on this device before the timed region: sdm_measure_fp64_peak (independent DFMA chains, "
+                                   "%.1f FMA/clk/SM); flops executed: DFMA = 2, DMUL = DADD = 1" % fp64_lanes,
+                    "fp64_issue_slot_frac": n_instr / slots if slots > 0 else None,
+                    "fp64_thread_instr_per_sd_substep": n_instr / max(subs, 1),
+                    "fp64_instr_mix": {k: v / n_instr for k, v in instr.items()}, "fp64_instr_source": FP64_INSTR_SOURCE,
+                    "traffic": NCU_COND_DRAM_BYTES[0] if full3d and a.real_bytes == 8 else None,
+                    "traffic_source": "from profile: " + NCU_COND_DRAM_BYTES[1]}
+    roofline.update({"evals_per_sd_substep": evals / max(subs, 1),
+                     "slow_list_fraction": (st1["cond_slow"] - st0["cond_slow"]) / max(subs, 1), "ms_per_launch": cond_ms / max(cond_n, 1),
+                     "share_of_step": (cond_ms / max(cond_n, 1)) / step_ms})
     bytes_step = BYTES_PER_SD_STEP[(ndim, a.real_bytes)] * (sd_steps / a.steps)
     hbm = {"bound": "hbm", "achieved": bytes_step / (step_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
            "frac": bytes_step / (step_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
@@ -332,16 +416,20 @@ def main():
     roofline_stages = {k: {"bytes_per_sd": sb[k], "achieved": sb[k] * (sd_steps / a.steps) / (stage_ms[k] * 1e-3) / 1e9, "unit": "GB/s",
                            "frac": sb[k] * (sd_steps / a.steps) / (stage_ms[k] * 1e-3) / 1e9 / hbm_peak}
                        for k in sb if stage_ms.get(k, 0.0) > 0}
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": warm,
            "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if a.cond_arith == 4 else "f64",
            "data": "synthetic", "config": dict(config_of(wa), state="fp64" if a.real_bytes == 8 else ("fp32 storage, fp32 condensation sweep (thermodynamics, feedback, coalescence probability, movement in fp64)" if a.cond_arith == 4 else "fp32 storage, fp64 arithmetic")), "clocks": clocks, "e2e": e2e,
-           "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "roofline": roofline, "roofline_step_hbm": hbm, "roofline_stages_hbm": roofline_stages,
-           "stage_ms": stage_ms, "n_sd_live": p.n_sd(), "n_sd_initial": n_sd0}
+           "gpu_launches": st1["kernel_launches"] - st0["kernel_launches"], "host_syncs_per_step": (st1["host_syncs"] - st0["host_syncs"]) / a.steps,
+           "roofline": roofline, "roofline_step_hbm": hbm, "roofline_stages_hbm": roofline_stages,
+           "stage_ms": stage_ms, "n_sd_live": st1["n_sd"], "n_sd_initial": n_sd0,
+           "launch_config": {k: st1[k] for k in ("cond_variant", "cond_tile_cells", "coal_tile_cells", "max_cell_count")}}
+    if long is not None:
+        out["long_run"] = long
     if a.recycle:
         out["config"]["recycling"] = "on (PAPER.md :641)"
         out["recycled"] = st1["recycled"] - st0["recycled"]
     if not a.no_cpu_baseline:
-        v, cores, desc, _ = oracle_rate(wa, 2, 1)
+        v, cores, desc, _, _ = oracle_rate(wa, 2, 1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                "value_1_thread": getattr(oracle_rate, "one_thread", None)}
     if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline:
@@ -351,7 +439,8 @@ def main():
             del p
             torch.cuda.empty_cache()
             cmd = [sys.executable, os.path.abspath(__file__), "--steps", str(a.steps), "--warmup", str(a.warmup), "--workload", a.workload,
-                   "--sd-per-cell", str(a.sd_per_cell), "--scale", str(a.scale), "--real-bytes", "4", "--cond-arith", "4", "--no-cpu-baseline"]
+                   "--sd-per-cell", str(a.sd_per_cell), "--scale", str(a.scale), "--real-bytes", "4", "--cond-arith", "4", "--no-cpu-baseline",
+                   "--long-run", "0"]
             r = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
             d = json.loads(r.stdout.strip().splitlines()[-1])
             out["fp32_mode"] = {k: d[k] for k in ("value", "unit", "ms_per_step", "dtype", "stage_ms", "gpu_launches")}

@@ -107,6 +107,12 @@ typedef struct {
   uint64_t sd_substeps;     /* condensation: SD-substeps solved */
   uint64_t cond_slow;       /* condensation: SD-substeps deferred to the second (compacted) solver pass */
   uint64_t recycled;        /* zero-multiplicity SDs recycled (sdm_set_recycle) */
+  /* launch configuration chosen by the last step (it follows the cell occupancy, which drifts as rain forms) */
+  uint64_t cond_variant;    /* condensation kernel: 1, 2, 3 = tile kernels of 800 / 1280 / 4096 SD slots, 0 = one cell per CTA in
+                               place in global memory; 100 + v: the fp32-arithmetic tile kernel v */
+  uint64_t cond_tile_cells; /* cells per condensation tile */
+  uint64_t coal_tile_cells; /* cells per tile of the fused coalescence + movement kernel; 0 = the per-cell kernel ran */
+  uint64_t host_syncs;      /* host synchronisations inside step_sync / step_async since creation */
 } sdm_stats_t;
 
 /* factory() of Listing 5.7 (:800-808).  Allocates all device memory for max_sd super-droplets on
@@ -186,6 +192,9 @@ const double* sdm_outbuf(sdm_ctx* ctx);
  * until the next step_sync.  sdm_export_order: after step_sync, the ids in sorted (cell, key, id)
  * order and the nx*ny*nz+1 segment offsets (DEVICE arrays).  All enqueue on `stream`. */
 int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd);
+/* sdm_n_live: the name SURVEY.md section 8(b) gives this call; the same number (after step_sync every SD in storage is
+ * live: the compaction of PAPER.md :641 is folded into the sort). */
+int sdm_n_live(sdm_ctx* ctx, uint64_t* n_live);
 int sdm_export_state(sdm_ctx* ctx, uint64_t* n, void* rw2, void* rd3, void* kappa,
                      void* x, void* y, void* z, uint32_t* id, void* stream);
 int sdm_export_order(sdm_ctx* ctx, uint32_t* ids_sorted, uint32_t* seg_start, void* stream);
@@ -232,6 +241,14 @@ int sdm_set_cond_arith(sdm_ctx* ctx, int bytes);
 /* Tuning override: growth-rate evaluations the dense condensation sweep spends on an SD before deferring it
  * to the compacted second pass (1..200, default 4).  Does not change results beyond the solver tolerance. */
 int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast);
+
+/* Measurement aid, not part of the step (the condensation kernel of PAPER.md eq. 17-24, which
+ * "takes most of the simulation time" (:912), is bound by fp64 arithmetic, so its roofline needs a MEASURED fp64 peak):
+ * runs a register-only kernel of independent fp64 FMA chains on every SM of the current device and returns the best of
+ * five timed launches (CUDA events on `stream`).  *fma_tflops: 2 flop per FMA, in TFLOP/s.  *dfma_per_clk_per_sm (may be
+ * NULL): thread-level FMAs retired per SM clock per SM, from clock64() inside the kernel (64 on sm_100).  HOST outputs;
+ * allocates and frees 1.3 MB of device memory.  Blocking.  SDM_ERR_NO_DEVICE without a device. */
+int sdm_measure_fp64_peak(double* fma_tflops, double* dfma_per_clk_per_sm, void* stream);
 
 #ifdef __cplusplus
 }

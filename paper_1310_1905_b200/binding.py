@@ -43,13 +43,15 @@ class ArrInfo(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [(k, C.c_uint64) for k in ("n_sd", "max_cell_count", "step", "kernel_launches", "pairs", "collisions",
-                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow", "recycled")]
+                                          "near_ties", "ill_posed", "newton_iters", "sd_substeps", "cond_slow", "recycled",
+                                          "cond_variant", "cond_tile_cells", "coal_tile_cells", "host_syncs")]
 
 
 EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_range", "sdm_init_from_arrays", "sdm_step_sync", "sdm_step_async",
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
-           "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_export_state", "sdm_export_order",
-           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith"]
+           "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_n_live", "sdm_export_state", "sdm_export_order",
+           "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith",
+           "sdm_measure_fp64_peak"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
@@ -85,6 +87,8 @@ def load_library():
     L.sdm_outbuf.argtypes = [vp]
     L.sdm_outbuf.restype = vp
     L.sdm_n_sd.argtypes = [vp, u64p]
+    L.sdm_n_live.argtypes = [vp, u64p]
+    L.sdm_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     L.sdm_export_state.argtypes = [vp] + [vp] * 8 + [vp]
     L.sdm_export_order.argtypes = [vp, vp, vp, vp]
     L.sdm_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -237,6 +241,11 @@ class Particles:
         self._ck(self.L.sdm_n_sd(self.h, C.byref(v)))
         return v.value
 
+    def n_live(self):
+        v = C.c_uint64()
+        self._ck(self.L.sdm_n_live(self.h, C.byref(v)))
+        return v.value
+
     def export_state(self):
         N = self.n_sd()
         dev = "cuda"
@@ -287,6 +296,15 @@ class Particles:
         cnt = (C.c_uint64 * len(STAGES))()
         self._ck(self.L.sdm_stage_times(self.h, ms, cnt, int(reset)))
         return {s: (ms[k], cnt[k]) for k, s in enumerate(STAGES)}
+
+
+def measure_fp64_peak():
+    """(TFLOP/s of fp64 FMA at 2 flop each, FMAs per SM clock per SM) measured on the current device."""
+    t, r = C.c_double(), C.c_double()
+    rc = load_library().sdm_measure_fp64_peak(C.byref(t), C.byref(r), _stream())
+    if rc != 0:
+        raise SdmError(f"sdm_measure_fp64_peak failed ({rc})")
+    return t.value, r.value
 
 
 def _as_tensor(ptr, n):

@@ -19,6 +19,7 @@ UNITS = {
     "sdm_diag.cu": ["-fmad=false"],
     "sdm_init.cu": ["-fmad=false"],
     "sdm_recycle.cu": [],
+    "sdm_peak.cu": [],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 
@@ -37,22 +38,26 @@ def build(force=False, verbose=False):
     env_extra = os.environ.get("SDM_NVCC_EXTRA", "").split()
     force = force or bool(env_extra)
     hdrs = [os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
-    objs = []
+    objs, jobs = [], []
     for src, extra in UNITS.items():
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + hdrs):
             cmd = [NVCC] + ARCH + COMMON + extra + env_extra + ["-c", s, "-o", o]
-            r = subprocess.run(cmd, capture_output=True, text=True)
-            log = r.stdout + r.stderr
-            with open(o + ".log", "w") as f:
-                f.write(" ".join(cmd) + "\n" + log)
-            if r.returncode != 0:
-                sys.stderr.write(log)
-                raise RuntimeError("nvcc failed on " + src)
-            if verbose:
-                print(log)
+            jobs.append((src, o, cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    failed = []
+    for src, o, cmd, proc in jobs:   # the translation units compile side by side
+        log = proc.communicate()[0]
+        with open(o + ".log", "w") as f:
+            f.write(" ".join(cmd) + "\n" + log)
+        if proc.returncode != 0:
+            sys.stderr.write(log)
+            failed.append(src)
+        elif verbose:
+            print(log)
+    if failed:
+        raise RuntimeError("nvcc failed on " + ", ".join(failed))
     if force or _stale(SO, objs):
         cmd = [NVCC] + ARCH + ["-shared", "-o", SO] + objs
         subprocess.check_call(cmd)

@@ -71,6 +71,8 @@ struct sdm_ctx {
   bool wait_h2d = false;
   cudaStream_t last_stream = nullptr;
   u64 launches = 0;
+  u64 host_syncs = 0;
+  int last_cond_variant = 0, last_cond_cpb = 0, last_coal_cpb = 0;
   double dry_lo = 0, dry_hi = 1e300, wet_lo = 0, wet_hi = 1e300;
   // optional per-stage timing with CUDA events on the launching stream (sdm_set_timing)
   bool timing = false;
@@ -425,6 +427,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     ctx->launches += 2;
     CK(cudaMemcpyAsync(ctx->h_rec, ctx->rec_info, 4 * sizeof(u32), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    ctx->host_syncs++;
     const u32 n_dead = ctx->h_rec[0], k = ctx->h_rec[1];
     if (k) {
       if (ctx->o.real_bytes == 8)
@@ -471,6 +474,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   ctx->launches += ctx->nslots ? 1 : 0;
   CK(cudaGetLastError());
   CK(cudaEventSynchronize(ctx->ev_info));   // the scatter runs while the host sizes the next launches
+  ctx->host_syncs++;
   ctx->cn ^= 1;
   ctx->cur ^= 1;
   ctx->nslots = ctx->h_info[ctx->cn];
@@ -509,6 +513,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
       if (v && (variant == 0 || v <= variant)) { cpb = cand; variant = v; }
     }
     CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
+    ctx->last_cond_cpb = cpb;
+    ctx->last_cond_variant = (ctx->o.real_bytes == 4 && arith32 && variant != 0 && op->sstp_cond <= 500) ? 100 + variant : variant;
     t_begin(ctx, SDM_STAGE_COND, st);
     if (ctx->o.real_bytes == 8)
       CK(launch_cond(cpb, variant, view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), ctx->rank, ctx->seg, g, thf,
@@ -549,6 +555,7 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
       if (coal_tile_fits(cand, (int)ctx->tile_max[k], ctx->o.real_bytes)) tile_cpb = cand;
     }
+    ctx->last_coal_cpb = tile_cpb;
     t_begin(ctx, SDM_STAGE_COAL_MOVE, st);
     const bool f64 = ctx->o.real_bytes == 8;
     if (tile_cpb && f64)
@@ -655,6 +662,8 @@ int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd) {
   return SDM_OK;
 }
 
+int sdm_n_live(sdm_ctx* ctx, uint64_t* n_live) { return sdm_n_sd(ctx, n_live); }
+
 int sdm_export_state(sdm_ctx* ctx, uint64_t* n, void* rw2, void* rd3, void* kappa, void* x, void* y, void* z,
                      uint32_t* id, void* stream) {
   if (!ctx) return SDM_ERR_INVALID;
@@ -695,6 +704,8 @@ int sdm_stats(sdm_ctx* ctx, sdm_stats_t* out) {
   out->pairs = s[0]; out->collisions = s[1]; out->near_ties = s[2]; out->ill_posed = s[3]; out->newton_iters = s[4];
   out->sd_substeps = s[5]; out->cond_slow = s[6];
   out->recycled = ctx->recycled;
+  out->cond_variant = (u64)ctx->last_cond_variant; out->cond_tile_cells = (u64)ctx->last_cond_cpb;
+  out->coal_tile_cells = (u64)ctx->last_coal_cpb; out->host_syncs = ctx->host_syncs;
   return SDM_OK;
 }
 

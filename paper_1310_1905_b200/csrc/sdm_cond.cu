@@ -90,11 +90,17 @@ enum {
   KC_D2Q, KC_B1, KC_B2, KC_B3, KC_B4, KC_B5,   // delta0^2/4; binomial series of (1+x)^(1/3) - 1
   KC_N
 };
+#ifndef SDM_COND_TOL
+#define SDM_COND_TOL 1e-11   // bound on the relative error left in r by a Newton step of the sweep
+#endif
+#ifndef SDM_COND_TOL1
+#define SDM_COND_TOL1 (1e-11 / 400.0)   // the same for the first step, whose curvature is bounded, not estimated
+#endif
 __constant__ double KC[KC_N] = {
     1.4426950408889634074, 6755399441055744.0 /* 1.5 * 2^52 */, 6.93147180369123816490e-01, 1.90821492927058770002e-10,
     1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0, 1.0 / 5040.0,
     1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5,
-    1e-11, 1e-11 / 400.0, 1e-15, cst::D_0, 0.5 * cst::D_0, cst::K_0, 0.5 * cst::K_0, 1.71,
+    SDM_COND_TOL, SDM_COND_TOL1, 1e-15, cst::D_0, 0.5 * cst::D_0, cst::K_0, 0.5 * cst::K_0, 1.71,
     cst::kc_delta0 * cst::kc_delta0 / 4.0, 1.0 / 3.0, -1.0 / 9.0, 5.0 / 81.0, -10.0 / 243.0, 22.0 / 729.0};
 
 // exp(t) for 0 <= t < 8 (t = A/r, the Kelvin exponent): n = rint(t log2 e) by the 1.5*2^52 trick,
@@ -402,7 +408,7 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
     y = yn;
     bool conv;
     if (newton) {
-      const double tol = 1e-11 * y;
+      const double tol = SDM_COND_TOL * y;
       const double d2 = d * d;
       conv = (dprev > 0.0) ? (d2 <= tol * y && d2 * d <= tol * (dprev * dprev)) : (100.0 * d2 <= tol * y);
       dprev = d;

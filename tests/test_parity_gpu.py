@@ -39,14 +39,23 @@ def rain_mix(w, seed=5, frac=0.25):
     return w
 
 
-def compare_states(p, o, positions=True, rtol=RTOL):
+def compare_states(p, o, positions=True, rtol=RTOL, drift=None):
+    """drift = (fraction, rtol_loose), for free-running trajectories of hundreds of steps only: the wet radii of all but
+    `fraction` of the SDs within rtol, every one within rtol_loose ("trajectory bar": a droplet that
+    evaporates towards its dry size multiplies a relative difference in r^2 by r^2_before / r^2_now, so a difference at
+    the rounding level surfaces, for the few steps that takes, above 1e-9 on a few SDs in 10^5, and decays again)."""
     g = sorted_by_id(p.export_state())
     r = sorted_by_id(o.get_state())
     assert len(g["id"]) == len(r["id"])
     np.testing.assert_array_equal(g["id"].astype(np.uint32), r["id"])
     np.testing.assert_array_equal(g["n"].astype(np.uint64), r["n"])      # multiplicities: bit-exact
     live = r["n"] > 0
-    np.testing.assert_allclose(np.sqrt(g["rw2"]), np.sqrt(r["rw2"]), rtol=rtol)
+    if drift is None:
+        np.testing.assert_allclose(np.sqrt(g["rw2"]), np.sqrt(r["rw2"]), rtol=rtol)
+    else:
+        rel = np.abs(np.sqrt(g["rw2"]) - np.sqrt(r["rw2"])) / np.sqrt(r["rw2"])
+        assert np.count_nonzero(rel > rtol) <= drift[0] * rel.size, (np.count_nonzero(rel > rtol), rel.size)
+        assert rel.max() <= drift[1], rel.max()
     np.testing.assert_allclose(np.cbrt(g["rd3"]), np.cbrt(r["rd3"]), rtol=rtol)
     np.testing.assert_allclose(g["kappa"], r["kappa"], rtol=rtol)
     if positions:
@@ -62,11 +71,11 @@ def compare_fields(th, rv, o, rtol=RTOL):
     np.testing.assert_allclose(np_(rv).ravel(), orv, rtol=rtol)
 
 
-def run_both(w, steps, group=0, opts=None, check_every=1, recycle=False, **override):
+def run_both(w, steps, group=0, opts=None, check_every=1, recycle=False, threads=4, **override):
     b = binding()
     kw = dict(w.opts)
     kw.update(opts or {})
-    o = make_oracle(w, threads=4, **override)
+    o = make_oracle(w, threads=threads, **override)
     p, th, rv = make_particles(w, **override)
     if recycle:
         o.set_recycle(True)
@@ -319,10 +328,14 @@ def test_runs_are_reproducible_bit_for_bit(mode):
 def test_full_size_3d_sampled_columns_match_oracle():
     """configs[3] at full size (128 x 128 x 64 cells, 67 108 864 SDs), in the launch configuration bench.py times.
     Every stage but the reorder is local to a column of cells, so the oracle can compute a sampled block of
-    columns on its own: after 3 steps of the whole domain on the GPU, the SDs of two 2 x 2 x 64 blocks are
-    handed to the oracle (same ids, same step counter, fields and Courant numbers sliced), both advance one
-    step, and the block's SDs are compared one by one.  Horizontal positions are compared modulo the block
-    width (an SD that leaves the block wraps in the oracle's small periodic domain)."""
+    columns on its own: after 3 steps of the whole domain on the GPU, the SDs of a 16 x 16 x 64 block (1.05 M SDs)
+    and of a 2 x 1 x 64 block whose cells touch both periodic borders are handed to the oracle (same ids, same step
+    counter, fields and Courant numbers sliced), both advance, and the blocks' SDs are compared one by one.
+    Horizontal positions are compared modulo the block width (an SD that leaves the block wraps in the oracle's small
+    periodic domain).  The large block is compared over TWO steps: after the first, its border columns have exchanged
+    SDs with the rest of the domain (in the oracle: with the opposite border), so the second step is compared on the
+    SDs and cells of its interior 14 x 14 columns, which no SD from outside can have reached (Courant numbers < 1)."""
+    import os
     b = binding()
     torch.cuda.empty_cache()
     w = W.cfg4_3d(device="cuda")
@@ -343,7 +356,7 @@ def test_full_size_3d_sampled_columns_match_oracle():
         p.step_async(po)
     st = p.export_state()                      # storage order, dead SDs of the last step still present
     N0 = st["id"].numel()
-    blocks = [(37, 90, 2, 2), (0, 127, 2, 1)]  # (i0, j0, bx, by); the second touches both periodic borders' cells
+    blocks = [(37, 90, 16, 16), (0, 127, 2, 1)]  # (i0, j0, bx, by); the second touches both periodic borders' cells
     ci = torch.clamp((st["x"] / dx).floor().long(), 0, nx - 1)
     cj = torch.clamp((st["y"] / dx).floor().long(), 0, ny - 1)
     oracles, picks = [], []
@@ -351,7 +364,7 @@ def test_full_size_3d_sampled_columns_match_oracle():
         m = (ci >= i0) & (ci < i0 + bx) & (cj >= j0) & (cj < j0 + by) & (st["n"] > 0)
         sel = torch.nonzero(m).flatten()
         o = oracle.Oracle(**dict(w.init, nx=bx, ny=by))
-        o.set_threads(4)
+        o.set_threads(os.cpu_count() or 4)
         sl = (slice(i0, i0 + bx), slice(j0, j0 + by))
         c1, c2, c3 = w.courants
         o.set_fields(th=np_(th[sl]).ravel(), rv=np_(rv[sl]).ravel(), rhod=np_(w.rhod[sl]).ravel(),
@@ -364,39 +377,68 @@ def test_full_size_3d_sampled_columns_match_oracle():
         oracles.append(o)
         picks.append(st["id"][sel].long())
         assert sel.numel() > 0.8 * 64 * bx * by * nz
-    del st, ci, cj
+    assert picks[0].numel() > 1000000
+    del st, ci, cj, m, sel
+
+    def compare(g, r, keep, i0, j0, bx, by):
+        """r: oracle state sorted by id; keep: mask over it; g: exported device state (dict of CUDA tensors)."""
+        where = torch.full((n_total,), -1, dtype=torch.int64, device="cuda")
+        where[g["id"].long()] = torch.arange(g["id"].numel(), device="cuda")
+        ids = torch.from_numpy(r["id"][keep].astype(np.int64)).cuda()
+        pos = where[ids]
+        assert bool((pos >= 0).all())
+        gg = {k: np_(v[pos]) for k, v in g.items()}
+        rr = {k: v[keep] for k, v in r.items()}
+        np.testing.assert_array_equal(gg["n"].astype(np.uint64), rr["n"])          # multiplicities: bit-exact
+        np.testing.assert_allclose(np.sqrt(gg["rw2"]), np.sqrt(rr["rw2"]), rtol=RTOL)
+        np.testing.assert_allclose(np.cbrt(gg["rd3"]), np.cbrt(rr["rd3"]), rtol=RTOL)
+        np.testing.assert_allclose(gg["kappa"], rr["kappa"], rtol=RTOL)
+        live = rr["n"] > 0
+        np.testing.assert_allclose(gg["z"][live], rr["z"][live], rtol=RTOL, atol=1e-9)
+        for k, o0, L, big in (("x", i0 * dx, bx * dx, nx * dx), ("y", j0 * dx, by * dx, ny * dx)):
+            d = np.mod(gg[k][live] - o0, big)            # the block may sit across the periodic border of the domain
+            d = np.mod(d - rr[k][live] + 0.5 * L, L) - 0.5 * L
+            assert np.max(np.abs(d)) < 1e-8
+        return int(keep.sum())
+
     th_before = th.clone()
     p.step_sync(po, th, rv)
     p.step_async(po)
     g = p.export_state()
-    where = torch.full((n_total,), -1, dtype=torch.int64, device="cuda")
-    where[g["id"].long()] = torch.arange(g["id"].numel(), device="cuda")
     ncoll = 0
-    for (i0, j0, bx, by), o, ids in zip(blocks, oracles, picks):
+    interior = None
+    for (i0, j0, bx, by), o in zip(blocks, oracles):
         o.step(oo)
         r = sorted_by_id(o.get_state())
-        ids_sorted, _ = torch.sort(ids)
-        pos = where[ids_sorted]
-        assert bool((pos >= 0).all())
-        gg = {k: np_(v[pos]) for k, v in g.items()}
-        np.testing.assert_array_equal(gg["id"].astype(np.uint32), r["id"])
-        np.testing.assert_array_equal(gg["n"].astype(np.uint64), r["n"])          # multiplicities: bit-exact
-        np.testing.assert_allclose(np.sqrt(gg["rw2"]), np.sqrt(r["rw2"]), rtol=RTOL)
-        np.testing.assert_allclose(np.cbrt(gg["rd3"]), np.cbrt(r["rd3"]), rtol=RTOL)
-        np.testing.assert_allclose(gg["kappa"], r["kappa"], rtol=RTOL)
-        live = r["n"] > 0
-        np.testing.assert_allclose(gg["z"][live], r["z"][live], rtol=RTOL, atol=1e-9)
-        for k, o0, L, big in (("x", i0 * dx, bx * dx, nx * dx), ("y", j0 * dx, by * dx, ny * dx)):
-            d = np.mod(gg[k][live] - o0, big)            # the block may sit across the periodic border of the domain
-            d = np.mod(d - r[k][live] + 0.5 * L, L) - 0.5 * L
-            assert np.max(np.abs(d)) < 1e-8
+        n_cmp = compare(g, r, np.ones(r["id"].shape, dtype=bool), i0, j0, bx, by)
+        assert n_cmp > 0.8 * 64 * bx * by * nz
         oth, orv = o.get_fields()
         sl = (slice(i0, i0 + bx), slice(j0, j0 + by))
         np.testing.assert_allclose(np_(th[sl]).ravel(), oth, rtol=RTOL)
         np.testing.assert_allclose(np_(rv[sl]).ravel(), orv, rtol=RTOL)
         assert not np.array_equal(np_(th_before[sl]).ravel(), oth)                 # condensation did act
         ncoll += o.counters()["collisions"]
+        if bx >= 4:   # SDs that start the second step in an interior column of the block
+            oi = np.clip(np.floor(r["x"] / dx).astype(np.int64), 0, bx - 1)
+            oj = np.clip(np.floor(r["y"] / dx).astype(np.int64), 0, by - 1)
+            interior = (r["n"] > 0) & (oi >= 1) & (oi <= bx - 2) & (oj >= 1) & (oj <= by - 2)
+            interior_ids = r["id"][interior]
     assert g["id"].numel() <= N0
+    del g
+    # second compared step: the interior of the large block
+    (i0, j0, bx, by), o = blocks[0], oracles[0]
+    p.step_sync(po, th, rv)
+    p.step_async(po)
+    g = p.export_state()
+    o.step(oo)
+    r = sorted_by_id(o.get_state())
+    keep = np.isin(r["id"], interior_ids)
+    assert keep.sum() == interior_ids.size > 0.7 * 64 * bx * by * nz
+    compare(g, r, keep, i0, j0, bx, by)
+    oth, orv = o.get_fields()
+    sl = (slice(i0 + 1, i0 + bx - 1), slice(j0 + 1, j0 + by - 1))
+    np.testing.assert_allclose(np_(th[sl]), oth.reshape(bx, by, nz)[1:-1, 1:-1], rtol=RTOL)
+    np.testing.assert_allclose(np_(rv[sl]), orv.reshape(bx, by, nz)[1:-1, 1:-1], rtol=RTOL)
 
 
 # ------------------------------------------------------------------------------------ init() (section 5.1.6)

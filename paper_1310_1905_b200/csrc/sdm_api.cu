@@ -26,6 +26,13 @@ constexpr double kCondTileTarget = SDM_COND_TILE_TARGET;   // SDs per condensati
 #endif
 constexpr double kCond32TileTarget = SDM_COND32_TILE_TARGET;   // the same for the fp32-arithmetic kernel (sdm_set_cond_arith)
 constexpr double kCondMaxCpb = 128.0;       // one thread per cell of the tile
+// SD slots of the small tile kernels (sdm_cond.cu: SDM_COND_CAP, SDM_COND32_CAP)
+#ifndef SDM_COND_TILE_SLOTS
+#define SDM_COND_TILE_SLOTS 800.0
+#endif
+#ifndef SDM_COND32_TILE_SLOTS
+#define SDM_COND32_TILE_SLOTS 800.0
+#endif
 }
 
 struct sdm_ctx {
@@ -45,6 +52,9 @@ struct sdm_ctx {
   double *cx = nullptr, *cy = nullptr, *cz = nullptr;
   double* outbuf = nullptr;
   double* flux_slots = nullptr;
+  double* flux_part = nullptr;   // per-CTA rain flux of k_coal_move_tile
+  int n_flux_part = 0;
+  bool hist_valid = false;       // cell, off, count of the next step were written by the last step_async
   double* d_flux = nullptr;  // [0] last step, [1] total
   unsigned long long* cnt_mem = nullptr;
   Counters cnt{};
@@ -225,14 +235,15 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   cudaError_t e;
   for (int b = 0; b < 2; ++b) {
     SdArrays& a = ctx->buf[b];
-    const size_t NR = o->real_bytes == 8 ? N : (N + 1) / 2;   // doubles that hold N reals
-    if ((e = dalloc(&a.n, N)) || (e = dalloc(&a.rw2, NR)) || (e = dalloc(&a.rd3, NR)) || (e = dalloc(&a.kappa, NR)) ||
-        (e = dalloc(&a.x, g.hx ? NR : 1)) || (e = dalloc(&a.y, g.hy ? NR : 1)) || (e = dalloc(&a.z, g.hz ? NR : 1)) ||
-        (e = dalloc(&a.id, N)))
+    // 4 elements to spare: the bulk copies of k_coal_move_tile fetch whole 16-byte units around a tile's run
+    const size_t NR = (o->real_bytes == 8 ? N : (N + 1) / 2) + 4;   // doubles that hold N reals
+    if ((e = dalloc(&a.n, N + 4)) || (e = dalloc(&a.rw2, NR)) || (e = dalloc(&a.rd3, NR)) || (e = dalloc(&a.kappa, NR)) ||
+        (e = dalloc(&a.x, g.hx ? NR : 4)) || (e = dalloc(&a.y, g.hy ? NR : 4)) || (e = dalloc(&a.z, g.hz ? NR : 4)) ||
+        (e = dalloc(&a.id, N + 4)))
       return bail(e, "particle state");
   }
   const int nb = scan_num_blocks(g.ncell);
-  if ((e = dalloc(&ctx->cell, N)) || (e = dalloc(&ctx->off, N)) || (e = dalloc(&ctx->rank, N)) ||
+  if ((e = dalloc(&ctx->cell, N)) || (e = dalloc(&ctx->off, N)) || (e = dalloc(&ctx->rank, N + 8)) ||
       (e = dalloc(&ctx->count, (size_t)g.ncell)) || (e = dalloc(&ctx->blocksum, (size_t)nb)) ||
       (e = dalloc(&ctx->seg, (size_t)g.ncell + 1)) || (e = dalloc(&ctx->d_info, 8)) ||
       (e = dalloc(&ctx->cf.rhod, (size_t)g.ncell)) || (e = dalloc(&ctx->cf.eta, (size_t)g.ncell)) ||
@@ -240,6 +251,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
       (e = dalloc(&ctx->th_dense, (size_t)g.ncell)) || (e = dalloc(&ctx->rv_dense, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->cx, (size_t)(g.NX + 1) * g.NY * g.NZ)) || (e = dalloc(&ctx->cy, (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = dalloc(&ctx->cz, (size_t)g.NX * g.NY * (g.NZ + 1))) || (e = dalloc(&ctx->flux_slots, NSLOT)) ||
+      (e = dalloc(&ctx->flux_part, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->d_flux, 2)) || (e = dalloc(&ctx->cnt_mem, N_COUNTERS * NSLOT)))
     return bail(e, "scratch");
   ctx->cf.cx = ctx->cx; ctx->cf.cy = ctx->cy; ctx->cf.cz = ctx->cz;
@@ -309,7 +321,7 @@ void sdm_destroy(sdm_ctx* ctx) {
   cudaFree(ctx->cell); cudaFree(ctx->off); cudaFree(ctx->rank); cudaFree(ctx->count); cudaFree(ctx->blocksum); cudaFree(ctx->seg);
   cudaFree(ctx->d_info); cudaFree(ctx->cf.rhod); cudaFree(ctx->cf.eta); cudaFree(ctx->cf.rho_a); cudaFree(ctx->outbuf);
   cudaFree(ctx->th_dense); cudaFree(ctx->rv_dense); cudaFree(ctx->cx); cudaFree(ctx->cy); cudaFree(ctx->cz);
-  cudaFree(ctx->flux_slots); cudaFree(ctx->d_flux); cudaFree(ctx->cnt_mem);
+  cudaFree(ctx->flux_slots); cudaFree(ctx->flux_part); cudaFree(ctx->d_flux); cudaFree(ctx->cnt_mem);
   cudaFree(ctx->d_effR); cudaFree(ctx->d_effq); cudaFree(ctx->d_efftab);
   if (ctx->h_info) cudaFreeHost(ctx->h_info);
   if (ctx->h_rec) cudaFreeHost(ctx->h_rec);
@@ -362,7 +374,7 @@ int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm
   CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
   CK(cudaMemsetAsync(ctx->outbuf, 0, sizeof(double) * g.ncell, st));
   CK(cudaStreamSynchronize(st));
-  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false;
+  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false; ctx->hist_valid = false;
   ctx->last_stream = st;
   return SDM_OK;
 }
@@ -401,7 +413,7 @@ int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arr
   CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
   CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
   CK(cudaStreamSynchronize(st));
-  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false;
+  ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false; ctx->hist_valid = false;
   ctx->last_stream = st;
   return SDM_OK;
 }
@@ -447,24 +459,42 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   CK(cudaMemsetAsync(ctx->d_info + 4, 0, 4 * sizeof(u32), st));
   // condensation tiles: about kCondTileTarget SDs per CTA at the occupancy seen before this step
   const bool arith32 = ctx->cond_arith == 4 && ctx->o.real_bytes == 4;
-  double tile_target = arith32 ? kCond32TileTarget : kCondTileTarget;
-  {  // a population that does not fill one wave of resident CTAs (5 per SM, 8 for the fp32 sweep): smaller tiles, so
-     // that every SM gets its share (configs[1]: 281 full-size tiles on 740 slots; measured 0.288 -> 0.250 ms per step;
-     // beyond one wave smaller tiles lose more to their fixed costs than the balance gains)
+  const double tile_target = arith32 ? kCond32TileTarget : kCondTileTarget;
+  const double mean_nc = (double)ctx->nslots / g.ncell;
+  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, tile_target / std::max(mean_nc, 1e-9)));
+  {  // A population of a few waves of resident CTAs (5 per SM, 8 for the fp32 sweep) is bound by the latency of one tile
+     // (10 substeps, each a sweep + a barrier + the cells' chain), not by throughput: the tiles of a launch then run in
+     // k = 1, 2, 3 FULL waves (a launch of 1.1 waves takes as long as one of 2), with the smallest k whose tiles fit the
+     // kernel's slots at mean + 5 sigma occupancy (configs[1], 180 000 SDs: 704 tiles of 8 cells on 740 slots;
+     // configs[2], 720 000 SDs: 1407 tiles of 4 cells = two waves).  Beyond ~4 waves the fixed costs of smaller tiles lose
+     // more than the balance gains.
     const double wave = (double)ctx->n_sm * (arith32 ? 8 : 5);
-    if ((double)ctx->nslots / tile_target < wave) tile_target = std::max(128.0, (double)ctx->nslots / (SDM_SMALL_WAVES * wave));
+    const double cap = arith32 ? SDM_COND32_TILE_SLOTS : SDM_COND_TILE_SLOTS;
+    if ((double)ctx->nslots / tile_target < 4.0 * wave && mean_nc > 0.0) {
+      for (int k = 1; k <= 4; ++k) {
+        const int cpb = (int)std::ceil((double)g.ncell / (k * wave));
+        const double expect = cpb * mean_nc;
+        if (cpb <= (int)kCondMaxCpb && expect + 5.0 * std::sqrt(expect) + 1.0 <= cap) { ctx->cond_cpb0 = std::max(cpb, 1); break; }
+      }
+    }
   }
-  ctx->cond_cpb0 = (int)std::min<double>(kCondMaxCpb, std::max(1.0, tile_target * g.ncell / std::max<double>(ctx->nslots, 1.0)));
-  t_begin(ctx, SDM_STAGE_HIST, st);
-  if (ctx->o.real_bytes == 8) launch_cellhist(view<double>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
-  else launch_cellhist(view<float>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
-  t_end(ctx, SDM_STAGE_HIST, st);
+  // a0-a1: the last step_async left cell, off and the histogram behind (k_coal_move_tile), unless recycling moved SDs since
+  const bool have_hist = ctx->hist_valid && !(ctx->recycle && ctx->nslots);
+  if (ctx->hist_valid && !have_hist) CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
+  ctx->hist_valid = false;
+  if (!have_hist) {
+    t_begin(ctx, SDM_STAGE_HIST, st);
+    if (ctx->o.real_bytes == 8) launch_cellhist(view<double>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+    else launch_cellhist(view<float>(ctx->buf[ctx->cur]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->count, st);
+    t_end(ctx, SDM_STAGE_HIST, st);
+    ctx->launches += ctx->nslots ? 1 : 0;
+  }
   t_begin(ctx, SDM_STAGE_SCAN, st);
   launch_scan(ctx->count, g.ncell, ctx->blocksum, ctx->seg, d_next, ctx->d_info + 2, st);
   t_end(ctx, SDM_STAGE_SCAN, st);
   launch_tile_max(ctx->seg, g.ncell, ctx->cond_cpb0, ctx->d_info + 4, st);
   ctx->launches++;
-  ctx->launches += (ctx->nslots ? 1 : 0) + 3;
+  ctx->launches += 3;
   CK(cudaMemcpyAsync(ctx->h_info, ctx->d_info, 8 * sizeof(u32), cudaMemcpyDeviceToHost, st));
   CK(cudaEventRecord(ctx->ev_info, st));
   t_begin(ctx, SDM_STAGE_SCATTER, st);
@@ -549,21 +579,23 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     bool in_smem = coal_smem_bytes(G, cap, sstp, true) <= kSmemLimit;
     if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
       return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
-    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step};
-    int tile_cpb = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
+    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step, ctx->recycle ? 0 : 1};
+    int tile_cpb = 0, tile_need = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
     for (int k = 0; k < 4 && !tile_cpb && sstp == 1 && !ctx->group_override; ++k) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
-      if (coal_tile_fits(cand, (int)ctx->tile_max[k], ctx->o.real_bytes)) tile_cpb = cand;
+      if (coal_tile_fits(cand, (int)ctx->tile_max[k], ctx->o.real_bytes)) { tile_cpb = cand; tile_need = (int)ctx->tile_max[k]; }
     }
     ctx->last_coal_cpb = tile_cpb;
     t_begin(ctx, SDM_STAGE_COAL_MOVE, st);
     const bool f64 = ctx->o.real_bytes == 8;
+    ctx->n_flux_part = tile_cpb ? (g.ncell + tile_cpb - 1) / tile_cpb : 0;
+    ctx->hist_valid = tile_cpb && mp.fold;
     if (tile_cpb && f64)
-      CK(launch_coal_move_tile(tile_cpb, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
-                               ctx->flux_slots, ctx->cnt, st));
+      CK(launch_coal_move_tile(tile_cpb, tile_need, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                               ctx->flux_part, ctx->cnt, ctx->cell, ctx->off, ctx->count, st));
     else if (tile_cpb)
-      CK(launch_coal_move_tile(tile_cpb, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
-                               ctx->flux_slots, ctx->cnt, st));
+      CK(launch_coal_move_tile(tile_cpb, tile_need, view<float>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
+                               ctx->flux_part, ctx->cnt, ctx->cell, ctx->off, ctx->count, st));
     else if (f64)
       CK(launch_coal_move(G, cap, in_smem, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
                           ctx->flux_slots, ctx->cnt, st));
@@ -573,7 +605,8 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     t_end(ctx, SDM_STAGE_COAL_MOVE, st);
     ctx->launches++;
   }
-  launch_flux_sum(ctx->flux_slots, ctx->d_flux, ctx->d_flux + 1, st);
+  else ctx->n_flux_part = 0;
+  launch_flux_sum(ctx->flux_slots, ctx->flux_part, ctx->n_flux_part, ctx->d_flux, ctx->d_flux + 1, st);
   ctx->launches++;
   CK(cudaGetLastError());
   CK(cudaEventRecord(ctx->ev_async, st));

@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a,
               pkap[k] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
             prd3[k] = rd3k + rd3j;
             const double r = cbrt(rw3);
-            prw2[k] = r * r;
+            prw2[k] = (PT)(double)(R)(r * r);   // what is stored is the radius from here on (as in k_coal_move_tile)
             pn[j] = nj - gam * nk;
           }
         }
@@ -222,164 +222,291 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a,
 }
 
 // ---- k_coal_move_tile: the same stages for sstp_coal == 1, tile-resident -----------------------------
-// A CTA of T threads owns a tile of `cpb` consecutive cells (at most CAP - cpb SDs).  n, r_w^2, id and the
-// positions of the tile's SDs are copied into shared memory IN STORAGE ORDER by asynchronous copies
-// (cp.async: no registers, no stall, every copy of the tile in flight at once); the sorted order enters
-// through an inverse map inv[sorted position] = slot, built with every cell's segment padded to an even
-// length, so that thread t owns the pair of sorted positions (2t, 2t+1): all lanes are busy whatever
-// the cell populations are.  r_d^3 and kappa are touched (in global memory) only by the rare pairs that
-// collide, and n, r_w^2 are written back only where they changed: per SD the kernel reads 46 B and writes
-// 24 B of HBM.  The terminal velocity of every SD is evaluated once, in the pair pass (the lone SD of an
-// odd cell by the thread of its padded slot), and reused by the sedimentation.  The arithmetic is,
-// expression by expression, that of k_coal_move above (-fmad=false).
-#ifndef SDM_COAL_UNROLL
-#define SDM_COAL_UNROLL 1
-#endif
-constexpr int kCoalUnroll = SDM_COAL_UNROLL;
+// A CTA of T threads owns a tile of `cpb` consecutive cells (at most CAP - cpb SDs).
+//  * n, r_w^2, id and the positions of the tile's SDs are one contiguous run per attribute in storage order: thread 0
+//    fetches each run with ONE bulk asynchronous copy (cp.async.bulk, the 1-D form of TMA: UBLKCP in SASS) signalled on an
+//    mbarrier, while all threads build the inverse map of the sorted order.  Bulk copies move multiples of 16 bytes between
+//    16-byte aligned addresses, so a run starts at the aligned element below its first one and element t of the tile sits
+//    at index t + sh of every shared array, sh = (first slot) mod 4 (the state arrays are allocated with 4 elements to spare).
+//  * The sorted order enters through inv[sorted position] = slot, built with every cell's segment padded to an even
+//    length, so that thread t owns the pair of sorted positions (2t, 2t+1): all lanes are busy whatever the cell
+//    populations are.  The thread of a pair does everything for its two SDs: terminal velocities, eq. 27-28, the Philox
+//    uniform, the Shima update, then eq. 16 and sedimentation, the cell index of the NEW position and its place in the
+//    next step's histogram.  There is no barrier between coalescence and movement and no per-SD search for the cell.
+//  * r_d^3 and kappa are touched (in global memory) only by the rare pairs that collide, n and r_w^2 are written back only
+//    where they changed; the new positions go back to shared memory and are stored coalesced in storage order.
+//  * Next step's a0-a1 (PAPER.md :547, :641): `cell` and `off` of every SD and the histogram `count` are produced here
+//    (SDs that stay in the tile's cells are counted in shared memory, one global atomic per cell and tile), so that
+//    step_sync need not read the positions again (k_cellhist stays for the first step, recycling and the per-cell kernel).
+//  * Arithmetic: the collision probability and the new positions need not be bit-identical to the oracle's (north_star
+//    counts near-tie decisions; positions are compared to 1e-9), so divisions by per-cell constants are multiplications by
+//    their IEEE reciprocals and square roots / reciprocals of per-SD values are the hardware seeds with two Newton steps
+//    (<= 2 ulp).  The CELL INDEX is different: floor(x/dx) decides which SDs meet, so it is the oracle's IEEE quotient
+//    whenever the fast quotient lies within 1e-9 of an integer.
 struct __align__(8) CoalCell {
-  double eta, rho_a, scale;                 // air properties; eq. 27 factor n(n-1)/2 / floor(n/2)
-  double Cxl, Cxh, Cyl, Cyh, Czl, Czh;      // Courant numbers at the cell's faces (rho_d C / rho_d)
-  int i, j, k, pad;
+  double kX, kv, scale;          // v_term: X = kX r^3, v = kv s^2 / r; eq. 27 factor n(n-1)/2 / floor(n/2)
+  double ax, bx, ay, by, az, bz; // eq. 16: x' = (x + a) b, a = dx (C_l - i dC), b = 1/(1 - dC)
 };
+
+// 1/sqrt(a) and 1/a: hardware seed (2^-22) and two Newton steps
+__device__ __forceinline__ double rsqrt_nr(double a) {
+  double x;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+  const double h = 0.5 * a;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const double e = fma(-h * x, x, 0.5);
+    x = fma(x, e, x);
+  }
+  return x;
+}
+__device__ __forceinline__ double rcp_nr2(double a) {
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const double e = fma(-a, x, 1.0);
+    x = fma(x, e, x);
+  }
+  return x;
+}
+// terminal velocity (PAPER.md :649, DESIGN.md R-vt) from y = r^2 with the cell's constants; also returns r
+__device__ __forceinline__ double v_term_cell(double y, const CoalCell& C, double& r_out) {
+  const double c1 = 4.0 / (cst::kc_delta0 * cst::kc_delta0 * 0.5403702434442518 /* sqrt(C0) */);
+  const double rinv = rsqrt_nr(y);
+  const double r = y * rinv;
+  r_out = r;
+  const double X = C.kX * (y * r);
+  const double e = c1 * (X * rsqrt_nr(X));
+  const double w = 1.0 + e;
+  const double s = e * rcp_nr2(fma(w, rsqrt_nr(w), 1.0));
+  return C.kv * (s * s) * rinv;
+}
+// cell index along one dimension, the oracle's floor(x/dx) clamped (eq. 15)
+__device__ __noinline__ double ieee_quotient(double x, double dx) { return x / dx; }   // rare: kept out of the hot loop
+__device__ __forceinline__ int cell_1d_fast(double x, double dx, double inv_dx, int n) {
+  double q = x * inv_dx;
+  const double f = q - floor(q);
+  if (__builtin_expect(f < 1e-9 || f > 1.0 - 1e-9, 0)) q = ieee_quotient(x, dx);
+  int i = (int)floor(q);
+  i = max(i, 0);
+  return min(i, n - 1);
+}
+
+// Outcome of gam collisions between j (the larger multiplicity, slot gj) and k (slot gk) in global memory (PAPER.md :639-643,
+// DESIGN.md R-outcome, R-kappa); returns the new r_w^2 of k as stored.  Rare: kept out of the hot loop.
+template <typename R>
+__device__ __noinline__ double shima_update(const SdArraysT<R>& a, u32 gj, u32 gk, u64 gam, u64 nj2, double yj, double yk, double rj,
+                                            double rk) {
+  const double gd = (double)gam;
+  const double rw3 = yk * rk + gd * (yj * rj);    // extensive attributes are summed (:643)
+  const double rd3j = gd * a.rd3[gj];
+  const double rd3k = a.rd3[gk];
+  const double kj = a.kappa[gj], kk = a.kappa[gk];
+  if (kj != kk)                                    // intensive ones averaged (:643)
+    a.kappa[gk] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
+  a.rd3[gk] = rd3k + rd3j;
+  const double r = cbrt(rw3);
+  const R y2 = (R)(r * r);   // what is stored is the radius from here on
+  a.rw2[gk] = y2;
+  a.n[gj] = nj2;
+  return (double)y2;
+}
 
 template <int CAP, int T, typename R>
-struct CoalTile {   // u64 n; R rw2, x, y, z; double vt; u32 id; u16 inv
+struct CoalTile {   // per slot: u64 n; R rw2, x, y, z; u32 id / new cell; u16 inv, off, rank; u8 cell of the pair
   static_assert(CAP % 16 == 0, "the arrays of the tile follow one another in shared memory: keep every one of them 16-byte aligned");
-  static constexpr size_t fixed_bytes = (size_t)CAP * (8 + 4 * sizeof(R) + 8 + 4 + 2);
-  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CoalCell) + (size_t)(cpb + 1) * 8 + 16; }
+  static constexpr int SLOTS = CAP + 16;   // room for the alignment shift of the bulk copies
+  static constexpr size_t fixed_bytes = (size_t)SLOTS * (8 + 4 * sizeof(R) + 4 + 2 + 2 + 2) + (size_t)(SLOTS / 2) * 2;
+  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * (sizeof(CoalCell) + 16) + 64; }
 };
 
-template <int BYTES>
-__device__ __forceinline__ void cp_async(void* smem_dst, const void* gmem_src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gmem_src), "n"(BYTES) : "memory");
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, unsigned bytes, unsigned long long* mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_u32(mbar))
+               : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int CAP, int T, int MINB, typename R>
 __global__ void __launch_bounds__(T, MINB)
 k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, CellFields cf, CoalParams kp,
-                 CoalMoveParams mp, double* flux_slots, Counters cnt, int cpb) {
+                 CoalMoveParams mp, double* __restrict__ flux_part, Counters cnt, int cpb, u32* __restrict__ cell_out,
+                 u32* __restrict__ off_out, u32* __restrict__ count) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using L = CoalTile<CAP, T, R>;
+  constexpr int SLOTS = L::SLOTS;
+  constexpr int NW = T / 32;
   constexpr u16 NONE = 0xFFFFu;
-  const int tid = threadIdx.x;
+  __shared__ __align__(8) unsigned long long mbar;
+  __shared__ double s_flux[NW];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c_first = blockIdx.x * cpb;
   const int nc = min(cpb, g.ncell - c_first);
   u64* s_n = reinterpret_cast<u64*>(smem_raw);
-  double* s_vt = reinterpret_cast<double*>(smem_raw) + CAP;
-  R* s_rw2 = reinterpret_cast<R*>(s_vt + CAP);
-  R* s_x = s_rw2 + CAP;
-  R* s_y = s_x + CAP;
-  R* s_z = s_y + CAP;
-  u32* s_id = reinterpret_cast<u32*>(s_z + CAP);
-  u16* inv = reinterpret_cast<u16*>(s_id + CAP);
+  R* s_rw2 = reinterpret_cast<R*>(s_n + SLOTS);
+  R* s_x = s_rw2 + SLOTS;
+  R* s_y = s_x + SLOTS;
+  R* s_z = s_y + SLOTS;
+  u32* s_id = reinterpret_cast<u32*>(s_z + SLOTS);      // id until the pair is done, then the SD's new cell
+  u16* inv = reinterpret_cast<u16*>(s_id + SLOTS);
+  u16* s_off = inv + SLOTS;                             // place among the SDs this tile sends to the new cell
+  u16* s_rk = s_off + SLOTS;                            // rank of the slot inside its cell (sdm_sort.cu), element t at t + (s0 mod 8)
+  u16* s_pc = s_rk + SLOTS;                             // cell (tile-local) of pair p
   CoalCell* s_cell = reinterpret_cast<CoalCell*>(smem_raw + L::fixed_bytes);
-  u32* segl = reinterpret_cast<u32*>(s_cell + cpb);   // storage offsets of the tile's cells
-  u32* segp = segl + cpb + 1;                          // padded (even) offsets of the sorted positions
+  u32* segl = reinterpret_cast<u32*>(s_cell + cpb);     // storage offsets of the tile's cells
+  u32* segp = segl + cpb + 1;                           // padded (even) offsets of the sorted positions
+  u32* s_cnt = segp + cpb + 1;                          // next step's histogram of the tile's own cells
+  u32* s_base = s_cnt + cpb;
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
+  const int sh = (int)(s0 & 3u);
   const bool moving = mp.adve || mp.sedi;
   const bool need_vt = mp.sedi && g.hz;
   unsigned n_pairs = 0, n_coll = 0, n_tie = 0;
   double flux = 0.0;
   if (M > 0) {
-    // everything that does not need the sorted order starts right away
-#pragma unroll kCoalUnroll
-    for (int t = tid; t < M; t += T) {
-      const u32 s = s0 + t;
-      cp_async<8>(s_n + t, a.n + s);
-      cp_async<sizeof(R)>(s_rw2 + t, a.rw2 + s);
-      if (mp.coal) cp_async<4>(s_id + t, a.id + s);
-      if (moving) {
-        if (g.hx) cp_async<sizeof(R)>(s_x + t, a.x + s);
-        if (g.hy) cp_async<sizeof(R)>(s_y + t, a.y + s);
-        if (g.hz) cp_async<sizeof(R)>(s_z + t, a.z + s);
-      }
+    if (tid == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar)) : "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      // the runs, from the 16-byte aligned element at or below the first one
+      const u32 lo4 = s0 - (u32)sh;                                   // 4-byte elements: multiple of 4
+      const unsigned n4 = (unsigned)((M + sh + 3) & ~3) * 4u;
+      const int sh8 = (int)(s0 & 1u);
+      const u32 lo8 = s0 - (u32)sh8;                                  // 8-byte elements: multiple of 2
+      const unsigned n8 = (unsigned)((M + sh8 + 1) & ~1) * 8u;
+      const int d8 = sh - sh8;                                        // even: 16-byte aligned in shared memory
+      constexpr bool R8 = sizeof(R) == 8;
+      const unsigned nR = R8 ? n8 : n4;
+      const u32 loR = R8 ? lo8 : lo4;
+      const int dR = R8 ? d8 : 0;
+      const int sh2 = (int)(s0 & 7u);                                 // 2-byte elements: multiple of 8
+      const unsigned n2 = (unsigned)((M + sh2 + 7) & ~7) * 2u;
+      unsigned total = n8 + nR + n2 + (mp.coal ? n4 : 0u);
+      if (g.hx) total += nR;
+      if (g.hy) total += nR;
+      if (g.hz) total += nR;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&mbar)), "r"(total) : "memory");
+      bulk_load(s_rk, rank + (s0 - (u32)sh2), n2, &mbar);
+      bulk_load(s_n + d8, a.n + lo8, n8, &mbar);
+      bulk_load(s_rw2 + dR, a.rw2 + loR, nR, &mbar);
+      if (mp.coal) bulk_load(s_id, a.id + lo4, n4, &mbar);
+      if (g.hx) bulk_load(s_x + dR, a.x + loR, nR, &mbar);
+      if (g.hy) bulk_load(s_y + dR, a.y + loR, nR, &mbar);
+      if (g.hz) bulk_load(s_z + dR, a.z + loR, nR, &mbar);
     }
     for (int cl = tid; cl < nc; cl += T) {
       const int c = c_first + cl;
       const u32 b0 = seg[c], b1 = seg[c + 1];
       segl[cl] = b0 - s0;
+      s_cnt[cl] = 0u;
       const int m = (int)(b1 - b0);
       CoalCell& C = s_cell[cl];
-      C.eta = cf.eta[c]; C.rho_a = cf.rho_a[c];
+      const double eta = cf.eta[c], rho_a = cf.rho_a[c];
+      C.kX = (32.0 / 3.0) * (cst::rho_w - rho_a) * cst::g * rho_a / (eta * eta);
+      C.kv = eta * (cst::kc_delta0 * cst::kc_delta0 / 4.0) / (2.0 * rho_a);
       C.scale = m >= 2 ? (double)((u64)m * (u64)(m - 1) / 2) / (double)(m / 2) : 0.0;
       const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
-      C.i = i; C.j = j; C.k = k;
       const double rhod = cf.rhod[c];
-      C.Cxl = C.Cxh = C.Cyl = C.Cyh = C.Czl = C.Czh = 0.0;
-      if (mp.adve) {
-        if (g.hx) { C.Cxl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod; C.Cxh = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod; }
-        if (g.hy) { C.Cyl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod; C.Cyh = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod; }
-        if (g.hz) { C.Czl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod; C.Czh = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod; }
+      C.ax = C.ay = C.az = 0.0;
+      C.bx = C.by = C.bz = 1.0;
+      if (mp.adve) {   // eq. 16 with the Courant numbers at the faces of the SD's time-n cell
+        if (g.hx) {
+          const double Cl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod, Ch = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod;
+          const double dC = Ch - Cl;
+          C.ax = g.dx * (Cl - (double)i * dC); C.bx = 1.0 / (1.0 - dC);
+        }
+        if (g.hy) {
+          const double Cl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod, Ch = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod;
+          const double dC = Ch - Cl;
+          C.ay = g.dy * (Cl - (double)j * dC); C.by = 1.0 / (1.0 - dC);
+        }
+        if (g.hz) {
+          const double Cl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod, Ch = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod;
+          const double dC = Ch - Cl;
+          C.az = g.dz * (Cl - (double)k * dC); C.bz = 1.0 / (1.0 - dC);
+        }
       }
     }
     if (tid == 0) segl[nc] = (u32)M;
     __syncthreads();
-    if (tid < 32) {   // padded offsets: warp scan over the cells, 32 at a time
+    // padded offsets: warp scan over the cells, 32 at a time; every warp does it for itself when the tile has at most 32
+    // cells (the same values from every warp: no barrier before the next phase)
+    if (nc < 32 || tid < 32) {
       u32 carry = 0;
       for (int c0 = 0; c0 <= nc; c0 += 32) {
-        const int cl = c0 + tid;
+        const int cl = c0 + lane;
         u32 v = 0;
         if (cl < nc) { const u32 m = segl[cl + 1] - segl[cl]; v = m + (m & 1u); }
         u32 inc = v;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const u32 t = __shfl_up_sync(0xffffffffu, inc, d); if (tid >= d) inc += t; }
+        for (int d = 1; d < 32; d <<= 1) { const u32 t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
         if (cl <= nc) segp[cl] = carry + inc - v;
         carry += __shfl_sync(0xffffffffu, inc, 31);
       }
+      __syncwarp();
     }
-    __syncthreads();
+    if (nc >= 32) __syncthreads();
     const int MP = (int)segp[nc];
-    // inverse map of the sorted order
-    for (int t = tid; t < M; t += T) {
-      int lo = 0, hi = nc;
-      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
-      inv[(int)segp[lo] + rank[s0 + t]] = (u16)t;
+    {   // the bulk copies have landed
+      unsigned done = 0;
+      while (!done)
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(done) : "r"(smem_u32(&mbar)) : "memory");
+    }
+    // inverse map of the sorted order and the cell of every pair; populated cells: a warp takes a cell at a time
+    const int sh2 = (int)(s0 & 7u);
+    const bool by_cell = M >= 24 * nc;
+    for (int q = by_cell ? warp : tid; q < (by_cell ? nc : M); q += by_cell ? NW : T) {
+      int cl, t0, t1;
+      if (by_cell) {
+        cl = q; t0 = (int)segl[cl] + lane; t1 = (int)segl[cl + 1];
+      } else {
+        int lo = 0, hi = nc;
+        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)q) lo = mid; else hi = mid; }
+        cl = lo; t0 = q; t1 = q + 1;
+      }
+      const int p0 = (int)segp[cl];
+      for (int t = t0; t < t1; t += 32) {
+        const int e = p0 + (int)s_rk[t + sh2];
+        inv[e] = (u16)(t + sh);
+        if ((e & 1) == 0) s_pc[e >> 1] = (u16)cl;
+      }
     }
     for (int cl = tid; cl < nc; cl += T) {   // the padding slot of an odd cell
       const u32 m = segl[cl + 1] - segl[cl];
       if (m & 1u) inv[segp[cl] + m] = NONE;
     }
-    cp_async_wait_all();
     __syncthreads();
-    // ---- pairs of sorted positions (2t, 2t+1) -------------------------------------------------------------
-    if (mp.coal || need_vt) {
-      const double dtdv = g.dt / g.dV;
-      for (int t = tid; 2 * t < MP; t += T) {
-        const u32 both = reinterpret_cast<const u32*>(inv)[t];
-        const int ia = (int)(both & 0xFFFFu), ib = (int)(both >> 16);
-        const bool lone = ib == (int)NONE;
-        int lo = 0, hi = nc;   // the pair's cell: segp[lo] <= 2t < segp[lo + 1]
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segp[mid] <= (u32)(2 * t)) lo = mid; else hi = mid; }
-        const CoalCell& C = s_cell[lo];
-        const double ya = s_rw2[ia];
-        const double ra = sqrt(ya);
-        if (lone || !mp.coal) {
-          if (need_vt) {
-            s_vt[ia] = v_term(ra, C.eta, C.rho_a);
-            if (!lone) s_vt[ib] = v_term(sqrt((double)s_rw2[ib]), C.eta, C.rho_a);
-          }
-          continue;
-        }
-        const u64 na = s_n[ia], nb = s_n[ib];
-        const double yb = s_rw2[ib];
-        const double rb = sqrt(yb);
+    // ---- pairs of sorted positions (2t, 2t+1): coalescence, then movement of both SDs ----------------------------------------
+    const double dtdv = g.dt / g.dV;
+    const double inv_dx = 1.0 / g.dx, inv_dy = 1.0 / g.dy, inv_dz = 1.0 / g.dz;
+    for (int t = tid; 2 * t < MP; t += T) {
+      const u32 both = reinterpret_cast<const u32*>(inv)[t];
+      const int ia = (int)(both & 0xFFFFu), ib = (int)(both >> 16);
+      const bool lone = ib == (int)NONE;
+      const int cl = (int)s_pc[t];
+      const CoalCell& C = s_cell[cl];
+      u64 na = s_n[ia], nb = lone ? 0ull : s_n[ib];
+      double ya = s_rw2[ia], yb = lone ? 1.0 : (double)s_rw2[ib];
+      double ra = 0.0, rb = 0.0, va = 0.0, vb = 0.0;
+      const bool geometric = kp.kernel != 1;
+      if (need_vt || (mp.coal && geometric)) {
+        va = v_term_cell(ya, C, ra);
+        if (!lone) vb = v_term_cell(yb, C, rb);
+      } else if (mp.coal) {
+        ra = ya * rsqrt_nr(ya); rb = yb * rsqrt_nr(yb);
+      }
+      if (mp.coal && !lone) {
         const bool afirst = na >= nb;            // j: larger N; tie -> first in order
-        const int j = afirst ? ia : ib, k = afirst ? ib : ia;
         const u64 nj = afirst ? na : nb, nk = afirst ? nb : na;
         const double yj = afirst ? ya : yb, yk = afirst ? yb : ya;
         const double rj = afirst ? ra : rb, rk = afirst ? rb : ra;
         double K;
-        if (kp.kernel == 1) {   // Golovin
+        if (!geometric) {   // Golovin
           const double vj = (4.0 / 3.0) * cst::pi * (yj * rj), vk = (4.0 / 3.0) * cst::pi * (yk * rk);
           K = kp.golovin_b * (vj + vk);
-          if (need_vt) { s_vt[j] = v_term(rj, C.eta, C.rho_a); s_vt[k] = v_term(rk, C.eta, C.rho_a); }
-        } else {                // eq. 28
-          const double vj = v_term(rj, C.eta, C.rho_a), vk = v_term(rk, C.eta, C.rho_a);
-          s_vt[j] = vj; s_vt[k] = vk;
-          K = cst::pi * ((rj + rk) * (rj + rk)) * fabs(vj - vk);
+        } else {            // eq. 28
+          K = cst::pi * ((rj + rk) * (rj + rk)) * fabs(va - vb);
           if (kp.kernel == 2) {
             const double rl = fmax(rj, rk), rs = fmin(rj, rk);
             K = K * eff_lookup(kp, rl, rs / rl);
@@ -387,9 +514,12 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
         }
         const double p = (((double)nj * K) * dtdv) * C.scale;   // eq. 27
         const double u = coal_uniform(s_id[ia], mp.step, 0u, kp.seed_lo, kp.seed_hi);
-        const u64 qmax = nj / nk;
         u64 gam;
-        if (kp.multi_coal) {
+        if (p < 1.0) {      // the usual case: floor(p) = 0, and nj >= nk allows one collision
+          if (fabs(u - p) < 1e-12) ++n_tie;
+          gam = (u < p) ? 1u : 0u;
+        } else if (kp.multi_coal) {
+          const u64 qmax = nj / nk;
           const double pf = floor(p);
           if (pf >= (double)qmax) gam = qmax;
           else {
@@ -400,58 +530,94 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
           }
         } else {
           if (fabs(u - p) < 1e-12) ++n_tie;
-          gam = (u < p) ? 1u : 0u;   // :639, :645
+          gam = 1u;   // u < 1 <= p (:639, :645)
         }
         ++n_pairs;
-        if (gam == 0) continue;
-        ++n_coll;
-        // the rare pair that collides updates global memory itself (r_d^3 and kappa are not staged)
-        const u32 gj = s0 + (u32)j, gk = s0 + (u32)k;
-        const double gd = (double)gam;
-        const double rw3 = yk * rk + gd * (yj * rj);    // extensive attributes are summed (:643)
-        const double rd3j = gd * a.rd3[gj];
-        const double rd3k = a.rd3[gk];
-        const double kj = a.kappa[gj], kk = a.kappa[gk];
-        if (kj != kk)                                    // intensive ones averaged (:643)
-          a.kappa[gk] = (rd3j * kj + rd3k * kk) / (rd3j + rd3k);
-        a.rd3[gk] = rd3k + rd3j;
-        const double r = cbrt(rw3);
-        const double y2 = (R)(r * r);   // what is stored is the radius from here on
-        s_rw2[k] = (R)y2; a.rw2[gk] = (R)y2;
-        s_n[j] = nj - gam * nk; a.n[gj] = nj - gam * nk;
-        if (need_vt) s_vt[k] = v_term(sqrt(y2), C.eta, C.rho_a);
+        if (gam != 0) {
+          ++n_coll;
+          // the rare pair that collides updates global memory itself (r_d^3 and kappa are not staged)
+          const int j = afirst ? ia : ib, k = afirst ? ib : ia;
+          const u32 gj = s0 + (u32)(j - sh), gk = s0 + (u32)(k - sh);
+          const u64 nj2 = nj - gam * nk;
+          const double y2 = shima_update(a, gj, gk, gam, nj2, yj, yk, rj, rk);
+          double rr;
+          const double v2 = need_vt ? v_term_cell(y2, C, rr) : 0.0;
+          if (afirst) { na = nj2; yb = y2; vb = v2; } else { nb = nj2; ya = y2; va = v2; }
+        }
+      }
+      // ---- eq. 16 + sedimentation of both SDs, the cell of the new position, its place in the next histogram --------
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        if (h == 1 && lone) break;
+        const int sl = h ? ib : ia;
+        const u64 n = h ? nb : na;
+        const double yy = h ? yb : ya, vt = h ? vb : va;
+        u32 cnew = CELL_DEAD;
+        if (n != 0) {
+          double xn = g.hx ? (double)s_x[sl] : 0.0, yn = g.hy ? (double)s_y[sl] : 0.0, zn = g.hz ? (double)s_z[sl] : 0.0;
+          if (moving) {
+            if (mp.adve) {
+              if (g.hx) xn = (xn + C.ax) * C.bx;
+              if (g.hy) yn = (yn + C.ay) * C.by;
+              if (g.hz) zn = (zn + C.az) * C.bz;
+            }
+            if (need_vt) zn = zn - vt * g.dt;                                   // explicit Euler (:649)
+            if (g.hx) { xn = wrap(xn, g.X); s_x[sl] = (R)xn; xn = (double)(R)xn; }  // periodic (:558)
+            if (g.hy) { yn = wrap(yn, g.Y); s_y[sl] = (R)yn; yn = (double)(R)yn; }
+            if (g.hz) { s_z[sl] = (R)zn; }
+          }
+          if (g.hz && moving && (zn < 0.0 || !(zn < g.Z))) {                     // left the domain (:651)
+            if (zn < 0.0) flux += (double)n * ((4.0 / 3.0) * cst::pi * cst::rho_w * (yy * (yy * rsqrt_nr(yy))));
+            a.n[s0 + (u32)(sl - sh)] = 0;
+          } else {
+            if (g.hz) zn = (double)(R)zn;
+            const int ci = g.hx ? cell_1d_fast(xn, g.dx, inv_dx, g.NX) : 0;
+            const int cj = g.hy ? cell_1d_fast(yn, g.dy, inv_dy, g.NY) : 0;
+            const int ck = g.hz ? cell_1d_fast(zn, g.dz, inv_dz, g.NZ) : 0;
+            cnew = (u32)((ci * g.NY + cj) * g.NZ + ck);
+          }
+        }
+        if (mp.fold) s_id[sl] = cnew;
+      }
+    }
+    __syncthreads();
+    if (mp.fold) {
+      // places in the next histogram, taken in STORAGE order (the reorder of the next step then writes runs, not a
+      // permutation of each cell): lanes that go to the same cell take consecutive places with one atomic, in shared
+      // memory for the tile's own cells
+      for (int t0 = 0; t0 < M; t0 += T) {
+        const int t = t0 + tid;
+        const u32 cnew = t < M ? s_id[t + sh] : CELL_DEAD;
+        const u32 peers = __match_any_sync(0xffffffffu, cnew);
+        const int leader = __ffs(peers) - 1;
+        const u32 rel = cnew - (u32)c_first;
+        u32 base = 0;
+        if (cnew != CELL_DEAD && lane == leader)
+          base = rel < (u32)nc ? atomicAdd(&s_cnt[rel], (u32)__popc(peers)) : atomicAdd(&count[cnew], (u32)__popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (cnew != CELL_DEAD) s_off[t + sh] = (u16)(base + __popc(peers & ((1u << lane) - 1u)));
       }
       __syncthreads();
+      for (int cl = tid; cl < nc; cl += T) { const u32 k = s_cnt[cl]; s_base[cl] = k ? atomicAdd(&count[c_first + cl], k) : 0u; }
+      __syncthreads();
     }
-    // ---- advection + sedimentation, SD by SD in storage order; everything is in shared memory -----------------
-    if (moving) {
-#pragma unroll kCoalUnroll
+    // ---- new positions, cell and offset back to global memory, coalesced in storage order ----------------------------------
+    if (moving || mp.fold) {
       for (int t = tid; t < M; t += T) {
-        const u64 n = s_n[t];
-        if (n == 0) continue;
-        int lo = 0, hi = nc;
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
         const u32 s = s0 + t;
-        const CoalCell& C = s_cell[lo];
-        double xn = 0, yn = 0, zn = 0;
-        if (g.hx) xn = s_x[t];
-        if (g.hy) yn = s_y[t];
-        if (g.hz) zn = s_z[t];
-        if (mp.adve) {   // eq. 16 with the Courant numbers at the edges of the SD's time-n cell
-          if (g.hx) { const double dC = C.Cxh - C.Cxl; xn = (xn + g.dx * (C.Cxl - (double)C.i * dC)) / (1.0 - dC); }
-          if (g.hy) { const double dC = C.Cyh - C.Cyl; yn = (yn + g.dy * (C.Cyl - (double)C.j * dC)) / (1.0 - dC); }
-          if (g.hz) { const double dC = C.Czh - C.Czl; zn = (zn + g.dz * (C.Czl - (double)C.k * dC)) / (1.0 - dC); }
+        const int sl = t + sh;
+        if (moving) {
+          if (g.hx) a.x[s] = s_x[sl];
+          if (g.hy) a.y[s] = s_y[sl];
+          if (g.hz) a.z[s] = s_z[sl];
         }
-        if (need_vt) zn = zn - s_vt[t] * g.dt;                                // explicit Euler (:649)
-        if (g.hx) { xn = wrap(xn, g.X); a.x[s] = xn; }                        // periodic (:558)
-        if (g.hy) { yn = wrap(yn, g.Y); a.y[s] = yn; }
-        if (g.hz) {
-          if (zn < 0.0 || !(zn < g.Z)) {                                       // left the domain (:651)
-            const double y = s_rw2[t];
-            if (zn < 0.0) flux += (double)n * ((4.0 / 3.0) * cst::pi * cst::rho_w * (y * sqrt(y)));
-            a.n[s] = 0;
+        if (mp.fold) {
+          const u32 cnew = s_id[sl];
+          cell_out[s] = cnew;
+          if (cnew != CELL_DEAD) {
+            const u32 rel = cnew - (u32)c_first;
+            off_out[s] = (u32)s_off[sl] + (rel < (u32)nc ? s_base[rel] : 0u);
           }
-          a.z[s] = zn;
         }
       }
     }
@@ -464,25 +630,33 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
     v2 += __shfl_xor_sync(0xffffffffu, v2, d);
     flux += __shfl_xor_sync(0xffffffffu, flux, d);
   }
-  if ((threadIdx.x & 31) == 0) {
-    const int slot = (blockIdx.x * (T / 32) + (threadIdx.x >> 5)) & (NSLOT - 1);
+  if (lane == 0) {
+    const int slot = (blockIdx.x * NW + warp) & (NSLOT - 1);
     if (v0) atomicAdd(&cnt.pairs[slot], (unsigned long long)v0);
     if (v1) atomicAdd(&cnt.collisions[slot], (unsigned long long)v1);
     if (v2) atomicAdd(&cnt.near_ties[slot], (unsigned long long)v2);
-    if (flux != 0.0) atomicAdd(&flux_slots[slot], flux);
+    s_flux[warp] = flux;
+  }
+  // rain flux: every thread sums its pairs in sorted order, the warp by a fixed butterfly, the CTA its warps in order, and
+  // k_flux_sum the CTAs in order: the same bits run after run (atomics would add in arrival order)
+  __syncthreads();
+  if (tid == 0) {
+    double f = 0.0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) f += s_flux[w];
+    flux_part[blockIdx.x] = f;
   }
 }
 
-// Tile capacity and CTAs per SM by storage type (swept on the 3D workload at 16.7 M SDs; the kernel is bound by the latency
-// of its IEEE divisions and square roots, so resident warps count): fp64 state 58 B of shared memory per SD -> 560 slots,
-// 7 CTAs per SM, 72 registers (672 / 6: +7 %, 816 / 5: +17 %, 448 / 8: +7 %); fp32 state 38 B per SD -> 816 slots, 7 CTAs,
-// 72 registers (5 CTAs: +23 %, 704 / 8: the same, 560 / 10: +9 %).  No spills in either.
+// Tile capacity and CTAs per SM by storage type (the kernel is bound by instruction issue and the latency of its square
+// roots and reciprocals, so resident warps count): fp64 state 50 B of shared memory per SD -> 592 slots, 7 CTAs per SM;
+// fp32 state 34 B per SD -> 864 slots, 7 CTAs.
 #ifndef SDM_COAL_CAP
-#define SDM_COAL_CAP 560
+#define SDM_COAL_CAP 592
 #define SDM_COAL_MINB 7
 #endif
 #ifndef SDM_COAL_CAP32
-#define SDM_COAL_CAP32 816
+#define SDM_COAL_CAP32 864
 #define SDM_COAL_MINB32 7
 #endif
 #ifndef SDM_COAL_T
@@ -490,37 +664,61 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
 #endif
 template <typename R> constexpr int coal_minb() { return sizeof(R) == 4 ? SDM_COAL_MINB32 : SDM_COAL_MINB; }
 template <typename R> constexpr int coal_cap() { return sizeof(R) == 4 ? SDM_COAL_CAP32 : SDM_COAL_CAP; }
-// can a tile of cpb cells whose most populated instance holds `need` SDs run in k_coal_move_tile?
+// sparse cells (8 SDs per cell: the per-cell records, 88 B each, outweigh the SDs): fewer SD slots, room for 100 cells and more
+template <typename R> constexpr int coal_cap_sparse() { return sizeof(R) == 4 ? 512 : 384; }
+template <typename R, int CAP>
+static bool coal_tile_fits_cap(int cpb, int need) {
+  const size_t smem = CoalTile<CAP, SDM_COAL_T, R>::smem(cpb);
+  return need + cpb <= CAP && cpb <= 4096 && smem <= (size_t)(228 * 1024 - coal_minb<R>() * 1024) / coal_minb<R>();
+}
+// can a tile of cpb cells whose most populated instance holds `need` SDs run in k_coal_move_tile?  1: the dense
+// instantiation, 2: the sparse one, 0: no
 template <typename R>
-static bool coal_tile_fits_t(int cpb, int need) {
-  const size_t smem = CoalTile<coal_cap<R>(), SDM_COAL_T, R>::smem(cpb);
-  return need + cpb <= coal_cap<R>() && cpb <= 4096 && smem <= (size_t)(228 * 1024 - coal_minb<R>() * 1024) / coal_minb<R>();
+static int coal_tile_fits_t(int cpb, int need) {
+  if (coal_tile_fits_cap<R, coal_cap<R>()>(cpb, need)) return 1;
+  if (coal_tile_fits_cap<R, coal_cap_sparse<R>()>(cpb, need)) return 2;
+  return 0;
 }
 bool coal_tile_fits(int cpb, int need, int real_bytes) {
-  return real_bytes == 8 ? coal_tile_fits_t<double>(cpb, need) : coal_tile_fits_t<float>(cpb, need);
+  return (real_bytes == 8 ? coal_tile_fits_t<double>(cpb, need) : coal_tile_fits_t<float>(cpb, need)) != 0;
 }
-template <typename R>
-cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
-                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
-                                  const Counters& cnt, cudaStream_t st) {
-  const size_t smem = CoalTile<coal_cap<R>(), SDM_COAL_T, R>::smem(cpb);
-  auto kern = k_coal_move_tile<coal_cap<R>(), SDM_COAL_T, coal_minb<R>(), R>;
+template <int CAP, typename R>
+static cudaError_t launch_coal_move_tile_cap(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
+                                             const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_part,
+                                             const Counters& cnt, u32* cell_out, u32* off_out, u32* count, cudaStream_t st) {
+  const size_t smem = CoalTile<CAP, SDM_COAL_T, R>::smem(cpb);
+  auto kern = k_coal_move_tile<CAP, SDM_COAL_T, coal_minb<R>(), R>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_slots, cnt, cpb);
+  kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_part, cnt, cpb, cell_out, off_out, count);
   return cudaGetLastError();
 }
+template <typename R>
+cudaError_t launch_coal_move_tile(int cpb, int need, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
+                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_part,
+                                  const Counters& cnt, u32* cell_out, u32* off_out, u32* count, cudaStream_t st) {
+  if (coal_tile_fits_t<R>(cpb, need) == 1)
+    return launch_coal_move_tile_cap<coal_cap<R>(), R>(cpb, a, rank, seg, g, cf, kp, mp, flux_part, cnt, cell_out, off_out, count, st);
+  return launch_coal_move_tile_cap<coal_cap_sparse<R>(), R>(cpb, a, rank, seg, g, cf, kp, mp, flux_part, cnt, cell_out, off_out, count, st);
+}
 
-// sums the NSLOT flux slots in a fixed order, then clears them
-__global__ void k_flux_sum(double* flux_slots, double* flux_out, double* flux_total) {
-  __shared__ double sh[NSLOT];
-  for (int t = threadIdx.x; t < NSLOT; t += blockDim.x) { sh[t] = flux_slots[t]; flux_slots[t] = 0.0; }
+// rain flux of the step: the per-CTA partial sums of k_coal_move_tile (n_part of them; every thread sums a strided subset in
+// order, then a fixed tree) plus the NSLOT atomic slots of the per-cell kernel (summed in order, then cleared)
+__global__ void __launch_bounds__(1024) k_flux_sum(double* flux_slots, const double* __restrict__ flux_part, int n_part, double* flux_out,
+                                                   double* flux_total) {
+  __shared__ double sh[1024];
+  double f = 0.0;
+  for (int t = threadIdx.x; t < n_part; t += 1024) f += flux_part[t];
+  for (int t = threadIdx.x; t < NSLOT; t += 1024) { f += flux_slots[t]; flux_slots[t] = 0.0; }
+  sh[threadIdx.x] = f;
   __syncthreads();
+  for (int d = 512; d >= 1; d >>= 1) {
+    if ((int)threadIdx.x < d) sh[threadIdx.x] += sh[threadIdx.x + d];
+    __syncthreads();
+  }
   if (threadIdx.x == 0) {
-    double s = 0.0;
-    for (int t = 0; t < NSLOT; ++t) s += sh[t];
-    *flux_out = s;
-    *flux_total += s;
+    *flux_out = sh[0];
+    *flux_total += sh[0];
   }
 }
 
@@ -567,13 +765,14 @@ cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArraysT<R>& a
   template cudaError_t launch_coal_move<R>(int, int, bool, const SdArraysT<R>&, const u16*, const u32*, const Grid&,          \
                                            const CellFields&, const CoalParams&, const CoalMoveParams&, double*, const Counters&, \
                                            cudaStream_t);                                                               \
-  template cudaError_t launch_coal_move_tile<R>(int, const SdArraysT<R>&, const u16*, const u32*, const Grid&, const CellFields&, \
-                                                const CoalParams&, const CoalMoveParams&, double*, const Counters&, cudaStream_t);
+  template cudaError_t launch_coal_move_tile<R>(int, int, const SdArraysT<R>&, const u16*, const u32*, const Grid&, const CellFields&, \
+                                                const CoalParams&, const CoalMoveParams&, double*, const Counters&, u32*, u32*, u32*, \
+                                                cudaStream_t);
 SDM_INSTANTIATE_REAL(SDM_INST)
 #undef SDM_INST
 
-void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st) {
-  k_flux_sum<<<1, 256, 0, st>>>(const_cast<double*>(flux_slots), flux_out, flux_total);
+void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, cudaStream_t st) {
+  k_flux_sum<<<1, 1024, 0, st>>>(flux_slots, flux_part, n_part, flux_out, flux_total);
 }
 
 }  // namespace sdm

@@ -283,13 +283,40 @@ __device__ __forceinline__ void slow_setup(double y0, double rd3, double krd3, c
   s.cDK = s.c0Dc * s.Kc;
 }
 
+// Root of g(y) = y - y0 - dt' f(y) in a bracket [a, b] with g(a) g(b) < 0 that holds exactly one root (single_root_bracket):
+// Newton steps kept inside the shrinking bracket, bisection where a step leaves it.  ga_pos: g(a) > 0.  The literal
+// bisection of the paper's procedure hands over to this as soon as its bracket is certified: what it would go on to
+// compute is this root to 1e-15 b, 40 evaluations later.
+__device__ __forceinline__ double newton_in_bracket(double a, double b, bool ga_pos, double y0, const SdK& s, const CellK& c, double dtp,
+                                                    unsigned& n_eval) {
+  double y = 0.5 * (a + b);
+  for (int it = 0; it < 100; ++it) {
+    double f, df;
+    growth_fd(y, s, c, f, df);
+    ++n_eval;
+    const double g = y - y0 - dtp * f, gp = fma(-dtp, df, 1.0);
+    if (g == 0.0) return y;
+    if ((g > 0.0) == ga_pos) a = y; else b = y;
+    double yn = y - g / gp;
+    const bool newton = yn > a && yn < b;
+    if (!newton) yn = 0.5 * (a + b);
+    const double d = fabs(yn - y);
+    y = yn;
+    // a Newton step of size d leaves ~d^2 |g''/2g'| <= d^2 (100/y): stop below 1e-13 y; a bisection step bounds the error directly
+    if (newton ? (100.0 * d * d <= 1e-13 * (y * y)) : (d <= 2e-16 * y)) return y;
+    if (!(b - a > 1e-15 * b)) return 0.5 * (a + b);
+  }
+  return y;
+}
+
 // The paper's procedure (:573-579) for one SD by a whole WARP: signs of g at both ends, (a+b)/2 if they agree,
 // else bisection - five levels per round: lane l = 1..31 is node l of the binary tree of midpoints below the
 // current interval (heap order), computes its midpoint with the very operations the serial bisection would use on
 // the way there, evaluates g, and the ballot of the signs lets every lane walk the five levels.  Same result
 // as the serial loop of the oracle, a fifth of its latency.  All lanes pass the same arguments.
 __device__ __forceinline__ double bisect_paper_warp(double a, double b, double f0, double y0, const SdK& s, const CellK& c,
-                                                    double dtp, int lane, unsigned& n_ill, unsigned& n_eval) {
+                                                    double dtp, int lane, unsigned& n_ill, unsigned& n_eval, double rd3, double krd3,
+                                                    double invA, double dtcD) {
   double f, df;
   double ga, gb;
   if (a == y0) ga = -dtp * f0; else { growth_fd(a, s, c, f, df); n_eval += (lane == 0); ga = a - y0 - dtp * f; }
@@ -326,6 +353,13 @@ __device__ __forceinline__ double bisect_paper_warp(double a, double b, double f
       if ((right >> node) & 1u) { a = mm; node = 2 * node + 1; } else { b = mm; node = 2 * node; }
     }
     if (done) break;
+    // five levels narrower: once the bracket provably holds one root, Newton finishes (the same on every lane)
+    if (single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, invA, dtcD)) {
+      unsigned ev = 0;
+      const double y = newton_in_bracket(a, b, ga_pos, y0, s, c, dtp, ev);
+      n_eval += (lane == 0) ? ev : 0u;
+      return y;
+    }
   }
   return 0.5 * (a + b);
 }
@@ -360,6 +394,7 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
         if (ga == 0.0) { y_out = a; return true; }
         if (gb == 0.0) { y_out = b; return true; }
         if ((ga > 0.0) == (gb > 0.0)) { n_ill += (b - a > 1e-9 * b); y_out = 0.5 * (a + b); return true; }
+        int level = 0;
         while (b - a > 1e-15 * b) {
           const double m = 0.5 * (a + b);
           if (m <= a || m >= b) break;
@@ -368,6 +403,10 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
           const double gm = m - y0 - dtp * f;
           if (gm == 0.0) { y_out = m; return true; }
           if ((gm > 0.0) == (ga > 0.0)) { a = m; ga = gm; } else { b = m; gb = gm; }
+          if (++level % 5 == 0 && single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc)) {
+            y_out = newton_in_bracket(a, b, ga > 0.0, y0, s, c, dtp, n_eval);   // one root left in the bracket: Newton finishes
+            return true;
+          }
         }
         y_out = 0.5 * (a + b);
         return true;
@@ -953,7 +992,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
           const double a = fmax(rd2, y0 + fmin(two, 0.0)), b = y0 + fmax(two, 0.0);   // eq. 18-19
           if (a < b && !single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, R.invA, dtp * s.c0Dc)) {
             ev = (lane == 0);
-            y1 = bisect_paper_warp(a, b, f, y0, s, c, dtp, lane, ill, ev);
+            y1 = bisect_paper_warp(a, b, f, y0, s, c, dtp, lane, ill, ev, rd3, krd3, R.invA, dtp * s.c0Dc);
             solved = true;
           }
         }
@@ -1327,7 +1366,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
           const double a_ = fmax(rd2, y0 + fmin(two, 0.0)), b_ = y0 + fmax(two, 0.0);   // eq. 18-19
           if (a_ < b_ && !single_root_bracket(a_, b_, y0, c.RH, rd3, krd3, c.A, R.invA, cp.dtp * s.c0Dc)) {
             ev = (lane == 0);
-            y1 = bisect_paper_warp(a_, b_, f, y0, s, c, cp.dtp, lane, ill, ev);
+            y1 = bisect_paper_warp(a_, b_, f, y0, s, c, cp.dtp, lane, ill, ev, rd3, krd3, R.invA, cp.dtp * s.c0Dc);
             solved = true;
           }
         }

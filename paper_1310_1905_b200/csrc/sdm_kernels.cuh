@@ -18,6 +18,7 @@ struct CondParams {
 struct CoalMoveParams {
   int coal, adve, sedi, sstp_coal;
   u32 step;
+  int fold;          // k_coal_move_tile also writes next step's cell index, offset and histogram (a0-a1 folded into a6)
 };
 struct CellFields {  // library-owned dense per-cell arrays
   double* rhod;      // copy of the caller's rhod
@@ -65,11 +66,12 @@ cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArraysT<R>& a
 size_t coal_smem_bytes(int G, int cap, int sstp_coal, bool in_smem);
 // tile-resident variant for sstp_coal == 1 (cpb cells per CTA, most populated tile `need` SDs)
 bool coal_tile_fits(int cpb, int need, int real_bytes);
+// flux_part: one double per CTA (ncell of them suffice); cell_out, off_out, count: next step's a0-a1 when mp.fold
 template <typename R>
-cudaError_t launch_coal_move_tile(int cpb, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
-                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_slots,
-                                  const Counters& cnt, cudaStream_t st);
-void launch_flux_sum(const double* flux_slots, double* flux_out, double* flux_total, cudaStream_t st);
+cudaError_t launch_coal_move_tile(int cpb, int need, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
+                                  const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_part,
+                                  const Counters& cnt, u32* cell_out, u32* off_out, u32* count, cudaStream_t st);
+void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, cudaStream_t st);
 
 // sdm_recycle.cu: recycling of zero-multiplicity SDs (PAPER.md :641, :651; reading R-recycle)
 struct __align__(16) RecItem { u64 key; u32 id; u32 slot; };   // ordered by (key, id); key = ~N for donors, 0 for dead SDs

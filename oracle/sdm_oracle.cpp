@@ -47,6 +47,7 @@ struct orc_opts_t {          // PAPER.md Listing 5.1 (:677-689)
   int adve, sedi, cond, coal;
   double RH_max;
   int sstp_cond, sstp_coal;
+  double cond_adapt_tol;     // > 0: per-cell number of condensation substeps (reading R-adapt; PAPER.md :566 "planned")
 };
 struct orc_counters_t {
   long long pairs, collisions, near_ties, ill_posed, f_evals, sd_substeps;
@@ -181,13 +182,40 @@ static void sort_stage(Ctx& c) {
 }
 
 // PAPER.md :560-618: condensation substeps with feedback on r_v, theta (eq. 25-26)
+// DESIGN.md reading R-adapt (PAPER.md :566: "the actual constraints for timestep length differ substantially, particularly
+// with the distance from cloud base.  An adaptive timestep choice mechanism is planned"): the number of condensation
+// substeps of a cell in this step.  What the substeps resolve is the explicit coupling of eq. 17 to r_v and theta, so the
+// measure is how far the cell's own condensation would move its supersaturation in one step:
+//   eps = |d r_v| / (r_v max(|RH - 1|, 1e-3)),  d r_v = eq. 25 with d(r_w^3) = (3/2) r_w dt f(y) at the start of the step
+// (eq. 20 with the cell's thermodynamics and the ventilation of the SD's own radius).  The cell takes the smallest divisor d
+// of sstp_cond with d >= sstp_cond eps / tol (eps >= tol: all sstp_cond substeps; haze in equilibrium: one).
+static int adaptive_substeps(const Ctx& c, long q, const orc_opts_t& op) {
+  const CellThermo ct = cell_thermo(c.th[q], c.rv[q], c.rhod[q], op.RH_max);
+  double est = 0.0;   // sum_i N_i (3/2) r_i dt f_i, sorted order
+  for (long p = c.seg[q]; p < c.seg[q + 1]; ++p) {
+    const long i = c.order[p];
+    const double y0 = c.rw2[i], r0 = std::sqrt(y0);
+    const double vt = v_term(r0, ct.eta, ct.rho_a);
+    const double Re = 2.0 * r0 * vt * ct.rho_a / ct.eta;
+    const double f0 = growth_f(y0, c.rd3[i], c.kappa[i], ct, vent(Re, ct.Sc), vent(Re, ct.Pr));
+    est += (double)c.n[i] * (1.5 * r0 * (c.o.dt * f0));
+  }
+  const double drv = (4.0 * pi * rho_w / 3.0) / (c.rhod[q] * c.dV) * std::fabs(est);
+  const double eps = drv / (c.rv[q] * std::max(std::fabs(ct.RH - 1.0), 1e-3));
+  const double want = op.sstp_cond * eps / op.cond_adapt_tol;
+  for (int d = 1; d < op.sstp_cond; ++d)
+    if (op.sstp_cond % d == 0 && (double)d >= want) return d;
+  return op.sstp_cond;
+}
+
 static void cond_stage(Ctx& c, const orc_opts_t& op) {
-  const double dtp = c.o.dt / op.sstp_cond;
   long long ill = 0, fev = 0, sds = 0;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(c.nthreads) reduction(+ : ill, fev, sds)
   for (long q = 0; q < c.ncell; ++q) {
     const long s0 = c.seg[q], s1 = c.seg[q + 1];
-    for (int sub = 0; sub < op.sstp_cond; ++sub) {
+    const int nsub = op.cond_adapt_tol > 0.0 ? adaptive_substeps(c, q, op) : op.sstp_cond;
+    const double dtp = c.o.dt / nsub;
+    for (int sub = 0; sub < nsub; ++sub) {
       const CellThermo ct = cell_thermo(c.th[q], c.rv[q], c.rhod[q], op.RH_max);
       double sum = 0.0;   // sum_i N_i (r_w^3 new - r_w^3 old), sorted order, plain fp64
       for (long p = s0; p < s1; ++p) {

@@ -656,6 +656,78 @@ def test_condensation_conserves_total_water_and_heats():
     assert o.counters()["sd_substeps"] == 5 * 10 * N
 
 
+def test_adaptive_condensation_substeps_rule_limits_and_water_budget():
+    """DESIGN.md reading R-adapt (PAPER.md :566 "An adaptive timestep choice mechanism is planned"): a cell takes the
+    smallest divisor d of sstp_cond with d >= sstp_cond eps / tol, eps = |d r_v| / (r_v max(|RH - 1|, 1e-3)) with d r_v the
+    vapour one explicit step of the cell's growth rates would take up (eq. 25, d(r_w^3) = (3/2) r_w dt f).  Pinned by
+    (i) the limits: tol -> 0 is the fixed-substep step bit for bit, tol -> infinity is one substep per cell; (ii) the
+    rule restated here on the growth rates (themselves pinned above) predicts every cell's substep count, and the
+    counts span 1, 2, 5, 10; (iii) condensation is cell-local, so each cell must end exactly where the fixed-substep
+    oracle with sstp_cond = d ends it; (iv) the water budget of eq. 25 holds whatever the counts are."""
+    from tests import pin_helpers as _ph
+
+    rng = np.random.default_rng(18)
+    nx, nz, N, sstp, dt = 4, 6, 2400, 10, 1.0
+    ncell = nx * nz
+    th0 = np.full(ncell, 289.0)
+    rhod = np.linspace(1.15, 1.05, ncell)
+    # from dry air to a 4 % supersaturation: haze in equilibrium below, activating droplets above
+    rv0 = np.array([_rv_for_RH(s) for s in np.linspace(0.80, 1.04, ncell)]) * 1.1 / rhod
+    rd = np.exp(rng.uniform(np.log(10e-9), np.log(0.3e-6), N))
+    x, z = rng.uniform(0, 20.0 * nx, N), rng.uniform(0, 20.0 * nz, N)
+    cell = np.floor(x / 20).astype(int) * nz + np.floor(z / 20).astype(int)
+    # fewer real particles per SD in the lower of the moist cells: their uptake, and with it eps, then spans two decades
+    n = (rng.integers(10**6, 10**9, N) * 10.0 ** np.clip(-1.5 + 0.15 * (cell - 12), -1.5, 0.0)).astype(np.uint64)
+    ct = [oracle.cell_thermo(th0[q], rv0[q], rhod[q]) for q in range(ncell)]
+    rw = np.array([_ph.equilibrium_rw_brentq(rd[i] ** 3, 0.61, min(0.95, ct[cell[i]]["RH"]), ct[cell[i]]["T"]) for i in range(N)])
+    # off equilibrium by 1e-7 (lowest cell) to 1e-2 (highest), so that eps spans decades
+    rw = rw * np.exp(rng.normal(0.0, 1.0, N) * 10.0 ** (-7.0 + 5.0 * cell / (ncell - 1)))
+
+    def run(steps=1, **kw):
+        o = oracle.Oracle(nx=nx, ny=0, nz=nz, dx=20.0, dy=1.0, dz=20.0, dt=dt, seed=3)
+        o.set_fields(th=th0, rv=rv0, rhod=rhod)
+        o.set_state(n, rw**2, rd**3, np.full(N, 0.61), x=x, z=z)
+        op = oracle.make_opts(adve=False, sedi=False, cond=True, coal=False, RH_max=1.05, **kw)
+        for _ in range(steps):
+            o.step(op)
+        st = o.get_state()
+        order = np.argsort(st["id"])
+        return {k: v[order] for k, v in st.items()}, o.get_fields(), o.counters()
+
+    fixed = {d: run(sstp_cond=d) for d in (1, 2, 5, 10)}
+    # (i) limits
+    for tol, d in ((1e-300, 10), (1e300, 1)):
+        st, (th, rv), cnt = run(sstp_cond=sstp, cond_adapt_tol=tol)
+        np.testing.assert_array_equal(st["rw2"], fixed[d][0]["rw2"])
+        np.testing.assert_array_equal(rv, fixed[d][1][1])
+        assert cnt["sd_substeps"] == d * N
+    # (ii) the rule, restated: eps per cell from the growth rates at the start of the step
+    tol = 0.006
+    f0 = np.array([L.orc_growth_f(rw[i] ** 2, rd[i] ** 3, 0.61, th0[cell[i]], rv0[cell[i]], rhod[cell[i]], 1.05, rw[i] ** 2) for i in range(N)])
+    est = np.bincount(cell, weights=n.astype(float) * 1.5 * rw * dt * f0, minlength=ncell)
+    RH = np.array([min(c["RH"], 1.05) for c in ct])
+    eps = 4 * np.pi * RHO_W / 3 / (rhod * 20.0 * 1.0 * 20.0) * np.abs(est) / (rv0 * np.maximum(np.abs(RH - 1.0), 1e-3))
+    want = sstp * eps / tol
+    n_c = np.array([next((d for d in (1, 2, 5) if d >= w), 10) for w in want])
+    assert set(n_c) == {1, 2, 5, 10}, (np.bincount(n_c), want)   # the case exercises every count
+    assert min(np.abs(want - d).min() for d in (1, 2, 5)) > 1e-6   # no cell sits on a threshold
+    st, (th, rv), cnt = run(sstp_cond=sstp, cond_adapt_tol=tol)
+    assert cnt["sd_substeps"] == int(np.sum(n_c[cell]))
+    # (iii) every cell ends where the fixed-substep oracle with its own count ends it
+    for d in (1, 2, 5, 10):
+        m = n_c[cell] == d
+        np.testing.assert_array_equal(st["rw2"][m], fixed[d][0]["rw2"][m])
+        np.testing.assert_array_equal(rv[n_c == d], fixed[d][1][1][n_c == d])
+        np.testing.assert_array_equal(th[n_c == d], fixed[d][1][0][n_c == d])
+    # (iv) eq. 25 over five adaptive steps
+    dV = 20.0 * 1.0 * 20.0
+    st5, (th5, rv5), _ = run(steps=5, sstp_cond=sstp, cond_adapt_tol=tol)
+    liq0 = np.bincount(cell, weights=n.astype(float) * rw**3, minlength=ncell)
+    liq5 = np.bincount(cell, weights=st5["n"].astype(float) * st5["rw2"] ** 1.5, minlength=ncell)
+    np.testing.assert_allclose(rv5 + 4 * np.pi * RHO_W / 3 * liq5 / (rhod * dV), rv0 + 4 * np.pi * RHO_W / 3 * liq0 / (rhod * dV), rtol=2e-14)
+    assert np.abs(rv5 - rv0).max() > 1e-6
+
+
 # ----------------------------------------------------------------------------- advection / sedimentation
 def test_advection_closed_form_solves_backward_euler():
     """:536-556: eq. 16 is the solution of eq. 13-15."""

@@ -78,6 +78,8 @@ def parse():
     ap.add_argument("--cond-arith", type=int, default=8, choices=[8, 4], help="arithmetic of the condensation sweep; 4 = fp32 (needs --real-bytes 4)")
     ap.add_argument("--recycle", action="store_true", help="the paper's recycling of zero-multiplicity SDs (:641) instead of compaction only")
     ap.add_argument("--real-bytes", type=int, default=8, choices=[8, 4], help="storage type of the SD attributes (configs[4]: fp32 state)")
+    ap.add_argument("--cond-adapt-tol", type=float, default=0.0, help="adaptive condensation substeps per cell (sdm_opts.cond_adapt_tol, DESIGN.md R-adapt); "
+                    "0 = the fixed sstp_cond of the paper and of the headline")
     ap.add_argument("--long-run", type=int, default=-1, help="after the timed region, continue the run to this many steps in all and report "
                     "ms/step, evaluations per SD-substep, slow-list fraction and the launch configuration per 100-step window "
                     "(default: 600 = the length of configs[3] for the default workload, 0 otherwise)")
@@ -263,7 +265,7 @@ def main():
     dev = f"cuda:{local}"
     warm = max(a.warmup, 3)
     full3d = wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64
-    long_run = a.long_run if a.long_run >= 0 else (600 if full3d and world == 1 and not a.recycle else 0)
+    long_run = a.long_run if a.long_run >= 0 else (600 if full3d and world == 1 and not a.recycle and a.cond_adapt_tol == 0.0 else 0)
 
     w = make_workload(wa, seed=replicas.replica_seed(42, rank), device=dev)
     p = make_particles(binding, torch, w, wa, a)
@@ -274,7 +276,7 @@ def main():
     ndim = 3 if wa["ny"] > 0 else 2
     del w
     torch.cuda.empty_cache()
-    po = binding.make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=1.05, sstp_cond=10, sstp_coal=1)
+    po = binding.make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=1.05, sstp_cond=10, sstp_coal=1, cond_adapt_tol=a.cond_adapt_tol)
     fp64_peak_tflops, fp64_lanes = binding.measure_fp64_peak()   # measured on this device, before the timed region
 
     def barrier():
@@ -425,6 +427,9 @@ def main():
            "launch_config": {k: st1[k] for k in ("cond_variant", "cond_tile_cells", "coal_tile_cells", "max_cell_count")}}
     if long is not None:
         out["long_run"] = long
+    if a.cond_adapt_tol > 0.0:
+        out["config"]["cond_adapt_tol"] = a.cond_adapt_tol
+        out["sd_substeps_per_sd_step"] = subs / max(sd_steps, 1)
     if a.recycle:
         out["config"]["recycling"] = "on (PAPER.md :641)"
         out["recycled"] = st1["recycled"] - st0["recycled"]
@@ -432,7 +437,7 @@ def main():
         v, cores, desc, _, _ = oracle_rate(wa, 2, 1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                "value_1_thread": getattr(oracle_rate, "one_thread", None)}
-    if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline:
+    if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline and a.cond_adapt_tol == 0.0:
         # the same workload and step counts in the fp32 mode of configs[4] (fp32 state, fp32 condensation sweep; radii to
         # 1e-4 instead of 1e-9): a second line of context, measured by the same code in a child process
         try:
@@ -451,6 +456,18 @@ def main():
             out["fp32_mode"]["parity"] = "radii within 1e-4 of the fp64 oracle (tests/test_parity_gpu.py::test_fp32_arithmetic_condensation_2d_3d_and_first_step)"
         except Exception as ex:   # context only: never fails the bench line
             out["fp32_mode"] = {"unavailable": str(ex)[:200]}
+        # ... and with the adaptive substepping the paper plans (:566; DESIGN.md R-adapt) at cond_adapt_tol = 5e-4: changes the
+        # results by its time-discretisation error (radii of droplets: 99th percentile 2e-3 after 70 steps), hence context only
+        try:
+            cmd = [sys.executable, os.path.abspath(__file__), "--steps", str(a.steps), "--warmup", str(a.warmup), "--workload", a.workload,
+                   "--sd-per-cell", str(a.sd_per_cell), "--scale", str(a.scale), "--cond-adapt-tol", "5e-4", "--no-cpu-baseline", "--long-run", "0"]
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+            out["adaptive_substeps_mode"] = {k: d[k] for k in ("value", "unit", "ms_per_step", "stage_ms", "sd_substeps_per_sd_step")}
+            out["adaptive_substeps_mode"]["cond_adapt_tol"] = 5e-4
+            out["adaptive_substeps_mode"]["parity"] = "tests/test_parity_gpu.py::test_adaptive_condensation_substeps_match_the_oracle"
+        except Exception as ex:
+            out["adaptive_substeps_mode"] = {"unavailable": str(ex)[:200]}
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()

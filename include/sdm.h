@@ -85,6 +85,13 @@ typedef struct {
   int adve, sedi, cond, coal; /* process toggles */
   double RH_max;              /* RH limit for drop growth (:685) */
   int sstp_cond, sstp_coal;   /* numbers of substeps (:688) */
+  double cond_adapt_tol;      /* 0 (default): every cell takes sstp_cond condensation substeps, as the paper does ("the number of
+                                 subtimesteps is kept constant throughout the domain", :566).  > 0: the adaptive choice the paper
+                                 plans (:566), per cell and step (reading R-adapt): with eps = |d r_v| / (r_v max(|RH - 1|,
+                                 1e-3)), d r_v the vapour one explicit step of the cell's growth rates would take up (eq. 25), the cell
+                                 takes the smallest divisor d of sstp_cond with d >= sstp_cond * eps / cond_adapt_tol substeps of dt / d.
+                                 Changes results (by the time-discretisation error it trades); fp64-arithmetic condensation only
+                                 (SDM_ERR_INVALID with sdm_set_cond_arith(ctx, 4)). */
 } sdm_opts;
 
 /* PAPER.md Listing 5.4 (:730-745) lgrngn::arrinfo_t: element (i,j,k) of the field lives at

@@ -34,7 +34,7 @@ class OptsInit(C.Structure):
 
 class Opts(C.Structure):
     _fields_ = [("adve", C.c_int), ("sedi", C.c_int), ("cond", C.c_int), ("coal", C.c_int),
-                ("RH_max", C.c_double), ("sstp_cond", C.c_int), ("sstp_coal", C.c_int)]
+                ("RH_max", C.c_double), ("sstp_cond", C.c_int), ("sstp_coal", C.c_int), ("cond_adapt_tol", C.c_double)]
 
 
 class ArrInfo(C.Structure):
@@ -103,8 +103,8 @@ def load_library():
     return L
 
 
-def make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=44.0, sstp_cond=10, sstp_coal=1):
-    return Opts(int(adve), int(sedi), int(cond), int(coal), float(RH_max), int(sstp_cond), int(sstp_coal))
+def make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=44.0, sstp_cond=10, sstp_coal=1, cond_adapt_tol=0.0):
+    return Opts(int(adve), int(sedi), int(cond), int(coal), float(RH_max), int(sstp_cond), int(sstp_coal), float(cond_adapt_tol))
 
 
 def arrinfo(t):

@@ -425,6 +425,8 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   const Grid& g = ctx->g;
   if (!th.data_zero || !rv.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: th and rv are mandatory");
   if (op->cond && (op->sstp_cond < 1 || !(op->RH_max > 0))) return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: sstp_cond >= 1 and RH_max > 0 required");
+  if (op->cond && op->cond_adapt_tol > 0.0 && ctx->cond_arith == 4)
+    return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: cond_adapt_tol needs the fp64-arithmetic condensation (sdm_set_cond_arith 8)");
   if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_step_sync: called twice without step_async");
   ctx->last_stream = st;
   if (rhod.data_zero) { launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st); ctx->launches++; }
@@ -542,7 +544,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
       const int v = arith32 ? cond_variant_f32(cand, (int)ctx->tile_max[k]) : cond_variant(cand, (int)ctx->tile_max[k]);
       if (v && (variant == 0 || v <= variant)) { cpb = cand; variant = v; }
     }
-    CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast};
+    CondParams cp{g.dt / op->sstp_cond, op->sstp_cond, op->RH_max, ctx->kfast, op->cond_adapt_tol > 0.0 ? op->cond_adapt_tol : 0.0};
     ctx->last_cond_cpb = cpb;
     ctx->last_cond_variant = (ctx->o.real_bytes == 4 && arith32 && variant != 0 && op->sstp_cond <= 500) ? 100 + variant : variant;
     t_begin(ctx, SDM_STAGE_COND, st);

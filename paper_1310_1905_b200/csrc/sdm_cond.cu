@@ -558,7 +558,52 @@ k_cond(SdArraysT<R> a, SdArraysT<R> alt, const u16* __restrict__ rank, const u32
   }
 
   unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
-  for (int sub = 0; sub < cp.sstp && M > 0; ++sub) {
+  int nsub = cp.sstp;
+  double dtp = cp.dtp;
+  if (cp.adapt_tol > 0.0 && M > 0 && cpb == 1) {   // R-adapt (see k_cond4): the cell's number of substeps in this step
+    __shared__ double s_red[COND_WARPS];
+    __shared__ int s_nsub;
+    if (tid == 0) {
+      CellK c;
+      cell_consts(th, rv, rhod, c_exn, cp.RH_max, c, T, lv);
+      s_cell[0] = c.RH; s_cell[1] = c.A; s_cell[2] = c.c0; s_cell[3] = c.lD; s_cell[4] = c.lK; s_cell[5] = c.heat;
+      s_cell[6] = c.kE; s_cell[7] = c.Sc; s_cell[8] = c.Pr;
+    }
+    __syncthreads();
+    CellK c;
+    c.RH = s_cell[0]; c.A = s_cell[1]; c.c0 = s_cell[2]; c.lD = s_cell[3]; c.lK = s_cell[4]; c.heat = s_cell[5];
+    c.kE = s_cell[6]; c.Sc = s_cell[7]; c.Pr = s_cell[8];
+    const double dt_full = cp.dtp * cp.sstp;
+    double acc = 0.0;
+    for (int t = tid; t < M; t += COND_THREADS) {
+      double y0, rd3, krd3, dn;
+      if constexpr (SMEM) { y0 = s_y[t]; rd3 = s_rd3[t]; krd3 = s_krd3[t]; dn = s_dn[t]; }
+      else { const u32 sl = s0 + t; y0 = a.rw2[sl]; rd3 = a.rd3[sl]; krd3 = a.kappa[sl] * rd3; dn = (double)a.n[sl]; }
+      SdK sk;
+      double Dc, f, df;
+      slow_setup(y0, rd3, krd3, c, sk, Dc);
+      growth_fd(y0, sk, c, f, df);
+      acc += dn * (1.5 * sqrt(y0) * (dt_full * f));
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if (lane == 0) s_red[warp] = acc;
+    __syncthreads();
+    if (tid == 0) {
+      double est = 0.0;
+      for (int w = 0; w < COND_WARPS; ++w) est += s_red[w];
+      const double eps = fabs(fbk * est) / (rv * fmax(fabs(c.RH - 1.0), 1e-3));
+      const double want = cp.sstp * eps / cp.adapt_tol;
+      int d = cp.sstp;
+      for (int k = cp.sstp - 1; k >= 1; --k)
+        if (cp.sstp % k == 0 && (double)k >= want) d = k;
+      s_nsub = d;
+    }
+    __syncthreads();
+    nsub = s_nsub;
+    dtp = dt_full / nsub;
+  }
+  for (int sub = 0; sub < nsub && M > 0; ++sub) {
     // A. feedback of the previous substep (eq. 25-26, old theta and T) and the new cell constants
     if (tid < nc) {
       if (sub > 0) {
@@ -604,7 +649,7 @@ k_cond(SdArraysT<R> a, SdArraysT<R> alt, const u16* __restrict__ rank, const u32
           c.kE = s_cell[6 * cpb + cl]; c.Sc = s_cell[7 * cpb + cl]; c.Pr = s_cell[8 * cpb + cl];
           double y1 = y0;
           unsigned ill = 0;
-          done = cond_solve(y0, rd2, rd3, krd3, c, cp.dtp, max_evals, y1, ill, n_eval);
+          done = cond_solve(y0, rd2, rd3, krd3, c, dtp, max_evals, y1, ill, n_eval);
           if (done) {
             n_ill += ill;
             ++n_sub;
@@ -707,8 +752,10 @@ struct __align__(16) CellRec {
   double th, rv, rhod, fbk;                     // theta, r_v (advanced every substep), rho_d, eq. 25 prefactor
   double T, invT, lv, pvs;                      // eq. 43, Table 2, [L] Clausius-Clapeyron
   double invA, pad;
+  double dtp;                                   // dt' of the cell in the current substep; 0: the cell sits this substep out (R-adapt)
+  double stride;                                // the cell takes every stride-th of the sstp_cond substeps (1 without R-adapt)
 };
-static_assert(sizeof(CellRec) == 192, "CellRec");
+static_assert(sizeof(CellRec) == 208, "CellRec");
 
 // everything the substep needs from (T, 1/T, p_vs, r_v, rho_d); square roots and reciprocals from fp32
 // seeds (sqrt_seeded, rcp_nr: relative error < 1e-14, they feed correction factors and RH to 1e-15)
@@ -832,8 +879,67 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     cidx[e] = (u16)lo;
   }
   unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
-  const double dtp = cp.dtp;
   const int nsub = M > 0 ? cp.sstp : 0;
+  const bool adapt = cp.adapt_tol > 0.0 && M > 0;
+  if (adapt) {
+    // R-adapt (PAPER.md :566; oracle: adaptive_substeps): substeps of each cell from the vapour its SDs would take up in one
+    // explicit step, eps = |d r_v| / (r_v max(|RH - 1|, 1e-3)); the smallest divisor d of sstp_cond with d >= sstp_cond eps / tol
+    __syncthreads();
+    if (tid < ((nc + 31) & ~31))
+      for (int cl = tid; cl < nc; cl += T) cell_init(s_cell[cl], cp.RH_max);
+    __syncthreads();
+    const double dt_full = cp.dtp * cp.sstp;
+    for (int q0 = warp * 32; q0 < M; q0 += NW * 32) {
+      const int e = q0 + lane;
+      if (e < M) {
+        const CellRec& R = s_cell[(int)cidx[e]];
+        const double r0 = s_r[e];
+        SdK s;
+        s.rd3 = s_rd3[e]; s.krd3 = s_krd3[e];
+        CellR c;
+        c.RH = R.RH; c.A = R.A; c.lD = R.lD; c.lK = R.lK; c.qD = R.qD; c.qK = R.qK; c.lD171 = R.lD171; c.lK171 = R.lK171;
+        sd_setup(r0, R.c0, R.heat, R.kE, R.Sc, R.Pr, s);
+        double y0, f, dfr, t;
+        growth_r(r0, s, c, y0, f, dfr, t);
+        if (!(t < 4.0)) {   // beyond the range of exp_kelvin: the plain evaluation
+          CellK ck;
+          ck.RH = R.RH; ck.A = R.A; ck.c0 = R.c0; ck.lD = R.lD; ck.lK = R.lK; ck.heat = R.heat; ck.kE = R.kE; ck.Sc = R.Sc; ck.Pr = R.Pr;
+          SdK ss;
+          double Dc, df;
+          slow_setup(y0, s.rd3, s.krd3, ck, ss, Dc);
+          growth_fd(y0, ss, ck, f, df);
+        }
+        s_con[e] = s_dn[e] * (1.5 * r0 * (dt_full * f));
+      }
+    }
+    __syncthreads();
+    {
+      const int l8 = lane & 7, grp = lane >> 3;
+      for (int cl = warp * 4 + grp; cl < ((nc + 3) & ~3); cl += NW * 4) {
+        double acc = 0.0;
+        if (cl < nc) {
+          const int b1 = (int)segl[cl + 1];
+          for (int e = (int)segl[cl] + l8; e < b1; e += 8) acc += s_con[e];
+        }
+        acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+        if (cl < nc && l8 == 0) {
+          CellRec& R = s_cell[cl];
+          const double drv = fabs(R.fbk * acc);
+          const double eps = drv / (R.rv * fmax(fabs(R.RH - 1.0), 1e-3));
+          const double want = cp.sstp * eps / cp.adapt_tol;
+          int d = cp.sstp;
+          for (int k = cp.sstp - 1; k >= 1; --k)
+            if (cp.sstp % k == 0 && (double)k >= want) d = k;
+          R.stride = (double)(cp.sstp / d);
+        }
+      }
+    }
+    __syncthreads();
+  } else {
+    for (int cl = tid; cl < nc; cl += T) s_cell[cl].stride = 1.0;
+  }
   for (int sub = 0; sub <= nsub; ++sub) {
     // D. per-cell sums of N d(r_w^3): 8 lanes per cell, fixed order (deterministic); R.pad carries the sum.
     // A. feedback (eq. 25-26) and the constants of the next substep, one lane per cell on the FIRST warp(s): the chain
@@ -843,21 +949,26 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       const int l8 = lane & 7, grp = lane >> 3;
       for (int cl = warp * 4 + grp; cl < ((nc + 3) & ~3); cl += NW * 4) {   // warp-uniform trip count
         double acc = 0.0;
-        if (cl < nc) {
+        const bool was_active = cl < nc && s_cell[cl].dtp > 0.0;   // the cell took part in the substep just done
+        if (was_active) {
           const int b1 = (int)segl[cl + 1];
           for (int e = (int)segl[cl] + l8; e < b1; e += 8) acc += s_con[e];
         }
         acc += __shfl_xor_sync(0xffffffffu, acc, 4);
         acc += __shfl_xor_sync(0xffffffffu, acc, 2);
         acc += __shfl_xor_sync(0xffffffffu, acc, 1);
-        if (cl < nc && l8 == 0) s_cell[cl].pad = acc;
+        if (was_active && l8 == 0) s_cell[cl].pad = acc;
       }
       __syncthreads();
     }
     if (tid < ((nc + 31) & ~31)) {
       for (int cl = tid; cl < nc; cl += T) {
         CellRec& R = s_cell[cl];
-        if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, R.pad, cp.RH_max, true);
+        const int stride = (int)R.stride;
+        const bool now = sub < nsub && sub % stride == 0;   // the cell takes part in this substep
+        if (sub == 0) { if (!adapt) cell_init(R, cp.RH_max); }
+        else if (now || sub == nsub) cell_advance(R, R.pad, cp.RH_max, true);   // the feedback of its last substep is pending
+        R.dtp = now ? cp.dtp * stride : 0.0;
       }
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
@@ -866,9 +977,11 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     // B. dense sweep.  st: 0 = iterating, 1 = solved, 2 = left to cond_solve (list)
     for (int q0 = warp * 32; q0 < M; q0 += NW * 32) {   // static chunks (a shared counter costs an atomic, a shuffle and two S2R per chunk)
       const int e = q0 + lane;
-      const bool valid = e < M;
       const int ec = min(e, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
       const CellRec& R = s_cell[(int)cidx[ec]];
+      const double dtp = R.dtp;
+      const bool valid = e < M && dtp > 0.0;
+      if (adapt && !__any_sync(0xffffffffu, valid)) continue;   // every cell of the chunk sits this substep out
       const double r0 = s_r[ec];
       const double rd2 = s_rd2[ec];
       SdK s;
@@ -976,6 +1089,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       for (int k = per_warp ? warp : tid; k < nlist; k += per_warp ? NW : T) {
         const int e = (int)list[k];
         const CellRec& R = s_cell[(int)cidx[e]];
+        const double dtp = R.dtp;
         CellK c;
         c.RH = R.RH; c.A = R.A; c.c0 = R.c0; c.lD = R.lD; c.lK = R.lK; c.heat = R.heat; c.kE = R.kE; c.Sc = R.Sc; c.Pr = R.Pr;
         const double r0 = s_r[e], y0 = r0 * r0;

@@ -14,6 +14,7 @@ struct CondParams {
   int sstp;
   double RH_max;
   int kfast;         // growth-rate evaluations per SD in the dense sweep before an SD is deferred to the second pass
+  double adapt_tol;  // > 0: per-cell substep counts (DESIGN.md R-adapt); fp64-arithmetic kernels only
 };
 struct CoalMoveParams {
   int coal, adve, sedi, sstp_coal;

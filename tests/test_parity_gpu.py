@@ -718,6 +718,45 @@ def test_fp32_arithmetic_condensation_2d_3d_and_first_step():
         make_particles(W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1))[0].set_cond_arith(4)   # fp64 state: refused
 
 
+# ----------------------------------------------------------------------------------------------- adaptive substeps
+def test_adaptive_condensation_substeps_match_the_oracle():
+    """sdm_opts.cond_adapt_tol > 0 (reading R-adapt; PAPER.md :566 "planned"): every cell takes the number of
+    substeps the oracle's rule gives it - the totals of SD-substeps are equal, far below the fixed count - and ends where
+    the oracle ends it, to the usual bars.  Full-height 2D column set (haze below, cloud base, supersaturated top), a 3D
+    case, the fp32 state with fp64 arithmetic, cells of ~1000 SDs (medium tile) and one crowded cell (in-place kernel)."""
+    b = binding()
+    w = rain_mix(W.cfg2_2d(sd_per_cell=32, nx=10, nz=75, seed=71))
+    for tol in (0.5, 0.05):
+        p, o, th, rv = run_both(w, 6, opts=dict(cond_adapt_tol=tol))
+        sp, so = p.stats(), o.counters()
+        assert sp["sd_substeps"] == so["sd_substeps"] and sp["ill_posed"] == so["ill_posed"]
+        assert sp["collisions"] == so["collisions"]
+        assert so["sd_substeps"] < 0.8 * 10 * 6 * w.n_sd
+    fixed = 10 * 6 * w.n_sd
+    assert so["sd_substeps"] > 0.15 * fixed        # the cloudy cells keep (most of) their substeps at the tighter tolerance
+    p, o, _, _ = run_both(rain_mix(W.cfg4_3d(sd_per_cell=64, nx=5, ny=4, nz=64, seed=72)), 3, opts=dict(cond_adapt_tol=0.2))
+    assert p.stats()["sd_substeps"] == o.counters()["sd_substeps"]
+    p, o, _, _ = run_both(rain_mix(W.cfg2_2d(sd_per_cell=1000, nx=2, nz=3, seed=73), frac=0.3), 2, opts=dict(sstp_cond=6, cond_adapt_tol=0.2))
+    assert p.stats()["sd_substeps"] == o.counters()["sd_substeps"] and p.stats()["cond_variant"] == 2
+    wc = rain_mix(W.cfg2_2d(sd_per_cell=1500, nx=2, nz=3, seed=74), frac=0.3)
+    wc.state["x"] = wc.state["x"] * 0.4
+    p, o, _, _ = run_both(wc, 2, group=32, opts=dict(sstp_cond=4, cond_adapt_tol=0.2))
+    assert p.stats()["sd_substeps"] == o.counters()["sd_substeps"] and p.stats()["cond_variant"] == 3
+    wc = rain_mix(W.cfg2_2d(sd_per_cell=1500, nx=2, nz=2, seed=76), frac=0.3)
+    wc.state["x"] = wc.state["x"] * 0.499
+    wc.state["z"] = wc.state["z"] * 0.499          # ~6000 SDs in one cell: beyond every tile kernel
+    p, o, _, _ = run_both(wc, 2, opts=dict(sstp_cond=4, cond_adapt_tol=0.2))
+    assert p.stats()["sd_substeps"] == o.counters()["sd_substeps"] and p.stats()["cond_variant"] == 0
+    p, o = _fp32_case(rain_mix(W.cfg2_2d(sd_per_cell=32, nx=6, nz=75, seed=75)), steps=2, cond_adapt_tol=0.3)
+    assert p.stats()["sd_substeps"] == o.counters()["sd_substeps"]
+    w4 = W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1)
+    w4.state = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in w4.state.items()}
+    q, th, rv = make_particles(w4, real_bytes=4)
+    q.set_cond_arith(4)
+    with pytest.raises(b.SdmError, match="cond_adapt_tol"):
+        q.step_sync(b.make_opts(cond_adapt_tol=0.1, RH_max=1.05), th, rv)
+
+
 # ----------------------------------------------------------------------------------------------- sync / async
 def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
     """PAPER.md :816 and Figure 7 (:833-848): step_sync returns th, rv for the host model, step_async (coalescence +

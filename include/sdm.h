@@ -249,6 +249,15 @@ int sdm_set_cond_arith(sdm_ctx* ctx, int bytes);
  * to the compacted second pass (1..200, default 4).  Does not change results beyond the solver tolerance. */
 int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast);
 
+/* The "prototype transport equation solver" of PAPER.md Figure 7 and section 5.2.2 (:831-852): one first-order upstream
+ * (donor-cell; :219-235) step of the scalar field psi (DEVICE, strided as the other Eulerian fields; overwritten) with the
+ * rho_d x Courant arrays and rho_d the context holds since sdm_init* / the last step_sync (:751): psi' = psi - sum over the
+ * dimensions of (F_hi - F_lo) / rho_d, F = max(rho_d C, 0) psi_donor-side + min(rho_d C, 0) psi_other at each face; periodic
+ * in x and y, psi continued by its boundary value below and above.  This is what the host model does to theta and r_v
+ * between step_sync and the next step_sync, on a stream of its own, while step_async runs (:816); the library's own step
+ * never calls it.  Enqueues 2 kernels on `stream`; the first call allocates nx*ny*nz doubles of scratch. */
+int sdm_upstream_advect(sdm_ctx* ctx, sdm_arrinfo psi, void* stream);
+
 /* Measurement aid, not part of the step (the condensation kernel of PAPER.md eq. 17-24, which
  * "takes most of the simulation time" (:912), is bound by fp64 arithmetic, so its roofline needs a MEASURED fp64 peak):
  * runs a register-only kernel of independent fp64 FMA chains on every SM of the current device and returns the best of

@@ -91,6 +91,7 @@ def lib():
         L.orc_get_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_order.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_get_counters.argtypes = [C.c_void_p, C.POINTER(_Counters)]
+        L.orc_upstream_advect.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_rain_flux_total.argtypes = [C.c_void_p]
         L.orc_rain_flux_total.restype = C.c_double
         L.orc_diag_mom.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int, C.c_void_p]
@@ -227,6 +228,13 @@ class Oracle:
         ids, seg = np.empty(N, np.uint32), np.empty(self.ncell + 1, np.int64)
         self.L.orc_get_order(self.h, _ptr(ids), _ptr(seg))
         return ids, seg
+
+    def upstream_advect(self, psi):
+        """One first-order upstream step (PAPER.md :219-235; the transport solver of Fig. 7) of the dense C-order field psi
+        with the rho_d x Courant arrays set by set_fields; returns the new field."""
+        out = np.ascontiguousarray(psi, dtype=np.float64).copy()
+        self.L.orc_upstream_advect(self.h, _ptr(out))
+        return out
 
     def counters(self):
         c = _Counters()

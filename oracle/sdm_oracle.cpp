@@ -616,6 +616,40 @@ void orc_get_order(void* h, u32* ids_sorted, long* seg) {
   for (size_t p = 0; p < c.order.size(); ++p) ids_sorted[p] = c.id[c.order[p]];
   memcpy(seg, c.seg.data(), (c.ncell + 1) * sizeof(long));
 }
+// One first-order upstream (donor-cell) step of a scalar field on the Arakawa-C grid (PAPER.md :219-235; the prototype
+// transport solver of Figure 7, :831-852) with the rho_d x Courant arrays of the context: psi' = psi - sum_dims (F_hi - F_lo) /
+// rho_d, F = max(rho_d C, 0) psi_donor-side + min(rho_d C, 0) psi_other; periodic in x and y, boundary value beyond bottom and top.
+void orc_upstream_advect(void* h, double* psi) {
+  const Ctx& c = *(Ctx*)h;
+  const int NX = c.NX, NY = c.NY, NZ = c.NZ;
+  const bool hx = c.o.nx > 0, hy = c.o.ny > 0, hz = c.o.nz > 0;
+  std::vector<double> out(c.ncell);
+  auto at = [&](int i, int j, int k) { return psi[((long)i * NY + j) * NZ + k]; };
+  for (int i = 0; i < NX; ++i)
+    for (int j = 0; j < NY; ++j)
+      for (int k = 0; k < NZ; ++k) {
+        const double pc = at(i, j, k);
+        double acc = 0.0;
+        if (hx) {
+          const double pm = at(i == 0 ? NX - 1 : i - 1, j, k), pp = at(i == NX - 1 ? 0 : i + 1, j, k);
+          const double Cl = c.cx[((long)i * NY + j) * NZ + k], Ch = c.cx[((long)(i + 1) * NY + j) * NZ + k];
+          acc = acc + ((std::fmax(Ch, 0.0) * pc + std::fmin(Ch, 0.0) * pp) - (std::fmax(Cl, 0.0) * pm + std::fmin(Cl, 0.0) * pc));
+        }
+        if (hy) {
+          const double pm = at(i, j == 0 ? NY - 1 : j - 1, k), pp = at(i, j == NY - 1 ? 0 : j + 1, k);
+          const double Cl = c.cy[((long)i * (NY + 1) + j) * NZ + k], Ch = c.cy[((long)i * (NY + 1) + j + 1) * NZ + k];
+          acc = acc + ((std::fmax(Ch, 0.0) * pc + std::fmin(Ch, 0.0) * pp) - (std::fmax(Cl, 0.0) * pm + std::fmin(Cl, 0.0) * pc));
+        }
+        if (hz) {
+          const double pm = at(i, j, k == 0 ? 0 : k - 1), pp = at(i, j, k == NZ - 1 ? k : k + 1);
+          const double Cl = c.cz[((long)i * NY + j) * (NZ + 1) + k], Ch = c.cz[((long)i * NY + j) * (NZ + 1) + k + 1];
+          acc = acc + ((std::fmax(Ch, 0.0) * pc + std::fmin(Ch, 0.0) * pp) - (std::fmax(Cl, 0.0) * pm + std::fmin(Cl, 0.0) * pc));
+        }
+        out[((long)i * NY + j) * NZ + k] = pc - acc / c.rhod[((long)i * NY + j) * NZ + k];
+      }
+  std::copy(out.begin(), out.end(), psi);
+}
+
 void orc_get_counters(void* h, orc_counters_t* out) { *out = ((Ctx*)h)->cnt; }
 double orc_rain_flux_total(void* h) { return ((Ctx*)h)->rain_flux_total; }
 

@@ -51,7 +51,7 @@ EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_n_live", "sdm_export_state", "sdm_export_order",
            "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith",
-           "sdm_measure_fp64_peak"]
+           "sdm_measure_fp64_peak", "sdm_upstream_advect"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
@@ -88,6 +88,7 @@ def load_library():
     L.sdm_outbuf.restype = vp
     L.sdm_n_sd.argtypes = [vp, u64p]
     L.sdm_n_live.argtypes = [vp, u64p]
+    L.sdm_upstream_advect.argtypes = [vp, ArrInfo, vp]
     L.sdm_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     L.sdm_export_state.argtypes = [vp] + [vp] * 8 + [vp]
     L.sdm_export_order.argtypes = [vp, vp, vp, vp]
@@ -240,6 +241,10 @@ class Particles:
         v = C.c_uint64()
         self._ck(self.L.sdm_n_sd(self.h, C.byref(v)))
         return v.value
+
+    def upstream_advect(self, psi):
+        """One upstream step of the field psi (overwritten) with the context's Courant numbers: the Eulerian solver of Fig. 7."""
+        self._ck(self.L.sdm_upstream_advect(self.h, arrinfo(psi), _stream()))
 
     def n_live(self):
         v = C.c_uint64()

@@ -20,6 +20,7 @@ UNITS = {
     "sdm_init.cu": ["-fmad=false"],
     "sdm_recycle.cu": [],
     "sdm_peak.cu": [],
+    "sdm_euler.cu": ["-fmad=false"],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 

@@ -51,6 +51,7 @@ struct sdm_ctx {
   CellFields cf{};
   double *cx = nullptr, *cy = nullptr, *cz = nullptr;
   double* outbuf = nullptr;
+  double* adv_tmp = nullptr;     // scratch of sdm_upstream_advect
   double* flux_slots = nullptr;
   double* flux_part = nullptr;   // per-CTA rain flux of k_coal_move_tile
   int n_flux_part = 0;
@@ -321,6 +322,7 @@ void sdm_destroy(sdm_ctx* ctx) {
   cudaFree(ctx->cell); cudaFree(ctx->off); cudaFree(ctx->rank); cudaFree(ctx->count); cudaFree(ctx->blocksum); cudaFree(ctx->seg);
   cudaFree(ctx->d_info); cudaFree(ctx->cf.rhod); cudaFree(ctx->cf.eta); cudaFree(ctx->cf.rho_a); cudaFree(ctx->outbuf);
   cudaFree(ctx->th_dense); cudaFree(ctx->rv_dense); cudaFree(ctx->cx); cudaFree(ctx->cy); cudaFree(ctx->cz);
+  cudaFree(ctx->adv_tmp);
   cudaFree(ctx->flux_slots); cudaFree(ctx->flux_part); cudaFree(ctx->d_flux); cudaFree(ctx->cnt_mem);
   cudaFree(ctx->d_effR); cudaFree(ctx->d_effq); cudaFree(ctx->d_efftab);
   if (ctx->h_info) cudaFreeHost(ctx->h_info);
@@ -694,6 +696,16 @@ const double* sdm_outbuf(sdm_ctx* ctx) { return ctx ? ctx->outbuf : nullptr; }
 int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd) {
   if (!ctx || !n_sd) return SDM_ERR_INVALID;
   *n_sd = ctx->nslots;
+  return SDM_OK;
+}
+
+int sdm_upstream_advect(sdm_ctx* ctx, sdm_arrinfo psi, void* stream) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (!psi.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_upstream_advect: psi is mandatory");
+  if (!ctx->adv_tmp) CK(dalloc(&ctx->adv_tmp, (size_t)ctx->g.ncell));
+  launch_upstream(make_field(ctx, psi), ctx->g, ctx->cf, ctx->adv_tmp, (cudaStream_t)stream);
+  ctx->launches += 2;
+  CK(cudaGetLastError());
   return SDM_OK;
 }
 

@@ -109,4 +109,7 @@ void launch_diag_mom(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_boun
                      double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st);
 void launch_dense_copy(Field src, double* dst, int n0, int n1, int n2, cudaStream_t st);
 
+// sdm_euler.cu: one upstream step of a scalar field with the context's rho_d x Courant arrays (tmp: ncell doubles); 2 launches
+void launch_upstream(Field psi, const Grid& g, const CellFields& cf, double* tmp, cudaStream_t st);
+
 }  // namespace sdm

@@ -728,6 +728,52 @@ def test_adaptive_condensation_substeps_rule_limits_and_water_budget():
     assert np.abs(rv5 - rv0).max() > 1e-6
 
 
+# ----------------------------------------------------------------------------- Eulerian transport (Fig. 7 prototype solver)
+def test_upstream_step_is_the_textbook_donor_cell_scheme():
+    """PAPER.md :219-235 (upstream scheme), Figure 7 (:831-852): the Eulerian step the host model takes between step_sync
+    and the next one.  Pinned by what the donor-cell scheme is known to do: a Courant number of +1 / -1 shifts the field
+    by exactly one cell down / up the axis, 1/2 averages a cell with its upwind neighbour, the flux form conserves
+    sum(rho_d psi) on the periodic domain, and a constant field is a fixed point of a discretely non-divergent flow."""
+    rng = np.random.default_rng(23)
+    # 1D along x: rho_d = 1, so the array holds plain Courant numbers
+    nx = 17
+    psi = rng.uniform(1.0, 2.0, nx)
+    for C, expect in ((1.0, np.roll(psi, 1)), (-1.0, np.roll(psi, -1)), (0.5, 0.5 * psi + 0.5 * np.roll(psi, 1)),
+                      (-0.25, 0.75 * psi + 0.25 * np.roll(psi, -1))):
+        o = oracle.Oracle(nx=nx, ny=0, nz=0, dx=1.0, dy=1.0, dz=1.0, dt=1.0)
+        o.set_fields(th=np.ones(nx), rv=np.ones(nx), rhod=np.ones(nx), cx=np.full(nx + 1, C))
+        np.testing.assert_allclose(o.upstream_advect(psi), expect, rtol=1e-15)
+    # 3D: a non-divergent flow from two stream functions differenced on the C-grid, rho_d varying with height
+    nx, ny, nz = 6, 5, 7
+    psi1, psi2 = rng.normal(size=(nx + 1, nz + 1)), rng.normal(size=(ny + 1, nz + 1))
+    psi1[-1], psi2[-1] = psi1[0], psi2[0]                         # periodic in x and y
+    psi1[:, 0] = psi1[:, -1] = psi2[:, 0] = psi2[:, -1] = 0.0     # no flow through bottom and top
+    cx = np.broadcast_to((-0.2 * (psi1[:, 1:] - psi1[:, :-1]))[:, None, :], (nx + 1, ny, nz))
+    cy = np.broadcast_to((-0.2 * (psi2[:, 1:] - psi2[:, :-1]))[None, :, :], (nx, ny + 1, nz))
+    cz = 0.2 * ((psi1[1:, :] - psi1[:-1, :])[:, None, :] + (psi2[1:, :] - psi2[:-1, :])[None, :, :])
+    rhod = np.broadcast_to(np.linspace(1.2, 1.0, nz), (nx, ny, nz)).ravel().copy()
+    o = oracle.Oracle(nx=nx, ny=ny, nz=nz, dx=1.0, dy=1.0, dz=1.0, dt=1.0)
+    o.set_fields(th=np.ones(nx * ny * nz), rv=np.ones(nx * ny * nz), rhod=rhod, cx=cx.ravel(), cy=cy.ravel(), cz=cz.ravel())
+    f = rng.uniform(280.0, 300.0, nx * ny * nz)
+    g = o.upstream_advect(f)
+    assert np.abs(g - f).max() > 1e-3                             # the field did move
+    np.testing.assert_allclose(np.sum(rhod * g), np.sum(rhod * f), rtol=1e-14)
+    const = np.full(nx * ny * nz, 289.0)
+    np.testing.assert_allclose(o.upstream_advect(const), const, rtol=1e-14)
+    # a y-only and a z-only shift, to pin the index arithmetic of every dimension
+    for dim, shift_axis in (("y", 1), ("z", 2)):
+        kw = dict(cx=np.zeros((nx + 1) * ny * nz), cy=np.zeros(nx * (ny + 1) * nz), cz=np.zeros(nx * ny * (nz + 1)))
+        kw["c" + dim] = np.ones_like(kw["c" + dim])
+        o.set_fields(th=const, rv=const, rhod=np.ones(nx * ny * nz), **kw)
+        h = o.upstream_advect(f).reshape(nx, ny, nz)
+        f3 = f.reshape(nx, ny, nz)
+        if dim == "y":
+            np.testing.assert_allclose(h, np.roll(f3, 1, axis=1), rtol=1e-15)
+        else:   # not periodic in z: the boundary value enters at the bottom
+            np.testing.assert_allclose(h[:, :, 1:], f3[:, :, :-1], rtol=1e-15)
+            np.testing.assert_allclose(h[:, :, 0], f3[:, :, 0], rtol=1e-15)
+
+
 # ----------------------------------------------------------------------------- advection / sedimentation
 def test_advection_closed_form_solves_backward_euler():
     """:536-556: eq. 16 is the solution of eq. 13-15."""

@@ -758,18 +758,37 @@ def test_adaptive_condensation_substeps_match_the_oracle():
 
 
 # ----------------------------------------------------------------------------------------------- sync / async
+def test_upstream_advect_matches_the_oracle_bit_for_bit():
+    """sdm_upstream_advect, the prototype transport solver of PAPER.md Figure 7 (:831-852; upstream scheme :219-235): the same
+    IEEE operations in the same order as the oracle's restatement, so the fields are equal to the bit - 2D and 3D, dense
+    and halo-padded (strided) fields, five steps in a row."""
+    for w in (W.cfg2_2d(sd_per_cell=4, nx=23, nz=17, seed=81), W.cfg4_3d(sd_per_cell=2, nx=9, ny=7, nz=11, seed=82)):
+        o = make_oracle(w)
+        p, th, rv = make_particles(w)
+        shape = tuple(th.shape)
+        pad = torch.zeros(tuple(n + 4 for n in shape), dtype=torch.float64, device="cuda")
+        view = pad[tuple(slice(2, 2 + n) for n in shape)]
+        view.copy_(th + 0.01 * torch.rand(shape, dtype=torch.float64, device="cuda"))
+        dense = view.clone()
+        ref = np_(dense).ravel()
+        for _ in range(5):
+            p.upstream_advect(dense)
+            p.upstream_advect(view)       # non-contiguous: strides of the padded array
+            ref = o.upstream_advect(ref)
+        np.testing.assert_array_equal(np_(dense).ravel(), ref)
+        np.testing.assert_array_equal(np_(view.contiguous()).ravel(), ref)
+        assert float(pad.sum()) == pytest.approx(float(view.sum()))   # the halo was not touched
+        assert np.abs(ref - np_(th).ravel()).max() > 1e-4
+
+
 def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
     """PAPER.md :816 and Figure 7 (:833-848): step_sync returns th, rv for the host model, step_async (coalescence +
-    movement, which touch neither) runs while the Eulerian solver advances th, rv.  Here the "solver" is a first-order
-    upstream shift of th, rv on a second stream, ordered after step_sync by an event.  Checked: step_async returns
-    to the host before its device work is done, the overlapped run equals the serialised one bit for bit, and it
-    matches the oracle driven the same way."""
+    movement, which touch neither) runs while the Eulerian solver advances th, rv.  The solver is the library's upstream
+    step (sdm_upstream_advect, Fig. 7's "prototype transport equation solver") on a second stream, ordered after
+    step_sync by an event.  Checked: step_async returns to the host before its device work is done, the overlapped run
+    equals the serialised one bit for bit, and it matches the oracle driven through the same calling sequence."""
     b = binding()
     w = W.cfg4_3d(sd_per_cell=64, nx=48, ny=48, nz=64, seed=61, device="cuda")
-
-    def solver(th, rv):   # stand-in for the host model's advection step (not part of libsdm)
-        th.copy_(0.75 * th + 0.25 * torch.roll(th, 1, 0))
-        rv.copy_(0.75 * rv + 0.25 * torch.roll(rv, 1, 0))
 
     def run(overlap):
         p, th, rv = make_particles(w)
@@ -790,7 +809,8 @@ def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
                 s1.synchronize()
             with torch.cuda.stream(s2):
                 s2.wait_event(ready)
-                solver(th, rv)
+                p.upstream_advect(th)
+                p.upstream_advect(rv)
             s1.wait_stream(s2)   # the next step_sync reads the solver's th, rv
             with torch.cuda.stream(s1):
                 p.step_async_result()
@@ -813,11 +833,10 @@ def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
         o.step_sync(oo)
         p.step_async(po)
         o.step_async(oo)
-        solver(th, rv)
+        p.upstream_advect(th)
+        p.upstream_advect(rv)
         oth, orv = o.get_fields()
-        oth, orv = torch.from_numpy(oth.reshape(th.shape).copy()), torch.from_numpy(orv.reshape(rv.shape).copy())
-        solver(oth, orv)
-        o.set_fields(th=oth.numpy().ravel(), rv=orv.numpy().ravel())
+        o.set_fields(th=o.upstream_advect(oth), rv=o.upstream_advect(orv))
     compare_states(p, o)
     compare_fields(th, rv, o)
 

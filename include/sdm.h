@@ -78,6 +78,9 @@ typedef struct {
   uint64_t max_sd;          /* capacity in super-droplets (HBM is allocated once, at creation) */
   int n_modes;              /* dry_distros (:703-708): number of lognormal modes, 0..8 (0: sdm_init unavailable) */
   const sdm_lognormal_mode* modes; /* HOST, n_modes entries; copied */
+  int open_x;               /* 0: x is periodic (PAPER.md :558).  1: this context is one slab of a domain decomposed along x
+                               (SURVEY.md section 8e): SDs moved beyond x < 0 or x >= nx*dx keep their coordinate and must be
+                               handed to the neighbour with sdm_pack_leavers before the next step_sync */
 } sdm_opts_init;
 
 /* PAPER.md Listing 5.1 (:677-689) lgrngn::opts_t */
@@ -248,6 +251,26 @@ int sdm_set_cond_arith(sdm_ctx* ctx, int bytes);
 /* Tuning override: growth-rate evaluations the dense condensation sweep spends on an SD before deferring it
  * to the compacted second pass (1..200, default 4).  Does not change results beyond the solver tolerance. */
 int sdm_set_cond_kfast(sdm_ctx* ctx, int kfast);
+
+/* Domain decomposition along x (PAPER.md :843 "in case of domain decomposition"): every stage but the
+ * movement of eq. 16 is local to a cell, so a rank owns a slab of columns (a context created with open_x = 1 on its own nx
+ * columns, coordinates relative to the slab) and after step_async exchanges the SDs that crossed its two faces.
+ * sdm_sd_buffers: one SoA set of DEVICE arrays, caller-owned; rw2 .. z of real_bytes-sized reals; y, z may be NULL when absent. */
+typedef struct {
+  uint64_t* n;
+  void *rw2, *rd3, *kappa, *x, *y, *z;
+  uint32_t* id;
+} sdm_sd_buffers;
+/* Moves every live SD with x < 0 into `left` and every one with x >= nx*dx into `right` (coordinates unchanged, any order)
+ * and marks its slot N = 0 (the next step_sync compacts it away).  cap: elements each buffer array holds.  *n_left,
+ * *n_right: HOST outputs.  If either count exceeds cap nothing is moved and SDM_ERR_CAPACITY is returned with the counts
+ * set.  To be called after step_async of the step; waits for it.  Blocking. */
+int sdm_pack_leavers(sdm_ctx* ctx, uint64_t cap, const sdm_sd_buffers* left, const sdm_sd_buffers* right, uint64_t* n_left,
+                     uint64_t* n_right, void* stream);
+/* Appends N SDs (a neighbour's `right` list with x_shift = minus that neighbour's slab width, or its `left` list with
+ * x_shift = plus this slab's width) behind the SDs in storage, x + x_shift being their coordinate in this slab.  Ids travel
+ * with the SDs (they key the Philox streams).  SDM_ERR_CAPACITY beyond max_sd.  Enqueues on `stream`. */
+int sdm_unpack_arrivals(sdm_ctx* ctx, uint64_t N, const sdm_sd_buffers* in, double x_shift, void* stream);
 
 /* The "prototype transport equation solver" of PAPER.md Figure 7 and section 5.2.2 (:831-852): one first-order upstream
  * (donor-cell; :219-235) step of the scalar field psi (DEVICE, strided as the other Eulerian fields; overwritten) with the

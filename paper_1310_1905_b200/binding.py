@@ -29,7 +29,7 @@ class OptsInit(C.Structure):
                 ("n_eff_R", C.c_int), ("n_eff_q", C.c_int),
                 ("eff_R", C.c_void_p), ("eff_q", C.c_void_p), ("eff_tab", C.c_void_p),
                 ("seed", C.c_uint64), ("real_bytes", C.c_int), ("multi_coal", C.c_int), ("max_sd", C.c_uint64),
-                ("n_modes", C.c_int), ("modes", C.c_void_p)]
+                ("n_modes", C.c_int), ("modes", C.c_void_p), ("open_x", C.c_int)]
 
 
 class Opts(C.Structure):
@@ -39,6 +39,11 @@ class Opts(C.Structure):
 
 class ArrInfo(C.Structure):
     _fields_ = [("data_zero", C.c_void_p), ("strides", C.c_int64 * 3)]
+
+
+class SdBuffers(C.Structure):
+    _fields_ = [("n", C.c_void_p), ("rw2", C.c_void_p), ("rd3", C.c_void_p), ("kappa", C.c_void_p), ("x", C.c_void_p),
+                ("y", C.c_void_p), ("z", C.c_void_p), ("id", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -51,7 +56,7 @@ EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_n_live", "sdm_export_state", "sdm_export_order",
            "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith",
-           "sdm_measure_fp64_peak", "sdm_upstream_advect"]
+           "sdm_measure_fp64_peak", "sdm_upstream_advect", "sdm_pack_leavers", "sdm_unpack_arrivals"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
@@ -89,6 +94,8 @@ def load_library():
     L.sdm_n_sd.argtypes = [vp, u64p]
     L.sdm_n_live.argtypes = [vp, u64p]
     L.sdm_upstream_advect.argtypes = [vp, ArrInfo, vp]
+    L.sdm_pack_leavers.argtypes = [vp, C.c_uint64, C.POINTER(SdBuffers), C.POINTER(SdBuffers), u64p, u64p, vp]
+    L.sdm_unpack_arrivals.argtypes = [vp, C.c_uint64, C.POINTER(SdBuffers), C.c_double, vp]
     L.sdm_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     L.sdm_export_state.argtypes = [vp] + [vp] * 8 + [vp]
     L.sdm_export_order.argtypes = [vp, vp, vp, vp]
@@ -134,7 +141,7 @@ class Particles:
 
     def __init__(self, nx=0, ny=0, nz=0, dx=1.0, dy=1.0, dz=1.0, dt=1.0, kernel="geometric", golovin_b=1500.0,
                  multi_coal=True, seed=42, eff_R=None, eff_q=None, eff_tab=None, max_sd=None, sd_conc_mean=0.0, modes=None,
-                 x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None, real_bytes=8):
+                 x0=0.0, y0=0.0, z0=0.0, x1=None, y1=None, z1=None, real_bytes=8, open_x=False):
         """real_bytes: 8 or 4, the storage type of rw2, rd3, kappa, x, y, z (fields stay float64).  modes: [(kappa, N_stp, r_mean, sigma_g), ...] of the dry spectrum, needed by init() only."""
         import numpy as np
         self.L = load_library()
@@ -153,6 +160,7 @@ class Particles:
             o.n_eff_R, o.n_eff_q = len(keep[0]), len(keep[1])
             o.eff_R, o.eff_q, o.eff_tab = (k.ctypes.data for k in keep)
         o.seed, o.real_bytes, o.multi_coal, o.max_sd = seed, int(real_bytes), int(multi_coal), int(max_sd)
+        o.open_x = int(bool(open_x))
         self.real = torch.float64 if int(real_bytes) == 8 else torch.float32
         self.h = C.c_void_p()
         rc = self.L.sdm_create(C.byref(o), C.byref(self.h))
@@ -241,6 +249,30 @@ class Particles:
         v = C.c_uint64()
         self._ck(self.L.sdm_n_sd(self.h, C.byref(v)))
         return v.value
+
+    def _sd_buffers(self, cap):
+        """A set of SoA device arrays for `cap` SDs (sdm_sd_buffers) and its ctypes view."""
+        t = dict(n=torch.empty(cap, dtype=torch.int64, device="cuda"), id=torch.empty(cap, dtype=torch.int32, device="cuda"))
+        for k in ("rw2", "rd3", "kappa", "x", "y", "z"):
+            t[k] = torch.zeros(cap, dtype=self.real, device="cuda")
+        return t, SdBuffers(*[_ptr(t[k]) for k in ("n", "rw2", "rd3", "kappa", "x", "y", "z", "id")])
+
+    def pack_leavers(self, cap):
+        """SDs that left the slab through x < 0 and through x >= nx*dx, as two dicts of tensors (open_x contexts only)."""
+        lt, lb = self._sd_buffers(max(cap, 1))
+        rt, rb = self._sd_buffers(max(cap, 1))
+        nl, nr = C.c_uint64(), C.c_uint64()
+        self._ck(self.L.sdm_pack_leavers(self.h, max(cap, 1), C.byref(lb), C.byref(rb), C.byref(nl), C.byref(nr), _stream()))
+        return {k: v[:nl.value] for k, v in lt.items()}, {k: v[:nr.value] for k, v in rt.items()}
+
+    def unpack_arrivals(self, sds, x_shift):
+        """Appends the SDs of `sds` (a dict as pack_leavers returns) with x + x_shift as their coordinate in this slab."""
+        N = int(sds["n"].numel())
+        if N == 0:
+            return
+        t = {k: v.contiguous() for k, v in sds.items()}
+        b = SdBuffers(*[_ptr(t[k]) for k in ("n", "rw2", "rd3", "kappa", "x", "y", "z", "id")])
+        self._ck(self.L.sdm_unpack_arrivals(self.h, N, C.byref(b), float(x_shift), _stream()))
 
     def upstream_advect(self, psi):
         """One upstream step of the field psi (overwritten) with the context's Courant numbers: the Eulerian solver of Fig. 7."""

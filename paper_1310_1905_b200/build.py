@@ -21,6 +21,7 @@ UNITS = {
     "sdm_recycle.cu": [],
     "sdm_peak.cu": [],
     "sdm_euler.cu": ["-fmad=false"],
+    "sdm_slab.cu": [],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 

@@ -222,6 +222,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
   Grid& g = ctx->g;
   g.NX = std::max(o->nx, 1); g.NY = std::max(o->ny, 1); g.NZ = std::max(o->nz, 1);
   g.hx = o->nx > 0; g.hy = o->ny > 0; g.hz = o->nz > 0;
+  g.open_x = (o->open_x && g.hx) ? 1 : 0;
   g.ncell = (int)ncell;
   g.dx = o->dx; g.dy = o->dy; g.dz = o->dz; g.dt = o->dt;
   g.dV = o->dx * o->dy * o->dz;
@@ -583,7 +584,8 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     bool in_smem = coal_smem_bytes(G, cap, sstp, true) <= kSmemLimit;
     if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
       return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
-    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step, ctx->recycle ? 0 : 1};
+    // (a slab hands SDs over after the step, recycling moves them before the next: the histogram is then built by k_cellhist)
+    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step, (ctx->recycle || g.open_x) ? 0 : 1};
     int tile_cpb = 0, tile_need = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
     for (int k = 0; k < 4 && !tile_cpb && sstp == 1 && !ctx->group_override; ++k) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
@@ -696,6 +698,71 @@ const double* sdm_outbuf(sdm_ctx* ctx) { return ctx ? ctx->outbuf : nullptr; }
 int sdm_n_sd(sdm_ctx* ctx, uint64_t* n_sd) {
   if (!ctx || !n_sd) return SDM_ERR_INVALID;
   *n_sd = ctx->nslots;
+  return SDM_OK;
+}
+
+}  // extern "C"
+
+namespace {
+template <typename R>
+SdArraysT<R> buffers_view(const sdm_sd_buffers& b) {
+  return SdArraysT<R>{b.n, (R*)b.rw2, (R*)b.rd3, (R*)b.kappa, (R*)b.x, (R*)b.y, (R*)b.z, b.id};
+}
+bool buffers_ok(const sdm_ctx* c, const sdm_sd_buffers* b) {
+  return b && b->n && b->rw2 && b->rd3 && b->kappa && b->x && b->id && (!c->g.hy || b->y) && (!c->g.hz || b->z);
+}
+}  // namespace
+
+extern "C" {
+
+int sdm_pack_leavers(sdm_ctx* ctx, uint64_t cap, const sdm_sd_buffers* left, const sdm_sd_buffers* right, uint64_t* n_left,
+                     uint64_t* n_right, void* stream) {
+  if (!ctx || !n_left || !n_right) return SDM_ERR_INVALID;
+  if (!ctx->g.open_x) return fail(ctx, SDM_ERR_ORDER, "sdm_pack_leavers: the context was not created with open_x = 1");
+  if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_pack_leavers: call it after step_async of the step");
+  if (!buffers_ok(ctx, left) || !buffers_ok(ctx, right)) return fail(ctx, SDM_ERR_INVALID, "sdm_pack_leavers: NULL buffer array");
+  cudaStream_t st = (cudaStream_t)stream;
+  ctx->last_stream = st;
+  CK(cudaStreamWaitEvent(st, ctx->ev_async, 0));
+  u32* cnt2 = ctx->d_info + 6;   // two of the tile-maximum words: free between step_async and the next step_sync
+  const bool f64 = ctx->o.real_bytes == 8;
+  if (f64) launch_count_leavers(view<double>(ctx->buf[ctx->cur]), (u32)ctx->nslots, ctx->g, cnt2, st);
+  else launch_count_leavers(view<float>(ctx->buf[ctx->cur]), (u32)ctx->nslots, ctx->g, cnt2, st);
+  u32 h[2] = {0, 0};
+  CK(cudaMemcpyAsync(h, cnt2, sizeof(h), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  ctx->launches += ctx->nslots ? 1 : 0;
+  *n_left = h[0]; *n_right = h[1];
+  if (h[0] > cap || h[1] > cap) return fail(ctx, SDM_ERR_CAPACITY, "sdm_pack_leavers: more leavers than the buffers hold");
+  if (h[0] + h[1] == 0) return SDM_OK;
+  if (f64) launch_pack_leavers(view<double>(ctx->buf[ctx->cur]), (u32)ctx->nslots, ctx->g, buffers_view<double>(*left), buffers_view<double>(*right), cnt2, st);
+  else launch_pack_leavers(view<float>(ctx->buf[ctx->cur]), (u32)ctx->nslots, ctx->g, buffers_view<float>(*left), buffers_view<float>(*right), cnt2, st);
+  ctx->launches++;
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(st));
+  ctx->hist_valid = false;
+  return SDM_OK;
+}
+
+int sdm_unpack_arrivals(sdm_ctx* ctx, uint64_t N, const sdm_sd_buffers* in, double x_shift, void* stream) {
+  if (!ctx) return SDM_ERR_INVALID;
+  if (!ctx->g.open_x) return fail(ctx, SDM_ERR_ORDER, "sdm_unpack_arrivals: the context was not created with open_x = 1");
+  if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_unpack_arrivals: call it between step_async and the next step_sync");
+  if (N == 0) return SDM_OK;
+  if (!buffers_ok(ctx, in)) return fail(ctx, SDM_ERR_INVALID, "sdm_unpack_arrivals: NULL buffer array");
+  if (ctx->nslots + N > ctx->cap_sd) return fail(ctx, SDM_ERR_CAPACITY, "sdm_unpack_arrivals: arrivals exceed max_sd");
+  cudaStream_t st = (cudaStream_t)stream;
+  ctx->last_stream = st;
+  CK(cudaStreamWaitEvent(st, ctx->ev_async, 0));
+  if (ctx->o.real_bytes == 8) launch_unpack_arrivals(view<double>(ctx->buf[ctx->cur]), (u32)ctx->nslots, (u32)N, ctx->g, buffers_view<double>(*in), x_shift, st);
+  else launch_unpack_arrivals(view<float>(ctx->buf[ctx->cur]), (u32)ctx->nslots, (u32)N, ctx->g, buffers_view<float>(*in), x_shift, st);
+  ctx->launches++;
+  ctx->nslots += N;
+  const u32 ns = (u32)ctx->nslots;
+  CK(cudaMemcpyAsync(ctx->d_info + ctx->cn, &ns, sizeof(u32), cudaMemcpyHostToDevice, st));
+  CK(cudaStreamSynchronize(st));   // &ns is a stack word
+  CK(cudaGetLastError());
+  ctx->hist_valid = false;
   return SDM_OK;
 }
 

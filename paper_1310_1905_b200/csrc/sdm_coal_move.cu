@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a,
           if (g.hz) { const double dC = Czh - Czl; zn = (zn + g.dz * (Czl - (double)k * dC)) / (1.0 - dC); }
         }
         if (mp.sedi && g.hz) zn = zn - v_term(sqrt(y), eta, rho_a) * g.dt;   // explicit Euler (:649)
-        if (g.hx) { xn = wrap(xn, g.X); a.x[s] = xn; }                        // periodic (:558)
+        if (g.hx) { if (!g.open_x) xn = wrap(xn, g.X); a.x[s] = xn; }         // periodic (:558) unless the context is a slab
         if (g.hy) { yn = wrap(yn, g.Y); a.y[s] = yn; }
         if (g.hz) {
           if (zn < 0.0 || !(zn < g.Z)) {                                       // left the domain (:651)
@@ -562,7 +562,7 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
               if (g.hz) zn = (zn + C.az) * C.bz;
             }
             if (need_vt) zn = zn - vt * g.dt;                                   // explicit Euler (:649)
-            if (g.hx) { xn = wrap(xn, g.X); s_x[sl] = (R)xn; xn = (double)(R)xn; }  // periodic (:558)
+            if (g.hx) { if (!g.open_x) xn = wrap(xn, g.X); s_x[sl] = (R)xn; xn = (double)(R)xn; }  // periodic (:558) unless a slab
             if (g.hy) { yn = wrap(yn, g.Y); s_y[sl] = (R)yn; yn = (double)(R)yn; }
             if (g.hz) { s_z[sl] = (R)zn; }
           }

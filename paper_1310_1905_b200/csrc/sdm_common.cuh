@@ -28,6 +28,7 @@ constexpr int NSLOT = 1024;   // spread-address accumulators for counters and ra
 struct Grid {
   int NX, NY, NZ;        // max(n?,1)
   int hx, hy, hz;        // dimension present
+  int open_x;            // x is not periodic: this context is a slab of a larger domain (sdm_opts_init.open_x)
   int ncell;
   double dx, dy, dz, dt, dV;
   double X, Y, Z;

@@ -109,6 +109,16 @@ void launch_diag_mom(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_boun
                      double r_mx, int k, int count_only, const double* rhod, double* out, cudaStream_t st);
 void launch_dense_copy(Field src, double* dst, int n0, int n1, int n2, cudaStream_t st);
 
+// sdm_slab.cu: exchange of SDs between slabs of a domain decomposed along x
+template <typename R>
+void launch_count_leavers(const SdArraysT<R>& a, u32 nslots, const Grid& g, u32* cnt2, cudaStream_t st);
+template <typename R>
+void launch_pack_leavers(const SdArraysT<R>& a, u32 nslots, const Grid& g, const SdArraysT<R>& left, const SdArraysT<R>& right, u32* cnt2,
+                         cudaStream_t st);
+template <typename R>
+void launch_unpack_arrivals(const SdArraysT<R>& a, u32 first, u32 count, const Grid& g, const SdArraysT<R>& in, double x_shift,
+                            cudaStream_t st);
+
 // sdm_euler.cu: one upstream step of a scalar field with the context's rho_d x Courant arrays (tmp: ncell doubles); 2 launches
 void launch_upstream(Field psi, const Grid& g, const CellFields& cf, double* tmp, cudaStream_t st);
 

@@ -841,6 +841,88 @@ def test_step_async_overlaps_an_eulerian_solver_on_another_stream():
     compare_fields(th, rv, o)
 
 
+# ----------------------------------------------------------------------------------------------- slabs along x
+@pytest.mark.parametrize("dims", ["2d", "3d"])
+def test_three_slabs_on_one_gpu_match_the_oracle_on_the_whole_domain(dims):
+    """the domain split into slabs of columns, one open_x context each (here all on one GPU, the
+    periodic neighbour of the last being the first), SDs that crossed a face handed over after every step
+    (sdm_pack_leavers / sdm_unpack_arrivals, slab.exchange_local).  Every other stage is local to a cell and the Philox
+    streams are keyed by the SD id, which travels with the SD: the union of the slabs must follow the oracle's
+    run on the whole periodic domain - multiplicities bit-exact, radii and fields to 1e-9, positions (in global
+    coordinates) to 1e-9 of the domain.  Unequal slab widths, rain mix, 8 steps; SDs do change slabs in both directions."""
+    from paper_1310_1905_b200 import slab
+
+    b = binding()
+    if dims == "2d":
+        w = rain_mix(W.cfg2_2d(sd_per_cell=24, nx=13, nz=20, seed=91))
+        w.courants = [c * 6.0 for c in w.courants]          # a brisk flow: Courant numbers up to ~0.4, many crossings
+    else:
+        w = rain_mix(W.cfg4_3d(sd_per_cell=16, nx=7, ny=4, nz=16, seed=92))
+        w.courants = [c * 4.0 for c in w.courants]
+    nx, dx = w.init["nx"], w.init["dx"]
+    cols = slab.split_columns(nx, 3)
+    widths = [n * dx for _, n in cols]
+    o = make_oracle(w, threads=4)
+    xs = w.state["x"]
+    parts, fields, n_moved = [], [], 0
+    for (i0, n) in cols:
+        m = (xs >= i0 * dx) & (xs < (i0 + n) * dx)
+        st = {k: (None if v is None else v[m].cuda()) for k, v in w.state.items()}
+        st["x"] = st["x"] - i0 * dx
+        p = b.Particles(max_sd=w.n_sd, sd_conc_mean=w.meta["sd_per_cell"], open_x=True, **dict(w.init, nx=n))
+        c = [cc.cuda() for cc in w.courants]
+        c[0] = c[0][i0:i0 + n + 1].contiguous()
+        c[1:] = [cc[i0:i0 + n].contiguous() for cc in c[1:]]
+        c += [None] * (3 - len(c))
+        p.init_from_arrays(w.rhod[i0:i0 + n].contiguous().cuda(), st["n"], st["rw2"], st["rd3"], st["kappa"], st["x"], st["y"], st["z"], st["id"],
+                           courant_1=c[0], courant_2=c[1], courant_3=c[2])
+        parts.append(p)
+        fields.append((w.th[i0:i0 + n].contiguous().cuda().clone(), w.rv[i0:i0 + n].contiguous().cuda().clone()))
+    po, oo = b.make_opts(**w.opts), oracle.make_opts(**w.opts)
+    for step in range(8):
+        fo = o.step(oo)
+        flux = 0.0
+        for p, (th, rv) in zip(parts, fields):
+            p.step_sync(po, th, rv)
+            p.step_async(po)
+            flux += p.step_async_result()
+        n_moved += sum(l + r for l, r in slab.exchange_local(parts, widths, cap=4096))
+        np.testing.assert_allclose(flux, fo, rtol=1e-8, atol=1e-300)
+        # the union of the slabs in global coordinates against the oracle
+        g = {k: [] for k in ("n", "rw2", "rd3", "kappa", "x", "y", "z", "id")}
+        for (i0, n), p in zip(cols, parts):
+            ex = p.export_state()
+            ex["x"] = ex["x"] + i0 * dx
+            for k in g:
+                g[k].append(ex[k])
+        g = sorted_by_id({k: torch.cat(v) for k, v in g.items()})
+        r = sorted_by_id(o.get_state())
+        keep = g["n"] != 0                         # a handed-over SD leaves a dead slot behind until the next compaction
+        g = {k: v[keep] for k, v in g.items()}
+        rk = r["n"] != 0
+        np.testing.assert_array_equal(g["id"].astype(np.uint32), r["id"][rk])
+        np.testing.assert_array_equal(g["n"].astype(np.uint64), r["n"][rk])
+        np.testing.assert_allclose(np.sqrt(g["rw2"]), np.sqrt(r["rw2"][rk]), rtol=RTOL)
+        np.testing.assert_allclose(np.cbrt(g["rd3"]), np.cbrt(r["rd3"][rk]), rtol=RTOL)
+        X = nx * dx
+        d = np.mod(g["x"] - r["x"][rk] + 0.5 * X, X) - 0.5 * X
+        assert np.abs(d).max() < 1e-9 * X
+        np.testing.assert_allclose(g["z"], r["z"][rk], rtol=RTOL, atol=1e-9)
+        if dims == "3d":
+            np.testing.assert_allclose(g["y"], r["y"][rk], rtol=RTOL, atol=1e-9)
+        oth, orv = o.get_fields()
+        th_all = torch.cat([f[0] for f in fields], 0)
+        rv_all = torch.cat([f[1] for f in fields], 0)
+        np.testing.assert_allclose(np_(th_all).ravel(), oth, rtol=RTOL)
+        np.testing.assert_allclose(np_(rv_all).ravel(), orv, rtol=RTOL)
+    assert n_moved > 100
+    assert sum(p.stats()["collisions"] for p in parts) == o.counters()["collisions"] > 0
+    # misuse is refused
+    q, th, rv = make_particles(W.cfg2_2d(sd_per_cell=4, nx=3, nz=3, seed=1))
+    with pytest.raises(b.SdmError, match="open_x"):
+        q.pack_leavers(16)
+
+
 def test_fp32_arithmetic_root_selection_scan_of_independent_sds():
     """The scan of test_root_selection_scan_of_independent_sds with the fp32 sweep: r_d from 1 nm to 2 um, sizes from
     barely wet to 3000 r_d, kappa 0.05-1.55, RH 0.3-1.05, multiplicity 1 (no feedback).  Whatever the fp32 certificate

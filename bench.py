@@ -44,13 +44,15 @@ def stage_bytes(ndim, rb):
             "coal_move": 2 * (8 + 3 * rb) + (ndim * rb + rb + 4) + (ndim * rb + 8)}   # a5 + a6
 
 
-# k_cond4, fp64 thread-instructions executed per unit of work, from the per-instruction execution counts of one
-# `ncu --set full --import-source on` capture of this build (profiles/r2_k_cond4_ncu_full.md: the SASS page summed by opcode and
-# by source line; "first" = everything an SD-substep costs with ONE growth-rate evaluation: ventilation set-up, eq. 18-19,
-# the certificate of R-roots, the evaluation, the Newton step, N d(r^3); "more" = every further evaluation with its
-# third-order corrected Newton step; "cell" = the cells' thermodynamics, spread over the SDs).  flops: DFMA = 2, DMUL = DADD = 1.
-FP64_INSTR = {"first": {"dfma": 62.0, "dmul": 58.0, "dadd": 19.0, "other": 11.0},
-              "more": {"dfma": 48.0, "dmul": 42.0, "dadd": 14.0, "other": 9.0}}
+# k_cond4, fp64 thread-instructions executed per unit of work, fitted to ncu's per-launch counters of 38 launches of this
+# build (profiles/r2_k_cond4_ncu_full.md: smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum and
+# smsp__inst_executed_pipe_fp64.sum against the SD-substeps and evaluations sdm_stats reports for the same launches).
+# "first" = everything an SD-substep costs with ONE growth-rate evaluation: ventilation set-up, eq. 18-19, the certificate of
+# R-roots, f and f', the Newton step, N d(r^3), its share of the cells' thermodynamics; "more" = every further evaluation with
+# its third-order corrected Newton step; "other" = the remaining lane slots of fp64-pipe warp instructions (DSETP, conversions,
+# lanes that are predicated off).  flops: DFMA = 2, DMUL = DADD = 1.
+FP64_INSTR = {"first": {"dfma": 55.2, "dmul": 60.3, "dadd": 22.7, "other": 50.9},
+              "more": {"dfma": 40.8, "dmul": 55.3, "dadd": 16.6, "other": 25.7}}
 FP64_INSTR_SOURCE = "profiles/r2_k_cond4_ncu_full.md"
 FP64_LANES_PER_SM = 64        # fp64 FMA lanes per SM per clock on sm_100 (B200_PROFILING.md; sdm_measure_fp64_peak confirms)
 # --cond-arith 4 (k_cond4f): fp32 operations of one evaluation with derivative and curvature bound (62 instructions, 20 of
@@ -59,7 +61,7 @@ FLOP_PER_EVAL_F32 = 86.0
 FLOP_PER_SETUP_F32 = 60.0
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x fp32 FMA lanes x 2 x max SM clock = 74.4
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch on the default workload, from the ncu capture named beside it
-NCU_COND_DRAM_BYTES = (2.317242e9 + 0.551745e9, "profiles/r1_k_cond4_v7_ncu_full.md (kernel of round 1; the staging code is unchanged)")
+NCU_COND_DRAM_BYTES = (2.314134e9 + 0.552060e9, "profiles/r2_k_cond4_ncu_full.md")
 NCU_COND32_DRAM_BYTES = (1.509464e9 + 0.313273e9, "profiles/r1_k_cond4f_ncu_full.md")
 
 
@@ -80,6 +82,8 @@ def parse():
     ap.add_argument("--real-bytes", type=int, default=8, choices=[8, 4], help="storage type of the SD attributes (configs[4]: fp32 state)")
     ap.add_argument("--cond-adapt-tol", type=float, default=0.0, help="adaptive condensation substeps per cell (sdm_opts.cond_adapt_tol, DESIGN.md R-adapt); "
                     "0 = the fixed sstp_cond of the paper and of the headline")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"], help="N > 1: independent replicas (default), or one domain of "
+                    "N x 128 columns decomposed into x-slabs, one per rank, SDs that cross a face exchanged every step (slab.py; weak scaling)")
     ap.add_argument("--long-run", type=int, default=-1, help="after the timed region, continue the run to this many steps in all and report "
                     "ms/step, evaluations per SD-substep, slow-list fraction and the launch configuration per 100-step window "
                     "(default: 600 = the length of configs[3] for the default workload, 0 otherwise)")
@@ -217,9 +221,12 @@ def config_of(wa):
             "parallelism": "independent replicas (single-GPU path, no collective)"}
 
 
-def make_particles(binding, torch, w, wa, a):
-    p = binding.Particles(max_sd=w.n_sd, sd_conc_mean=wa["sd"], real_bytes=a.real_bytes, **w.init)
+def make_particles(binding, torch, w, wa, a, rank=0):
+    slab_mode = a.decomp == "slab"
+    p = binding.Particles(max_sd=int(w.n_sd * (1.05 if slab_mode else 1.0)), sd_conc_mean=wa["sd"], real_bytes=a.real_bytes, open_x=slab_mode, **w.init)
     s = w.state
+    if slab_mode:   # ids are unique over the whole domain: they key the Philox streams and travel with the SDs
+        s = dict(s, id=(s["id"].to(torch.int64) + rank * w.n_sd).to(torch.int32))
     if a.real_bytes == 4:
         s = {k: (v if v is None or k in ("n", "id") else v.to(torch.float32)) for k, v in s.items()}
     cs = list(w.courants) + [None] * (3 - len(w.courants))
@@ -265,11 +272,17 @@ def main():
     dev = f"cuda:{local}"
     warm = max(a.warmup, 3)
     full3d = wa["kind"] == "3d" and a.scale == 1.0 and wa["sd"] == 64
-    long_run = a.long_run if a.long_run >= 0 else (600 if full3d and world == 1 and not a.recycle and a.cond_adapt_tol == 0.0 else 0)
+    long_run = a.long_run if a.long_run >= 0 else (600 if full3d and world == 1 and not a.recycle and a.cond_adapt_tol == 0.0 and a.decomp == "replicas" else 0)
 
     w = make_workload(wa, seed=replicas.replica_seed(42, rank), device=dev)
-    p = make_particles(binding, torch, w, wa, a)
-    p_host = make_particles(binding, torch, w, wa, a)   # a second, identically initialised context for the end-to-end leg
+    p = make_particles(binding, torch, w, wa, a, rank)
+    p_host = make_particles(binding, torch, w, wa, a, rank)   # a second, identically initialised context for the end-to-end leg
+    slab_widths = [wa["nx"] * 20.0] * world
+    from paper_1310_1905_b200 import slab
+
+    def hand_over(q):   # --decomp slab: SDs that crossed a face of this rank's slab go to the neighbour (nccl send/recv)
+        if a.decomp == "slab":
+            slab.exchange(q, slab_widths, 1 << 20, rank, world)
     n_sd0 = w.n_sd
     th, rv = w.th.clone(), w.rv.clone()
     th_h, rv_h = w.th.cpu().pin_memory(), w.rv.cpu().pin_memory()
@@ -288,6 +301,7 @@ def main():
     for _ in range(warm):
         p.step_sync(po, th, rv)
         p.step_async(po)
+        hand_over(p)
     # ---- device-resident timing ------------------------------------------------------------------
     p.set_timing(True)
     p.stage_times(reset=True)
@@ -302,6 +316,7 @@ def main():
         p.step_sync(po, th, rv)
         sd_steps += p.n_sd()      # live SDs of this step (host-known after the sort, no extra sync)
         p.step_async(po)
+        hand_over(p)
     ev1.record()
     barrier()
     clocks = sampler.stop()
@@ -316,11 +331,13 @@ def main():
     # pinned host memory, copied in and out inside every timed step through sdm_step_host ------------------------------
     for _ in range(warm):
         p_host.step_host(po, th_h, rv_h)
+        hand_over(p_host)
     barrier()
     e_sd, t0 = 0, time.perf_counter()
     for _ in range(a.steps):
         e_sd += p_host.n_sd()
         p_host.step_host(po, th_h, rv_h)
+        hand_over(p_host)
     torch.cuda.synchronize()
     e_dt = time.perf_counter() - t0
     e_s, e_tot = replicas.job_totals(e_dt, e_sd, device=dev)
@@ -430,6 +447,8 @@ def main():
     if a.cond_adapt_tol > 0.0:
         out["config"]["cond_adapt_tol"] = a.cond_adapt_tol
         out["sd_substeps_per_sd_step"] = subs / max(sd_steps, 1)
+    if a.decomp == "slab":
+        out["config"]["parallelism"] = "one domain of %d x %d columns in x-slabs, one per rank; leavers exchanged every step (slab.py)" % (world, wa["nx"])
     if a.recycle:
         out["config"]["recycling"] = "on (PAPER.md :641)"
         out["recycled"] = st1["recycled"] - st0["recycled"]
@@ -437,7 +456,7 @@ def main():
         v, cores, desc, _, _ = oracle_rate(wa, 2, 1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                "value_1_thread": getattr(oracle_rate, "one_thread", None)}
-    if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline and a.cond_adapt_tol == 0.0:
+    if world == 1 and a.real_bytes == 8 and a.cond_arith == 8 and not a.recycle and not a.no_fp32_mode and not a.no_cpu_baseline and a.cond_adapt_tol == 0.0 and a.decomp == "replicas":
         # the same workload and step counts in the fp32 mode of configs[4] (fp32 state, fp32 condensation sweep; radii to
         # 1e-4 instead of 1e-9): a second line of context, measured by the same code in a child process
         try:

@@ -59,10 +59,12 @@ def exchange_lists(left, right, rank=None, world=None, group=None):
             ops.append(dist.P2POp(dist.isend, left[k].contiguous(), ln, group, tag=2 * t))
         if right[k].numel():
             ops.append(dist.P2POp(dist.isend, right[k].contiguous(), rn, group, tag=2 * t + 1))
-        if n_from_left:
-            ops.append(dist.P2POp(dist.irecv, from_left[k], ln, group, tag=2 * t + 1))
+        # receives in the order the peer sends (its left list, then its right list): nccl matches messages between two
+        # ranks in posting order and ignores tags
         if n_from_right:
             ops.append(dist.P2POp(dist.irecv, from_right[k], rn, group, tag=2 * t))
+        if n_from_left:
+            ops.append(dist.P2POp(dist.irecv, from_left[k], ln, group, tag=2 * t + 1))
     if ops:
         for req in dist.batch_isend_irecv(ops):
             req.wait()

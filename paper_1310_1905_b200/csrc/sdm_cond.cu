@@ -1,18 +1,19 @@
-// Stage a4: condensational growth, all sstp_cond substeps fused in one
-// tile-resident kernel.  A CTA of 256 threads owns a TILE of consecutive grid cells (about 1800
-// super-droplets): the SDs are staged once in shared memory in sorted order and stay there for all
-// substeps.  Per substep
-//   A. one thread per cell applies the feedback of the previous substep (eq. 25-26) and
-//      diagnoses T, p, rho_vs, RH.. from theta, r_v, rho_d (eq. 43-44, Table 2),
-//   B. all threads sweep the tile's SDs DENSELY (lane utilisation does not depend on the cell
-//      populations) and solve eq. 17 by a bracketed Newton iteration on r_w^2 inside the interval of
-//      eq. 18-19 (the paper bisects, :579, and names a faster root finder as the first optimisation,
-//      :912); the sweep spends at most `kfast` growth-rate evaluations per SD,
-//   C. the few SDs that did not converge in B are collected in a list and solved to the end in a second,
-//      again densely packed, pass (so one slow SD does not hold 31 lanes for its whole iteration),
-//   D. one warp per cell sums N (r_w^3' - r_w^3) in sorted order (deterministic) for the next feedback.
-// The solver is a small state machine around ONE inlined growth-rate evaluation, so that lanes of a
-// warp differ only in their trip count.  fp64 throughout; this kernel is fp64-ALU bound.
+// Stage a4: condensational growth (eq. 17-26), all sstp_cond substeps fused in one
+// tile-resident kernel.  Kernels of this file:
+//   k_cond4   the fp64 kernel of the step: a CTA of 128 threads owns a tile of ~10 consecutive cells (<= 800 SDs, 5 CTAs per
+//             SM; 256 / 1280 and 512 / 4096 variants for crowded cells); r_w, r_d^3, kappa r_d^3, N of the tile stay in shared
+//             memory in sorted order for all substeps.  Per substep: (D) 8-lane groups sum N d(r_w^3) of the cells in a fixed
+//             order; (A) one lane per cell on the first warp applies the feedback (eq. 25-26) and advances T, p_vs .. by short
+//             series; (B) the warps sweep the tile's SDs in 32-SD chunks and solve eq. 17 by a Newton iteration in r = sqrt(y)
+//             bracketed by eq. 18-19 (the paper bisects, :579, and names a faster root finder as the first optimisation, :912);
+//             (C) whatever is irregular - an iterate leaving the bracket, a bracket that may hold several roots, a Kelvin
+//             exponent out of range - was put on a list and is solved by cond_solve (bracketed Newton / bisection state
+//             machine) or by the paper's literal bisection, which hands over to Newton once its bracket holds one root.
+//             With cp.adapt_tol > 0 every cell takes its own number of substeps (reading R-adapt).
+//   k_cond4f  the same design with the sweep in fp32 arithmetic for the fp32 state (sdm_set_cond_arith 4).
+//   k_cond    one crowded cell (beyond 4096 SDs) per CTA, in place in global memory, cond_solve only.
+//   k_thermo  eta, rho_a per cell when condensation is switched off.
+// fp64 throughout unless stated; k_cond4 is bound by latency in front of the fp64 pipe.
 #include "sdm_kernels.cuh"
 
 namespace sdm {

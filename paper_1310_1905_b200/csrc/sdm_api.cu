@@ -56,7 +56,7 @@ struct sdm_ctx {
   double* flux_part = nullptr;   // per-CTA rain flux of k_coal_move_tile
   int n_flux_part = 0;
   bool hist_valid = false;       // cell, off, count of the next step were written by the last step_async
-  double* d_flux = nullptr;  // [0] last step, [1] total
+  double* d_flux = nullptr;  // [0] last step, [1] total, [2] the device error flag of the step (copied by k_flux_sum)
   unsigned long long* cnt_mem = nullptr;
   Counters cnt{};
   CoalParams kp{};
@@ -174,6 +174,17 @@ void t_fold(sdm_ctx* c) {   // caller has synchronised the stream
   cudaGetLastError();
 }
 
+// The rank kernels of step_sync raise d_info[3] when a cell holds more SDs than the launch was sized for; the step's device work
+// is complete when this is called, so the flag is that of THIS step.  Cleared once reported.
+int check_device_flag(sdm_ctx* ctx, const char* who, double* rain_flux) {
+  double h[3] = {0, 0, 0};   // flux of the step, total, error flag: one read-back
+  CK(cudaMemcpy(h, ctx->d_flux, sizeof(h), cudaMemcpyDeviceToHost));
+  if (rain_flux) *rain_flux = h[0];
+  if (h[2] == 0.0) return SDM_OK;
+  cudaMemset(ctx->d_info + 3, 0, sizeof(u32));
+  return fail(ctx, SDM_ERR_CUDA, std::string(who) + ": device-side error flag set (a cell outgrew the launch its ranks were sized for)");
+}
+
 int pick_group(const sdm_ctx* c, double mean) {
   if (c->group_override) return c->group_override;
   if (mean < 12.0) return 4;
@@ -254,7 +265,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
       (e = dalloc(&ctx->cx, (size_t)(g.NX + 1) * g.NY * g.NZ)) || (e = dalloc(&ctx->cy, (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = dalloc(&ctx->cz, (size_t)g.NX * g.NY * (g.NZ + 1))) || (e = dalloc(&ctx->flux_slots, NSLOT)) ||
       (e = dalloc(&ctx->flux_part, (size_t)g.ncell)) ||
-      (e = dalloc(&ctx->d_flux, 2)) || (e = dalloc(&ctx->cnt_mem, N_COUNTERS * NSLOT)))
+      (e = dalloc(&ctx->d_flux, 4)) || (e = dalloc(&ctx->cnt_mem, N_COUNTERS * NSLOT)))
     return bail(e, "scratch");
   ctx->cf.cx = ctx->cx; ctx->cf.cy = ctx->cy; ctx->cf.cz = ctx->cz;
   if ((e = cudaMallocHost((void**)&ctx->h_info, 8 * sizeof(u32)))) return bail(e, "pinned info");
@@ -263,7 +274,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
       (e = cudaMemset(ctx->cx, 0, sizeof(double) * (size_t)(g.NX + 1) * g.NY * g.NZ)) ||
       (e = cudaMemset(ctx->cy, 0, sizeof(double) * (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = cudaMemset(ctx->cz, 0, sizeof(double) * (size_t)g.NX * g.NY * (g.NZ + 1))) ||
-      (e = cudaMemset(ctx->flux_slots, 0, sizeof(double) * NSLOT)) || (e = cudaMemset(ctx->d_flux, 0, 2 * sizeof(double))) ||
+      (e = cudaMemset(ctx->flux_slots, 0, sizeof(double) * NSLOT)) || (e = cudaMemset(ctx->d_flux, 0, 4 * sizeof(double))) ||
       (e = cudaMemset(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT)) ||
       (e = cudaMemset(ctx->outbuf, 0, sizeof(double) * g.ncell)))
     return bail(e, "memset");
@@ -374,7 +385,7 @@ int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm
   CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
   CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT, st));
   CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
-  CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
+  CK(cudaMemsetAsync(ctx->d_flux, 0, 4 * sizeof(double), st));
   CK(cudaMemsetAsync(ctx->outbuf, 0, sizeof(double) * g.ncell, st));
   CK(cudaStreamSynchronize(st));
   ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false; ctx->hist_valid = false;
@@ -414,7 +425,7 @@ int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arr
   CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));
   CK(cudaMemsetAsync(ctx->cnt_mem, 0, sizeof(unsigned long long) * N_COUNTERS * NSLOT, st));
   CK(cudaMemsetAsync(ctx->flux_slots, 0, sizeof(double) * NSLOT, st));
-  CK(cudaMemsetAsync(ctx->d_flux, 0, 2 * sizeof(double), st));
+  CK(cudaMemsetAsync(ctx->d_flux, 0, 4 * sizeof(double), st));
   CK(cudaStreamSynchronize(st));
   ctx->nslots = N; ctx->max_nc = 0; ctx->step = 0; ctx->synced = false; ctx->have_order = false; ctx->hist_valid = false;
   ctx->last_stream = st;
@@ -515,7 +526,10 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   ctx->nslots = ctx->h_info[ctx->cn];
   ctx->max_nc = ctx->h_info[2];
   for (int k = 0; k < 4; ++k) ctx->tile_max[k] = ctx->h_info[4 + k];
-  if (ctx->h_info[3]) return fail(ctx, SDM_ERR_CUDA, "sdm_step_sync: device-side error flag set (corrupted segment sizes)");
+  if (ctx->h_info[3]) {   // raised by a rank kernel of the step before (reported here at the latest; cleared once reported)
+    cudaMemsetAsync(ctx->d_info + 3, 0, sizeof(u32), st);
+    return fail(ctx, SDM_ERR_CUDA, "sdm_step_sync: device-side error flag set (corrupted segment sizes)");
+  }
 
   // launch sizing from the measured occupancy
   const double mean = (double)ctx->nslots / g.ncell;
@@ -612,7 +626,7 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     ctx->launches++;
   }
   else ctx->n_flux_part = 0;
-  launch_flux_sum(ctx->flux_slots, ctx->flux_part, ctx->n_flux_part, ctx->d_flux, ctx->d_flux + 1, st);
+  launch_flux_sum(ctx->flux_slots, ctx->flux_part, ctx->n_flux_part, ctx->d_flux, ctx->d_flux + 1, ctx->d_info + 3, st);
   ctx->launches++;
   CK(cudaGetLastError());
   CK(cudaEventRecord(ctx->ev_async, st));
@@ -625,8 +639,7 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
 int sdm_step_async_result(sdm_ctx* ctx, double* rain_flux) {
   if (!ctx) return SDM_ERR_INVALID;
   CK(cudaEventSynchronize(ctx->ev_async));
-  if (rain_flux) CK(cudaMemcpy(rain_flux, ctx->d_flux, sizeof(double), cudaMemcpyDeviceToHost));
-  return SDM_OK;
+  return check_device_flag(ctx, "sdm_step_async_result", rain_flux);
 }
 
 int sdm_step_host(sdm_ctx* ctx, const sdm_opts* op, double* th_host, double* rv_host, double* rain_flux, void* stream) {
@@ -663,8 +676,7 @@ int sdm_step_host(sdm_ctx* ctx, const sdm_opts* op, double* th_host, double* rv_
   if (int rc = sdm_step_async(ctx, op, stream)) return rc;
   CK(cudaStreamSynchronize(st));
   CK(cudaStreamSynchronize(cs));
-  if (rain_flux) CK(cudaMemcpy(rain_flux, ctx->d_flux, sizeof(double), cudaMemcpyDeviceToHost));
-  return SDM_OK;
+  return check_device_flag(ctx, "sdm_step_host", rain_flux);
 }
 
 static int diag_launch(sdm_ctx* ctx, int wet, double lo, double hi, int k, int count_only, void* stream) {

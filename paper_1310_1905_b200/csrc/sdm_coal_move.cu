@@ -705,7 +705,7 @@ cudaError_t launch_coal_move_tile(int cpb, int need, const SdArraysT<R>& a, cons
 // rain flux of the step: the per-CTA partial sums of k_coal_move_tile (n_part of them; every thread sums a strided subset in
 // order, then a fixed tree) plus the NSLOT atomic slots of the per-cell kernel (summed in order, then cleared)
 __global__ void __launch_bounds__(1024) k_flux_sum(double* flux_slots, const double* __restrict__ flux_part, int n_part, double* flux_out,
-                                                   double* flux_total) {
+                                                   double* flux_total, const u32* __restrict__ d_flag) {
   __shared__ double sh[1024];
   double f = 0.0;
   for (int t = threadIdx.x; t < n_part; t += 1024) f += flux_part[t];
@@ -719,6 +719,7 @@ __global__ void __launch_bounds__(1024) k_flux_sum(double* flux_slots, const dou
   if (threadIdx.x == 0) {
     *flux_out = sh[0];
     *flux_total += sh[0];
+    flux_out[2] = (double)*d_flag;   // the host reads flux and flag in one copy
   }
 }
 
@@ -771,8 +772,9 @@ cudaError_t launch_coal_move(int G, int cap, bool in_smem, const SdArraysT<R>& a
 SDM_INSTANTIATE_REAL(SDM_INST)
 #undef SDM_INST
 
-void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, cudaStream_t st) {
-  k_flux_sum<<<1, 1024, 0, st>>>(flux_slots, flux_part, n_part, flux_out, flux_total);
+void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, const u32* d_flag,
+                     cudaStream_t st) {
+  k_flux_sum<<<1, 1024, 0, st>>>(flux_slots, flux_part, n_part, flux_out, flux_total, d_flag);
 }
 
 }  // namespace sdm

@@ -72,7 +72,9 @@ template <typename R>
 cudaError_t launch_coal_move_tile(int cpb, int need, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                   const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_part,
                                   const Counters& cnt, u32* cell_out, u32* off_out, u32* count, cudaStream_t st);
-void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, cudaStream_t st);
+// also copies the step's device error flag into flux_out[2], so that one read-back serves both
+void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, const u32* d_flag,
+                     cudaStream_t st);
 
 // sdm_recycle.cu: recycling of zero-multiplicity SDs (PAPER.md :641, :651; reading R-recycle)
 struct __align__(16) RecItem { u64 key; u32 id; u32 slot; };   // ordered by (key, id); key = ~N for donors, 0 for dead SDs

@@ -718,6 +718,17 @@ def test_fp32_arithmetic_condensation_2d_3d_and_first_step():
         make_particles(W.cfg2_2d(sd_per_cell=8, nx=2, nz=2, seed=1))[0].set_cond_arith(4)   # fp64 state: refused
 
 
+def test_measured_fp64_peak_and_n_live():
+    """sdm_measure_fp64_peak (the denominator of the condensation roofline): a B200 retires 64 fp64 FMAs per clock
+    per SM; the measurement must land within a few per cent of that and of 148 x 64 x 2 x clock.  sdm_n_live = sdm_n_sd."""
+    b = binding()
+    tflops, per_clk = b.measure_fp64_peak()
+    assert 58.0 < per_clk <= 64.5, per_clk
+    assert 25.0 < tflops < 40.0, tflops
+    p, th, rv = make_particles(W.cfg2_2d(sd_per_cell=8, nx=4, nz=4, seed=3))
+    assert p.n_live() == p.n_sd() == 128
+
+
 # ----------------------------------------------------------------------------------------------- adaptive substeps
 def test_adaptive_condensation_substeps_match_the_oracle():
     """sdm_opts.cond_adapt_tol > 0 (reading R-adapt; PAPER.md :566 "planned"): every cell takes the number of

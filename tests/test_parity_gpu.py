@@ -724,7 +724,7 @@ def test_measured_fp64_peak_and_n_live():
     b = binding()
     tflops, per_clk = b.measure_fp64_peak()
     assert 58.0 < per_clk <= 64.5, per_clk
-    assert 25.0 < tflops < 40.0, tflops
+    assert 15.0 < tflops < 40.0, tflops   # 36.6 at 1965 MHz; a power-capped clock lowers it
     p, th, rv = make_particles(W.cfg2_2d(sd_per_cell=8, nx=4, nz=4, seed=3))
     assert p.n_live() == p.n_sd() == 128
 

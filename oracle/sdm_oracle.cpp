@@ -48,6 +48,7 @@ struct orc_opts_t {          // PAPER.md Listing 5.1 (:677-689)
   double RH_max;
   int sstp_cond, sstp_coal;
   double cond_adapt_tol;     // > 0: per-cell number of condensation substeps (reading R-adapt; PAPER.md :566 "planned")
+  int coal_adapt_max;        // > 1: per-cell number of coalescence substeps from P_ij (reading R-adapt-coal; PAPER.md :645 "planned")
 };
 struct orc_counters_t {
   long long pairs, collisions, near_ties, ill_posed, f_evals, sd_substeps;
@@ -276,15 +277,38 @@ static double coal_kernel(const Ctx& c, long j, long k, const CellThermo& ct) {
 }
 
 // PAPER.md :622-645: SDM coalescence on the pairs (0,1),(2,3).. of each cell's sorted segment
+// DESIGN.md reading R-adapt-coal (PAPER.md :645: "It is planned ... to use the values of P_ij to control an adaptive timestep
+// logic"): with P_max the largest probability of eq. 27 among the pairs of the cell's first grouping, for the substep length
+// dt / sstp_coal, the cell takes sstp_coal * m substeps, m = min(coal_adapt_max, ceil(P_max)) (at least 1): just enough for
+// every pair of that grouping to have P <= 1, where an event stands for one collision per pair of real droplets.
+static int coal_substep_multiplier(const Ctx& c, const std::vector<long>& L, const CellThermo& ct, const orc_opts_t& op) {
+  const u64 nc = L.size();
+  if (op.coal_adapt_max <= 1 || nc < 2) return 1;
+  const double dtpp = c.o.dt / op.sstp_coal;
+  const double scale = (double)(nc * (nc - 1) / 2) / (double)(nc / 2);
+  double pmax = 0.0;
+  for (u64 m = 0; m + 1 < nc; m += 2) {
+    const long a = L[m], b = L[m + 1];
+    long j, k;
+    if (c.n[a] >= c.n[b]) { j = a; k = b; } else { j = b; k = a; }
+    const double p = (((double)c.n[j] * coal_kernel(c, j, k, ct)) * (dtpp / c.dV)) * scale;
+    pmax = std::max(pmax, p);
+  }
+  const double want = std::ceil(pmax);
+  if (want >= (double)op.coal_adapt_max) return op.coal_adapt_max;
+  return std::max(1, (int)want);
+}
+
 static void coal_stage(Ctx& c, const orc_opts_t& op) {
   if ((long)c.thermo.size() != c.ncell) thermo_stage(c, op);
-  const double dtpp = c.o.dt / op.sstp_coal;
   long long pairs = 0, colls = 0, ties = 0;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(c.nthreads) reduction(+ : pairs, colls, ties)
   for (long q = 0; q < c.ncell; ++q) {
     std::vector<long> L(c.order.begin() + c.seg[q], c.order.begin() + c.seg[q + 1]);
     const CellThermo& ct = c.thermo[q];
-    for (int sub = 0; sub < op.sstp_coal; ++sub) {
+    const int nsub = op.sstp_coal * coal_substep_multiplier(c, L, ct, op);
+    const double dtpp = c.o.dt / nsub;
+    for (int sub = 0; sub < nsub; ++sub) {
       if (sub > 0) {   // new random grouping each substep (:624); SDs at N=0 drop out
         std::vector<long> M; M.reserve(L.size());
         for (long i : L) if (c.n[i] > 0) M.push_back(i);

@@ -122,6 +122,72 @@ def test_pair_probability_bruteforce(nsd):
         assert abs(hits[pr] - T * p) < 4.5 * max(sd / np.sqrt(scale), 3.0), (pr, hits[pr], T * p)
 
 
+def test_adaptive_coalescence_substeps_from_pij():
+    """DESIGN.md reading R-adapt-coal (PAPER.md :645 "use the values of P_ij to control an adaptive timestep logic"): a cell
+    takes sstp_coal * m substeps, m = min(coal_adapt_max, ceil(max P_ij over its first grouping)).  Pinned by (i) the
+    paper's variant without multiple coalescence on a pair with P = 3.7: one substep yields exactly one event per step (the
+    undersampling :645 describes), m = 2 exactly two, and m = 4 substeps of P' = 0.925 a Binomial(4, 0.925) number whose mean
+    is the 3.7 collisions the probability stands for; (ii) the rule restated on a 9-SD Golovin cell from the grouping the
+    oracle reports: the candidate pairs examined are m * floor(n/2); (iii) coal_adapt_max <= 1 is the fixed step bit for bit."""
+    b, dV, dt = 1500.0, 1.0, 1.0
+    rj, rk, nj = 1e-6, 30e-6, 10**9            # many small droplets (j) against one big drop (k): k hardly changes when hit
+    K = b * 4 / 3 * np.pi * (rj**3 + rk**3)
+    dV = nj * K * dt / 3.7                     # P = N_j K dt / dV = 3.7 (two SDs: the factor of eq. 27 is 1)
+    side = dV ** (1 / 3)
+    T = 3000
+
+    def mean_drop(**kw):
+        o = oracle.Oracle(dx=side, dy=side, dz=side, dt=dt, kernel="golovin", golovin_b=b, multi_coal=False, seed=11)
+        op = oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, **kw)
+        drops = []
+        for t in range(T):
+            o.set_state(np.array([nj, 1], np.uint64), np.array([rj**2, rk**2]), np.full(2, 1e-27), np.full(2, 0.5))
+            o.set_step(t)
+            o.stage("sort")
+            o.stage("coal", op)
+            drops.append(nj - int(o.get_state()["n"][0]))
+        return np.array(drops)
+
+    assert set(mean_drop()) == {1}                                   # fixed: u < 1 < P every step, one event, 2.7 lost
+    assert set(mean_drop(coal_adapt_max=2)) == {2}                   # capped at m = 2: P' = 1.85 still above 1
+    d = mean_drop(coal_adapt_max=8)                                  # m = ceil(3.7) = 4, P' = 0.925
+    assert d.max() == 4 and d.min() >= 1
+    assert abs(d.mean() - 3.7) < 4.5 * np.sqrt(4 * 0.925 * 0.075 / T)
+    assert set(mean_drop(coal_adapt_max=8, sstp_coal=2)) <= {1, 2, 3, 4}   # P(dt/2) = 1.85 -> m = 2: again 4 substeps
+    # (ii) the rule on a cell of 9 SDs
+    rng = np.random.default_rng(12)
+    nsd = 9
+    n = (np.array([7, 11, 13, 17, 19, 23, 29, 31, 37]) * 10**6).astype(np.uint64)
+    r = rng.uniform(10e-6, 30e-6, nsd)
+    v = 4 / 3 * np.pi * r**3
+    scale = (nsd * (nsd - 1) / 2) / (nsd // 2)
+    for want_m, cap in ((1, 8), (3, 8), (6, 8), (5, 5)):
+        o = oracle.Oracle(dx=1.0, dy=1.0, dz=1.0, dt=dt, kernel="golovin", golovin_b=b, seed=77)
+        o.set_state(n, r**2, np.full(nsd, 1e-27), np.full(nsd, 0.5))
+        o.stage("sort")
+        ids, _ = o.get_order()
+        P1 = max(float(max(n[i], n[j])) * b * (v[i] + v[j]) * dt * scale for i, j in zip(ids[0:-1:2], ids[1::2]))   # at dV = 1
+        target = {1: 0.8, 3: 2.5, 6: 5.5, 5: 7.3}[want_m]            # the P_max this case is built to have
+        side = (P1 / target) ** (1 / 3)
+        o = oracle.Oracle(dx=side, dy=side, dz=side, dt=dt, kernel="golovin", golovin_b=b, seed=77)
+        o.set_state(n, r**2, np.full(nsd, 1e-27), np.full(nsd, 0.5))
+        o.stage("sort")
+        ids2, _ = o.get_order()
+        np.testing.assert_array_equal(ids, ids2)                    # the grouping does not depend on the cell volume
+        o.stage("coal", oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, coal_adapt_max=cap))
+        assert o.counters()["pairs"] == want_m * (nsd // 2), (want_m, o.counters()["pairs"])
+    # (iii) off means off
+    for mx in (0, 1):
+        a = oracle.Oracle(dx=0.01, dy=0.01, dz=0.01, dt=dt, kernel="golovin", golovin_b=b, seed=5)
+        f = oracle.Oracle(dx=0.01, dy=0.01, dz=0.01, dt=dt, kernel="golovin", golovin_b=b, seed=5)
+        for o, kw in ((a, dict(coal_adapt_max=mx)), (f, {})):
+            o.set_state(n, r**2, np.full(nsd, 1e-27), np.full(nsd, 0.5))
+            for _ in range(5):
+                o.step(oracle.make_opts(adve=False, sedi=False, cond=False, coal=True, **kw))
+        for k in ("n", "rw2", "rd3"):
+            np.testing.assert_array_equal(a.get_state()[k], f.get_state()[k])
+
+
 def _stokes(r, eta, rho_a):
     """Stokes fall speed 2 r^2 g (rho_w - rho_a) / (9 eta): the r -> 0 limit of the terminal-velocity formula (:649),
     within 3e-3 of it up to 1 um (test_terminal_velocity_stokes_limit_and_textbook)."""

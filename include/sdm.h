@@ -95,6 +95,11 @@ typedef struct {
                                  takes the smallest divisor d of sstp_cond with d >= sstp_cond * eps / cond_adapt_tol substeps of dt / d.
                                  Changes results (by the time-discretisation error it trades); fp64-arithmetic condensation only
                                  (SDM_ERR_INVALID with sdm_set_cond_arith(ctx, 4)). */
+  int coal_adapt_max;         /* 0 or 1 (default): every cell takes sstp_coal coalescence substeps.  > 1: the adaptive logic the paper
+                                 plans (:645 "use the values of P_ij to control an adaptive timestep logic"; DESIGN.md reading
+                                 R-adapt-coal): a cell takes sstp_coal * m substeps with new random pairs each, m = min(coal_adapt_max,
+                                 ceil(P_max)), P_max the largest probability of eq. 27 among the pairs of its first grouping at
+                                 dt / sstp_coal: enough for every such pair to have P <= 1.  Changes results wherever P_max > 1. */
 } sdm_opts;
 
 /* PAPER.md Listing 5.4 (:730-745) lgrngn::arrinfo_t: element (i,j,k) of the field lives at

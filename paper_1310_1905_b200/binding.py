@@ -34,7 +34,7 @@ class OptsInit(C.Structure):
 
 class Opts(C.Structure):
     _fields_ = [("adve", C.c_int), ("sedi", C.c_int), ("cond", C.c_int), ("coal", C.c_int),
-                ("RH_max", C.c_double), ("sstp_cond", C.c_int), ("sstp_coal", C.c_int), ("cond_adapt_tol", C.c_double)]
+                ("RH_max", C.c_double), ("sstp_cond", C.c_int), ("sstp_coal", C.c_int), ("cond_adapt_tol", C.c_double), ("coal_adapt_max", C.c_int)]
 
 
 class ArrInfo(C.Structure):
@@ -111,8 +111,9 @@ def load_library():
     return L
 
 
-def make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=44.0, sstp_cond=10, sstp_coal=1, cond_adapt_tol=0.0):
-    return Opts(int(adve), int(sedi), int(cond), int(coal), float(RH_max), int(sstp_cond), int(sstp_coal), float(cond_adapt_tol))
+def make_opts(adve=True, sedi=True, cond=True, coal=True, RH_max=44.0, sstp_cond=10, sstp_coal=1, cond_adapt_tol=0.0, coal_adapt_max=0):
+    return Opts(int(adve), int(sedi), int(cond), int(coal), float(RH_max), int(sstp_cond), int(sstp_coal), float(cond_adapt_tol),
+                int(coal_adapt_max))
 
 
 def arrinfo(t):

@@ -595,13 +595,15 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     int cap = (int)((ctx->max_nc + 3) / 4 * 4);
     cap = std::max(cap, 4);
     const int sstp = op->coal ? op->sstp_coal : 1;
-    bool in_smem = coal_smem_bytes(G, cap, sstp, true) <= kSmemLimit;
-    if (!in_smem && coal_smem_bytes(G, cap, sstp, false) > kSmemLimit)
+    const int adapt_max = (op->coal && op->coal_adapt_max > 1) ? op->coal_adapt_max : 0;
+    const int multi = (sstp > 1 || adapt_max) ? 2 : 1;   // several groupings per step: the per-cell kernel with its sort buffers
+    bool in_smem = coal_smem_bytes(G, cap, multi, true) <= kSmemLimit;
+    if (!in_smem && coal_smem_bytes(G, cap, multi, false) > kSmemLimit)
       return fail(ctx, SDM_ERR_CAPACITY, "sdm_step_async: a cell holds more super-droplets than one CTA can pair");
     // (a slab hands SDs over after the step, recycling moves them before the next: the histogram is then built by k_cellhist)
-    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step, (ctx->recycle || g.open_x) ? 0 : 1};
+    CoalMoveParams mp{op->coal, op->adve, op->sedi, sstp, (u32)ctx->step, (ctx->recycle || g.open_x) ? 0 : 1, adapt_max};
     int tile_cpb = 0, tile_need = 0;   // tile-resident kernel: largest candidate tile that fits (one set of pairs per step only)
-    for (int k = 0; k < 4 && !tile_cpb && sstp == 1 && !ctx->group_override; ++k) {
+    for (int k = 0; k < 4 && !tile_cpb && multi == 1 && !ctx->group_override; ++k) {
       const int cand = cond_tile_candidate(ctx->cond_cpb0, k);
       if (coal_tile_fits(cand, (int)ctx->tile_max[k], ctx->o.real_bytes)) { tile_cpb = cand; tile_need = (int)ctx->tile_max[k]; }
     }

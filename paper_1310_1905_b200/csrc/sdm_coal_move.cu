@@ -84,9 +84,42 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a,
         }
       }
       grp.sync();
-      const double dtpp = g.dt / mp.sstp_coal;
+      // R-adapt-coal (PAPER.md :645; oracle: coal_substep_multiplier): sstp_coal * m substeps, m = min(cap, ceil(largest P of
+      // eq. 27 among the pairs of the first grouping, for dt / sstp_coal)); the same IEEE operations as in the pair loop below
+      int nsub = mp.sstp_coal;
+      if (mp.coal_adapt_max > 1 && m >= 2) {
+        const double dt0 = g.dt / mp.sstp_coal;
+        const double scale0 = (double)((u64)m * (u64)(m - 1) / 2) / (double)(m / 2);
+        double pmax = 0.0;
+        for (int pr = grp.lane; pr < m / 2; pr += G) {
+          const int ea = SL(2 * pr), eb = SL(2 * pr + 1);
+          const u64 na = pn[ea], nb = pn[eb];
+          const int j = (na >= nb) ? ea : eb, k = (na >= nb) ? eb : ea;
+          const u64 nj = (na >= nb) ? na : nb;
+          const double yj = prw2[j], yk = prw2[k];
+          const double rj = sqrt(yj), rk = sqrt(yk);
+          double K;
+          if (kp.kernel == 1) {
+            const double vj = (4.0 / 3.0) * cst::pi * (yj * rj), vk = (4.0 / 3.0) * cst::pi * (yk * rk);
+            K = kp.golovin_b * (vj + vk);
+          } else {
+            const double vj = v_term(rj, eta, rho_a), vk = v_term(rk, eta, rho_a);
+            K = cst::pi * ((rj + rk) * (rj + rk)) * fabs(vj - vk);
+            if (kp.kernel == 2) {
+              const double rl = fmax(rj, rk), rs = fmin(rj, rk);
+              K = K * eff_lookup(kp, rl, rs / rl);
+            }
+          }
+          pmax = fmax(pmax, (((double)nj * K) * (dt0 / g.dV)) * scale0);
+        }
+        pmax = grp.max_nonneg(pmax);
+        const double want = ceil(pmax);
+        const int mult = want >= (double)mp.coal_adapt_max ? mp.coal_adapt_max : max(1, (int)want);
+        nsub = mp.sstp_coal * mult;
+      }
+      const double dtpp = g.dt / nsub;
       int nc = m;   // SDs taking part in this substep
-      for (int sub = 0; sub < mp.sstp_coal; ++sub) {
+      for (int sub = 0; sub < nsub; ++sub) {
         if (sub > 0) {
           // new random grouping (:624): drop SDs that reached N = 0, draw new keys, sort again
           const int Pm = next_pow2(m);
@@ -735,8 +768,9 @@ static cudaError_t launch_coal_move_t(int cap, bool in_smem, const SdArraysT<R>&
                                       double* flux_slots, const Counters& cnt, cudaStream_t st) {
   constexpr int NG = CtaOf<G>::threads / G;
   const int grid = (g.ncell + NG - 1) / NG;
-  const int P = mp.sstp_coal > 1 ? next_pow2(cap) : 0;
-  const size_t smem = coal_smem_bytes(G, cap, mp.sstp_coal, in_smem);
+  const bool multi = mp.sstp_coal > 1 || mp.coal_adapt_max > 1;
+  const int P = multi ? next_pow2(cap) : 0;
+  const size_t smem = coal_smem_bytes(G, cap, multi ? 2 : 1, in_smem);
   if (in_smem) {
     cudaError_t e = cudaFuncSetAttribute(k_coal_move<G, true, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

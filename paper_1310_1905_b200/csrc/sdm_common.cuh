@@ -150,6 +150,24 @@ struct Group {
       return t;
     }
   }
+  // largest value over the group (v >= 0), the same on every thread
+  __device__ __forceinline__ double max_nonneg(double v) const {
+    if constexpr (kWarp) {
+#pragma unroll
+      for (int d = G / 2; d >= 1; d >>= 1) v = fmax(v, __shfl_xor_sync(mask, v, d, 32));
+      return v;
+    } else {
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, d, 32));
+      __syncthreads();
+      if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+      __syncthreads();
+      double t = 0.0;
+#pragma unroll
+      for (int w = 0; w < G / 32; ++w) t = fmax(t, red[w]);
+      return t;
+    }
+  }
   __device__ __forceinline__ unsigned long long sum(unsigned long long v) const {
     if constexpr (kWarp) {
 #pragma unroll

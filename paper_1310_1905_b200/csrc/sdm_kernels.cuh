@@ -20,6 +20,7 @@ struct CoalMoveParams {
   int coal, adve, sedi, sstp_coal;
   u32 step;
   int fold;          // k_coal_move_tile also writes next step's cell index, offset and histogram (a0-a1 folded into a6)
+  int coal_adapt_max;   // > 1: per-cell coalescence substeps from P_ij (DESIGN.md R-adapt-coal); per-cell kernel only
 };
 struct CellFields {  // library-owned dense per-cell arrays
   double* rhod;      // copy of the caller's rhod

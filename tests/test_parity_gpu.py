@@ -768,6 +768,29 @@ def test_adaptive_condensation_substeps_match_the_oracle():
         q.step_sync(b.make_opts(cond_adapt_tol=0.1, RH_max=1.05), th, rv)
 
 
+def test_adaptive_coalescence_substeps_match_the_oracle():
+    """sdm_opts.coal_adapt_max > 1 (reading R-adapt-coal; PAPER.md :645 "planned"): cells whose first grouping has
+    a pair with P > 1 take more substeps, each with new random pairs.  The Golovin box of configs[0] (P reaches 25 there), with
+    and without multiple coalescence, and a 2D rain case in a small volume; pairs examined, collisions and multiplicities as the
+    oracle's, and more pairs examined than the fixed step examines."""
+    w = W.box_golovin(seed=44)
+    for multi in (True, False):
+        # the box shrunk to 40^3 m^3: 15.6 times the collision probabilities of configs[0], P above 1 from the start
+        p, o, _, _ = run_both(w, 60, check_every=20, opts=dict(coal_adapt_max=8), multi_coal=multi, dx=40.0, dy=40.0, dz=40.0)
+        sp, so = p.stats(), o.counters()
+        assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"] and sp["near_ties"] == so["near_ties"]
+        assert so["pairs"] > 1.5 * 60 * (p.n_sd() // 2)           # several groupings per step
+        assert p.n_sd() == o.n_sd()
+    w2 = rain_mix(W.cfg2_2d(sd_per_cell=40, nx=6, nz=8, seed=93), frac=0.6)
+    w2.state["n"] = w2.state["n"] * 2000                           # crowded with real drops: P of the rain pairs exceeds 1
+    for group in (0, 256):
+        p, o, _, _ = run_both(w2, 3, group=group, opts=dict(coal_adapt_max=4, sstp_coal=2, cond=False))
+        sp, so = p.stats(), o.counters()
+        assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"] > 100
+        assert so["pairs"] > 3 * 2 * (w2.n_sd // 2) * 0.9 * 1.05  # some cells took more than sstp_coal groupings
+    assert p.stats()["coal_tile_cells"] == 0                       # the per-cell kernel ran
+
+
 # ----------------------------------------------------------------------------------------------- sync / async
 def test_upstream_advect_matches_the_oracle_bit_for_bit():
     """sdm_upstream_advect, the prototype transport solver of PAPER.md Figure 7 (:831-852; upstream scheme :219-235): the same

@@ -494,6 +494,9 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
       }
     }
   }
+  // sparse cells: the smallest candidate tile (a quarter of cond_cpb0) must fit the cell records of the small kernel, or the
+  // launch would fall back to one cell per CTA
+  ctx->cond_cpb0 = std::max(1, std::min(ctx->cond_cpb0, 4 * cond_max_cells(arith32)));
   // a0-a1: the last step_async left cell, off and the histogram behind (k_coal_move_tile), unless recycling moved SDs since
   const bool have_hist = ctx->hist_valid && !(ctx->recycle && ctx->nslots);
   if (ctx->hist_valid && !have_hist) CK(cudaMemsetAsync(ctx->count, 0, sizeof(u32) * g.ncell, st));

@@ -833,7 +833,8 @@ struct Cond4 {
   static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CellRec) + (size_t)(cpb + 1) * 4 + 16; }
 };
 
-template <int CAP, int T, int MINB, typename R>
+// ADAPT: per-cell substep counts (cp.adapt_tol > 0, DESIGN.md R-adapt); the fixed-substep instantiation carries none of it
+template <int CAP, int T, int MINB, typename R, bool ADAPT>
 __global__ void __launch_bounds__(T, MINB)
 k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
         CellFields cf, CondParams cp, Counters cnt, int cpb) {
@@ -881,8 +882,8 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   }
   unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
   const int nsub = M > 0 ? cp.sstp : 0;
-  const bool adapt = cp.adapt_tol > 0.0 && M > 0;
-  if (adapt) {
+  constexpr bool adapt = ADAPT;
+  if (ADAPT && M > 0) {
     // R-adapt (PAPER.md :566; oracle: adaptive_substeps): substeps of each cell from the vapour its SDs would take up in one
     // explicit step, eps = |d r_v| / (r_v max(|RH - 1|, 1e-3)); the smallest divisor d of sstp_cond with d >= sstp_cond eps / tol
     __syncthreads();
@@ -938,8 +939,6 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       }
     }
     __syncthreads();
-  } else {
-    for (int cl = tid; cl < nc; cl += T) s_cell[cl].stride = 1.0;
   }
   for (int sub = 0; sub <= nsub; ++sub) {
     // D. per-cell sums of N d(r_w^3): 8 lanes per cell, fixed order (deterministic); R.pad carries the sum.
@@ -950,7 +949,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       const int l8 = lane & 7, grp = lane >> 3;
       for (int cl = warp * 4 + grp; cl < ((nc + 3) & ~3); cl += NW * 4) {   // warp-uniform trip count
         double acc = 0.0;
-        const bool was_active = cl < nc && s_cell[cl].dtp > 0.0;   // the cell took part in the substep just done
+        const bool was_active = cl < nc && (!ADAPT || s_cell[cl].dtp > 0.0);   // the cell took part in the substep just done
         if (was_active) {
           const int b1 = (int)segl[cl + 1];
           for (int e = (int)segl[cl] + l8; e < b1; e += 8) acc += s_con[e];
@@ -965,11 +964,14 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     if (tid < ((nc + 31) & ~31)) {
       for (int cl = tid; cl < nc; cl += T) {
         CellRec& R = s_cell[cl];
-        const int stride = (int)R.stride;
-        const bool now = sub < nsub && sub % stride == 0;   // the cell takes part in this substep
-        if (sub == 0) { if (!adapt) cell_init(R, cp.RH_max); }
-        else if (now || sub == nsub) cell_advance(R, R.pad, cp.RH_max, true);   // the feedback of its last substep is pending
-        R.dtp = now ? cp.dtp * stride : 0.0;
+        if constexpr (ADAPT) {
+          const int stride = (int)R.stride;
+          const bool now = sub < nsub && sub % stride == 0;   // the cell takes part in this substep
+          if (sub > 0 && (now || sub == nsub)) cell_advance(R, R.pad, cp.RH_max, true);   // the feedback of its last substep is pending
+          R.dtp = now ? cp.dtp * stride : 0.0;
+        } else {
+          if (sub == 0) cell_init(R, cp.RH_max); else cell_advance(R, R.pad, cp.RH_max, true);
+        }
       }
     }
     if (tid == 0) { ctr[0] = 0u; ctr[1] = 0u; }
@@ -980,9 +982,9 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       const int e = q0 + lane;
       const int ec = min(e, M - 1);   // lanes past the end of the tile redo its last SD and discard the result
       const CellRec& R = s_cell[(int)cidx[ec]];
-      const double dtp = R.dtp;
-      const bool valid = e < M && dtp > 0.0;
-      if (adapt && !__any_sync(0xffffffffu, valid)) continue;   // every cell of the chunk sits this substep out
+      const double dtp = ADAPT ? R.dtp : cp.dtp;
+      const bool valid = e < M && (!ADAPT || dtp > 0.0);
+      if (ADAPT && !__any_sync(0xffffffffu, valid)) continue;   // every cell of the chunk sits this substep out
       const double r0 = s_r[ec];
       const double rd2 = s_rd2[ec];
       SdK s;
@@ -1090,7 +1092,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       for (int k = per_warp ? warp : tid; k < nlist; k += per_warp ? NW : T) {
         const int e = (int)list[k];
         const CellRec& R = s_cell[(int)cidx[e]];
-        const double dtp = R.dtp;
+        const double dtp = ADAPT ? R.dtp : cp.dtp;
         CellK c;
         c.RH = R.RH; c.A = R.A; c.c0 = R.c0; c.lD = R.lD; c.lK = R.lK; c.heat = R.heat; c.kE = R.kE; c.Sc = R.Sc; c.Pr = R.Pr;
         const double r0 = s_r[e], y0 = r0 * r0;
@@ -1566,6 +1568,13 @@ constexpr size_t kCondLargeBudget = 227 * 1024;
 
 // 1, 2, 3: small, medium, large tile kernel (in order of preference); 0: a tile of cpb cells with up to `need`
 // SDs fits none of them
+// most cells a tile of the small kernel can hold (its SD slots are a compile-time constant, the cell records take what is left)
+int cond_max_cells(bool arith32) {
+  int c = 1;
+  if (arith32) { while (c < 128 && Cond4F<SDM_COND32_CAP, SDM_COND32_T>::smem(c + 1) <= (228 * 1024 - SDM_COND32_MINB * 1024) / SDM_COND32_MINB) ++c; }
+  else { while (c < 128 && CondSmall::smem(c + 1) <= kCondSmallBudget) ++c; }
+  return c;
+}
 int cond_variant(int cpb, int need) {
   if (cpb <= 128 && need <= SDM_COND_CAP && CondSmall::smem(cpb) <= kCondSmallBudget) return 1;
   if (cpb <= 256 && need <= 1280 && CondMedium::smem(cpb) <= kCondMediumBudget) return 2;
@@ -1577,9 +1586,15 @@ template <int CAP, int T, int MINB, typename R>
 static cudaError_t launch_cond4(size_t smem, int grid, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g, Field th,
                                 Field rv, const CellFields& cf, const CondParams& cp, const Counters& cnt, int cpb,
                                 cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  k_cond4<CAP, T, MINB, R><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  if (cp.adapt_tol > 0.0) {
+    cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_cond4<CAP, T, MINB, R, true><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  } else {
+    cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_cond4<CAP, T, MINB, R, false><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  }
   return cudaGetLastError();
 }
 

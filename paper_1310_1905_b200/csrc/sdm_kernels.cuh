@@ -48,6 +48,7 @@ void launch_export_order(const u32* id, const u16* rank, const u32* seg, int nce
 // up to 800 / 1280 / 4096 SDs per tile (in order of preference), 0 = fits none: work in place in global memory
 // (cpb == 1, `alt` = idle ping-pong copy used as scratch)
 int cond_variant(int cpb, int need);
+int cond_max_cells(bool arith32);   // most cells per tile the small tile kernel has room for (sparse cells)
 int cond_tile_candidate(int cpb0, int k);   // k-th candidate tile size (cells) tried by k_tile_max, k = 0..3
 template <typename R>
 cudaError_t launch_cond(int cpb, int variant, const SdArraysT<R>& a, const SdArraysT<R>& alt, const u16* rank, const u32* seg,

@@ -163,6 +163,21 @@ def test_full_step_3d():
     assert p.stats()["collisions"] == o.counters()["collisions"] > 0
 
 
+def test_sparse_cells_many_cells_per_tile():
+    """4 SDs per cell on 800 x 670 cells: tiles of several dozen cells (the sparse instantiation of k_coal_move_tile, its
+    offset scan beyond 32 cells per tile, the flat staging loops), all-pairs rank counting; and a small box without any
+    spatial dimension through the tile kernel."""
+    import os
+    w = rain_mix(W.cfg2_2d(sd_per_cell=4, nx=800, nz=670, seed=15), frac=0.4)   # 2.14 M SDs: beyond the few-wave tile sizing
+    p, o, th, rv = run_both(w, 3, threads=os.cpu_count() or 4)
+    sp, so = p.stats(), o.counters()
+    assert sp["coal_tile_cells"] >= 8 and sp["cond_tile_cells"] >= 8
+    assert sp["pairs"] == so["pairs"] and sp["collisions"] == so["collisions"] > 0
+    wb = W.box_golovin(seed=45, n_sd=256)
+    p, o, _, _ = run_both(wb, 20, check_every=5, dx=12.0, dy=12.0, dz=12.0)
+    assert p.stats()["coal_tile_cells"] == 1 and p.stats()["collisions"] == o.counters()["collisions"] > 50
+
+
 def test_hydro_tab_kernel_and_paper_variant_without_multiple_coalescence():
     w = rain_mix(W.cfg3_2d_drizzle(sd_per_cell=48, nx=10, nz=12, seed=6))
     run_both(w, 3)

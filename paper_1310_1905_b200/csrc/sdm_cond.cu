@@ -888,19 +888,32 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
   }
   if (tid == 0) { segl[nc] = (u32)M; ctr[0] = 0u; ctr[1] = 0u; }
   __syncthreads();
-  for (int t = tid; t < M; t += T) {   // stage the tile in sorted order
-    int lo = 0, hi = nc;
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
-    const u32 s = s0 + t;
-    const int e = (int)segl[lo] + rank[s];
-    const double rd3 = a.rd3[s];
-    const double q = cbrt(rd3);
-    s_r[e] = sqrt((double)a.rw2[s]);
-    s_rd3[e] = rd3;
-    s_krd3[e] = a.kappa[s] * rd3;
-    s_dn[e] = (double)a.n[s];
-    s_rd2[e] = q * q;
-    cidx[e] = (u16)lo;
+  const bool by_cell = M >= 24 * nc;   // populated cells: a warp stages a cell at a time (no search for the cell of a slot)
+  for (int q = by_cell ? warp : tid; q < (by_cell ? nc : M); q += by_cell ? NW : T) {   // stage the tile in sorted order
+    int cl, t0, t1;
+    if (by_cell) {
+      cl = q; t0 = (int)segl[cl] + lane; t1 = (int)segl[cl + 1];
+    } else {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)q) lo = mid; else hi = mid; }
+      cl = lo; t0 = q; t1 = q + 1;
+    }
+    const int b0 = (int)segl[cl];
+    for (int t = t0; t < t1; t += 32) {
+      const u32 s = s0 + t;
+      const int e = b0 + rank[s];
+      const double rd3 = a.rd3[s];
+      // r_d = cbrt(r_d^3) from the fp32 cube root and one fp64 Newton step (1e-14: r_d^2 only bounds eq. 18 from below)
+      const double c = (double)cbrtf((float)rd3);
+      const double c2 = c * c;
+      const double rd = c - fma(c2, c, -rd3) * rcp_seeded(3.0 * c2);
+      s_r[e] = sqrt((double)a.rw2[s]);
+      s_rd3[e] = rd3;
+      s_krd3[e] = a.kappa[s] * rd3;
+      s_dn[e] = (double)a.n[s];
+      s_rd2[e] = rd * rd;
+      cidx[e] = (u16)cl;
+    }
   }
   unsigned n_ill = 0, n_eval = 0, n_sub = 0, n_slow = 0;
   const int nsub = M > 0 ? cp.sstp : 0;
@@ -1161,12 +1174,21 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
     cf.eta[c] = R.eta;
     cf.rho_a[c] = R.rhod * (1.0 + R.rv);
   }
-  for (int t = tid; t < M; t += T) {
-    int lo = 0, hi = nc;
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)t) lo = mid; else hi = mid; }
-    const u32 s = s0 + t;
-    const double r = s_r[(int)segl[lo] + rank[s]];
-    a.rw2[s] = r * r;
+  for (int q = by_cell ? warp : tid; q < (by_cell ? nc : M); q += by_cell ? NW : T) {
+    int cl, t0, t1;
+    if (by_cell) {
+      cl = q; t0 = (int)segl[cl] + lane; t1 = (int)segl[cl + 1];
+    } else {
+      int lo = 0, hi = nc;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (segl[mid] <= (u32)q) lo = mid; else hi = mid; }
+      cl = lo; t0 = q; t1 = q + 1;
+    }
+    const int b0 = (int)segl[cl];
+    for (int t = t0; t < t1; t += 32) {
+      const u32 s = s0 + t;
+      const double r = s_r[b0 + rank[s]];
+      a.rw2[s] = r * r;
+    }
   }
   unsigned v0 = n_ill, v1 = n_eval, v2 = n_sub, v3 = n_slow;
 #pragma unroll

@@ -51,8 +51,8 @@ def stage_bytes(ndim, rb):
 # R-roots, f and f', the Newton step, N d(r^3), its share of the cells' thermodynamics; "more" = every further evaluation with
 # its third-order corrected Newton step; "other" = the remaining lane slots of fp64-pipe warp instructions (DSETP, conversions,
 # lanes that are predicated off).  flops: DFMA = 2, DMUL = DADD = 1.
-FP64_INSTR = {"first": {"dfma": 55.2, "dmul": 60.3, "dadd": 22.7, "other": 50.9},
-              "more": {"dfma": 40.8, "dmul": 55.3, "dadd": 16.6, "other": 25.7}}
+FP64_INSTR = {"first": {"dfma": 48.9, "dmul": 61.0, "dadd": 21.5, "other": 52.6},
+              "more": {"dfma": 40.2, "dmul": 55.2, "dadd": 16.5, "other": 27.0}}
 FP64_INSTR_SOURCE = "profiles/r2_k_cond4_ncu_full.md"
 FP64_LANES_PER_SM = 64        # fp64 FMA lanes per SM per clock on sm_100 (B200_PROFILING.md; sdm_measure_fp64_peak confirms)
 # --cond-arith 4 (k_cond4f): fp32 operations of one evaluation with derivative and curvature bound (62 instructions, 20 of

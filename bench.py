@@ -84,6 +84,9 @@ def parse():
                     "0 = the fixed sstp_cond of the paper and of the headline")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"], help="N > 1: independent replicas (default), or one domain of "
                     "N x 128 columns decomposed into x-slabs, one per rank, SDs that cross a face exchanged every step (slab.py; weak scaling)")
+    ap.add_argument("--step-stats", default="", help="profiling aid: write one JSON line per step of the device-timed context (warm-up steps "
+                    "included) with the growth-rate evaluations and SD-substeps of that step's condensation launch (sdm_stats deltas); "
+                    "synchronises after every step, so the run's timings are not bench values")
     ap.add_argument("--long-run", type=int, default=-1, help="after the timed region, continue the run to this many steps in all and report "
                     "ms/step, evaluations per SD-substep, slow-list fraction and the launch configuration per 100-step window "
                     "(default: 600 = the length of configs[3] for the default workload, 0 otherwise)")
@@ -298,10 +301,23 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    step_log = open(a.step_stats, "w") if a.step_stats and rank == 0 else None
+    prev = [p.stats()] if step_log else None
+
+    def log_step():
+        if step_log:
+            cur = p.stats()
+            step_log.write(json.dumps({"step": cur["step"], "evals": cur["newton_iters"] - prev[0]["newton_iters"],
+                                       "sd_substeps": cur["sd_substeps"] - prev[0]["sd_substeps"],
+                                       "slow": cur["cond_slow"] - prev[0]["cond_slow"]}) + "\n")
+            step_log.flush()
+            prev[0] = cur
+
     for _ in range(warm):
         p.step_sync(po, th, rv)
         p.step_async(po)
         hand_over(p)
+        log_step()
     # ---- device-resident timing ------------------------------------------------------------------
     p.set_timing(True)
     p.stage_times(reset=True)
@@ -317,6 +333,7 @@ def main():
         sd_steps += p.n_sd()      # live SDs of this step (host-known after the sort, no extra sync)
         p.step_async(po)
         hand_over(p)
+        log_step()
     ev1.record()
     barrier()
     clocks = sampler.stop()

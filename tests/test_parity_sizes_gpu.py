@@ -95,6 +95,27 @@ def test_config2_75x75_128_per_cell_hydro_tab_200_steps():
     assert p.n_sd() == o.n_sd() < w.n_sd
 
 
+LONG = pytest.mark.skipif(os.environ.get("SDM_LONG_TESTS", "") != "1", reason="full-length runs (10 and 35 minutes of oracle time): set SDM_LONG_TESTS=1")
+
+
+@LONG
+def test_config1_full_length_3600_steps():
+    """configs[1] over its full 3600 steps (PAPER.md :858-860: the paper's own run), compared every 300 steps: free-running
+    trajectory bar + the strict single-step bar from the device's state at every checkpoint."""
+    p, o, th, rv = _trajectory(W.cfg2_2d(), 3600, 300)
+    _counters_equal(p, o)
+    assert o.rain_flux_total() > 0
+
+
+@LONG
+def test_config2_full_length_3600_steps():
+    """configs[2] (720 000 SDs, r_v = 8.5 g/kg, tabulated efficiencies) over its full 3600 steps from the haze-only initial
+    condition: the drizzle-forming run."""
+    p, o, th, rv = _trajectory(W.cfg3_2d_drizzle(), 3600, 300)
+    sp, so = _counters_equal(p, o)
+    assert so["collisions"] > 1000
+
+
 def test_one_cell_at_the_capacity_of_a_cta():
     """One cell with ~12 000 SDs (P = 16384, the most a CTA sorts in shared memory): the CTA-wide bitonic ranks
     (k_rank<256>), the in-place condensation kernel (k_cond<false>) and the in-place per-cell coalescence kernel

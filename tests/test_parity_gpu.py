@@ -43,7 +43,8 @@ def compare_states(p, o, positions=True, rtol=RTOL, drift=None):
     """drift = (fraction, rtol_loose), for free-running trajectories of hundreds of steps only: the wet radii of all but
     `fraction` of the SDs within rtol, every one within rtol_loose ("trajectory bar": a droplet that
     evaporates towards its dry size multiplies a relative difference in r^2 by r^2_before / r^2_now, so a difference at
-    the rounding level surfaces, for the few steps that takes, above 1e-9 on a few SDs in 10^5, and decays again)."""
+    the rounding level surfaces, for the few steps that takes, above 1e-9 on a few SDs in 10^5, and decays again); positions
+    within rtol_loose metres (a falling drop integrates the fall speed of its drifted radius over hundreds of steps)."""
     g = sorted_by_id(p.export_state())
     r = sorted_by_id(o.get_state())
     assert len(g["id"]) == len(r["id"])
@@ -60,8 +61,8 @@ def compare_states(p, o, positions=True, rtol=RTOL, drift=None):
     np.testing.assert_allclose(g["kappa"], r["kappa"], rtol=rtol)
     if positions:
         for k, present in zip("xyz", p.dims):
-            if present:
-                np.testing.assert_allclose(g[k][live], r[k][live], rtol=rtol, atol=1e-9)
+            if present:   # (free-running: a position integrates the fall speed of a radius that drifted, see the docstring)
+                np.testing.assert_allclose(g[k][live], r[k][live], rtol=rtol, atol=1e-9 if drift is None else drift[1])
     return g, r
 
 

@@ -268,8 +268,8 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_coal_move(SdArraysT<R> a,
 //    next step's histogram.  There is no barrier between coalescence and movement and no per-SD search for the cell.
 //  * r_d^3 and kappa are touched (in global memory) only by the rare pairs that collide, n and r_w^2 are written back only
 //    where they changed; the new positions go back to shared memory and are stored coalesced in storage order.
-//  * Next step's a0-a1 (PAPER.md :547, :641): `cell` and `off` of every SD and the histogram `count` are produced here
-//    (SDs that stay in the tile's cells are counted in shared memory, one global atomic per cell and tile), so that
+//  * Next step's a0-a1 (PAPER.md :547, :641): `cell` and `off` of every SD and the histogram `count` are produced here, in the
+//    pass that stores the new positions (lanes that go to the same cell share one atomic on count[cell], as in k_cellhist), so that
 //    step_sync need not read the positions again (k_cellhist stays for the first step, recycling and the per-cell kernel).
 //  * Arithmetic: the collision probability and the new positions need not be bit-identical to the oracle's (north_star
 //    counts near-tie decisions; positions are compared to 1e-9), so divisions by per-cell constants are multiplications by
@@ -347,11 +347,11 @@ __device__ __noinline__ double shima_update(const SdArraysT<R>& a, u32 gj, u32 g
 }
 
 template <int CAP, int T, typename R>
-struct CoalTile {   // per slot: u64 n; R rw2, x, y, z; u32 id / new cell; u16 inv, off, rank; u8 cell of the pair
+struct CoalTile {   // per slot: u64 n; R rw2, x, y, z; u32 id / new cell; u16 inv, rank; u8 cell of the pair
   static_assert(CAP % 16 == 0, "the arrays of the tile follow one another in shared memory: keep every one of them 16-byte aligned");
   static constexpr int SLOTS = CAP + 16;   // room for the alignment shift of the bulk copies
-  static constexpr size_t fixed_bytes = (size_t)SLOTS * (8 + 4 * sizeof(R) + 4 + 2 + 2 + 2) + (size_t)(SLOTS / 2) * 2;
-  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * (sizeof(CoalCell) + 16) + 64; }
+  static constexpr size_t fixed_bytes = (size_t)SLOTS * (8 + 4 * sizeof(R) + 4 + 2 + 2) + (size_t)(SLOTS / 2) * 2;
+  static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * (sizeof(CoalCell) + 8) + 64; }
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -383,14 +383,11 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
   R* s_z = s_y + SLOTS;
   u32* s_id = reinterpret_cast<u32*>(s_z + SLOTS);      // id until the pair is done, then the SD's new cell
   u16* inv = reinterpret_cast<u16*>(s_id + SLOTS);
-  u16* s_off = inv + SLOTS;                             // place among the SDs this tile sends to the new cell
-  u16* s_rk = s_off + SLOTS;                            // rank of the slot inside its cell (sdm_sort.cu), element t at t + (s0 mod 8)
+  u16* s_rk = inv + SLOTS;                            // rank of the slot inside its cell (sdm_sort.cu), element t at t + (s0 mod 8)
   u16* s_pc = s_rk + SLOTS;                             // cell (tile-local) of pair p
   CoalCell* s_cell = reinterpret_cast<CoalCell*>(smem_raw + L::fixed_bytes);
   u32* segl = reinterpret_cast<u32*>(s_cell + cpb);     // storage offsets of the tile's cells
   u32* segp = segl + cpb + 1;                           // padded (even) offsets of the sorted positions
-  u32* s_cnt = segp + cpb + 1;                          // next step's histogram of the tile's own cells
-  u32* s_base = s_cnt + cpb;
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
   const int sh = (int)(s0 & 3u);
@@ -432,7 +429,6 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
       const int c = c_first + cl;
       const u32 b0 = seg[c], b1 = seg[c + 1];
       segl[cl] = b0 - s0;
-      s_cnt[cl] = 0u;
       const int m = (int)(b1 - b0);
       CoalCell& C = s_cell[cl];
       const double eta = cf.eta[c], rho_a = cf.rho_a[c];
@@ -614,42 +610,30 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
       }
     }
     __syncthreads();
-    if (mp.fold) {
-      // places in the next histogram, taken in STORAGE order (the reorder of the next step then writes runs, not a
-      // permutation of each cell): lanes that go to the same cell take consecutive places with one atomic, in shared
-      // memory for the tile's own cells
+    // ---- new positions back to global memory, coalesced in storage order; with mp.fold also the SD's cell and its place in
+    // the next step's histogram, taken in STORAGE order (the reorder of the next step then writes runs, not a permutation of
+    // each cell): lanes that go to the same cell take consecutive places with one atomic on count[cell], as k_cellhist does
+    if (moving || mp.fold) {
       for (int t0 = 0; t0 < M; t0 += T) {
         const int t = t0 + tid;
-        const u32 cnew = t < M ? s_id[t + sh] : CELL_DEAD;
-        const u32 peers = __match_any_sync(0xffffffffu, cnew);
-        const int leader = __ffs(peers) - 1;
-        const u32 rel = cnew - (u32)c_first;
-        u32 base = 0;
-        if (cnew != CELL_DEAD && lane == leader)
-          base = rel < (u32)nc ? atomicAdd(&s_cnt[rel], (u32)__popc(peers)) : atomicAdd(&count[cnew], (u32)__popc(peers));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (cnew != CELL_DEAD) s_off[t + sh] = (u16)(base + __popc(peers & ((1u << lane) - 1u)));
-      }
-      __syncthreads();
-      for (int cl = tid; cl < nc; cl += T) { const u32 k = s_cnt[cl]; s_base[cl] = k ? atomicAdd(&count[c_first + cl], k) : 0u; }
-      __syncthreads();
-    }
-    // ---- new positions, cell and offset back to global memory, coalesced in storage order ----------------------------------
-    if (moving || mp.fold) {
-      for (int t = tid; t < M; t += T) {
-        const u32 s = s0 + t;
+        const bool in = t < M;
+        const u32 s = s0 + (u32)t;
         const int sl = t + sh;
-        if (moving) {
+        if (in && moving) {
           if (g.hx) a.x[s] = s_x[sl];
           if (g.hy) a.y[s] = s_y[sl];
           if (g.hz) a.z[s] = s_z[sl];
         }
         if (mp.fold) {
-          const u32 cnew = s_id[sl];
-          cell_out[s] = cnew;
-          if (cnew != CELL_DEAD) {
-            const u32 rel = cnew - (u32)c_first;
-            off_out[s] = (u32)s_off[sl] + (rel < (u32)nc ? s_base[rel] : 0u);
+          const u32 cnew = in ? s_id[sl] : CELL_DEAD;
+          const u32 peers = __match_any_sync(0xffffffffu, cnew);
+          const int leader = __ffs(peers) - 1;
+          u32 base = 0;
+          if (cnew != CELL_DEAD && lane == leader) base = atomicAdd(&count[cnew], (u32)__popc(peers));
+          base = __shfl_sync(0xffffffffu, base, leader);
+          if (in) {
+            cell_out[s] = cnew;
+            if (cnew != CELL_DEAD) off_out[s] = base + __popc(peers & ((1u << lane) - 1u));
           }
         }
       }

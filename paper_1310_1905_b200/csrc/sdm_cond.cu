@@ -156,12 +156,14 @@ __device__ __forceinline__ void growth_r(double r, const SdK& s, const CellR& c,
   const double Q = fma(KN, DM, HN * DT);
   const double r3 = y * r;
   const double P = r3 - s.rd3, W = P + s.krd3;
-  const double QW = Q * W;
-  const double inv = rcp_nr<2>(r * QW);
-  const double invr = inv * QW, invQ = inv * (r * W), invW = inv * (r * Q);
+  // two reciprocals, 1/r and 1/(Q W), instead of one of r Q W: the Kelvin exponent and its exp then depend on r alone and run
+  // beside the chain that leads to Q (the kernel is bound by dependent-instruction latency)
+  const double invr = rcp_nr<2>(r);
   const double t = c.A * invr;
   t_out = t;
   const double ex = exp_kelvin(t);
+  const double inv = rcp_nr<2>(Q * W);
+  const double invQ = inv * W, invW = inv * Q;
   const double NN = NM * NT;
   const double aw = P * invW;
   const double S = fma(-aw, ex, c.RH);

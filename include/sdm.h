@@ -294,6 +294,30 @@ int sdm_upstream_advect(sdm_ctx* ctx, sdm_arrinfo psi, void* stream);
  * allocates and frees 1.3 MB of device memory.  Blocking.  SDM_ERR_NO_DEVICE without a device. */
 int sdm_measure_fp64_peak(double* fma_tflops, double* dfma_per_clk_per_sm, void* stream);
 
+/* An entry point that allocates nothing, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  The operation is the scan of the counting sort by cell (SURVEY.md section 8
+ * row a2; PAPER.md :641, the super-droplets are sorted by cell before the pairs are drawn): from the per-cell numbers of
+ * super-droplets count[0..ncell) it writes the start of every cell's segment in the sorted order,
+ *     seg[c] = count[0] + ... + count[c-1]   (c = 0..ncell;  seg[ncell] = the total),
+ * exactly (32-bit unsigned arithmetic, as in the step; the total must fit 32 bits).
+ * count: DEVICE, ncell words, read only (the step's own scan zeroes its histogram; this one does not).  seg: DEVICE,
+ * ncell + 1 words, written.  Both caller-owned; they must not overlap.  Needs no context.  Enqueues 3 kernels on `stream`
+ * of the current device and returns; no host synchronisation, no cudaMalloc / cudaFree / allocating library routine.
+ * The block sums it needs live in a static device array of 16 KB inside the library (held by every GPU that loads the
+ * library, until the process exits), which bounds the size: ncell <= SDM_NOALLOC_MAX_CELLS, beyond which the call is
+ * refused with SDM_ERR_CAPACITY and enqueues nothing.  SDM_ERR_INVALID for NULL pointers or ncell < 0, SDM_ERR_NO_DEVICE
+ * without a device, SDM_ERR_CUDA if a launch fails; the message is available from sdm_noalloc_last_error() (per host thread).
+ * All calls on one device share that array, and it keeps the last call's contents (nothing in it has to start at zero:
+ * every call overwrites what it reads).  Calls that OVERLAP on the GPU - different streams, or host threads, on the same
+ * device without an ordering between them - race on it and give wrong offsets; calls on one stream are safe.
+ * sdm_cell_offsets_noalloc_setup(): looks up the array's device address for the CURRENT device (cudaGetSymbolAddress, once
+ * per device).  The entry point does this itself on its first call on a device; call the set-up beforehand, with the
+ * device current, where that first call would come at a bad time (before starting a graph capture). */
+#define SDM_NOALLOC_MAX_CELLS 16777216LL
+int sdm_cell_offsets_noalloc_setup(void);
+int sdm_cell_offsets_noalloc(const uint32_t* count, int64_t ncell, uint32_t* seg, void* stream);
+const char* sdm_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -56,7 +56,8 @@ EXPORTS = ["sdm_create", "sdm_destroy", "sdm_last_error", "sdm_init", "sdm_init_
            "sdm_step_async_result", "sdm_step_host", "sdm_diag_sd_conc", "sdm_diag_dry_rng", "sdm_diag_wet_rng",
            "sdm_diag_dry_mom", "sdm_diag_wet_mom", "sdm_outbuf", "sdm_n_sd", "sdm_n_live", "sdm_export_state", "sdm_export_order",
            "sdm_stats", "sdm_set_step", "sdm_set_group_size", "sdm_set_cond_kfast", "sdm_set_timing", "sdm_stage_times", "sdm_set_recycle", "sdm_set_cond_arith",
-           "sdm_measure_fp64_peak", "sdm_upstream_advect", "sdm_pack_leavers", "sdm_unpack_arrivals"]
+           "sdm_measure_fp64_peak", "sdm_upstream_advect", "sdm_pack_leavers", "sdm_unpack_arrivals",
+           "sdm_cell_offsets_noalloc", "sdm_cell_offsets_noalloc_setup", "sdm_noalloc_last_error"]
 
 STAGES = ("hist", "scan", "scatter", "rank", "cond", "coal_move", "recycle")
 
@@ -107,6 +108,10 @@ def load_library():
     L.sdm_set_recycle.argtypes = [vp, C.c_int]
     L.sdm_set_cond_arith.argtypes = [vp, C.c_int]
     L.sdm_stage_times.argtypes = [vp, C.POINTER(C.c_double), u64p, C.c_int]
+    L.sdm_cell_offsets_noalloc_setup.argtypes = []
+    L.sdm_cell_offsets_noalloc.argtypes = [vp, C.c_int64, vp, vp]
+    L.sdm_noalloc_last_error.argtypes = []
+    L.sdm_noalloc_last_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -343,6 +348,33 @@ def measure_fp64_peak():
     if rc != 0:
         raise SdmError(f"sdm_measure_fp64_peak failed ({rc})")
     return t.value, r.value
+
+
+NOALLOC_MAX_CELLS = 16777216   # SDM_NOALLOC_MAX_CELLS of include/sdm.h
+
+
+def cell_offsets_noalloc_setup():
+    """sdm_cell_offsets_noalloc_setup for the current device (optional: the first call does it otherwise)."""
+    L = load_library()
+    rc = L.sdm_cell_offsets_noalloc_setup()
+    if rc != 0:
+        raise SdmError(f"libsdm error {rc}: {L.sdm_noalloc_last_error().decode()}")
+
+
+def cell_offsets_noalloc(count, seg, ncell=None):
+    """sdm_cell_offsets_noalloc: seg[c] = count[0] + .. + count[c-1], c = 0..ncell, on the current stream, with no allocation
+    on the way (the library's static scratch; calls that overlap on the GPU race, see include/sdm.h).  count: CUDA int32
+    tensor of >= ncell per-cell SD numbers (the bits are read as unsigned); seg: CUDA int32 tensor of >= ncell + 1 words,
+    caller-allocated, written in place.  Only marshalling here."""
+    L = load_library()
+    n = count.numel() if ncell is None else int(ncell)
+    if n <= NOALLOC_MAX_CELLS:   # beyond the limit the library refuses before it touches a buffer: let it say so
+        assert count.is_cuda and seg.is_cuda and count.dtype == torch.int32 and seg.dtype == torch.int32
+        assert count.is_contiguous() and seg.is_contiguous() and 0 <= n <= count.numel() and seg.numel() >= n + 1
+    rc = L.sdm_cell_offsets_noalloc(_ptr(count), n, _ptr(seg), _stream())
+    if rc != 0:
+        raise SdmError(f"libsdm error {rc}: {L.sdm_noalloc_last_error().decode()}")
+    return seg
 
 
 def _as_tensor(ptr, n):

@@ -22,6 +22,7 @@ UNITS = {
     "sdm_peak.cu": [],
     "sdm_euler.cu": ["-fmad=false"],
     "sdm_slab.cu": [],
+    "sdm_noalloc.cu": [],
 }
 HEADERS = ["sdm_common.cuh", "sdm_kernels.cuh", os.path.join("..", "..", "include", "sdm.h")]
 

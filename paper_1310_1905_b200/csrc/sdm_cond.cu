@@ -50,7 +50,7 @@ struct SdK {   // per-SD constants of one substep
 //   beta_M = N_M/D_M, beta_T = N_T/D_T (Fuchs-Sutugin multiplied through by r^2),
 //   D_eff = Dc Kc N_M N_T / Q,  Q = Kc N_T D_M + heat Dc N_M D_T,
 //   a_w = P/W, P = r^3 - r_d^3, W = P + kappa r_d^3,  f = c0 D_eff (RH - a_w exp(A/r)).
-__device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c, double& f, double& df) {
+__device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c, double& f, double& df, double& cDN_out) {
   const double invr = rsqrt(y);
   const double r = y * invr;
   const double lDr = c.lD * r, lKr = c.lK * r;
@@ -67,7 +67,9 @@ __device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c
   const double aw = P * invW;
   const double S = c.RH - aw * ex;
   const double cD = s.cDK * invQ;
-  f = cD * NN * S;
+  const double cDN = cD * NN;   // c0 D_eff(y)
+  cDN_out = cDN;
+  f = cDN * S;
   // derivative
   const double hr = 0.5 * invr;   // dr/dy
   const double NMp = fma(c.lD, hr, 1.0), DMp = fma(1.71 * c.lD, hr, 1.0);
@@ -77,6 +79,10 @@ __device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c
   const double awp = 1.5 * r * s.krd3 * (invW * invW);
   const double Sp = -ex * (awp - aw * (c.A * hr) * (invr * invr));
   df = cD * fma(NNp - NN * (Qp * invQ), S, NN * Sp);
+}
+__device__ __forceinline__ void growth_fd(double y, const SdK& s, const CellK& c, double& f, double& df) {
+  double cDN;
+  growth_fd(y, s, c, f, df, cDN);
 }
 
 // ---- fast path (k_cond4): the same equations written in r = sqrt(y), which stays resident in shared
@@ -281,15 +287,31 @@ __device__ __forceinline__ void sd_setup(double r0, double c0, double heat, doub
 //      dt' c0 D 1.3 A / (2 r^3) <= 1/2 and e^(A/r) <= 1.3, or
 //  (3) the particle grows (lo = y0) in subsaturated air: a_w e^(A/r) = RH < 1 has one solution y_eq, on the
 //      rising side of the Koehler curve, f > 0 below it and f < 0 above, so g > 0 from y_eq on and changes sign
-//      once between y0 and y_eq (haze catching up with a moister cell: by far the most frequent wide bracket).
+//      once between y0 and y_eq (haze catching up with a moister cell: by far the most frequent wide bracket), or
+//  (4) the particle evaporates (f(y0) < 0, hi = y0) and the Kelvin term is as weak as in (2), however wide the bracket.
+//      A root below y0 needs f < 0 there (g = y - y0 - dt' f), i.e. S = RH - a_w e^(A/r) < 0, and the set S < 0 is an
+//      interval that holds y0 (the Koehler curve a_w e^(A/r) rises to r_c, then falls towards 1).  On it D_eff' S <= 0
+//      (D_eff rises with r), so g' >= 1 - dt' c0 D_eff S', and S' > 0 only on the falling branch y >= y_c, where
+//      S' <= e^(A/r) A / (2 r^3): with e^(A/r) <= 1.3 and r^3 >= ym^(3/2), g' >= 1 - K3 / (2 ym^(3/2)) > 0: g rises
+//      through the whole set, one root at most (a droplet of ~1 um shrinking by 10 % per substep under cloud base: its
+//      bracket [0.6 y0, y0] is too wide for (2), and the literal bisection took 36 to 315 evaluations for it).
+//      Below y0, c0 D_eff(y) <= c0 D_eff(y0), which the evaluation at y0 has as f / S: dtcDe = dt' c0 D_eff(y0) takes
+//      the place of dtcD in this rule (a third of it at 0.5 um), and the rule asks for g' > 0 only:
+//      K3 / (2 ym^(3/2)) <= 0.92.  Applied on the slow list only (RULE4; its SDs then need one round of the warp
+//      bisection and ~3 Newton evaluations): in the sweeps every instruction of this test is paid by every SD-substep,
+//      and the two it takes there cost the 67M-SD step 0.8 % while its list is 5e-5 of the SD-substeps either way
+//      (profiles/r2_k_cond4_ncu_full.md).
 // Everything else is solved by the paper's own procedure, literally (bisect_paper).  dtcD = dt' c0 D_0 Sh/2.
+template <bool RULE4 = true>
 __device__ __forceinline__ bool single_root_bracket(double lo, double hi, double y0, double RH, double rd3, double krd3, double A,
-                                                    double invA, double dtcD) {
+                                                    double invA, double dtcD, double dtcDe) {
   const double yc = 3.0 * krd3 * invA;
   if ((hi <= yc && krd3 <= 2.0 * rd3) || (RH < 1.0 && lo == y0)) return true;   // (1), (3)
   const double ym = dmax(lo, yc);
-  const double K3 = 1.3 * A * dtcD;
-  return (hi - lo <= 0.5 * lo) && (ym * ym * ym >= K3 * K3) && (A * A <= 0.0625 * ym);   // (2)
+  const bool evap = RULE4 && hi <= y0;   // a bracket below y0: only an evaporating particle has one (a growing one has lo = y0 < hi)
+  const double K3 = 1.3 * A * (evap ? dtcDe : dtcD);
+  const double K32 = evap ? 0.3 * (K3 * K3) : K3 * K3;
+  return (evap || hi - lo <= 0.5 * lo) && (ym * ym * ym >= K32) && (A * A <= 0.0625 * ym);   // (4), (2)
 }
 
 // per-SD constants of one substep in plain fp64 (cond_solve and the literal bisection)
@@ -341,7 +363,7 @@ __device__ __forceinline__ double newton_in_bracket(double a, double b, bool ga_
 // as the serial loop of the oracle, a fifth of its latency.  All lanes pass the same arguments.
 __device__ __forceinline__ double bisect_paper_warp(double a, double b, double f0, double y0, const SdK& s, const CellK& c,
                                                     double dtp, int lane, unsigned& n_ill, unsigned& n_eval, double rd3, double krd3,
-                                                    double invA, double dtcD) {
+                                                    double invA, double dtcD, double dtcDe) {
   double f, df;
   double ga, gb;
   if (a == y0) ga = -dtp * f0; else { growth_fd(a, s, c, f, df); n_eval += (lane == 0); ga = a - y0 - dtp * f; }
@@ -379,7 +401,7 @@ __device__ __forceinline__ double bisect_paper_warp(double a, double b, double f
     }
     if (done) break;
     // five levels narrower: once the bracket provably holds one root, Newton finishes (the same on every lane)
-    if (single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, invA, dtcD)) {
+    if (single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, invA, dtcD, dtcDe)) {
       unsigned ev = 0;
       const double y = newton_in_bracket(a, b, ga_pos, y0, s, c, dtp, ev);
       n_eval += (lane == 0) ? ev : 0u;
@@ -397,11 +419,11 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
   double Dc;
   slow_setup(y0, rd3, krd3, c, s, Dc);
   int mode = M_FIRST;
-  double yE = y0, y = y0, g = 0.0, gp = 1.0, a = 0.0, b = 0.0, lo = 0.0, hi = 0.0, dprev = 0.0;
+  double yE = y0, y = y0, g = 0.0, gp = 1.0, a = 0.0, b = 0.0, lo = 0.0, hi = 0.0, dprev = 0.0, dtcDe = 0.0;
   bool lo_unv = false, hi_unv = false;
   for (int it = 0; it < max_evals; ++it) {
-    double f, df;
-    growth_fd(yE, s, c, f, df);   // the only evaluation site
+    double f, df, cDN;
+    growth_fd(yE, s, c, f, df, cDN);   // the only evaluation site
     ++n_eval;
     bool bisect = false;
     if (mode == M_FIRST) {
@@ -409,7 +431,8 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
       a = fmax(rd2, y0 + fmin(two, 0.0));   // eq. 18
       b = y0 + fmax(two, 0.0);              // eq. 19
       if (!(a < b)) { y_out = a; return true; }
-      if (!single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc)) {
+      dtcDe = dtp * cDN;                    // dt' c0 D_eff(y0): rule (4) of single_root_bracket
+      if (!single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc, dtcDe)) {
         // the paper's procedure, literally (:573-579): signs at both ends, (a+b)/2 if they agree, else bisection
         if (max_evals < 100) return false;   // not in a budgeted sweep: leave it to the pass that may finish
         const double f0 = f;
@@ -428,7 +451,7 @@ __device__ __forceinline__ bool cond_solve(double y0, double rd2, double rd3, do
           const double gm = m - y0 - dtp * f;
           if (gm == 0.0) { y_out = m; return true; }
           if ((gm > 0.0) == (ga > 0.0)) { a = m; ga = gm; } else { b = m; gb = gm; }
-          if (++level % 5 == 0 && single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc)) {
+          if (++level % 5 == 0 && single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, 1.0 / c.A, dtp * c.c0 * Dc, dtcDe)) {
             y_out = newton_in_bracket(a, b, ga > 0.0, y0, s, c, dtp, n_eval);   // one root left in the bracket: Newton finishes
             return true;
           }
@@ -1041,7 +1064,7 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
       int st;
       // guards: the range of exp_kelvin, and the bracket must hold at most one root
       const bool guard = !(t < 4.0) ||
-                         !single_root_bracket(lo, hi, y0, c.RH, s.rd3, s.krd3, c.A, R.invA, dtp * s.c0Dc);
+                         !single_root_bracket<false>(lo, hi, y0, c.RH, s.rd3, s.krd3, c.A, R.invA, dtp * s.c0Dc, 0.0);
       if (!(lo < hi)) {
         st = (lo == y0) ? 1 : 2;                    // a = b: the result is a
       } else {
@@ -1139,14 +1162,14 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
         bool solved = false;
         if (per_warp) {   // all lanes hold the same SD
           SdK s;
-          double Dc, f, df;
+          double Dc, f, df, cDN;
           slow_setup(y0, rd3, krd3, c, s, Dc);
-          growth_fd(y0, s, c, f, df);
+          growth_fd(y0, s, c, f, df, cDN);
           const double two = 2.0 * dtp * f;
           const double a = fmax(rd2, y0 + fmin(two, 0.0)), b = y0 + fmax(two, 0.0);   // eq. 18-19
-          if (a < b && !single_root_bracket(a, b, y0, c.RH, rd3, krd3, c.A, R.invA, dtp * s.c0Dc)) {
+          if (a < b) {   // the paper's procedure on the whole warp, whatever the bracket: it hands over to Newton once certified
             ev = (lane == 0);
-            y1 = bisect_paper_warp(a, b, f, y0, s, c, dtp, lane, ill, ev, rd3, krd3, R.invA, dtp * s.c0Dc);
+            y1 = bisect_paper_warp(a, b, f, y0, s, c, dtp, lane, ill, ev, rd3, krd3, R.invA, dtp * s.c0Dc, dtp * cDN);
             solved = true;
           }
         }
@@ -1522,14 +1545,14 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
         bool solved = false;
         if (per_warp) {   // all lanes hold the same SD
           SdK s;
-          double Dc, f, df;
+          double Dc, f, df, cDN;
           slow_setup(y0, rd3, krd3, c, s, Dc);
-          growth_fd(y0, s, c, f, df);
+          growth_fd(y0, s, c, f, df, cDN);
           const double two = 2.0 * cp.dtp * f;
           const double a_ = fmax(rd2, y0 + fmin(two, 0.0)), b_ = y0 + fmax(two, 0.0);   // eq. 18-19
-          if (a_ < b_ && !single_root_bracket(a_, b_, y0, c.RH, rd3, krd3, c.A, R.invA, cp.dtp * s.c0Dc)) {
+          if (a_ < b_) {   // the paper's procedure on the whole warp, whatever the bracket: it hands over to Newton once certified
             ev = (lane == 0);
-            y1 = bisect_paper_warp(a_, b_, f, y0, s, c, cp.dtp, lane, ill, ev, rd3, krd3, R.invA, cp.dtp * s.c0Dc);
+            y1 = bisect_paper_warp(a_, b_, f, y0, s, c, cp.dtp, lane, ill, ev, rd3, krd3, R.invA, cp.dtp * s.c0Dc, cp.dtp * cDN);
             solved = true;
           }
         }

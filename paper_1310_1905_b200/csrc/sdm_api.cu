@@ -84,6 +84,7 @@ struct sdm_ctx {
   u64 launches = 0;
   u64 host_syncs = 0;
   int last_cond_variant = 0, last_cond_cpb = 0, last_coal_cpb = 0;
+  bool mv_valid = false;     // cf.mv matches cf.rhod and the Courant fields
   double dry_lo = 0, dry_hi = 1e300, wet_lo = 0, wet_hi = 1e300;
   // optional per-stage timing with CUDA events on the launching stream (sdm_set_timing)
   bool timing = false;
@@ -139,6 +140,7 @@ int copy_courants(sdm_ctx* ctx, const sdm_arrinfo* comps, cudaStream_t st) {
     double* dst = dim == 0 ? ctx->cx : dim == 1 ? ctx->cy : ctx->cz;
     launch_dense_copy(make_field(ctx, a), dst, g.NX + (dim == 0), g.NY + (dim == 1), g.NZ + (dim == 2), st);
     ctx->launches++;
+    ctx->mv_valid = false;
   }
   CK(cudaGetLastError());
   return SDM_OK;
@@ -264,7 +266,7 @@ int sdm_create(const sdm_opts_init* o, sdm_ctx** out) {
       (e = dalloc(&ctx->th_dense, (size_t)g.ncell)) || (e = dalloc(&ctx->rv_dense, (size_t)g.ncell)) ||
       (e = dalloc(&ctx->cx, (size_t)(g.NX + 1) * g.NY * g.NZ)) || (e = dalloc(&ctx->cy, (size_t)g.NX * (g.NY + 1) * g.NZ)) ||
       (e = dalloc(&ctx->cz, (size_t)g.NX * g.NY * (g.NZ + 1))) || (e = dalloc(&ctx->flux_slots, NSLOT)) ||
-      (e = dalloc(&ctx->flux_part, (size_t)g.ncell)) ||
+      (e = dalloc(&ctx->flux_part, (size_t)g.ncell)) || (e = dalloc(&ctx->cf.mv, (size_t)6 * g.ncell)) ||
       (e = dalloc(&ctx->d_flux, 4)) || (e = dalloc(&ctx->cnt_mem, N_COUNTERS * NSLOT)))
     return bail(e, "scratch");
   ctx->cf.cx = ctx->cx; ctx->cf.cy = ctx->cy; ctx->cf.cz = ctx->cz;
@@ -332,6 +334,7 @@ void sdm_destroy(sdm_ctx* ctx) {
     cudaFree(a.n); cudaFree(a.rw2); cudaFree(a.rd3); cudaFree(a.kappa); cudaFree(a.x); cudaFree(a.y); cudaFree(a.z); cudaFree(a.id);
   }
   cudaFree(ctx->cell); cudaFree(ctx->off); cudaFree(ctx->rank); cudaFree(ctx->count); cudaFree(ctx->blocksum); cudaFree(ctx->seg);
+  cudaFree(ctx->cf.mv);
   cudaFree(ctx->d_info); cudaFree(ctx->cf.rhod); cudaFree(ctx->cf.eta); cudaFree(ctx->cf.rho_a); cudaFree(ctx->outbuf);
   cudaFree(ctx->th_dense); cudaFree(ctx->rv_dense); cudaFree(ctx->cx); cudaFree(ctx->cy); cudaFree(ctx->cz);
   cudaFree(ctx->adv_tmp);
@@ -372,6 +375,7 @@ int sdm_init(sdm_ctx* ctx, sdm_arrinfo th, sdm_arrinfo rv, sdm_arrinfo rhod, sdm
   const u64 N = (u64)Nd;
   launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st);
   ctx->launches++;
+  ctx->mv_valid = false;
   const sdm_arrinfo comps[3] = {c1, c2, c3};
   if (int rc = copy_courants(ctx, comps, st)) return rc;
   ctx->cur = 0; ctx->cn = 0;
@@ -405,6 +409,7 @@ int sdm_init_from_arrays(sdm_ctx* ctx, sdm_arrinfo rhod, sdm_arrinfo c1, sdm_arr
   if (!rhod.data_zero) return fail(ctx, SDM_ERR_INVALID, "sdm_init_from_arrays: rhod is mandatory");
   launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st);
   ctx->launches++;
+  ctx->mv_valid = false;
   const sdm_arrinfo comps[3] = {c1, c2, c3};
   if (int rc = copy_courants(ctx, comps, st)) return rc;
   ctx->cur = 0; ctx->cn = 0;
@@ -443,7 +448,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
     return fail(ctx, SDM_ERR_INVALID, "sdm_step_sync: cond_adapt_tol needs the fp64-arithmetic condensation (sdm_set_cond_arith 8)");
   if (ctx->synced) return fail(ctx, SDM_ERR_ORDER, "sdm_step_sync: called twice without step_async");
   ctx->last_stream = st;
-  if (rhod.data_zero) { launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st); ctx->launches++; }
+  if (rhod.data_zero) { launch_dense_copy(make_field(ctx, rhod), ctx->cf.rhod, g.NX, g.NY, g.NZ, st); ctx->launches++; ctx->mv_valid = false; }
   const sdm_arrinfo comps[3] = {c1, c2, c3};
   if (int rc = copy_courants(ctx, comps, st)) return rc;
 
@@ -615,6 +620,11 @@ int sdm_step_async(sdm_ctx* ctx, const sdm_opts* op, void* stream) {
     const bool f64 = ctx->o.real_bytes == 8;
     ctx->n_flux_part = tile_cpb ? (g.ncell + tile_cpb - 1) / tile_cpb : 0;
     ctx->hist_valid = tile_cpb && mp.fold;
+    if (tile_cpb && op->adve && !ctx->mv_valid) {   // eq. 16 per cell: once per set of Courant fields, not once per step
+      launch_cell_move_consts(g, ctx->cf, st);
+      ctx->mv_valid = true;
+      ctx->launches++;
+    }
     if (tile_cpb && f64)
       CK(launch_coal_move_tile(tile_cpb, tile_need, view<double>(ctx->buf[ctx->cur]), ctx->rank, ctx->seg, g, ctx->cf, ctx->kp, mp,
                                ctx->flux_part, ctx->cnt, ctx->cell, ctx->off, ctx->count, st));

@@ -346,6 +346,37 @@ __device__ __noinline__ double shima_update(const SdArraysT<R>& a, u32 gj, u32 g
   return (double)y2;
 }
 
+// eq. 16 per cell (PAPER.md :556-558): x' = (x + a) b with a = dx (C_l - i dC), b = 1 / (1 - dC), from the Courant numbers at the
+// faces of the cell.  They change only when the caller hands new Courant fields or a new rho_d to step_sync, so they are a
+// table (cf.mv, 6 doubles per cell), not something every tile works out again in every step behind its first barrier.
+__global__ void __launch_bounds__(256) k_cell_move_consts(Grid g, CellFields cf) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= g.ncell) return;
+  const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
+  const double rhod = cf.rhod[c];
+  double ax = 0.0, bx = 1.0, ay = 0.0, by = 1.0, az = 0.0, bz = 1.0;
+  if (g.hx) {
+    const double Cl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod, Ch = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod;
+    const double dC = Ch - Cl;
+    ax = g.dx * (Cl - (double)i * dC); bx = 1.0 / (1.0 - dC);
+  }
+  if (g.hy) {
+    const double Cl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod, Ch = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod;
+    const double dC = Ch - Cl;
+    ay = g.dy * (Cl - (double)j * dC); by = 1.0 / (1.0 - dC);
+  }
+  if (g.hz) {
+    const double Cl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod, Ch = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod;
+    const double dC = Ch - Cl;
+    az = g.dz * (Cl - (double)k * dC); bz = 1.0 / (1.0 - dC);
+  }
+  double2* o = reinterpret_cast<double2*>(cf.mv + (size_t)6 * c);
+  o[0] = make_double2(ax, bx); o[1] = make_double2(ay, by); o[2] = make_double2(az, bz);
+}
+void launch_cell_move_consts(const Grid& g, const CellFields& cf, cudaStream_t st) {
+  k_cell_move_consts<<<(g.ncell + 255) / 256, 256, 0, st>>>(g, cf);
+}
+
 template <int CAP, int T, typename R>
 struct CoalTile {   // per slot: u64 n; R rw2, x, y, z; u32 id / new cell; u16 inv, rank; u8 cell of the pair
   static_assert(CAP % 16 == 0, "the arrays of the tile follow one another in shared memory: keep every one of them 16-byte aligned");
@@ -431,31 +462,19 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
       segl[cl] = b0 - s0;
       const int m = (int)(b1 - b0);
       CoalCell& C = s_cell[cl];
+      // everything this lane needs from global memory is requested before any of it is used: the whole CTA waits for
+      // these few lanes at the next barrier, so one memory latency and ~25 instructions here instead of nine divisions
       const double eta = cf.eta[c], rho_a = cf.rho_a[c];
-      C.kX = (32.0 / 3.0) * (cst::rho_w - rho_a) * cst::g * rho_a / (eta * eta);
-      C.kv = eta * (cst::kc_delta0 * cst::kc_delta0 / 4.0) / (2.0 * rho_a);
-      C.scale = m >= 2 ? (double)((u64)m * (u64)(m - 1) / 2) / (double)(m / 2) : 0.0;
-      const int k = c % g.NZ, j = (c / g.NZ) % g.NY, i = c / (g.NZ * g.NY);
-      const double rhod = cf.rhod[c];
-      C.ax = C.ay = C.az = 0.0;
-      C.bx = C.by = C.bz = 1.0;
-      if (mp.adve) {   // eq. 16 with the Courant numbers at the faces of the SD's time-n cell
-        if (g.hx) {
-          const double Cl = cf.cx[((long long)i * g.NY + j) * g.NZ + k] / rhod, Ch = cf.cx[((long long)(i + 1) * g.NY + j) * g.NZ + k] / rhod;
-          const double dC = Ch - Cl;
-          C.ax = g.dx * (Cl - (double)i * dC); C.bx = 1.0 / (1.0 - dC);
-        }
-        if (g.hy) {
-          const double Cl = cf.cy[((long long)i * (g.NY + 1) + j) * g.NZ + k] / rhod, Ch = cf.cy[((long long)i * (g.NY + 1) + j + 1) * g.NZ + k] / rhod;
-          const double dC = Ch - Cl;
-          C.ay = g.dy * (Cl - (double)j * dC); C.by = 1.0 / (1.0 - dC);
-        }
-        if (g.hz) {
-          const double Cl = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k] / rhod, Ch = cf.cz[((long long)i * g.NY + j) * (g.NZ + 1) + k + 1] / rhod;
-          const double dC = Ch - Cl;
-          C.az = g.dz * (Cl - (double)k * dC); C.bz = 1.0 / (1.0 - dC);
-        }
+      double2 mx = make_double2(0.0, 1.0), my = mx, mz = mx;
+      if (mp.adve) {   // eq. 16 with the Courant numbers at the faces of the SD's time-n cell: the table of k_cell_move_consts
+        const double2* mvp = reinterpret_cast<const double2*>(cf.mv + (size_t)6 * c);
+        mx = mvp[0]; my = mvp[1]; mz = mvp[2];
       }
+      C.kX = ((32.0 / 3.0 * cst::g) * ((cst::rho_w - rho_a) * rho_a)) * rcp_nr2(eta * eta);
+      C.kv = (eta * (cst::kc_delta0 * cst::kc_delta0 / 8.0)) * rcp_nr2(rho_a);
+      // eq. 27: n (n - 1) / 2 pairs over floor(n / 2) drawn = n - 1 for even n, n for odd n
+      C.scale = m >= 2 ? (double)((m & 1) ? m : m - 1) : 0.0;
+      C.ax = mx.x; C.bx = mx.y; C.ay = my.x; C.by = my.y; C.az = mz.x; C.bz = mz.y;
     }
     if (tid == 0) segl[nc] = (u32)M;
     __syncthreads();
@@ -614,26 +633,46 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
     // the next step's histogram, taken in STORAGE order (the reorder of the next step then writes runs, not a permutation of
     // each cell): lanes that go to the same cell take consecutive places with one atomic on count[cell], as k_cellhist does
     if (moving || mp.fold) {
-      for (int t0 = 0; t0 < M; t0 += T) {
-        const int t = t0 + tid;
-        const bool in = t < M;
-        const u32 s = s0 + (u32)t;
-        const int sl = t + sh;
-        if (in && moving) {
+      // the places are asked for first, for the whole tile (one atomic per group of lanes and pass, none waited for), the
+      // positions are stored while they are on their way, and only then does the warp pick the answers up: the latency
+      // of the atomics is paid once per tile, not once per 128 SDs
+      constexpr int NIT = (CAP + T - 1) / T;
+      u32 base_r[NIT];
+      if (mp.fold) {
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+          base_r[it] = 0;
+          if (it * T < M) {
+            const int t = it * T + tid;
+            const u32 cnew = t < M ? s_id[t + sh] : CELL_DEAD;
+            const u32 peers = __match_any_sync(0xffffffffu, cnew);
+            if (cnew != CELL_DEAD && lane == __ffs(peers) - 1) base_r[it] = atomicAdd(&count[cnew], (u32)__popc(peers));
+          }
+        }
+      }
+      if (moving) {
+        for (int t = tid; t < M; t += T) {
+          const u32 s = s0 + (u32)t;
+          const int sl = t + sh;
           if (g.hx) a.x[s] = s_x[sl];
           if (g.hy) a.y[s] = s_y[sl];
           if (g.hz) a.z[s] = s_z[sl];
         }
-        if (mp.fold) {
-          const u32 cnew = in ? s_id[sl] : CELL_DEAD;
-          const u32 peers = __match_any_sync(0xffffffffu, cnew);
-          const int leader = __ffs(peers) - 1;
-          u32 base = 0;
-          if (cnew != CELL_DEAD && lane == leader) base = atomicAdd(&count[cnew], (u32)__popc(peers));
-          base = __shfl_sync(0xffffffffu, base, leader);
-          if (in) {
-            cell_out[s] = cnew;
-            if (cnew != CELL_DEAD) off_out[s] = base + __popc(peers & ((1u << lane) - 1u));
+      }
+      if (mp.fold) {
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+          if (it * T < M) {
+            const int t = it * T + tid;
+            const bool in = t < M;
+            const u32 cnew = in ? s_id[t + sh] : CELL_DEAD;
+            const u32 peers = __match_any_sync(0xffffffffu, cnew);
+            const u32 base = __shfl_sync(0xffffffffu, base_r[it], __ffs(peers) - 1);
+            if (in) {
+              const u32 s = s0 + (u32)t;
+              cell_out[s] = cnew;
+              if (cnew != CELL_DEAD) off_out[s] = base + __popc(peers & ((1u << lane) - 1u));
+            }
           }
         }
       }

@@ -27,6 +27,7 @@ struct CellFields {  // library-owned dense per-cell arrays
   double* eta;       // viscosity after the condensation feedback (for v_term)
   double* rho_a;     // air density rhod (1 + rv)
   const double *cx, *cy, *cz;   // rho_d * Courant on the Arakawa-C grid, dense C order
+  double* mv;        // eq. 16 per cell, 6 doubles: ax, bx, ay, by, az, bz (k_cell_move_consts; rebuilt when rhod or a Courant field changes)
 };
 
 // sdm_sort.cu
@@ -74,6 +75,8 @@ template <typename R>
 cudaError_t launch_coal_move_tile(int cpb, int need, const SdArraysT<R>& a, const u16* rank, const u32* seg, const Grid& g,
                                   const CellFields& cf, const CoalParams& kp, const CoalMoveParams& mp, double* flux_part,
                                   const Counters& cnt, u32* cell_out, u32* off_out, u32* count, cudaStream_t st);
+// the table cf.mv from cf.rhod and the Courant fields
+void launch_cell_move_consts(const Grid& g, const CellFields& cf, cudaStream_t st);
 // also copies the step's device error flag into flux_out[2], so that one read-back serves both
 void launch_flux_sum(double* flux_slots, const double* flux_part, int n_part, double* flux_out, double* flux_total, const u32* d_flag,
                      cudaStream_t st);

@@ -419,6 +419,22 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
   CoalCell* s_cell = reinterpret_cast<CoalCell*>(smem_raw + L::fixed_bytes);
   u32* segl = reinterpret_cast<u32*>(s_cell + cpb);     // storage offsets of the tile's cells
   u32* segp = segl + cpb + 1;                           // padded (even) offsets of the sorted positions
+  // what the lanes that own a cell of the tile need from global memory, requested together with the tile's bounds below:
+  // the whole CTA waits for these few lanes at the first barrier, so they should wait for ONE memory latency, not two
+  struct CellIn { u32 b0, b1; double eta, rho_a; double2 mx, my, mz; };
+  auto load_cell = [&](int c) {
+    CellIn in;
+    in.b0 = seg[c]; in.b1 = seg[c + 1];
+    in.eta = cf.eta[c]; in.rho_a = cf.rho_a[c];
+    in.mx = make_double2(0.0, 1.0); in.my = in.mx; in.mz = in.mx;
+    if (mp.adve) {   // eq. 16 with the Courant numbers at the faces of the SD's time-n cell: the table of k_cell_move_consts
+      const double2* mvp = reinterpret_cast<const double2*>(cf.mv + (size_t)6 * c);
+      in.mx = mvp[0]; in.my = mvp[1]; in.mz = mvp[2];
+    }
+    return in;
+  };
+  CellIn pre;
+  if (tid < nc) pre = load_cell(c_first + tid);
   const u32 s0 = seg[c_first];
   const int M = (int)(seg[c_first + nc] - s0);
   const int sh = (int)(s0 & 3u);
@@ -458,18 +474,12 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
     }
     for (int cl = tid; cl < nc; cl += T) {
       const int c = c_first + cl;
-      const u32 b0 = seg[c], b1 = seg[c + 1];
-      segl[cl] = b0 - s0;
-      const int m = (int)(b1 - b0);
+      const CellIn in = cl == tid ? pre : load_cell(c);
+      segl[cl] = in.b0 - s0;
+      const int m = (int)(in.b1 - in.b0);
       CoalCell& C = s_cell[cl];
-      // everything this lane needs from global memory is requested before any of it is used: the whole CTA waits for
-      // these few lanes at the next barrier, so one memory latency and ~25 instructions here instead of nine divisions
-      const double eta = cf.eta[c], rho_a = cf.rho_a[c];
-      double2 mx = make_double2(0.0, 1.0), my = mx, mz = mx;
-      if (mp.adve) {   // eq. 16 with the Courant numbers at the faces of the SD's time-n cell: the table of k_cell_move_consts
-        const double2* mvp = reinterpret_cast<const double2*>(cf.mv + (size_t)6 * c);
-        mx = mvp[0]; my = mvp[1]; mz = mvp[2];
-      }
+      const double eta = in.eta, rho_a = in.rho_a;
+      const double2 mx = in.mx, my = in.my, mz = in.mz;
       C.kX = ((32.0 / 3.0 * cst::g) * ((cst::rho_w - rho_a) * rho_a)) * rcp_nr2(eta * eta);
       C.kv = (eta * (cst::kc_delta0 * cst::kc_delta0 / 8.0)) * rcp_nr2(rho_a);
       // eq. 27: n (n - 1) / 2 pairs over floor(n / 2) drawn = n - 1 for even n, n for odd n
@@ -527,7 +537,7 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
     __syncthreads();
     // ---- pairs of sorted positions (2t, 2t+1): coalescence, then movement of both SDs ----------------------------------------
     const double dtdv = g.dt / g.dV;
-    const double inv_dx = 1.0 / g.dx, inv_dy = 1.0 / g.dy, inv_dz = 1.0 / g.dz;
+    const double inv_dx = mp.inv_dx, inv_dy = mp.inv_dy, inv_dz = mp.inv_dz;
     for (int t = tid; 2 * t < MP; t += T) {
       const u32 both = reinterpret_cast<const u32*>(inv)[t];
       const int ia = (int)(both & 0xFFFFu), ib = (int)(both >> 16);
@@ -746,7 +756,9 @@ static cudaError_t launch_coal_move_tile_cap(int cpb, const SdArraysT<R>& a, con
   auto kern = k_coal_move_tile<CAP, SDM_COAL_T, coal_minb<R>(), R>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mp, flux_part, cnt, cpb, cell_out, off_out, count);
+  CoalMoveParams mq = mp;
+  mq.inv_dx = 1.0 / g.dx; mq.inv_dy = 1.0 / g.dy; mq.inv_dz = 1.0 / g.dz;
+  kern<<<(g.ncell + cpb - 1) / cpb, SDM_COAL_T, smem, st>>>(a, rank, seg, g, cf, kp, mq, flux_part, cnt, cpb, cell_out, off_out, count);
   return cudaGetLastError();
 }
 template <typename R>

@@ -21,6 +21,7 @@ struct CoalMoveParams {
   u32 step;
   int fold;          // k_coal_move_tile also writes next step's cell index, offset and histogram (a0-a1 folded into a6)
   int coal_adapt_max;   // > 1: per-cell coalescence substeps from P_ij (DESIGN.md R-adapt-coal); per-cell kernel only
+  double inv_dx, inv_dy, inv_dz;   // 1/dx .. (IEEE), filled in by launch_coal_move_tile
 };
 struct CellFields {  // library-owned dense per-cell arrays
   double* rhod;      // copy of the caller's rhod

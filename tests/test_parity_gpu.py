@@ -247,6 +247,37 @@ def test_strided_fields_and_optional_arguments():
         np.testing.assert_array_equal(a[k], c[k])
 
 
+def test_new_courant_fields_and_rhod_handed_to_step_sync_mid_run():
+    """step_sync with new Courant fields and a new rho_d in the middle of a run (:751, :816: "may be omitted when unchanged"):
+    k_coal_move_tile takes its eq. 16 coefficients from a per-cell table (k_cell_move_consts) that must be rebuilt exactly
+    then; the oracle is handed the same fields before the same step."""
+    from tests.util import courant_xyz
+
+    b = binding()
+    w = rain_mix(W.cfg2_2d(sd_per_cell=24, nx=12, nz=16, seed=61))
+    o = make_oracle(w)
+    p, th, rv = make_particles(w)
+    oo, po = oracle.make_opts(**w.opts), b.make_opts(**w.opts)
+    c = courant_xyz(w)
+    for s in range(6):
+        kw = {}
+        if s == 2:     # the flow reversed and halved from here on (rho_d C stays non-divergent)
+            cx2, cz2 = (-0.5 * c["x"]).contiguous(), (-0.5 * c["z"]).contiguous()
+            o.set_fields(cx=np_(cx2).ravel(), cz=np_(cz2).ravel())
+            kw = dict(courant_1=cx2.cuda(), courant_2=cz2.cuda())
+        if s == 4:     # a new rho_d alone (the table divides the Courant fields by it)
+            rhod2 = (1.002 * w.rhod).contiguous()
+            o.set_fields(rhod=np_(rhod2).ravel())
+            kw = dict(rhod=rhod2.cuda())
+        fo = o.step(oo)
+        p.step_sync(po, th, rv, **kw)
+        p.step_async(po)
+        np.testing.assert_allclose(p.step_async_result(), fo, rtol=3 * RTOL, atol=1e-300)
+        compare_states(p, o, positions=True)
+        compare_fields(th, rv, o)
+    assert p.stats()["coal_tile_cells"] > 0     # the tile kernel (and its table) did run
+
+
 def test_step_host_matches_device_path():
     b = binding()
     w = rain_mix(W.cfg2_2d(sd_per_cell=16, nx=9, nz=7, seed=14))

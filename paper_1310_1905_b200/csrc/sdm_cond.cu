@@ -880,8 +880,9 @@ struct Cond4 {
   static size_t smem(int cpb) { return fixed_bytes + (size_t)cpb * sizeof(CellRec) + (size_t)(cpb + 1) * 4 + 16; }
 };
 
-// ADAPT: per-cell substep counts (cp.adapt_tol > 0, DESIGN.md R-adapt); the fixed-substep instantiation carries none of it
-template <int CAP, int T, int MINB, typename R, bool ADAPT>
+// ADAPT: per-cell substep counts (cp.adapt_tol > 0, DESIGN.md R-adapt); the fixed-substep instantiation carries none of it.
+// KF: evaluations per SD-substep in the sweep as a compile-time constant (0: cp.kfast, sdm_set_cond_kfast)
+template <int CAP, int T, int MINB, typename R, bool ADAPT, int KF = 0>
 __global__ void __launch_bounds__(T, MINB)
 k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ seg, Grid g, Field th_f, Field rv_f,
         CellFields cf, CondParams cp, Counters cnt, int cpb) {
@@ -1086,7 +1087,8 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
 #endif
       if (guard) st = 2;
       if (!valid) st = 1;
-      for (int it = 1; it < cp.kfast; ++it) {
+#pragma unroll 1
+      for (int it = 1; it < (KF ? KF : cp.kfast); ++it) {   // KF: the bound as an immediate (0.6 % of the kernel); unrolling costs 4 %
         if (!__any_sync(0xffffffffu, st == 0)) break;
         if (st == 0) {
           double y;
@@ -1659,6 +1661,10 @@ static cudaError_t launch_cond4(size_t smem, int grid, const SdArraysT<R>& a, co
     cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_cond4<CAP, T, MINB, R, true><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
+  } else if (CAP == SDM_COND_CAP && cp.kfast == 4) {   // the default of the small tile kernel
+    cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R, false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_cond4<CAP, T, MINB, R, false, 4><<<grid, T, smem, st>>>(a, rank, seg, g, th, rv, cf, cp, cnt, cpb);
   } else {
     cudaError_t e = cudaFuncSetAttribute(k_cond4<CAP, T, MINB, R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

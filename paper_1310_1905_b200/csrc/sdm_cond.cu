@@ -1136,13 +1136,9 @@ k_cond4(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __restrict__ se
         s_r[e] = r;
         ++n_sub;
       }
-      const unsigned need = __ballot_sync(0xffffffffu, st == 2);
-      if (need) {   // warp-aggregated append to the tile's slow list
-        u32 base = 0;
-        if (lane == 0) base = atomicAdd(&ctr[1], (u32)__popc(need));
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (st == 2) list[base + __popc(need & ((1u << lane) - 1u))] = (u16)e;
-      }
+      // append to the tile's slow list: one shared atomic per listed SD.  Listed SDs are rare (5e-5 of the SD-substeps), a vote
+      // that aggregates them per warp is paid by every chunk (0.65 % of the kernel); the order of the list does not matter
+      if (st == 2) list[atomicAdd(&ctr[1], 1u)] = (u16)e;
     }
     __syncthreads();
     // C. the listed rest, from the start of the substep: cond_solve (bracketed Newton) or the paper's literal
@@ -1521,13 +1517,7 @@ k_cond4f(SdArraysT<float> a, const u16* __restrict__ rank, const u32* __restrict
         s_r[e] = r0 + d;
         n_es += 0x100000u;
       }
-      const unsigned need = __ballot_sync(0xffffffffu, st == 2);
-      if (need) {   // warp-aggregated append to the tile's slow list
-        u32 base = 0;
-        if (lane == 0) base = atomicAdd(&ctr[1], (u32)__popc(need));
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (st == 2) list[base + __popc(need & ((1u << lane) - 1u))] = (u16)e;
-      }
+      if (st == 2) list[atomicAdd(&ctr[1], 1u)] = (u16)e;   // as in k_cond4: no vote per chunk for the rare listed SD
     }
     __syncthreads();
     // C. the listed rest in fp64 (SI units), exactly as k_cond4 does: cond_solve or the paper's literal bisection

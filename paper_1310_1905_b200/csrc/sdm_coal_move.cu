@@ -648,15 +648,18 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
       // of the atomics is paid once per tile, not once per 128 SDs
       constexpr int NIT = (CAP + T - 1) / T;
       u32 base_r[NIT];
+      u32 peers_r[NIT];   // the groups of lanes that go to the same cell (a second __match_any per pass costs more than NIT registers)
       if (mp.fold) {
 #pragma unroll
         for (int it = 0; it < NIT; ++it) {
           base_r[it] = 0;
+          peers_r[it] = 0;
           if (it * T < M) {
             const int t = it * T + tid;
             const u32 cnew = t < M ? s_id[t + sh] : CELL_DEAD;
             const u32 peers = __match_any_sync(0xffffffffu, cnew);
             if (cnew != CELL_DEAD && lane == __ffs(peers) - 1) base_r[it] = atomicAdd(&count[cnew], (u32)__popc(peers));
+            peers_r[it] = peers;
           }
         }
       }
@@ -676,7 +679,7 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
             const int t = it * T + tid;
             const bool in = t < M;
             const u32 cnew = in ? s_id[t + sh] : CELL_DEAD;
-            const u32 peers = __match_any_sync(0xffffffffu, cnew);
+            const u32 peers = peers_r[it];
             const u32 base = __shfl_sync(0xffffffffu, base_r[it], __ffs(peers) - 1);
             if (in) {
               const u32 s = s0 + (u32)t;
@@ -688,14 +691,11 @@ k_coal_move_tile(SdArraysT<R> a, const u16* __restrict__ rank, const u32* __rest
       }
     }
   }
-  unsigned v0 = n_pairs, v1 = n_coll, v2 = n_tie;
+  // integer counters by the warp-reduce instruction (REDUX), the flux by a butterfly in a fixed order
+  const unsigned v0 = __reduce_add_sync(0xffffffffu, n_pairs), v1 = __reduce_add_sync(0xffffffffu, n_coll),
+                 v2 = __reduce_add_sync(0xffffffffu, n_tie);
 #pragma unroll
-  for (int d = 16; d >= 1; d >>= 1) {
-    v0 += __shfl_xor_sync(0xffffffffu, v0, d);
-    v1 += __shfl_xor_sync(0xffffffffu, v1, d);
-    v2 += __shfl_xor_sync(0xffffffffu, v2, d);
-    flux += __shfl_xor_sync(0xffffffffu, flux, d);
-  }
+  for (int d = 16; d >= 1; d >>= 1) flux += __shfl_xor_sync(0xffffffffu, flux, d);
   if (lane == 0) {
     const int slot = (blockIdx.x * NW + warp) & (NSLOT - 1);
     if (v0) atomicAdd(&cnt.pairs[slot], (unsigned long long)v0);

@@ -525,7 +525,7 @@ int sdm_step_sync(sdm_ctx* ctx, const sdm_opts* op, sdm_arrinfo th, sdm_arrinfo 
   if (ctx->o.real_bytes == 8) launch_scatter(view<double>(ctx->buf[ctx->cur]), view<double>(ctx->buf[ctx->cur ^ 1]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
   else launch_scatter(view<float>(ctx->buf[ctx->cur]), view<float>(ctx->buf[ctx->cur ^ 1]), d_cur, (u32)ctx->nslots, g, ctx->cell, ctx->off, ctx->seg, st);
   t_end(ctx, SDM_STAGE_SCATTER, st);
-  ctx->launches += ctx->nslots ? 1 : 0;
+  ctx->launches += ctx->nslots ? scatter_parts((u32)ctx->nslots) : 0;   // one launch, or two halves (sdm_sort.cu)
   CK(cudaGetLastError());
   CK(cudaEventSynchronize(ctx->ev_info));   // the scatter runs while the host sizes the next launches
   ctx->host_syncs++;

@@ -36,6 +36,7 @@ template <typename R>
 void launch_cellhist(const SdArraysT<R>& a, const u32* d_nslots, u32 nslots_bound, const Grid& g, u32* cell, u32* off,
                      u32* count, cudaStream_t st);
 int scan_num_blocks(int ncell);
+int scatter_parts(u32 nslots_bound);   // launches of the reorder (1 or 2)
 void launch_scan(u32* count, int ncell, u32* blocksum, u32* seg, u32* d_nslots_next, u32* d_maxcount, cudaStream_t st);
 void launch_tile_max(const u32* seg, int ncell, int cpb0, u32* d_tilemax4, cudaStream_t st);
 template <typename R>

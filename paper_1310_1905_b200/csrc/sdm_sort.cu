@@ -124,30 +124,49 @@ __global__ void __launch_bounds__(256) k_tile_max(const u32* __restrict__ seg, i
 }
 
 // ---- a3: scatter the SoA state into cell-sorted storage (drops dead SDs) ----------------------------
-template <typename R>
+// The eight attributes move in SCATTER_PARTS = 2 launches of four attributes each (n, r_w^2, r_d^3, kappa | x, y, z, id), each
+// of which reads the SD's cell and offset again: with all eight in one kernel (9 read and 8 scattered write streams at once)
+// the reorder ran at 0.79 of the copy rate on its DRAM bytes, in two halves at 0.87 although they move 8 B per SD more
+// (1.72 -> 1.55 ms at 67 M SDs; three parts 1.64, four 1.81, eight 2.81 ms: profiles/r2_k_scatter_ncu_full.md).  Populations of a few
+// million SDs gain nothing (8.4 M: 0.176 / 0.174 ms) or lose the second launch (2.1 M: 0.053 -> 0.056 ms): one part below 2^24 SDs.
+constexpr int SCATTER_PARTS = 2;
+int scatter_parts(u32 nslots_bound) { return nslots_bound < (1u << 24) ? 1 : SCATTER_PARTS; }
+template <typename R, int PARTS, int PART>
 __global__ void __launch_bounds__(256) k_scatter(SdArraysT<R> src, SdArraysT<R> dst, const u32* __restrict__ d_nslots, Grid g,
                                                  const u32* __restrict__ cell, const u32* __restrict__ off,
                                                  const u32* __restrict__ seg) {
   const u32 i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= *d_nslots) return;
+  constexpr auto mine = [](int k) { return k * PARTS / 8 == PART; };   // attribute k = n, rw2, rd3, kappa, x, y, z, id
   // all loads first, and none of them behind the test for a dead SD: the two copies of the state are not declared
   // disjoint, so a store between two loads would order them
   const u32 c = cell[i];
   const u32 o = off[i];
-  const u64 n = src.n[i];
-  const R rw2 = src.rw2[i], rd3 = src.rd3[i], kappa = src.kappa[i];
-  const R x = g.hx ? src.x[i] : R(0), y = g.hy ? src.y[i] : R(0), z = g.hz ? src.z[i] : R(0);
-  const u32 id = src.id[i];
+  u64 n = 0; R rw2 = R(0), rd3 = R(0), kappa = R(0), x = R(0), y = R(0), z = R(0); u32 id = 0;
+  if (mine(0)) n = src.n[i];
+  if (mine(1)) rw2 = src.rw2[i];
+  if (mine(2)) rd3 = src.rd3[i];
+  if (mine(3)) kappa = src.kappa[i];
+  if (mine(4) && g.hx) x = src.x[i];
+  if (mine(5) && g.hy) y = src.y[i];
+  if (mine(6) && g.hz) z = src.z[i];
+  if (mine(7)) id = src.id[i];
   if (c == CELL_DEAD) return;
   const u32 d = seg[c] + o;
-  dst.n[d] = n;
-  dst.rw2[d] = rw2;
-  dst.rd3[d] = rd3;
-  dst.kappa[d] = kappa;
-  if (g.hx) dst.x[d] = x;
-  if (g.hy) dst.y[d] = y;
-  if (g.hz) dst.z[d] = z;
-  dst.id[d] = id;
+  if (mine(0)) dst.n[d] = n;
+  if (mine(1)) dst.rw2[d] = rw2;
+  if (mine(2)) dst.rd3[d] = rd3;
+  if (mine(3)) dst.kappa[d] = kappa;
+  if (mine(4) && g.hx) dst.x[d] = x;
+  if (mine(5) && g.hy) dst.y[d] = y;
+  if (mine(6) && g.hz) dst.z[d] = z;
+  if (mine(7)) dst.id[d] = id;
+}
+template <typename R, int PARTS, int PART = 0>
+static void launch_scatter_parts(const SdArraysT<R>& src, const SdArraysT<R>& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
+                                 const u32* cell, const u32* off, const u32* seg, cudaStream_t st) {
+  k_scatter<R, PARTS, PART><<<(nslots_bound + 255) / 256, 256, 0, st>>>(src, dst, d_nslots, g, cell, off, seg);
+  if constexpr (PART + 1 < PARTS) launch_scatter_parts<R, PARTS, PART + 1>(src, dst, d_nslots, nslots_bound, g, cell, off, seg, st);
 }
 
 // ---- a2 (second level): rank of every SD inside its cell under (Philox key, id) ----------------------
@@ -331,7 +350,8 @@ template <typename R>
 void launch_scatter(const SdArraysT<R>& src, const SdArraysT<R>& dst, const u32* d_nslots, u32 nslots_bound, const Grid& g,
                     const u32* cell, const u32* off, const u32* seg, cudaStream_t st) {
   if (nslots_bound == 0) return;
-  k_scatter<R><<<(nslots_bound + 255) / 256, 256, 0, st>>>(src, dst, d_nslots, g, cell, off, seg);
+  if (scatter_parts(nslots_bound) == 1) launch_scatter_parts<R, 1>(src, dst, d_nslots, nslots_bound, g, cell, off, seg, st);
+  else launch_scatter_parts<R, SCATTER_PARTS>(src, dst, d_nslots, nslots_bound, g, cell, off, seg, st);
 }
 
 #define SDM_INST(R)                                                                                              \

@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) k_tile_max(const u32* __restrict__ seg, i
 // ---- a3: scatter the SoA state into cell-sorted storage (drops dead SDs) ----------------------------
 // The eight attributes move in SCATTER_PARTS = 2 launches of four attributes each (n, r_w^2, r_d^3, kappa | x, y, z, id), each
 // of which reads the SD's cell and offset again: with all eight in one kernel (9 read and 8 scattered write streams at once)
-// the reorder ran at 0.79 of the copy rate on its DRAM bytes, in two halves at 0.87 although they move 8 B per SD more
+// the reorder ran at 0.79 of the copy rate on its DRAM bytes, in two halves at 0.90 although they move 8 B per SD more
 // (1.72 -> 1.55 ms at 67 M SDs; three parts 1.64, four 1.81, eight 2.81 ms: profiles/r2_k_scatter_ncu_full.md).  Populations of a few
 // million SDs gain nothing (8.4 M: 0.176 / 0.174 ms) or lose the second launch (2.1 M: 0.053 -> 0.056 ms): one part below 2^24 SDs.
 constexpr int SCATTER_PARTS = 2;

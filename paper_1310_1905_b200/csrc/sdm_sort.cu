@@ -257,6 +257,18 @@ __global__ void __launch_bounds__(128) k_rank_count(const u32* __restrict__ id, 
 // it: ~16 compares per SD instead of the log^2 m barriers and swaps of the bitonic network (which stays for cells
 // beyond 8192 SDs).  G = 32: a warp per cell, 4 cells per CTA; G = 256: a CTA per cell.
 // Shared memory per group: u64 keys[P], u64 sorted[P], u32 hist[P/16].
+// Buckets per cell for P key slots (P = the largest cell, rounded up to a power of two).  The compare loop inside the bucket is half
+// of the kernel's instructions at ~8 keys per bucket, the histogram and its scan are cheap while they fit a few words per lane:
+// ~2 keys per bucket up to 128 buckets (a cell of 64 SDs in P = 128: 0.73 -> 0.59 ms at 67 M SDs), ~16 for the CTA-wide path of
+// crowded cells, whose scan runs on one warp.
+#ifdef SDM_RANK_BUCKET_SHIFT
+__host__ __device__ inline int rank_buckets(int P) { return (P >> SDM_RANK_BUCKET_SHIFT) > 4 ? (P >> SDM_RANK_BUCKET_SHIFT) : 4; }
+#else
+__host__ __device__ inline int rank_buckets(int P) {
+  const int nb = P <= 256 ? P >> 1 : P <= 512 ? P >> 2 : P >> 4;
+  return nb > 4 ? nb : 4;
+}
+#endif
 template <int G>
 __global__ void __launch_bounds__(CtaOf<G>::threads) k_rank_bucket(const u32* __restrict__ id, const u32* __restrict__ seg,
                                                                    int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
@@ -265,7 +277,7 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_rank_bucket(const u32* __
   constexpr int NG = CtaOf<G>::threads / G;
   const int gi = threadIdx.x / G;
   const Group<G> grp = make_group<G>(nullptr);
-  const int NB = max(P >> 4, 4);               // buckets (power of two)
+  const int NB = rank_buckets(P);              // buckets (power of two)
   const int shift = 64 - (31 - __clz(NB));     // key >> shift = bucket
   unsigned char* base = smem_raw + (size_t)gi * ((size_t)P * 16 + (size_t)NB * 4);
   u64* skey = reinterpret_cast<u64*>(base);
@@ -387,7 +399,7 @@ template <int G>
 static cudaError_t launch_rank_bucket_t(const u32* id, const u32* seg, int ncell, u32 step, u32 seed_lo, u32 seed_hi, int P,
                                         u16* rank, int* d_error, cudaStream_t st) {
   constexpr int NG = CtaOf<G>::threads / G;
-  const size_t smem = (size_t)NG * ((size_t)P * 16 + (size_t)std::max(P >> 4, 4) * 4);
+  const size_t smem = (size_t)NG * ((size_t)P * 16 + (size_t)rank_buckets(P) * 4);
   cudaError_t e = cudaFuncSetAttribute(k_rank_bucket<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   k_rank_bucket<G><<<(ncell + NG - 1) / NG, CtaOf<G>::threads, smem, st>>>(id, seg, ncell, step, seed_lo, seed_hi, P, rank, d_error);

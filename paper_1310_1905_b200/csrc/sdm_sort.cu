@@ -322,7 +322,12 @@ __global__ void __launch_bounds__(CtaOf<G>::threads) k_rank_bucket(const u32* __
     const u32 b = (u32)(key >> shift);
     const int lo = b ? (int)hist[b - 1] : 0, hi = (int)hist[b];
     int r = lo;
-    for (int j = lo; j < hi; ++j) r += (ssort[j] < key);
+    if constexpr (G < 256) {   // ~2 keys per bucket: a 4-fold unrolled loop with its remainder costs more than it saves (0.59 -> 0.54 ms)
+#pragma unroll 1
+      for (int j = lo; j < hi; ++j) r += (ssort[j] < key);
+    } else {
+      for (int j = lo; j < hi; ++j) r += (ssort[j] < key);
+    }
     rank[s0 + t] = (u16)r;
   }
 }

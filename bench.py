@@ -68,8 +68,8 @@ NCU_COND32_DRAM_BYTES = (1.509464e9 + 0.313273e9, "profiles/r1_k_cond4f_ncu_full
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="3d", choices=["3d", "2d", "sweep"])
     ap.add_argument("--sd-per-cell", type=int, default=0)
